@@ -1,0 +1,255 @@
+"""Seeded synthetic inputs for the five BASELINE.json configs (and reduced-size variants).
+
+This module serves BOTH the CPU oracle and the CUDA path and therefore holds none of the method's
+arithmetic: it only builds node coordinates, initial states and boundary data (numpy, seeded with
+numpy.random.default_rng).  The inputs are synthetic stand-ins with the shapes, sizes and value ranges of
+the paper's workloads; the paper's own
+grids and data are not in the container and nothing here reproduces them.
+
+Every generator returns a dict:
+  params   plain dict with the fields of the params struct (ni,nj,nk,periodic,period,viscous,...)
+  x,y,z    node coordinates, shape (nk+1, nj+1, ni+1), float64
+  dx_mode,dy_mode,dz_mode   node displacement modes (moving meshes only)
+  U0       initial conservative state, shape (5, nk, nj, ni)
+  inflow   {face: P_in (5, n2, n1)}       (optional)
+  sigma, U_ref                            (optional sponge)
+  dt, steps, name, t0
+"""
+import hashlib
+import json
+import os
+
+import numpy as np
+
+GAMMA = 1.4
+
+
+def cell_centres(a):
+    """8-vertex mean of a node array -- geometry preprocessing for the initial data."""
+    return 0.125 * (a[:-1, :-1, :-1] + a[:-1, :-1, 1:] + a[:-1, 1:, :-1] + a[:-1, 1:, 1:]
+                    + a[1:, :-1, :-1] + a[1:, :-1, 1:] + a[1:, 1:, :-1] + a[1:, 1:, 1:])
+
+
+def conservative(rho, u, v, w, p, gamma=GAMMA):
+    """(rho,u,v,w,p) -> Q of Eq. 5; input packing only."""
+    E = p / (gamma - 1.0) + 0.5 * rho * (u * u + v * v + w * w)
+    return np.ascontiguousarray(np.stack([rho, rho * u, rho * v, rho * w, E]))
+
+
+def sha256(*arrays):
+    h = hashlib.sha256()
+    for a in arrays:
+        h.update(np.ascontiguousarray(a).tobytes())
+    return h.hexdigest()
+
+
+def _base_params(ni, nj, nk, **kw):
+    p = dict(ni=ni, nj=nj, nk=nk, periodic=[1, 1, 1], period=[[0.0] * 3 for _ in range(3)], scheme=0,
+             viscous=0, gamma=GAMMA, r_gas=1.0, prandtl=0.71, mu_ref=0.0, t_ref=1.0, s_suth=-1.0,
+             mp_alpha=4.0, moving=0, omega=0.0, bc=[0] * 6, p_out=0.0)
+    p.update(kw)
+    return p
+
+
+def _comp_coords(n, L):
+    """computational coordinates of the nodes, (nk+1,nj+1,ni+1) each, spanning [0,L]"""
+    ni, nj, nk = n
+    xi = np.arange(ni + 1) * (L[0] / ni)
+    et = np.arange(nj + 1) * (L[1] / nj)
+    ze = np.arange(nk + 1) * (L[2] / nk)
+    Z, E, X = np.meshgrid(ze, et, xi, indexing="ij")
+    return X, E, Z
+
+
+_DT_FILE = os.path.join(os.path.dirname(os.path.abspath(__file__)), "..", "tests", "golden", "dt.json")
+
+
+def stored_dt(name):
+    """Time steps written by tests/golden/make_dt.py (oracle's Eq. B.2/B.3); None if not stored."""
+    try:
+        with open(_DT_FILE) as f:
+            return json.load(f).get(name)
+    except FileNotFoundError:
+        return None
+
+
+# --------------------------------------------------------------------------------------------------
+def wavy_periodic_grid(n, L, amp, centre=True):
+    """x = xi + amp sin(2 pi eta/L) sin(2 pi zeta/L) and cyclic (config 1; form of Eq. 45)."""
+    X, E, Z = _comp_coords((n, n, n), (L, L, L))
+    s = lambda a: np.sin(2.0 * np.pi * a / L)
+    x = X + amp * s(E) * s(Z)
+    y = E + amp * s(Z) * s(X)
+    z = Z + amp * s(X) * s(E)
+    if centre:
+        x, y, z = x - L / 2, y - L / 2, z - L / 2
+    return x, y, z
+
+
+def random_periodic_grid(n, L, frac, seed, centre=True):
+    """uniform grid with every node moved by U(-frac,frac) x spacing, identical on periodic images."""
+    X, E, Z = _comp_coords((n, n, n), (L, L, L))
+    rng = np.random.default_rng(seed)
+    out = []
+    for base in (X, E, Z):
+        r = rng.uniform(-frac, frac, size=(n, n, n)) * (L / n)
+        full = np.empty((n + 1, n + 1, n + 1))
+        full[:n, :n, :n] = r
+        full[n, :, :] = full[0, :, :]
+        full[:, n, :] = full[:, 0, :]
+        full[:, :, n] = full[:, :, 0]
+        out.append(base + full - (L / 2 if centre else 0.0))
+    return out
+
+
+def isentropic_vortex(xc, yc, mach=0.5, eps=5.0, gamma=GAMMA):
+    """z-aligned isentropic vortex on a Mach `mach` +x stream, rho_inf = p_inf = 1 (config 1)."""
+    r2 = xc * xc + yc * yc
+    f = eps / (2.0 * np.pi) * np.exp(0.5 * (1.0 - r2))
+    u = mach * np.sqrt(gamma) - yc * f
+    v = xc * f
+    T = 1.0 - (gamma - 1.0) * eps * eps / (8.0 * gamma * np.pi ** 2) * np.exp(1.0 - r2)
+    rho = T ** (1.0 / (gamma - 1.0))
+    p = rho ** gamma
+    return rho, u, v, np.zeros_like(u), p
+
+
+def c1_vortex(n=32, wavy=True, steps=10):
+    """Config 1: inviscid isentropic vortex, periodic [-5,5]^3, wavy mesh amplitude 0.1, CFL 0.5."""
+    L = 10.0
+    x, y, z = wavy_periodic_grid(n, L, 0.1 if wavy else 0.0)
+    rho, u, v, w, p = isentropic_vortex(cell_centres(x), cell_centres(y))
+    prm = _base_params(n, n, n, period=[[L, 0, 0], [0, L, 0], [0, 0, L]])
+    name = "c1_vortex_%d%s" % (n, "" if wavy else "_cart")
+    return dict(name=name, params=prm, x=x, y=y, z=z, U0=conservative(rho, u, v, w, p), dt=stored_dt(name),
+                cfl=0.5, steps=steps, t0=0.0)
+
+
+def freestream_state(shape, mach=0.5, gamma=GAMMA):
+    """(rho,u,v,w,p) = (1,1,0,0,1/(gamma M^2))"""
+    one = np.ones(shape)
+    return one, one.copy(), 0 * one, 0 * one, one / (gamma * mach * mach)
+
+
+def freestream_static(n=20, kind="wavy", seed=7):
+    """Sec. 8.1.1 analogue: uniform flow on a sinusoidal or 20%-randomised periodic grid, L=4."""
+    L = 4.0
+    if kind == "wavy":
+        # Eq. 45: amplitude = one grid spacing, half-wave sin(pi ...) over [0,L] made periodic
+        X, E, Z = _comp_coords((n, n, n), (L, L, L))
+        h = L / n
+        s = lambda a: np.sin(2.0 * np.pi * a / L)
+        x = X + h * s(E) * s(Z) - L / 2
+        y = E + h * s(Z) * s(X) - L / 2
+        z = Z + h * s(X) * s(E) - L / 2
+    else:
+        x, y, z = random_periodic_grid(n, L, 0.2, seed)
+    prm = _base_params(n, n, n, period=[[L, 0, 0], [0, L, 0], [0, 0, L]])
+    U0 = conservative(*freestream_state((n, n, n)))
+    return dict(name="freestream_%s_%d" % (kind, n), params=prm, x=x, y=y, z=z, U0=U0, dt=None, cfl=0.2,
+                steps=10, t0=0.0)
+
+
+def c2_dynamic_freestream(n=64, steps=100, seed=20231):
+    """Config 2: uniform Mach 0.5 flow, periodic unit cube, nodes move as 0.08 sin(2 pi t) sin sin (+-2% jitter)."""
+    L = 1.0
+    X, E, Z = _comp_coords((n, n, n), (L, L, L))
+    xj, yj, zj = random_periodic_grid(n, L, 0.02, seed)
+    s = lambda a: np.sin(2.0 * np.pi * a)
+    dxm = 0.08 * s(E) * s(Z)
+    dym = 0.08 * s(Z) * s(X)
+    dzm = 0.08 * s(X) * s(E)
+    prm = _base_params(n, n, n, period=[[L, 0, 0], [0, L, 0], [0, 0, L]], moving=1, omega=1.0)
+    U0 = conservative(*freestream_state((n, n, n)))
+    name = "c2_dynfree_%d" % n
+    return dict(name=name, params=prm, x=xj, y=yj, z=zj, dx_mode=dxm, dy_mode=dym, dz_mode=dzm, U0=U0,
+                dt=stored_dt(name), cfl=0.2, steps=steps, t0=0.0)
+
+
+def tgv_state(xc, yc, zc, mach=0.1, gamma=GAMMA):
+    p0 = 1.0 / (gamma * mach * mach)
+    u = np.sin(xc) * np.cos(yc) * np.cos(zc)
+    v = -np.cos(xc) * np.sin(yc) * np.cos(zc)
+    w = np.zeros_like(u)
+    p = p0 + (np.cos(2 * xc) + np.cos(2 * yc)) * (np.cos(2 * zc) + 2.0) / 16.0
+    rho = p / p0
+    return rho, u, v, w, p
+
+
+def c3_tgv(n=128, steps=200, seed=1600, amp=0.05, scheme=0, re=1600.0):
+    """Config 3 (and 5 with scheme=1): viscous Taylor-Green vortex, Re 1600, Ma 0.1, wavy periodic mesh."""
+    L = 2.0 * np.pi
+    X, E, Z = _comp_coords((n, n, n), (L, L, L))
+    rng = np.random.default_rng(seed)
+    k = rng.integers(1, 4, size=(3, 2))
+    ph = rng.uniform(0.0, 2.0 * np.pi, size=(3, 2))
+    x = X - np.pi + amp * np.sin(k[0, 0] * E + ph[0, 0]) * np.sin(k[0, 1] * Z + ph[0, 1])
+    y = E - np.pi + amp * np.sin(k[1, 0] * Z + ph[1, 0]) * np.sin(k[1, 1] * X + ph[1, 1])
+    z = Z - np.pi + amp * np.sin(k[2, 0] * X + ph[2, 0]) * np.sin(k[2, 1] * E + ph[2, 1])
+    mach = 0.1
+    p0 = 1.0 / (GAMMA * mach * mach)
+    prm = _base_params(n, n, n, period=[[L, 0, 0], [0, L, 0], [0, 0, L]], viscous=1, r_gas=p0,
+                       mu_ref=1.0 / re, t_ref=1.0, s_suth=110.4 / 293.0, scheme=scheme)
+    rho, u, v, w, p = tgv_state(cell_centres(x), cell_centres(y), cell_centres(z), mach)
+    name = "c%d_tgv_%d" % (5 if scheme else 3, n)
+    return dict(name=name, params=prm, x=x, y=y, z=z, U0=conservative(rho, u, v, w, p), dt=stored_dt(name),
+                cfl=0.2, steps=steps, t0=0.0)
+
+
+def jet_exit_state(mj=1.35, tn=1.0, gamma=GAMMA):
+    """Eq. 55 in units rho_inf = a_inf = 1."""
+    pe = (1.0 / gamma) * ((2.0 + (gamma - 1.0) * mj * mj) / (gamma + 1.0)) ** (gamma / (gamma - 1.0))
+    rhoe = gamma * (gamma + 1.0) * pe / (2.0 * tn)
+    ue = np.sqrt(2.0 * tn / (gamma + 1.0))
+    return rhoe, ue, pe
+
+
+def c4_jet(ni=320, nj=200, nk=200, steps=500, seed=135, re=1.0e4):
+    """Config 4: under-expanded Mach 1.35 jet on a tanh-stretched Cartesian-topology mesh, inflow/outflow,
+    sponge, viscous Re_D = 1e4.  Constant dt = 2e-3 (the paper's dt a_inf/D)."""
+    Lx, bx, Lr, br = 25.0, 2.0, 8.0, 2.0
+    s = np.arange(ni + 1) / ni
+    xs = Lx * (1.0 - np.tanh(bx * (1.0 - s)) / np.tanh(bx))
+
+    def radial(n):
+        sg = 2.0 * np.arange(n + 1) / n - 1.0
+        return np.sign(sg) * Lr * (1.0 - np.tanh(br * (1.0 - np.abs(sg))) / np.tanh(br))
+
+    ys, zs = radial(nj), radial(nk)
+    z, y, x = np.meshgrid(zs, ys, xs, indexing="ij")
+    x, y, z = (np.ascontiguousarray(a) for a in (x, y, z))
+    g = GAMMA
+    rhoe, ue, pe = jet_exit_state()
+    shape = (nk, nj, ni)
+    amb = (np.ones(shape), np.zeros(shape), np.zeros(shape), np.zeros(shape), np.full(shape, 1.0 / g))
+    U0 = conservative(*amb)
+    # inflow face imin: top-hat of diameter 1, 1% seeded velocity perturbation
+    yc = 0.5 * (ys[:-1] + ys[1:])
+    zc = 0.5 * (zs[:-1] + zs[1:])
+    ZC, YC = np.meshgrid(zc, yc, indexing="ij")
+    core = (YC * YC + ZC * ZC) < 0.25
+    rng = np.random.default_rng(seed)
+    pert = 1.0 + 0.01 * rng.uniform(-1.0, 1.0, size=core.shape)
+    pin = np.zeros((5, nk, nj))
+    pin[0] = np.where(core, rhoe, 1.0)
+    pin[1] = np.where(core, ue * pert, 0.0)
+    pin[4] = np.where(core, pe, 1.0 / g)
+    # sponge: sigma = 2 s^2 over the last 15% of x and the outer 15% of |y|,|z|
+    xc3, yc3, zc3 = cell_centres(x), cell_centres(y), cell_centres(z)
+    ramp = lambda a, L: np.clip((a - 0.85 * L) / (0.15 * L), 0.0, 1.0)
+    sp = np.maximum(ramp(xc3, Lx), np.maximum(ramp(np.abs(yc3), Lr), ramp(np.abs(zc3), Lr)))
+    sigma = 2.0 * sp * sp
+    # viscosity: Re_D = rho_e u_e D / mu(T_e) with Sutherland (t_ref = T_inf = 1, S = 110.4/293)
+    r_gas = 1.0 / g
+    Te = pe / (rhoe * r_gas)
+    S = 110.4 / 293.0
+    mu_e = rhoe * ue / re
+    mu_ref = mu_e / (Te ** 1.5 * (1.0 + S) / (Te + S))
+    prm = _base_params(ni, nj, nk, periodic=[0, 0, 0], viscous=1, r_gas=r_gas, mu_ref=mu_ref, t_ref=1.0,
+                       s_suth=S, bc=[1, 2, 2, 2, 2, 2], p_out=1.0 / g)
+    return dict(name="c4_jet_%dx%dx%d" % (ni, nj, nk), params=prm, x=x, y=y, z=z, U0=U0, inflow={0: pin},
+                sigma=sigma, U_ref=U0.copy(), dt=2.0e-3, cfl=None, steps=steps, t0=0.0)
+
+
+def c5_tgv_mig4(n=384, steps=50):
+    return c3_tgv(n=n, steps=steps, scheme=1)
