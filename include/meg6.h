@@ -1,0 +1,114 @@
+/*
+ * meg6.h -- C ABI of the B200 (sm_100a) implementation of the MEG6 right-hand side + SSP-RK3 step of
+ * arXiv 2303.10785 (Chandravamsi et al., gradient-based reconstruction on curvilinear / dynamic meshes).
+ *
+ * Citations: "P:n" = line n of the paper text; "Rn" = reading n of a garbled or silent
+ * passage, listed in DESIGN.md.
+ *
+ * Conventions (all entry points):
+ *  - Every array pointer is a DEVICE pointer owned by the caller unless stated otherwise; FP64 only.
+ *  - State arrays U, dUdt are interior-only structure-of-arrays [5][nk][nj][ni] of the conservative
+ *    variables Q = (rho, rho u, rho v, rho w, E), index ((c*nk + k)*nj + j)*ni + i, xi fastest.
+ *  - Node coordinate arrays are [(nk+1)][(nj+1)][(ni+1)], xi fastest (hexahedral cell vertices).
+ *  - The library never allocates device memory: the caller passes one workspace block of
+ *    meg6_workspace_bytes() bytes (256-byte aligned) that must outlive the grid handle.
+ *  - All work is enqueued on the CUDA stream given at grid_create; nothing synchronises the stream
+ *    except meg6_limiter_stats, meg6_cfl_dt and meg6_get_array (which copy to the host).
+ *  - Every function returns a status code; meg6_last_error() gives a message for the last failure on
+ *    the calling thread.  Nothing throws.  There is no CPU fallback: without a CUDA device every
+ *    compute entry point returns MEG6_ECUDA.
+ */
+#ifndef MEG6_H
+#define MEG6_H
+#include <stddef.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct meg6_grid meg6_grid; /* opaque; host memory owned by the library */
+
+typedef enum {
+  MEG6_OK = 0,
+  MEG6_EINVAL = 1, /* bad argument (null pointer, size < stencil, unsupported option) */
+  MEG6_ENOMEM = 2, /* workspace too small                                            */
+  MEG6_ECUDA = 3,  /* CUDA runtime error (message in meg6_last_error)                */
+  MEG6_ESTATE = 4  /* call order violated (e.g. rhs before metrics_compute)          */
+} meg6_status;
+
+typedef struct {
+  int ni, nj, nk;     /* interior cells per direction; each >= 10 (periodic wrap of the 10-deep metric halo) */
+  int periodic[3];    /* per direction; a periodic direction ignores bc[] of its two faces           */
+  double period[3][3];/* period[d] = (dx,dy,dz) added to ghost-cell coordinates across direction d (R14) */
+  int scheme;         /* 0 = MEG6 (E6 gradients, Eq. 17).  1 = MIG4 is not built: MEG6_EINVAL   */
+  int viscous;        /* 0: Euler; 1: + alpha-damping viscous flux (Eq. 29-35)            */
+  double gamma, r_gas, prandtl; /* T = p/(rho r_gas); kappa = mu gamma r_gas/((gamma-1) Pr)   */
+  double mu_ref, t_ref, s_suth; /* mu = mu_ref (T/t_ref)^1.5 (t_ref+s_suth)/(T+s_suth); s_suth<0: mu = mu_ref (R15) */
+  double mp_alpha;    /* alpha of the MP limiter (App. E; R7), 4 by default              */
+  int moving;         /* 0 static mesh; 1: nodes x(t) = x0 + sin(2 pi omega t) * dx_mode (form of Eq. 49) */
+  double omega;
+  int bc[6];          /* faces imin,imax,jmin,jmax,kmin,kmax of non-periodic directions:
+                         1 fixed inflow (ghost = 2 P_in - P_mirror), 2 outflow (ghost = last interior cell,
+                         p = p_out where the outward normal Mach number < 1)   (Table 1, R20) */
+  double p_out;
+} meg6_params;
+
+/* Bytes of device workspace the grid needs (0 on invalid params). */
+size_t meg6_workspace_bytes(const meg6_params* p);
+
+/* Creates a grid.  x,y,z: node coordinates (device); dx_mode,dy_mode,dz_mode: node displacement modes
+ * (device; NULL when moving == 0).  The node arrays are copied into the workspace (the caller may free
+ * them after the call has been enqueued and the stream synchronised).  cuda_stream is a cudaStream_t
+ * (NULL = default stream).  *out is written on success only. */
+meg6_status meg6_grid_create(const meg6_params* p, const double* x, const double* y, const double* z,
+                             const double* dx_mode, const double* dy_mode, const double* dz_mode,
+                             void* workspace, size_t workspace_bytes, void* cuda_stream, meg6_grid** out);
+void meg6_grid_destroy(meg6_grid* g);
+
+/* Metric/Jacobian kernels (Sec. 4 and 7): cell centres = 8-vertex mean; ghost coordinates
+ * (R13, R14); Thomas-Lombard conservative metrics Eq. 10 with every derivative the consistent
+ * central derivative of Eq. 36-37 / 41; 1/J Eq. 13; time metrics Eq. 11; interface values by
+ * the central interpolation Eq. 38; (1/J)_t Eq. 14 from the same interface values.
+ * Static meshes: t ignored, idempotent.  Moving meshes: geometry at time t. */
+meg6_status meg6_metrics_compute(meg6_grid* g, double t);
+
+/* Inflow data of one bc==1 face: P_in[5][n2][n1] = (rho,u,v,w,p) per face cell, (n1,n2) = the two
+ * transverse extents in storage order (i before j before k).  Copied into the workspace. */
+meg6_status meg6_set_inflow(meg6_grid* g, int face, const double* P_in);
+/* Sponge source -sigma (Q - Q_ref) (R16): sigma[nk][nj][ni], U_ref[5][nk][nj][ni]; the POINTERS are
+ * kept (caller keeps the arrays alive); NULL, NULL switches the sponge off. */
+meg6_status meg6_set_sponge(meg6_grid* g, const double* sigma, const double* U_ref);
+
+/* dUdt = dQ/dt = J (Res - (1/J)_t Q) - sigma (Q - Q_ref) with Res of Eq. 8-9: E6 gradients
+ * (Eq. 17), characteristic gradient-based reconstruction (Eq. 19-23), improved MP limiter (App. E),
+ * contravariant HLLC (Eq. 26-27), alpha-damping viscous flux (Eq. 29-35), at the geometry of the last
+ * metrics_compute.  U and dUdt must not overlap. */
+meg6_status meg6_rhs(meg6_grid* g, const double* U, double* dUdt);
+
+/* One SSP-RK3 step (Eq. B.1) in place on U, from time t to t+dt.  Moving meshes recompute the
+ * geometry at the stage times t, t+dt, t+dt/2 (R17) and leave it at t+dt/2. */
+meg6_status meg6_rk3_step(meg6_grid* g, double* U, double t, double dt);
+
+/* Eq. B.2 / B.3 time step for the state U at the geometry of the last metrics_compute.
+ * Synchronises the stream.  *dt is a HOST pointer. */
+meg6_status meg6_cfl_dt(meg6_grid* g, const double* U, double cfl, double* dt);
+
+/* Counters of interface-components tested / limited by the MP limiter (test E.1 failed) since grid
+ * creation, accumulated only while enabled (default off; costs atomics).  HOST pointers; synchronises. */
+meg6_status meg6_limiter_stats_enable(meg6_grid* g, int on);
+meg6_status meg6_limiter_stats(meg6_grid* g, unsigned long long* n_limited, unsigned long long* n_tested);
+
+/* Inspection for tests: copies an internal array to HOST memory `out` (interior cells, [nk][nj][ni], or
+ * for interface arrays n_d+1 entries along d).  kind 0: cell array `which` = 0..8 hatted metrics
+ * (xi_x..zeta_z), 9 = 1/J, 10..12 = hatted time metrics, 13 = (1/J)_t, 14..16 = cell-centre x,y,z;
+ * kind 1: interface array, which = 16*d + q, q = 0..8 hatted metrics, 9 = 1/J, 10 = own time metric;
+ * kind 2: primitive field which = 0..5 (rho,u,v,w,p,T) after the last rhs. */
+meg6_status meg6_get_array(meg6_grid* g, int kind, int which, double* out);
+
+const char* meg6_last_error(void);
+/* Library/ABI version: 1000*major + minor. */
+int meg6_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif
