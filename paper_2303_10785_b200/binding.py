@@ -1,0 +1,192 @@
+"""ctypes binding of csrc/libmeg6.so -- same names as include/meg6.h, argument marshalling only.
+
+PyTorch is used for device memory and streams.  Nothing here computes: every method forwards to the C ABI.
+"""
+import ctypes as C
+import os
+
+from . import build as _build
+
+EXPORTS = ["meg6_workspace_bytes", "meg6_grid_create", "meg6_grid_destroy", "meg6_metrics_compute",
+           "meg6_set_inflow", "meg6_set_sponge", "meg6_rhs", "meg6_rk3_step", "meg6_cfl_dt",
+           "meg6_limiter_stats_enable", "meg6_limiter_stats", "meg6_get_array", "meg6_last_error",
+           "meg6_version"]
+
+
+class Meg6Error(RuntimeError):
+    pass
+
+
+class Params(C.Structure):
+    _fields_ = [("ni", C.c_int), ("nj", C.c_int), ("nk", C.c_int),
+                ("periodic", C.c_int * 3), ("period", (C.c_double * 3) * 3),
+                ("scheme", C.c_int), ("viscous", C.c_int),
+                ("gamma", C.c_double), ("r_gas", C.c_double), ("prandtl", C.c_double),
+                ("mu_ref", C.c_double), ("t_ref", C.c_double), ("s_suth", C.c_double),
+                ("mp_alpha", C.c_double), ("moving", C.c_int), ("omega", C.c_double),
+                ("bc", C.c_int * 6), ("p_out", C.c_double)]
+
+
+def make_params(cfg):
+    p = Params()
+    p.ni, p.nj, p.nk = cfg["ni"], cfg["nj"], cfg["nk"]
+    for d in range(3):
+        p.periodic[d] = int(cfg["periodic"][d])
+        for c in range(3):
+            p.period[d][c] = float(cfg["period"][d][c])
+    p.scheme = int(cfg.get("scheme", 0))
+    p.viscous = int(cfg.get("viscous", 0))
+    p.gamma = cfg.get("gamma", 1.4)
+    p.r_gas = cfg.get("r_gas", 1.0)
+    p.prandtl = cfg.get("prandtl", 0.71)
+    p.mu_ref = cfg.get("mu_ref", 0.0)
+    p.t_ref = cfg.get("t_ref", 1.0)
+    p.s_suth = cfg.get("s_suth", -1.0)
+    p.mp_alpha = cfg.get("mp_alpha", 4.0)
+    p.moving = int(cfg.get("moving", 0))
+    p.omega = cfg.get("omega", 0.0)
+    for f in range(6):
+        p.bc[f] = int(cfg.get("bc", [0] * 6)[f])
+    p.p_out = cfg.get("p_out", 0.0)
+    return p
+
+
+_lib = None
+_vp = C.c_void_p
+
+
+def lib_path():
+    return _build.SO
+
+
+def lib():
+    """Loads (building first if the sources are newer) the CUDA library.  Raises if it cannot."""
+    global _lib
+    if _lib is None:
+        so = _build.build()
+        L = C.CDLL(so)
+        L.meg6_workspace_bytes.restype = C.c_size_t
+        L.meg6_workspace_bytes.argtypes = [C.POINTER(Params)]
+        L.meg6_grid_create.restype = C.c_int
+        L.meg6_grid_create.argtypes = [C.POINTER(Params)] + [_vp] * 6 + [_vp, C.c_size_t, _vp, C.POINTER(_vp)]
+        L.meg6_grid_destroy.argtypes = [_vp]
+        L.meg6_metrics_compute.restype = C.c_int
+        L.meg6_metrics_compute.argtypes = [_vp, C.c_double]
+        L.meg6_set_inflow.restype = C.c_int
+        L.meg6_set_inflow.argtypes = [_vp, C.c_int, _vp]
+        L.meg6_set_sponge.restype = C.c_int
+        L.meg6_set_sponge.argtypes = [_vp, _vp, _vp]
+        L.meg6_rhs.restype = C.c_int
+        L.meg6_rhs.argtypes = [_vp, _vp, _vp]
+        L.meg6_rk3_step.restype = C.c_int
+        L.meg6_rk3_step.argtypes = [_vp, _vp, C.c_double, C.c_double]
+        L.meg6_cfl_dt.restype = C.c_int
+        L.meg6_cfl_dt.argtypes = [_vp, _vp, C.c_double, C.POINTER(C.c_double)]
+        L.meg6_limiter_stats_enable.restype = C.c_int
+        L.meg6_limiter_stats_enable.argtypes = [_vp, C.c_int]
+        L.meg6_limiter_stats.restype = C.c_int
+        L.meg6_limiter_stats.argtypes = [_vp, C.POINTER(C.c_ulonglong), C.POINTER(C.c_ulonglong)]
+        L.meg6_get_array.restype = C.c_int
+        L.meg6_get_array.argtypes = [_vp, C.c_int, C.c_int, _vp]
+        L.meg6_last_error.restype = C.c_char_p
+        L.meg6_version.restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def _check(status, what):
+    if status != 0:
+        raise Meg6Error("%s failed (status %d): %s" % (what, status, lib().meg6_last_error().decode()))
+
+
+class Grid:
+    """Handle around meg6_grid.  All tensors are torch CUDA float64; U is (5, nk, nj, ni) contiguous."""
+
+    def __init__(self, wl, device="cuda:0", stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise Meg6Error("no CUDA device: the MEG6 path has no CPU fallback")
+        L = lib()
+        self.torch = torch
+        self.device = torch.device(device)
+        self.cfg = wl["params"]
+        self.p = make_params(self.cfg)
+        self.shape = (self.cfg["nk"], self.cfg["nj"], self.cfg["ni"])
+        nbytes = L.meg6_workspace_bytes(C.byref(self.p))
+        if nbytes == 0:
+            raise Meg6Error("meg6_workspace_bytes: " + L.meg6_last_error().decode())
+        self.workspace_bytes = nbytes
+        with torch.cuda.device(self.device):
+            self.ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            base = (self.ws.data_ptr() + 255) // 256 * 256
+            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            dev = lambda a: torch.as_tensor(a, dtype=torch.float64).contiguous().to(self.device)
+            x, y, z = dev(wl["x"]), dev(wl["y"]), dev(wl["z"])
+            modes = [None, None, None]
+            if self.p.moving:
+                modes = [dev(wl["dx_mode"]), dev(wl["dy_mode"]), dev(wl["dz_mode"])]
+            h = _vp()
+            _check(L.meg6_grid_create(C.byref(self.p), x.data_ptr(), y.data_ptr(), z.data_ptr(),
+                                      *(m.data_ptr() if m is not None else None for m in modes),
+                                      base, nbytes, self.stream.cuda_stream, C.byref(h)), "meg6_grid_create")
+            self.h = h
+            for face, pin in wl.get("inflow", {}).items():
+                t = dev(pin)
+                _check(L.meg6_set_inflow(self.h, int(face), t.data_ptr()), "meg6_set_inflow")
+            self.sigma = self.uref = None
+            if wl.get("sigma") is not None:
+                self.sigma, self.uref = dev(wl["sigma"]), dev(wl["U_ref"])
+                _check(L.meg6_set_sponge(self.h, self.sigma.data_ptr(), self.uref.data_ptr()), "meg6_set_sponge")
+            self.stream.synchronize()   # node / inflow staging copies done before the temporaries die
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.torch.cuda.synchronize(self.device)
+            lib().meg6_grid_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _chk_state(self, U):
+        assert U.is_cuda and U.dtype == self.torch.float64 and U.is_contiguous() and tuple(U.shape) == (5,) + self.shape
+
+    def metrics_compute(self, t=0.0):
+        _check(lib().meg6_metrics_compute(self.h, float(t)), "meg6_metrics_compute")
+
+    def rhs(self, U, out=None):
+        self._chk_state(U)
+        if out is None:
+            out = self.torch.empty_like(U)
+        _check(lib().meg6_rhs(self.h, U.data_ptr(), out.data_ptr()), "meg6_rhs")
+        return out
+
+    def rk3_step(self, U, t, dt):
+        self._chk_state(U)
+        _check(lib().meg6_rk3_step(self.h, U.data_ptr(), float(t), float(dt)), "meg6_rk3_step")
+
+    def cfl_dt(self, U, cfl):
+        self._chk_state(U)
+        dt = C.c_double()
+        _check(lib().meg6_cfl_dt(self.h, U.data_ptr(), float(cfl), C.byref(dt)), "meg6_cfl_dt")
+        return dt.value
+
+    def limiter_stats_enable(self, on=True):
+        _check(lib().meg6_limiter_stats_enable(self.h, int(on)), "meg6_limiter_stats_enable")
+
+    def limiter_stats(self):
+        a, b = C.c_ulonglong(), C.c_ulonglong()
+        _check(lib().meg6_limiter_stats(self.h, C.byref(a), C.byref(b)), "meg6_limiter_stats")
+        return a.value, b.value
+
+    def get_array(self, kind, which):
+        import numpy as np
+        shp = list(self.shape)
+        if kind == 1:
+            shp[2 - which // 16] += 1
+        out = np.empty(shp, dtype=np.float64)
+        _check(lib().meg6_get_array(self.h, kind, which, out.ctypes.data), "meg6_get_array")
+        return out

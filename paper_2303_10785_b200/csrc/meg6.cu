@@ -1,0 +1,343 @@
+// meg6.cu -- host side of the C ABI declared in include/meg6.h: workspace carving, kernel launches.
+// Single translation unit of libmeg6.so (sm_100a).  No CPU fallback; shares nothing with oracle/.
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+#include <new>
+
+#include "meg6_common.cuh"
+#include "meg6_flow.cuh"
+#include "meg6_flux.cuh"
+
+using namespace meg6;
+
+static thread_local char g_err[512] = "";
+
+static meg6_status fail(meg6_status s, const char* fmt, const char* a = "") {
+  snprintf(g_err, sizeof(g_err), fmt, a);
+  return s;
+}
+#define CUDA_OK(call)                                                              \
+  do {                                                                             \
+    cudaError_t e_ = (call);                                                       \
+    if (e_ != cudaSuccess) return fail(MEG6_ECUDA, #call ": %s", cudaGetErrorString(e_)); \
+  } while (0)
+
+static bool params_ok(const meg6_params* p) {
+  if (!p) return false;
+  if (p->ni < 10 || p->nj < 10 || p->nk < 10) return false;
+  if (p->scheme != 0) return false;
+  if (!(p->gamma > 1.0) || !(p->r_gas > 0.0)) return false;
+  for (int d = 0; d < 3; ++d)
+    if (!p->periodic[d])
+      for (int s = 0; s < 2; ++s)
+        if (p->bc[2 * d + s] != 1 && p->bc[2 * d + s] != 2) return false;
+  if (p->viscous && !(p->prandtl > 0.0)) return false;
+  return true;
+}
+
+static Consts make_consts(const meg6_params* p) {
+  Consts c;
+  memset(&c, 0, sizeof(c));
+  c.n[0] = p->ni; c.n[1] = p->nj; c.n[2] = p->nk;
+  for (int d = 0; d < 3; ++d) {
+    c.periodic[d] = p->periodic[d] ? 1 : 0;
+    for (int q = 0; q < 3; ++q) c.period[d][q] = p->period[d][q];
+  }
+  c.viscous = p->viscous ? 1 : 0;
+  c.moving = p->moving ? 1 : 0;
+  for (int f = 0; f < 6; ++f) c.bc[f] = p->bc[f];
+  c.gamma = p->gamma; c.r_gas = p->r_gas; c.prandtl = p->prandtl;
+  c.mu_ref = p->mu_ref; c.t_ref = p->t_ref; c.s_suth = p->s_suth;
+  c.mp_alpha = p->mp_alpha; c.p_out = p->p_out;
+  c.kappa_fac = p->viscous ? p->gamma * p->r_gas / ((p->gamma - 1.0) * p->prandtl) : 0.0;
+  c.LX = make_lay(p->ni, p->nj, p->nk, GX, GX, GX);
+  c.LP = make_lay(p->ni, p->nj, p->nk, GPI, GPJ, GPK);
+  c.LG = make_lay(p->ni, p->nj, p->nk, GGI, GGJ, GGK);
+  c.LC = make_lay(p->ni, p->nj, p->nk, 0, 0, 0);
+  c.LF[0] = make_lay(p->ni + 1, p->nj, p->nk, 0, 0, 0);
+  c.LF[1] = make_lay(p->ni, p->nj + 1, p->nk, 0, 0, 0);
+  c.LF[2] = make_lay(p->ni, p->nj, p->nk + 1, 0, 0, 0);
+  return c;
+}
+
+// Carves the workspace; with g == nullptr only sizes it.
+static size_t carve(const meg6_params* p, const Consts& c, meg6_grid* g, char* base) {
+  size_t off = 0;
+  auto take = [&](long long n_doubles) -> double* {
+    double* ptr = base ? (double*)(base + off) : nullptr;
+    off += ((size_t)n_doubles * sizeof(double) + 255) / 256 * 256;
+    return ptr;
+  };
+  const long long nn = (long long)(p->ni + 1) * (p->nj + 1) * (p->nk + 1);
+  meg6_grid tmp;
+  meg6_grid* G = g ? g : &tmp;
+  for (int q = 0; q < 3; ++q) G->nodes[q] = take(nn);
+  for (int q = 0; q < 3; ++q) G->modes[q] = p->moving ? take(nn) : nullptr;
+  for (int q = 0; q < 3; ++q) G->xc[q] = take(c.LX.n);
+  for (int q = 0; q < 3; ++q) G->xt[q] = p->moving ? take(c.LX.n) : nullptr;
+  for (int q = 0; q < 9; ++q) G->cd[q] = take(c.LX.n);
+  for (int q = 0; q < 9; ++q) G->met[q] = take(c.LX.n);
+  G->rj = take(c.LX.n);
+  for (int q = 0; q < 3; ++q) G->mt[q] = p->moving ? take(c.LX.n) : nullptr;
+  for (int d = 0; d < 3; ++d) {
+    for (int q = 0; q < 10; ++q) {
+      const bool own = (q >= 3 * d && q < 3 * d + 3);
+      G->fmet[d][q] = (own || p->viscous) ? take(c.LF[d].n) : nullptr;
+    }
+    G->fmt[d] = p->moving ? take(c.LF[d].n) : nullptr;
+  }
+  G->rjt = p->moving ? take(c.LC.n) : nullptr;
+  for (int f = 0; f < 6; ++f) G->P[f] = take(c.LP.n);
+  for (int e = 0; e < 3; ++e)
+    for (int f = 0; f < 4; ++f) G->G[e][f] = p->viscous ? take(c.LG.n) : nullptr;
+  G->res = take(5 * c.LC.n);
+  G->U0 = take(5 * c.LC.n);
+  for (int f = 0; f < 6; ++f) {
+    const int d = f / 2;
+    G->inflow[f] = nullptr;
+    if (!p->periodic[d] && p->bc[f] == 1) {
+      int a = (d + 1) % 3, b = (d + 2) % 3;
+      G->inflow[f] = take(5LL * c.n[a] * c.n[b]);
+    }
+  }
+  G->stats = (unsigned long long*)take(2);
+  G->red = take(2 * CFL_BLOCKS);
+  return off;
+}
+
+static inline unsigned nblk(long long n, int t) { return (unsigned)((n + t - 1) / t); }
+namespace meg6 { cudaError_t launch_geometry(meg6_grid* g, double t); }
+
+extern "C" {
+
+int meg6_version(void) { return 1000; }
+const char* meg6_last_error(void) { return g_err; }
+
+size_t meg6_workspace_bytes(const meg6_params* p) {
+  if (!params_ok(p)) { fail(MEG6_EINVAL, "invalid params%s"); return 0; }
+  Consts c = make_consts(p);
+  return carve(p, c, nullptr, nullptr);
+}
+
+meg6_status meg6_grid_create(const meg6_params* p, const double* x, const double* y, const double* z,
+                             const double* dxm, const double* dym, const double* dzm, void* workspace,
+                             size_t workspace_bytes, void* cuda_stream, meg6_grid** out) {
+  if (!params_ok(p)) return fail(MEG6_EINVAL, "invalid params%s");
+  if (!x || !y || !z || !workspace || !out) return fail(MEG6_EINVAL, "null pointer%s");
+  if (p->moving && (!dxm || !dym || !dzm)) return fail(MEG6_EINVAL, "moving mesh needs displacement modes%s");
+  if (((uintptr_t)workspace & 255) != 0) return fail(MEG6_EINVAL, "workspace must be 256-byte aligned%s");
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return fail(MEG6_ECUDA, "no CUDA device%s");
+  meg6_grid* g = new (std::nothrow) meg6_grid();
+  if (!g) return fail(MEG6_ENOMEM, "host allocation failed%s");
+  memset((void*)g, 0, sizeof(*g));
+  g->p = *p;
+  g->c = make_consts(p);
+  g->stream = (cudaStream_t)cuda_stream;
+  g->ws = (char*)workspace; g->ws_bytes = workspace_bytes;
+  const size_t need = carve(p, g->c, g, g->ws);
+  if (need > workspace_bytes) { delete g; return fail(MEG6_ENOMEM, "workspace too small%s"); }
+  const size_t nn = (size_t)(p->ni + 1) * (p->nj + 1) * (p->nk + 1) * sizeof(double);
+  const double* src[3] = {x, y, z};
+  const double* msrc[3] = {dxm, dym, dzm};
+  cudaError_t e = cudaMemsetAsync(g->ws, 0, need, g->stream);
+  for (int q = 0; q < 3 && e == cudaSuccess; ++q) {
+    e = cudaMemcpyAsync(g->nodes[q], src[q], nn, cudaMemcpyDeviceToDevice, g->stream);
+    if (e == cudaSuccess && p->moving) e = cudaMemcpyAsync(g->modes[q], msrc[q], nn, cudaMemcpyDeviceToDevice, g->stream);
+  }
+  if (e == cudaSuccess) {
+    // opt in to the dynamic shared memory the flux kernels need
+    e = cudaFuncSetAttribute(k_flux<0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(FluxCfg<0, false>::SMEM_DOUBLES * 8));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_flux<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(FluxCfg<1, false>::SMEM_DOUBLES * 8));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_flux<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(FluxCfg<2, false>::SMEM_DOUBLES * 8));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_flux<0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(FluxCfg<0, true>::SMEM_DOUBLES * 8));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_flux<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(FluxCfg<1, true>::SMEM_DOUBLES * 8));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_flux<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(FluxCfg<2, true>::SMEM_DOUBLES * 8));
+  }
+  if (e != cudaSuccess) { delete g; return fail(MEG6_ECUDA, "grid_create: %s", cudaGetErrorString(e)); }
+  *out = g;
+  return MEG6_OK;
+}
+
+void meg6_grid_destroy(meg6_grid* g) { delete g; }
+
+meg6_status meg6_metrics_compute(meg6_grid* g, double t) {
+  if (!g) return fail(MEG6_EINVAL, "null grid%s");
+  if (g->have_metrics && !g->p.moving) return MEG6_OK;   // static: idempotent
+  cudaError_t e = meg6::launch_geometry(g, t);            // meg6_geom.cu (compiled with -fmad=false)
+  if (e != cudaSuccess) return fail(MEG6_ECUDA, "metrics_compute: %s", cudaGetErrorString(e));
+  g->have_metrics = true;
+  return MEG6_OK;
+}
+
+meg6_status meg6_set_inflow(meg6_grid* g, int face, const double* P_in) {
+  if (!g || !P_in || face < 0 || face > 5) return fail(MEG6_EINVAL, "set_inflow: bad argument%s");
+  if (!g->inflow[face]) return fail(MEG6_EINVAL, "set_inflow: face is not a fixed-inflow face%s");
+  const int d = face / 2, a = (d + 1) % 3, b = (d + 2) % 3;
+  CUDA_OK(cudaMemcpyAsync(g->inflow[face], P_in, sizeof(double) * 5 * (size_t)g->c.n[a] * g->c.n[b],
+                          cudaMemcpyDeviceToDevice, g->stream));
+  return MEG6_OK;
+}
+
+meg6_status meg6_set_sponge(meg6_grid* g, const double* sigma, const double* U_ref) {
+  if (!g) return fail(MEG6_EINVAL, "null grid%s");
+  if ((sigma == nullptr) != (U_ref == nullptr)) return fail(MEG6_EINVAL, "set_sponge: both or neither%s");
+  g->sigma = sigma; g->uref = U_ref;
+  return MEG6_OK;
+}
+
+// residual of Eq. 8-9 into g->res for the state U (all kernels of one RK stage but the update)
+static meg6_status residual(meg6_grid* g, const double* U) {
+  const Consts& c = g->c;
+  P6 P;
+  for (int f = 0; f < 6; ++f) P.p[f] = g->P[f];
+  const int T = 256;
+  k_prim<<<nblk(c.LC.n, T), T, 0, g->stream>>>(c, U, P);
+  for (int d = 0; d < 3; ++d) {
+    int a = (d + 1) % 3, b = (d + 2) % 3;
+    if (a > b) { int t = a; a = b; b = t; }
+    const long long ea = c.n[a] + ((a < d) ? 12 : 0), eb = c.n[b] + ((b < d) ? 12 : 0);
+    GhostIn gin;
+    gin.inflow[0] = g->inflow[2 * d]; gin.inflow[1] = g->inflow[2 * d + 1];
+    gin.mx = g->met[3 * d]; gin.my = g->met[3 * d + 1]; gin.mz = g->met[3 * d + 2];
+    k_ghost<<<nblk(ea * eb * 2, 128), 128, 0, g->stream>>>(c, d, P, gin);
+  }
+  if (g->p.viscous) {
+    P12 G;
+    for (int e = 0; e < 3; ++e)
+      for (int f = 0; f < 4; ++f) G.p[4 * e + f] = g->G[e][f];
+    const long long ng = (long long)(c.n[0] + 2) * (c.n[1] + 2) * (c.n[2] + 2);
+    k_grad<<<nblk(ng, T), T, 0, g->stream>>>(c, P, G);
+  }
+  for (int d = 0; d < 3; ++d) {
+    FluxIn in;
+    for (int f = 0; f < 6; ++f) in.P[f] = g->P[f];
+    for (int q = 0; q < 10; ++q) in.m[q] = g->fmet[d][q];
+    in.mt = g->p.moving ? g->fmt[d] : nullptr;
+    for (int e = 0; e < 3; ++e)
+      for (int f = 0; f < 4; ++f) in.G[4 * e + f] = g->G[e][f];
+    in.res = g->res;
+    in.stats = g->stats_on ? g->stats : nullptr;
+    in.first = (d == 0);
+    const bool V = g->p.viscous != 0;
+    if (d == 0) {
+      dim3 grid(nblk(c.n[0], FluxCfg<0, false>::TS), nblk(c.n[1], FluxCfg<0, false>::TT), c.n[2]);
+      if (V) k_flux<0, true><<<grid, FluxCfg<0, true>::NT, FluxCfg<0, true>::SMEM_DOUBLES * 8, g->stream>>>(c, in);
+      else k_flux<0, false><<<grid, FluxCfg<0, false>::NT, FluxCfg<0, false>::SMEM_DOUBLES * 8, g->stream>>>(c, in);
+    } else if (d == 1) {
+      dim3 grid(nblk(c.n[0], FluxCfg<1, false>::TT), nblk(c.n[1], FluxCfg<1, false>::TS), c.n[2]);
+      if (V) k_flux<1, true><<<grid, FluxCfg<1, true>::NT, FluxCfg<1, true>::SMEM_DOUBLES * 8, g->stream>>>(c, in);
+      else k_flux<1, false><<<grid, FluxCfg<1, false>::NT, FluxCfg<1, false>::SMEM_DOUBLES * 8, g->stream>>>(c, in);
+    } else {
+      dim3 grid(nblk(c.n[0], FluxCfg<2, false>::TT), c.n[1], nblk(c.n[2], FluxCfg<2, false>::TS));
+      if (V) k_flux<2, true><<<grid, FluxCfg<2, true>::NT, FluxCfg<2, true>::SMEM_DOUBLES * 8, g->stream>>>(c, in);
+      else k_flux<2, false><<<grid, FluxCfg<2, false>::NT, FluxCfg<2, false>::SMEM_DOUBLES * 8, g->stream>>>(c, in);
+    }
+  }
+  CUDA_OK(cudaGetLastError());
+  return MEG6_OK;
+}
+
+static void launch_update(meg6_grid* g, const double* U, double* out, int mode, double a, double b, double dt) {
+  UpdIn in;
+  in.res = g->res; in.rj = g->rj; in.rjt = g->p.moving ? g->rjt : nullptr;
+  in.sigma = g->sigma; in.uref = g->uref;
+  in.U = U; in.U0 = g->U0; in.out = out; in.a = a; in.b = b; in.dt = dt; in.mode = mode;
+  k_update<<<nblk(g->c.LC.n, 256), 256, 0, g->stream>>>(g->c, in);
+}
+
+meg6_status meg6_rhs(meg6_grid* g, const double* U, double* dUdt) {
+  if (!g || !U || !dUdt) return fail(MEG6_EINVAL, "rhs: null pointer%s");
+  if (!g->have_metrics) return fail(MEG6_ESTATE, "rhs called before metrics_compute%s");
+  meg6_status s = residual(g, U);
+  if (s != MEG6_OK) return s;
+  launch_update(g, U, dUdt, 0, 0.0, 0.0, 0.0);
+  CUDA_OK(cudaGetLastError());
+  return MEG6_OK;
+}
+
+meg6_status meg6_rk3_step(meg6_grid* g, double* U, double t, double dt) {
+  if (!g || !U) return fail(MEG6_EINVAL, "rk3_step: null pointer%s");
+  if (!g->have_metrics && !g->p.moving) return fail(MEG6_ESTATE, "rk3_step called before metrics_compute%s");
+  CUDA_OK(cudaMemcpyAsync(g->U0, U, sizeof(double) * 5 * (size_t)g->c.LC.n, cudaMemcpyDeviceToDevice, g->stream));
+  const double ts[3] = {t, t + dt, t + 0.5 * dt};
+  const double aa[3] = {0.0, 3.0 / 4.0, 1.0 / 3.0}, bb[3] = {1.0, 1.0 / 4.0, 2.0 / 3.0};
+  for (int s = 0; s < 3; ++s) {
+    meg6_status st;
+    if (g->p.moving && (st = meg6_metrics_compute(g, ts[s])) != MEG6_OK) return st;
+    if ((st = residual(g, U)) != MEG6_OK) return st;
+    launch_update(g, U, U, 1, aa[s], bb[s], dt);
+  }
+  CUDA_OK(cudaGetLastError());
+  return MEG6_OK;
+}
+
+meg6_status meg6_cfl_dt(meg6_grid* g, const double* U, double cfl, double* dt) {
+  if (!g || !U || !dt) return fail(MEG6_EINVAL, "cfl_dt: null pointer%s");
+  if (!g->have_metrics) return fail(MEG6_ESTATE, "cfl_dt called before metrics_compute%s");
+  CflIn in;
+  for (int q = 0; q < 9; ++q) in.met[q] = g->met[q];
+  for (int q = 0; q < 3; ++q) in.mt[q] = g->mt[q];
+  in.rj = g->rj;
+  const int nb = (int)((g->c.LC.n + 255) / 256 < CFL_BLOCKS ? (g->c.LC.n + 255) / 256 : CFL_BLOCKS);
+  k_cfl<<<nb, 256, 0, g->stream>>>(g->c, U, in, g->red);
+  static thread_local double host[2 * CFL_BLOCKS];
+  CUDA_OK(cudaMemcpyAsync(host, g->red, sizeof(double) * 2 * nb, cudaMemcpyDeviceToHost, g->stream));
+  CUDA_OK(cudaStreamSynchronize(g->stream));
+  double a = INFINITY, b = INFINITY;
+  for (int q = 0; q < nb; ++q) { a = fmin(a, host[2 * q]); b = fmin(b, host[2 * q + 1]); }
+  double r = a;
+  if (g->p.viscous) r = fmin(r, b / 4.0);   // R25: the alpha of Eq. B.3 read as alpha^D = 4
+  *dt = cfl * r;
+  return MEG6_OK;
+}
+
+meg6_status meg6_limiter_stats_enable(meg6_grid* g, int on) {
+  if (!g) return fail(MEG6_EINVAL, "null grid%s");
+  g->stats_on = on ? 1 : 0;
+  return MEG6_OK;
+}
+
+meg6_status meg6_limiter_stats(meg6_grid* g, unsigned long long* n_limited, unsigned long long* n_tested) {
+  if (!g || !n_limited || !n_tested) return fail(MEG6_EINVAL, "limiter_stats: null pointer%s");
+  unsigned long long h[2];
+  CUDA_OK(cudaMemcpyAsync(h, g->stats, sizeof(h), cudaMemcpyDeviceToHost, g->stream));
+  CUDA_OK(cudaStreamSynchronize(g->stream));
+  *n_limited = h[0]; *n_tested = h[1];
+  return MEG6_OK;
+}
+
+meg6_status meg6_get_array(meg6_grid* g, int kind, int which, double* out) {
+  if (!g || !out) return fail(MEG6_EINVAL, "get_array: null pointer%s");
+  const Consts& c = g->c;
+  const double* src = nullptr;
+  Lay L = c.LX;
+  int ext[3] = {c.n[0], c.n[1], c.n[2]};
+  if (kind == 0) {
+    if (which >= 0 && which < 9) src = g->met[which];
+    else if (which == 9) src = g->rj;
+    else if (which >= 10 && which < 13) src = g->mt[which - 10];
+    else if (which == 13) { src = g->rjt; L = c.LC; }
+    else if (which >= 14 && which < 17) src = g->xc[which - 14];
+  } else if (kind == 1) {
+    const int d = which / 16, q = which % 16;
+    if (d >= 0 && d < 3 && q >= 0 && q <= 10) { src = (q < 10) ? g->fmet[d][q] : g->fmt[d]; L = c.LF[d]; ext[d] += 1; }
+  } else if (kind == 2) {
+    if (which >= 0 && which < 6) { src = g->P[which]; L = c.LP; }
+  }
+  if (!src) return fail(MEG6_EINVAL, "get_array: no such array%s");
+  // strided device-to-host copy of the interior box
+  cudaMemcpy3DParms p3;
+  memset(&p3, 0, sizeof(p3));
+  p3.srcPtr = make_cudaPitchedPtr((void*)src, (size_t)L.pi * sizeof(double), L.pi, L.pj);
+  p3.srcPos = make_cudaPos((size_t)L.gi * sizeof(double), L.gj, L.gk);
+  p3.dstPtr = make_cudaPitchedPtr(out, (size_t)ext[0] * sizeof(double), ext[0], ext[1]);
+  p3.extent = make_cudaExtent((size_t)ext[0] * sizeof(double), ext[1], ext[2]);
+  p3.kind = cudaMemcpyDeviceToHost;
+  CUDA_OK(cudaMemcpy3DAsync(&p3, g->stream));
+  CUDA_OK(cudaStreamSynchronize(g->stream));
+  return MEG6_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,89 @@
+// meg6_common.cuh -- layouts, constants and the grid object of the B200 MEG6 library.
+// Part of the single translation unit meg6.cu.  Shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "../../include/meg6.h"
+
+namespace meg6 {
+
+// Ghost depths.  GX: cell-centre coordinates and metrics (two nested consistent derivatives of reach 5,
+// Eq. 10 + Eq. 41).  Primitives need 6 cells beyond an interface stencil (P' on i-2..i+3 from P on i-5..i+6);
+// the i-axis ghost is widened to 8 so that interior rows start on a 64-byte boundary.
+constexpr int GX = 10;
+constexpr int GPI = 8, GPJ = 6, GPK = 6;
+constexpr int GGI = 4, GGJ = 1, GGK = 1;   // stored gradients: one ghost layer (cells i and i+1 of boundary faces)
+
+// Consistent central derivative, Eq. 41: delta f_i = sum_m CD[m-1] (f_{i+m} - f_{i-m})
+__device__ constexpr double CD1 = 2282.0 / 2880.0, CD2 = -546.0 / 2880.0, CD3 = 89.0 / 2880.0,
+                            CD4 = -3.0 / 2880.0, CD5 = -1.0 / 2880.0;
+// Central interface value, Eq. 36/38 with Eq. 17 and 19 substituted:
+// H_{i+1/2} = sum_{q=1..5} CH[q-1] (f_{i+1-q} + f_{i+q})
+__device__ constexpr double CH1 = 1821.0 / 2880.0, CH2 = -461.0 / 2880.0, CH3 = 85.0 / 2880.0,
+                            CH4 = -4.0 / 2880.0, CH5 = -1.0 / 2880.0;
+// E6 gradient, Eq. 17
+__device__ constexpr double CE1 = 3.0 / 4.0, CE2 = -3.0 / 20.0, CE3 = 1.0 / 60.0;
+// Eq. 19 with Eq. 17 substituted: D2 f_i = CS0 f_i + sum_{m=1..4} CS[m] (f_{i+m} + f_{i-m})
+__device__ constexpr double CS0 = -13.0 / 4.0, CS1 = 77.0 / 40.0, CS2 = -11.0 / 30.0, CS3 = 3.0 / 40.0,
+                            CS4 = -1.0 / 120.0;
+
+struct Lay {   // padded 3-D layout, i fastest
+  int gi, gj, gk;
+  int pi, pj, pk;
+  long long sj, sk, n;
+  __host__ __device__ __forceinline__ long long at(int i, int j, int k) const {
+    return (long long)(k + gk) * sk + (long long)(j + gj) * sj + (long long)(i + gi);
+  }
+  __host__ __device__ __forceinline__ long long stride(int d) const { return d == 0 ? 1 : d == 1 ? sj : sk; }
+};
+
+inline Lay make_lay(int ni, int nj, int nk, int gi, int gj, int gk, int align_i = 1) {
+  Lay L;
+  L.gi = gi; L.gj = gj; L.gk = gk;
+  L.pi = ni + 2 * gi;
+  if (align_i > 1) L.pi = (L.pi + align_i - 1) / align_i * align_i;
+  L.pj = nj + 2 * gj; L.pk = nk + 2 * gk;
+  L.sj = L.pi; L.sk = (long long)L.pi * L.pj;
+  L.n = L.sk * L.pk;
+  return L;
+}
+
+struct Consts {   // per-grid constants passed by value to kernels
+  int n[3];
+  int periodic[3];
+  double period[3][3];
+  int viscous, moving;
+  int bc[6];
+  double gamma, r_gas, prandtl, mu_ref, t_ref, s_suth, mp_alpha, p_out;
+  double kappa_fac;   // gamma r_gas / ((gamma-1) Pr)
+  Lay LX, LP, LG, LC; // coordinates/metrics, primitives, gradients, interior cells
+  Lay LF[3];          // interface families
+};
+
+}  // namespace meg6
+
+struct meg6_grid {
+  meg6_params p;
+  meg6::Consts c;
+  cudaStream_t stream;
+  char* ws; size_t ws_bytes;
+  // geometry inputs (copied nodes)
+  double* nodes[3]; double* modes[3];
+  // geometry
+  double* xc[3]; double* xt[3];
+  double* cd[9];      // delta_d(x_c): cd[3*c + d]
+  double* met[9]; double* rj; double* mt[3];
+  double* fmet[3][10]; double* fmt[3];
+  double* rjt;
+  // flow
+  double* P[6];
+  double* G[3][4];    // D1 gradients of (u,v,w,T) along xi,eta,zeta (viscous)
+  double* res;        // [5][N]
+  double* U0;         // [5][N]
+  double* inflow[6];
+  const double* sigma; const double* uref;
+  unsigned long long* stats;   // [2] device counters: limited, tested
+  double* red;                 // reduction scratch
+  int stats_on;
+  bool have_metrics;
+};

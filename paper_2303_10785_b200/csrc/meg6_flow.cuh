@@ -1,0 +1,201 @@
+// meg6_flow.cuh -- primitive conversion, ghost fill, stored gradients, residual assembly + SSP-RK3 update,
+// CFL reduction.
+#pragma once
+#include "meg6_common.cuh"
+
+namespace meg6 {
+
+struct P5c { const double* p[5]; };
+struct P6 { double* p[6]; };
+struct P12 { double* p[12]; };
+
+// G(a): Q -> P = (rho,u,v,w,p) (Eq. 5, P:83 inverted) and T = p/(rho R), interior cells.
+__global__ void __launch_bounds__(256) k_prim(Consts c, const double* __restrict__ U, P6 P) {
+  const long long N = c.LC.n;
+  const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (tid >= N) return;
+  const int i = (int)(tid % c.n[0]), j = (int)((tid / c.n[0]) % c.n[1]), k = (int)(tid / ((long long)c.n[0] * c.n[1]));
+  const double r = U[tid], ir = 1.0 / r;
+  const double u = U[N + tid] * ir, v = U[2 * N + tid] * ir, w = U[3 * N + tid] * ir;
+  const double p = (c.gamma - 1.0) * (U[4 * N + tid] - 0.5 * r * (u * u + v * v + w * w));
+  const long long at = c.LP.at(i, j, k);
+  P.p[0][at] = r; P.p[1][at] = u; P.p[2][at] = v; P.p[3][at] = w; P.p[4][at] = p;
+  P.p[5][at] = p / (r * c.r_gas);
+}
+
+struct GhostIn { const double* inflow[2]; const double* mx; const double* my; const double* mz; };
+
+// B: ghost layers of direction d (6 deep), after the lower directions have been filled: periodic wrap, fixed
+// inflow ghost = 2 P_in - P_mirror, outflow ghost = last interior cell with p = p_out where the outward normal
+// Mach number is below one (Table 1, R20).  One thread per transverse position and side.
+__global__ void k_ghost(Consts c, int d, P6 P, GhostIn in) {
+  int a = (d + 1) % 3, b = (d + 2) % 3;
+  if (a > b) { int t = a; a = b; b = t; }
+  const int g[3] = {GPJ, GPJ, GPK};   // ghost depth filled per direction (6 everywhere)
+  // transverse ranges: directions below d are already extended
+  const int loa = (a < d) ? -g[a] : 0, ea = c.n[a] + ((a < d) ? 2 * g[a] : 0);
+  const int lob = (b < d) ? -g[b] : 0, eb = c.n[b] + ((b < d) ? 2 * g[b] : 0);
+  const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (tid >= (long long)ea * eb * 2) return;
+  const int side = (int)(tid / ((long long)ea * eb));
+  const long long r = tid % ((long long)ea * eb);
+  const int ta = loa + (int)(r % ea), tb = lob + (int)(r / ea);
+  int ix[3];
+  ix[a] = ta; ix[b] = tb;
+  const int n = c.n[d];
+  const long long s = c.LP.stride(d);
+  ix[d] = 0;
+  const long long base = c.LP.at(ix[0], ix[1], ix[2]);   // cell 0 of this line
+  const int NG = 6;
+  if (c.periodic[d]) {
+    for (int q = 1; q <= NG; ++q)
+#pragma unroll
+      for (int f = 0; f < 6; ++f) {
+        if (side == 0) P.p[f][base - q * s] = P.p[f][base + (long long)(n - q) * s];
+        else P.p[f][base + (long long)(n - 1 + q) * s] = P.p[f][base + (long long)(q - 1) * s];
+      }
+    return;
+  }
+  const int face = 2 * d + side, bc = c.bc[face];
+  const int last = side ? n - 1 : 0, sg = side ? 1 : -1;
+  const int ca = min(max(ta, 0), c.n[a] - 1), cb = min(max(tb, 0), c.n[b] - 1);
+  if (bc == 1) {
+    const long long nf = (long long)c.n[a] * c.n[b];
+    const double* pin = in.inflow[side] + (long long)cb * c.n[a] + ca;
+    double pi5[5];
+#pragma unroll
+    for (int f = 0; f < 5; ++f) pi5[f] = pin[f * nf];
+    for (int q = 1; q <= NG; ++q) {
+      double v[5];
+#pragma unroll
+      for (int f = 0; f < 5; ++f) {
+        v[f] = 2.0 * pi5[f] - P.p[f][base + (long long)(last - sg * (q - 1)) * s];
+        P.p[f][base + (long long)(last + sg * q) * s] = v[f];
+      }
+      P.p[5][base + (long long)(last + sg * q) * s] = v[4] / (v[0] * c.r_gas);
+    }
+  } else {
+    double pv[5];
+#pragma unroll
+    for (int f = 0; f < 5; ++f) pv[f] = P.p[f][base + (long long)last * s];
+    int im[3];
+    im[a] = ca; im[b] = cb; im[d] = last;
+    const long long am = c.LX.at(im[0], im[1], im[2]);
+    const double mx = in.mx[am], my = in.my[am], mz = in.mz[am];
+    const double gm = sqrt(mx * mx + my * my + mz * mz);
+    const double cs = sqrt(c.gamma * pv[4] / pv[0]);
+    const double mn = sg * (mx * pv[1] + my * pv[2] + mz * pv[3]) / (gm * cs);
+    if (mn < 1.0) pv[4] = c.p_out;
+    const double T = pv[4] / (pv[0] * c.r_gas);
+    for (int q = 1; q <= NG; ++q) {
+#pragma unroll
+      for (int f = 0; f < 5; ++f) P.p[f][base + (long long)(last + sg * q) * s] = pv[f];
+      P.p[5][base + (long long)(last + sg * q) * s] = T;
+    }
+  }
+}
+
+// E6 gradient, Eq. 17 (R1)
+__device__ __forceinline__ double d1_op(const double* __restrict__ f, long long s) {
+  double r = CE1 * (f[s] - f[-s]);
+  r = fma(CE2, f[2 * s] - f[-2 * s], r);
+  r = fma(CE3, f[3 * s] - f[-3 * s], r);
+  return r;
+}
+
+// G(b): stored gradients of (u,v,w,T) along xi, eta, zeta on cells [-1, n+1)^3 (viscous flux, Fig. 5 P:295;
+// R18: T is differentiated with the same E6 scheme).  G.p[4*e + f].
+__global__ void __launch_bounds__(256) k_grad(Consts c, P6 P, P12 G) {
+  const int ei = c.n[0] + 2, ej = c.n[1] + 2;
+  const long long total = (long long)ei * ej * (c.n[2] + 2);
+  const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (tid >= total) return;
+  const int i = (int)(tid % ei) - 1, j = (int)((tid / ei) % ej) - 1, k = (int)(tid / ((long long)ei * ej)) - 1;
+  const long long ap = c.LP.at(i, j, k), ag = c.LG.at(i, j, k);
+#pragma unroll
+  for (int e = 0; e < 3; ++e) {
+    const long long s = c.LP.stride(e);
+#pragma unroll
+    for (int f = 0; f < 4; ++f) {
+      const int pf = (f < 3) ? f + 1 : 5;
+      G.p[4 * e + f][ag] = d1_op(P.p[pf] + ap, s);
+    }
+  }
+}
+
+// S + T: dQ/dt = J (Res - (1/J)_t Q) - sigma (Q - Q_ref) (Eq. 9, 12, 14; R16) and one SSP-RK3 stage
+// (Eq. B.1):  U <- a U0 + b (U + dt dQ/dt).   mode 0: write dQ/dt to out (meg6_rhs);
+// mode 1: stage update in place on U (a = 0 for stage 1).
+struct UpdIn {
+  const double* res; const double* rj; const double* rjt; const double* sigma; const double* uref;
+  const double* U; const double* U0; double* out;
+  double a, b, dt; int mode;
+};
+
+__global__ void __launch_bounds__(256) k_update(Consts c, UpdIn in) {
+  const long long N = c.LC.n;
+  const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (tid >= N) return;
+  const int i = (int)(tid % c.n[0]), j = (int)((tid / c.n[0]) % c.n[1]), k = (int)(tid / ((long long)c.n[0] * c.n[1]));
+  const double J = 1.0 / in.rj[c.LX.at(i, j, k)];
+  const double rjt = in.rjt ? in.rjt[tid] : 0.0;
+  const double sg = in.sigma ? in.sigma[tid] : 0.0;
+#pragma unroll
+  for (int f = 0; f < 5; ++f) {
+    const double u = in.U[f * N + tid];
+    double L = J * (in.res[f * N + tid] - rjt * u);
+    if (in.sigma) L -= sg * (u - in.uref[f * N + tid]);
+    if (in.mode == 0) in.out[f * N + tid] = L;
+    else {
+      double v = u + in.dt * L;
+      if (in.a != 0.0) v = in.a * in.U0[f * N + tid] + in.b * v;
+      in.out[f * N + tid] = v;
+    }
+  }
+}
+
+// Eq. B.2 / B.3: per-block minima of 1/(|U|+c|grad xi|) and 1/(mu |grad xi|^2) over cells and
+// directions (un-hatted metrics = hatted * J).  red[2*b], red[2*b+1]; the host finishes the reduction.
+struct CflIn { const double* met[9]; const double* mt[3]; const double* rj; };
+
+__device__ __forceinline__ double sutherland(const Consts& c, double T) {
+  if (c.s_suth < 0.0) return c.mu_ref;
+  const double r = T / c.t_ref;
+  return c.mu_ref * r * sqrt(r) * (c.t_ref + c.s_suth) / (T + c.s_suth);
+}
+
+constexpr int CFL_BLOCKS = 1024;
+
+__global__ void __launch_bounds__(256) k_cfl(Consts c, const double* __restrict__ U, CflIn in, double* __restrict__ red) {
+  const long long N = c.LC.n;
+  double inv_min = INFINITY, vis_min = INFINITY;
+  for (long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x; tid < N; tid += (long long)gridDim.x * blockDim.x) {
+    const int i = (int)(tid % c.n[0]), j = (int)((tid / c.n[0]) % c.n[1]), k = (int)(tid / ((long long)c.n[0] * c.n[1]));
+    const long long at = c.LX.at(i, j, k);
+    const double r = U[tid], u = U[N + tid] / r, v = U[2 * N + tid] / r, w = U[3 * N + tid] / r;
+    const double p = (c.gamma - 1.0) * (U[4 * N + tid] - 0.5 * r * (u * u + v * v + w * w));
+    const double cs = sqrt(c.gamma * p / r), J = 1.0 / in.rj[at];
+    const double mu = c.viscous ? sutherland(c, p / (r * c.r_gas)) : 0.0;
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      const double mx = J * in.met[3 * d][at], my = J * in.met[3 * d + 1][at], mz = J * in.met[3 * d + 2][at];
+      const double mtt = c.moving ? J * in.mt[d][at] : 0.0;
+      const double gn = sqrt(mx * mx + my * my + mz * mz);
+      inv_min = fmin(inv_min, 1.0 / (fabs(mtt + mx * u + my * v + mz * w) + cs * gn));
+      if (c.viscous) vis_min = fmin(vis_min, 1.0 / (mu * gn * gn));
+    }
+  }
+  __shared__ double sa[256], sb[256];
+  sa[threadIdx.x] = inv_min; sb[threadIdx.x] = vis_min;
+  __syncthreads();
+  for (int o = 128; o > 0; o >>= 1) {
+    if ((int)threadIdx.x < o) {
+      sa[threadIdx.x] = fmin(sa[threadIdx.x], sa[threadIdx.x + o]);
+      sb[threadIdx.x] = fmin(sb[threadIdx.x], sb[threadIdx.x + o]);
+    }
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) { red[2 * blockIdx.x] = sa[0]; red[2 * blockIdx.x + 1] = sb[0]; }
+}
+
+}  // namespace meg6
