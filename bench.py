@@ -1,0 +1,302 @@
+#!/usr/bin/env python
+"""bench.py -- FP64 MEG6 RHS + SSP-RK3 throughput on B200 (BASELINE.json metric).
+
+One "step" = one rk3_step = three passes of the whole hot path (primitives, ghosts, gradients, three flux
+kernels, assembly + update) over the workload.  value = N_cells * 3 * steps / seconds, in Mcell-updates/s per
+RK stage, summed over all ranks (independent replicas for --gpus > 1: the path is single-GPU).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c4|c3|c1|c2] [--impl reference]
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+import workloads as W  # noqa: E402
+
+METRIC = "FP64 MEG6 RHS Mcell-updates/s per RK stage"
+UNIT = "Mcell-updates/s/stage"
+# FP64 (DFMA-pipe) warp-instruction peak: 148 SMs x 64 lanes/clk x clock
+FP64_LANES_PER_SM_CLK = 64
+N_SM = 148
+
+
+def make_workload(name):
+    if name == "c4":
+        return W.c4_jet()
+    if name == "c4_small":
+        return W.c4_jet(ni=160, nj=100, nk=100)
+    if name == "c3":
+        return W.c3_tgv(n=128)
+    if name == "c1":
+        return W.c1_vortex(n=32)
+    if name == "c2":
+        return W.c2_dynamic_freestream(n=64)
+    raise SystemExit("unknown workload " + name)
+
+
+def peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            p = json.load(f)
+        return p["hbm_gbs"], p.get("sm_max_mhz", 1965.0), "measured (MEASURED_PEAKS.json)"
+    except Exception:
+        return 6650.0, 1965.0, "fallback (B200_PROFILING.md)"
+
+
+def bytes_per_cell_stage(prm, sponge):
+    """Compulsory HBM doubles per cell per RK stage of the shipped kernel set."""
+    v, m = prm["viscous"], prm["moving"]
+    k = {}
+    k["prim"] = 5 + 6
+    k["grad"] = (4 + 12) if v else 0
+    met = (10 if v else 3) + (1 if m else 0)
+    k["flux_xi"] = (6 if v else 5) + met + (8 if v else 0) + 5
+    k["flux_eta"] = k["flux_xi"] + 5
+    k["flux_zeta"] = k["flux_xi"] + 5
+    k["update"] = 5 + 5 + 10.0 / 3 + 1 + (1 if m else 0) + ((1 + 5) if sponge else 0) + 5
+    k["copy_Un"] = 10.0 / 3
+    k["metrics"] = (6 + 3 + 9 + 9 + 1 + 6 + 3 * met + 1) if m else 0   # nodes+modes, xc, cd, met, rj, xt+mt, faces, rjt
+    return {a: 8.0 * b for a, b in k.items()}
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu):
+        self.rows, self.proc, self.gpu = [], None, gpu
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.gpu), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[1])); mx.append(float(r[2]))
+                for n, v in zip(names, r[5:9]):
+                    if v.lower().startswith("active"):
+                        reasons.add(n)
+            except Exception:
+                pass
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def oracle_sample(threads=None):
+    """The CPU oracle as it stands, timed on a bounded sample of the C4 workload (1/8 of the cells)."""
+    from oracle import meg6_oracle as O
+    nthr = threads or (os.cpu_count() or 1)
+    O.set_threads(nthr)
+    wl = W.c4_jet(ni=160, nj=100, nk=100)
+    g = O.Grid(wl)
+    g.metrics_compute(0.0)
+    U = wl["U0"].copy()
+    t0 = time.perf_counter()
+    g.rk3_step(U, 0.0, wl["dt"])
+    dt = time.perf_counter() - t0
+    n = U[0].size
+    return {"value": n * 3 / dt / 1e6, "unit": UNIT, "cores": O.get_threads(), "kind": "oracle",
+            "sample": "c4_jet 160x100x100 (1.6 M cells, 1/8 of the workload), 1 RK3 step, %.1f s" % dt}, dt
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    vals = []
+    base = None
+    for s in range(args.warmup + args.steps):
+        base, dt = oracle_sample()
+        if s >= args.warmup:
+            vals.append((base["value"], dt))
+    v = float(np.mean([a for a, _ in vals]))
+    ms = float(np.mean([b for _, b in vals])) * 1e3
+    base["value"] = v
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "c4_jet_320x200x200", "sample": base["sample"]},
+            "cpu_baseline": base,
+            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+def run_ours(args):
+    import torch
+    from paper_2303_10785_b200 import Grid
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    wl = make_workload(args.workload)
+    prm = wl["params"]
+    ncell = prm["ni"] * prm["nj"] * prm["nk"]
+    g = Grid(wl, device=dev)
+    g.metrics_compute(wl["t0"])
+    U = torch.as_tensor(wl["U0"], device=dev).contiguous()
+    if wl["dt"] is not None:
+        dt = wl["dt"]
+    else:
+        dt = g.cfl_dt(U, wl["cfl"])      # on-device Eq. B.2/B.3 (no oracle on the product path)
+    stream = torch.cuda.current_stream(dev)
+
+    def barrier():
+        torch.cuda.synchronize(dev)
+        if dist:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    # ---------------- device-resident timing ----------------
+    t = wl["t0"]
+    for _ in range(args.warmup):
+        g.rk3_step(U, t, dt); t += dt
+    g.profile_enable(True)
+    g.profile_read()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(args.steps):
+        g.rk3_step(U, t, dt); t += dt
+    e1.record(stream)
+    barrier()
+    ms = e0.elapsed_time(e1)
+    clocks = sampler.stop() if rank == 0 else None
+    prof = g.profile_read()
+    g.profile_enable(False)
+    finite = bool(torch.isfinite(U).all().item())
+
+    # ---------------- end to end: host buffers, copies inside the timed region ----------------
+    Uh = torch.empty(U.shape, dtype=torch.float64).pin_memory()
+    Uh.copy_(U)
+    Ud = torch.empty_like(U)
+    for _ in range(2):
+        Ud.copy_(Uh, non_blocking=True); g.rk3_step(Ud, t, dt); Uh.copy_(Ud, non_blocking=True)
+    barrier()
+    f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    f0.record(stream)
+    for _ in range(args.steps):
+        Ud.copy_(Uh, non_blocking=True)          # host -> device copy of this step's input state
+        g.rk3_step(Ud, t, dt)
+        Uh.copy_(Ud, non_blocking=True)          # device -> host read of the step's result
+        t += dt
+    f1.record(stream)
+    barrier()
+    ms_e2e = f0.elapsed_time(f1)
+
+    tms = torch.tensor([ms, ms_e2e], dtype=torch.float64, device=dev)
+    if dist:
+        dist.all_reduce(tms, op=dist.ReduceOp.MAX)
+    ms, ms_e2e = float(tms[0]), float(tms[1])
+    if rank != 0:
+        if dist:
+            dist.destroy_process_group()
+        return
+
+    value = ncell * 3 * args.steps * world / (ms * 1e-3) / 1e6
+    e2e_value = ncell * 3 * args.steps * world / (ms_e2e * 1e-3) / 1e6
+    hbm, sm_max, peak_src = peaks()
+    bpc = bytes_per_cell_stage(prm, wl.get("sigma") is not None)
+    stage_bytes = sum(bpc.values())
+    # per-kernel breakdown measured live with CUDA events on the launching stream
+    tot_prof = sum(v[0] for v in prof.values())
+    kernels = {}
+    launches = 0
+    for k, (kms, kn) in prof.items():
+        if kms == 0 and kn == 0:
+            continue
+        launches += kn
+        per_stage = kms / (3 * args.steps)
+        kernels[k] = {"ms_per_stage": per_stage, "share": kms / tot_prof, "launches": int(kn),
+                      "algorithmic_GBps": (bpc.get(k, 0) * ncell / (per_stage * 1e-3) / 1e9) if per_stage else None}
+    dom = max((k for k in kernels if k.startswith("flux")), key=lambda k: kernels[k]["ms_per_stage"])
+    dsec = kernels[dom]["ms_per_stage"] * 1e-3
+    ach = bpc[dom] * ncell / dsec / 1e9
+    clk = (clocks or {}).get("sm_mhz") or sm_max
+    roof = {"kernel": "k_flux<%s,%s>" % (dom[5:], "visc" if prm["viscous"] else "inv"), "bound": "hbm",
+            "achieved": ach, "peak": hbm, "unit": "GB/s", "frac": ach / hbm, "traffic": None,
+            "peak_source": peak_src, "bytes_per_cell": bpc[dom], "cells_per_launch": ncell,
+            "avg_launch_ms": dsec * 1e3,
+            "fp64_pipe_peak_Tinst_s_at_sampled_clock": N_SM * FP64_LANES_PER_SM_CLK * clk * 1e6 / 1e12}
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": wl["name"], "cells": ncell, "viscous": prm["viscous"], "moving": prm["moving"],
+                       "dt": dt, "parallelism": "replicas x%d" % world,
+                       "l2": "working set %.1f GB per stage >> 126 MB L2 (no flush needed)" % (stage_bytes * ncell / 1e9)},
+            "clocks": clocks, "gpu_launches": int(launches), "finite": finite,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(U.numel() * 8),
+                    "d2h_bytes_per_step": int(U.numel() * 8), "ms_per_step": ms_e2e / args.steps},
+            "roofline": roof,
+            "hbm_roofline_step": {"bytes_per_cell_stage": stage_bytes,
+                                  "achieved_GBps": stage_bytes * ncell * 3 * args.steps / (ms * 1e-3) / 1e9,
+                                  "frac": stage_bytes * ncell * 3 * args.steps / (ms * 1e-3) / 1e9 / hbm,
+                                  "peak": hbm, "peak_source": peak_src},
+            "kernels": kernels}
+    if world == 1 and not args.no_cpu_baseline:
+        line["cpu_baseline"], _ = oracle_sample()
+    print(json.dumps(line))
+    if dist:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="c4")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

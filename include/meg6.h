@@ -104,6 +104,15 @@ meg6_status meg6_limiter_stats(meg6_grid* g, unsigned long long* n_limited, unsi
  * kind 2: primitive field which = 0..5 (rho,u,v,w,p,T) after the last rhs. */
 meg6_status meg6_get_array(meg6_grid* g, int kind, int which, double* out);
 
+/* Per-kernel timing for bench.py: while enabled, every kernel launch of the library is bracketed by CUDA
+ * events on the grid's stream.  meg6_profile_read synchronises the stream, adds up the elapsed time and the
+ * number of kernel launches per kind since the last read, and clears the record.  HOST pointers, 16 entries
+ * each.  Kinds: 0 metric/Jacobian kernels (all of one metrics_compute), 1 primitive conversion, 2 ghost fill,
+ * 3 stored E6 gradients, 4/5/6 flux kernel along xi/eta/zeta, 7 residual assembly + RK3 update,
+ * 8 copy of U^n (memcpy, not counted as a kernel launch), 9 CFL reduction. */
+meg6_status meg6_profile_enable(meg6_grid* g, int on);
+meg6_status meg6_profile_read(meg6_grid* g, double* ms_per_kind, unsigned long long* launches_per_kind);
+
 const char* meg6_last_error(void);
 /* Library/ABI version: 1000*major + minor. */
 int meg6_version(void);

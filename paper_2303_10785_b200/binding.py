@@ -9,7 +9,8 @@ from . import build as _build
 
 EXPORTS = ["meg6_workspace_bytes", "meg6_grid_create", "meg6_grid_destroy", "meg6_metrics_compute",
            "meg6_set_inflow", "meg6_set_sponge", "meg6_rhs", "meg6_rk3_step", "meg6_cfl_dt",
-           "meg6_limiter_stats_enable", "meg6_limiter_stats", "meg6_get_array", "meg6_last_error",
+           "meg6_limiter_stats_enable", "meg6_limiter_stats", "meg6_get_array", "meg6_profile_enable",
+           "meg6_profile_read", "meg6_last_error",
            "meg6_version"]
 
 
@@ -88,6 +89,10 @@ def lib():
         L.meg6_limiter_stats.argtypes = [_vp, C.POINTER(C.c_ulonglong), C.POINTER(C.c_ulonglong)]
         L.meg6_get_array.restype = C.c_int
         L.meg6_get_array.argtypes = [_vp, C.c_int, C.c_int, _vp]
+        L.meg6_profile_enable.restype = C.c_int
+        L.meg6_profile_enable.argtypes = [_vp, C.c_int]
+        L.meg6_profile_read.restype = C.c_int
+        L.meg6_profile_read.argtypes = [_vp, C.POINTER(C.c_double), C.POINTER(C.c_ulonglong)]
         L.meg6_last_error.restype = C.c_char_p
         L.meg6_version.restype = C.c_int
         _lib = L
@@ -181,6 +186,19 @@ class Grid:
         a, b = C.c_ulonglong(), C.c_ulonglong()
         _check(lib().meg6_limiter_stats(self.h, C.byref(a), C.byref(b)), "meg6_limiter_stats")
         return a.value, b.value
+
+    PROFILE_KINDS = ["metrics", "prim", "ghost", "grad", "flux_xi", "flux_eta", "flux_zeta", "update",
+                     "copy_Un", "cfl"]
+
+    def profile_enable(self, on=True):
+        _check(lib().meg6_profile_enable(self.h, int(on)), "meg6_profile_enable")
+
+    def profile_read(self):
+        """{kind: (milliseconds, kernel launches)} since the last read"""
+        ms = (C.c_double * 16)()
+        n = (C.c_ulonglong * 16)()
+        _check(lib().meg6_profile_read(self.h, ms, n), "meg6_profile_read")
+        return {k: (ms[i], n[i]) for i, k in enumerate(self.PROFILE_KINDS)}
 
     def get_array(self, kind, which):
         import numpy as np

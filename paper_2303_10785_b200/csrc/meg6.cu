@@ -8,6 +8,8 @@
 #include "meg6_common.cuh"
 #include "meg6_flow.cuh"
 #include "meg6_flux.cuh"
+#include "meg6_flux_tma.cuh"
+#include <stdlib.h>
 
 using namespace meg6;
 
@@ -52,12 +54,17 @@ static Consts make_consts(const meg6_params* p) {
   c.mp_alpha = p->mp_alpha; c.p_out = p->p_out;
   c.kappa_fac = p->viscous ? p->gamma * p->r_gas / ((p->gamma - 1.0) * p->prandtl) : 0.0;
   c.LX = make_lay(p->ni, p->nj, p->nk, GX, GX, GX);
-  c.LP = make_lay(p->ni, p->nj, p->nk, GPI, GPJ, GPK);
-  c.LG = make_lay(p->ni, p->nj, p->nk, GGI, GGJ, GGK);
+  // row pitches are even so that every TMA global stride is a multiple of 16 bytes
+  c.LP = make_lay(p->ni, p->nj, p->nk, GPI, GPJ, GPK, 2);
+  c.LG = make_lay(p->ni, p->nj, p->nk, GGI, GGJ, GGK, 2);
   c.LC = make_lay(p->ni, p->nj, p->nk, 0, 0, 0);
-  c.LF[0] = make_lay(p->ni + 1, p->nj, p->nk, 0, 0, 0);
-  c.LF[1] = make_lay(p->ni, p->nj + 1, p->nk, 0, 0, 0);
-  c.LF[2] = make_lay(p->ni, p->nj, p->nk + 1, 0, 0, 0);
+  c.LR = make_lay(p->ni, p->nj, p->nk, 0, 0, 0, 2);
+  c.LF[0] = make_lay(p->ni + 1, p->nj, p->nk, 0, 0, 0, 2);
+  c.LF[1] = make_lay(p->ni, p->nj + 1, p->nk, 0, 0, 0, 2);
+  c.LF[2] = make_lay(p->ni, p->nj, p->nk + 1, 0, 0, 0, 2);
+  auto fs = [](long long n) { return (long long)(((size_t)n * 8 + 255) / 256 * 256 / 8); };
+  c.fsP = fs(c.LP.n); c.fsG = fs(c.LG.n); c.fsR = fs(c.LR.n);
+  for (int d = 0; d < 3; ++d) c.fsM[d] = fs(c.LF[d].n);
   return c;
 }
 
@@ -70,7 +77,7 @@ static size_t carve(const meg6_params* p, const Consts& c, meg6_grid* g, char* b
     return ptr;
   };
   const long long nn = (long long)(p->ni + 1) * (p->nj + 1) * (p->nk + 1);
-  meg6_grid tmp;
+  meg6_grid tmp = meg6_grid();
   meg6_grid* G = g ? g : &tmp;
   for (int q = 0; q < 3; ++q) G->nodes[q] = take(nn);
   for (int q = 0; q < 3; ++q) G->modes[q] = p->moving ? take(nn) : nullptr;
@@ -91,7 +98,8 @@ static size_t carve(const meg6_params* p, const Consts& c, meg6_grid* g, char* b
   for (int f = 0; f < 6; ++f) G->P[f] = take(c.LP.n);
   for (int e = 0; e < 3; ++e)
     for (int f = 0; f < 4; ++f) G->G[e][f] = p->viscous ? take(c.LG.n) : nullptr;
-  G->res = take(5 * c.LC.n);
+  G->res = take(c.LR.n);
+  for (int f = 1; f < 5; ++f) take(c.LR.n);   // fields c.fsR apart
   G->U0 = take(5 * c.LC.n);
   for (int f = 0; f < 6; ++f) {
     const int d = f / 2;
@@ -109,7 +117,116 @@ static size_t carve(const meg6_params* p, const Consts& c, meg6_grid* g, char* b
 static inline unsigned nblk(long long n, int t) { return (unsigned)((n + t - 1) / t); }
 namespace meg6 { cudaError_t launch_geometry(meg6_grid* g, double t); }
 
+// ---- TMA descriptors (cuTensorMapEncodeTiled through the runtime's driver entry point: no libcuda link) ----
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static bool make_map4(EncodeTiledFn fn, CUtensorMap* tm, const double* base, const Lay& L, long long fs, int nfields,
+                      const int box[4]) {
+  cuuint64_t dims[4] = {(cuuint64_t)L.pi, (cuuint64_t)L.pj, (cuuint64_t)L.pk, (cuuint64_t)nfields};
+  cuuint64_t strides[3] = {(cuuint64_t)L.sj * 8, (cuuint64_t)L.sk * 8, (cuuint64_t)fs * 8};
+  cuuint32_t bx[4] = {(cuuint32_t)box[0], (cuuint32_t)box[1], (cuuint32_t)box[2], (cuuint32_t)box[3]};
+  cuuint32_t es[4] = {1, 1, 1, 1};
+  return fn(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, (void*)base, dims, strides, bx, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+            CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+template <int DIR, bool VISC>
+static bool make_maps_dir(EncodeTiledFn fn, meg6_grid* g) {
+  using C = TmaCfg<DIR, VISC>;
+  const Consts& c = g->c;
+  TmaMaps& t = g->tmaps[DIR];
+  auto box = [](int sweep, int trans, int nf, int out[4]) {
+    if (DIR == 0) { out[0] = sweep; out[1] = trans; out[2] = 1; }
+    else if (DIR == 1) { out[0] = trans; out[1] = sweep; out[2] = 1; }
+    else { out[0] = trans; out[1] = 1; out[2] = sweep; }
+    out[3] = nf;
+  };
+  int b[4];
+  bool ok = true;
+  box(C::LP, C::TT, C::NF, b);
+  ok = ok && make_map4(fn, &t.P, g->P[0], c.LP, c.fsP, 6, b);
+  box(C::LF, C::TT, C::NM, b);
+  ok = ok && make_map4(fn, &t.M, VISC ? g->fmet[DIR][0] : g->fmet[DIR][3 * DIR], c.LF[DIR], c.fsM[DIR], C::NM, b);
+  if (g->p.moving) {
+    box(C::LF, C::TT, 1, b);
+    ok = ok && make_map4(fn, &t.Mt, g->fmt[DIR], c.LF[DIR], c.fsM[DIR], 1, b);
+  }
+  if (VISC) {
+    box(C::LG, C::TT, 4, b);
+    ok = ok && make_map4(fn, &t.G, g->G[0][0], c.LG, c.fsG, 12, b);
+  }
+  box(C::TS, C::TT, 5, b);
+  ok = ok && make_map4(fn, &t.R, g->res, c.LR, c.fsR, 5, b);
+  return ok;
+}
+
+static cudaError_t setup_tma(meg6_grid* g) {
+  g->use_tma = 0;
+  const char* env = getenv("MEG6_FLUX");
+  if (env && strcmp(env, "v1") == 0) return cudaSuccess;   // A/B switch: plain shared-memory staging kernel
+  void* fp = nullptr;
+  cudaDriverEntryPointQueryResult qr;
+  cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fp, cudaEnableDefault, &qr);
+  if (e != cudaSuccess) return e;
+  if (!fp || qr != cudaDriverEntryPointSuccess) return cudaErrorNotSupported;
+  EncodeTiledFn fn = (EncodeTiledFn)fp;
+  bool ok;
+  if (g->p.viscous) ok = make_maps_dir<0, true>(fn, g) && make_maps_dir<1, true>(fn, g) && make_maps_dir<2, true>(fn, g);
+  else ok = make_maps_dir<0, false>(fn, g) && make_maps_dir<1, false>(fn, g) && make_maps_dir<2, false>(fn, g);
+  if (!ok) return cudaErrorInvalidValue;
+#define SET_SMEM(D, V)                                                                                      \
+  if ((e = cudaFuncSetAttribute(k_flux_tma<D, V>, cudaFuncAttributeMaxDynamicSharedMemorySize,              \
+                                TmaCfg<D, V>::SMEM_BYTES)) != cudaSuccess) return e;
+  SET_SMEM(0, false) SET_SMEM(1, false) SET_SMEM(2, false) SET_SMEM(0, true) SET_SMEM(1, true) SET_SMEM(2, true)
+#undef SET_SMEM
+  g->use_tma = 1;
+  return cudaSuccess;
+}
+
+// ---- per-kernel timing: one event pair per launch (or launch group) while profiling is enabled ----
+struct ProfScope {
+  meg6_grid* g; size_t rec;
+  ProfScope(meg6_grid* g_, int kind, int launches) : g(g_), rec((size_t)-1) {
+    if (!g->prof_on) return;
+    while (g->prof_pool.size() < g->prof_used + 2) {
+      cudaEvent_t e;
+      if (cudaEventCreate(&e) != cudaSuccess) return;
+      g->prof_pool.push_back(e);
+    }
+    meg6_grid::ProfRec r;
+    r.kind = kind; r.launches = launches; r.e0 = g->prof_used; r.e1 = g->prof_used + 1;
+    g->prof_used += 2;
+    cudaEventRecord(g->prof_pool[r.e0], g->stream);
+    g->prof_recs.push_back(r);
+    rec = g->prof_recs.size() - 1;
+  }
+  ~ProfScope() {
+    if (rec != (size_t)-1) cudaEventRecord(g->prof_pool[g->prof_recs[rec].e1], g->stream);
+  }
+};
+
 extern "C" {
+
+meg6_status meg6_profile_enable(meg6_grid* g, int on) {
+  if (!g) return fail(MEG6_EINVAL, "null grid%s");
+  g->prof_on = on ? 1 : 0;
+  return MEG6_OK;
+}
+
+meg6_status meg6_profile_read(meg6_grid* g, double* ms, unsigned long long* launches) {
+  if (!g || !ms || !launches) return fail(MEG6_EINVAL, "profile_read: null pointer%s");
+  CUDA_OK(cudaStreamSynchronize(g->stream));
+  for (int k = 0; k < 16; ++k) { ms[k] = 0.0; launches[k] = 0; }
+  for (const meg6_grid::ProfRec& r : g->prof_recs) {
+    float t = 0.f;
+    CUDA_OK(cudaEventElapsedTime(&t, g->prof_pool[r.e0], g->prof_pool[r.e1]));
+    ms[r.kind] += t; launches[r.kind] += r.launches;
+  }
+  g->prof_recs.clear(); g->prof_used = 0;
+  return MEG6_OK;
+}
 
 int meg6_version(void) { return 1000; }
 const char* meg6_last_error(void) { return g_err; }
@@ -129,9 +246,8 @@ meg6_status meg6_grid_create(const meg6_params* p, const double* x, const double
   if (((uintptr_t)workspace & 255) != 0) return fail(MEG6_EINVAL, "workspace must be 256-byte aligned%s");
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return fail(MEG6_ECUDA, "no CUDA device%s");
-  meg6_grid* g = new (std::nothrow) meg6_grid();
+  meg6_grid* g = new (std::nothrow) meg6_grid();   // value-initialised: all pointers null, flags zero
   if (!g) return fail(MEG6_ENOMEM, "host allocation failed%s");
-  memset((void*)g, 0, sizeof(*g));
   g->p = *p;
   g->c = make_consts(p);
   g->stream = (cudaStream_t)cuda_stream;
@@ -155,17 +271,26 @@ meg6_status meg6_grid_create(const meg6_params* p, const double* x, const double
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_flux<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(FluxCfg<1, true>::SMEM_DOUBLES * 8));
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_flux<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(FluxCfg<2, true>::SMEM_DOUBLES * 8));
   }
+  if (e == cudaSuccess) e = setup_tma(g);
   if (e != cudaSuccess) { delete g; return fail(MEG6_ECUDA, "grid_create: %s", cudaGetErrorString(e)); }
   *out = g;
   return MEG6_OK;
 }
 
-void meg6_grid_destroy(meg6_grid* g) { delete g; }
+void meg6_grid_destroy(meg6_grid* g) {
+  if (!g) return;
+  for (cudaEvent_t e : g->prof_pool) cudaEventDestroy(e);
+  delete g;
+}
 
 meg6_status meg6_metrics_compute(meg6_grid* g, double t) {
   if (!g) return fail(MEG6_EINVAL, "null grid%s");
   if (g->have_metrics && !g->p.moving) return MEG6_OK;   // static: idempotent
-  cudaError_t e = meg6::launch_geometry(g, t);            // meg6_geom.cu (compiled with -fmad=false)
+  cudaError_t e;
+  {
+    ProfScope ps(g, 0, 3 + 3 + (g->p.moving ? 1 : 0));
+    e = meg6::launch_geometry(g, t);                      // meg6_geom.cu (compiled with -fmad=false)
+  }
   if (e != cudaSuccess) return fail(MEG6_ECUDA, "metrics_compute: %s", cudaGetErrorString(e));
   g->have_metrics = true;
   return MEG6_OK;
@@ -193,7 +318,7 @@ static meg6_status residual(meg6_grid* g, const double* U) {
   P6 P;
   for (int f = 0; f < 6; ++f) P.p[f] = g->P[f];
   const int T = 256;
-  k_prim<<<nblk(c.LC.n, T), T, 0, g->stream>>>(c, U, P);
+  { ProfScope ps(g, 1, 1); k_prim<<<nblk(c.LC.n, T), T, 0, g->stream>>>(c, U, P); }
   for (int d = 0; d < 3; ++d) {
     int a = (d + 1) % 3, b = (d + 2) % 3;
     if (a > b) { int t = a; a = b; b = t; }
@@ -201,6 +326,7 @@ static meg6_status residual(meg6_grid* g, const double* U) {
     GhostIn gin;
     gin.inflow[0] = g->inflow[2 * d]; gin.inflow[1] = g->inflow[2 * d + 1];
     gin.mx = g->met[3 * d]; gin.my = g->met[3 * d + 1]; gin.mz = g->met[3 * d + 2];
+    ProfScope ps(g, 2, 1);
     k_ghost<<<nblk(ea * eb * 2, 128), 128, 0, g->stream>>>(c, d, P, gin);
   }
   if (g->p.viscous) {
@@ -208,6 +334,7 @@ static meg6_status residual(meg6_grid* g, const double* U) {
     for (int e = 0; e < 3; ++e)
       for (int f = 0; f < 4; ++f) G.p[4 * e + f] = g->G[e][f];
     const long long ng = (long long)(c.n[0] + 2) * (c.n[1] + 2) * (c.n[2] + 2);
+    ProfScope ps(g, 3, 1);
     k_grad<<<nblk(ng, T), T, 0, g->stream>>>(c, P, G);
   }
   for (int d = 0; d < 3; ++d) {
@@ -221,7 +348,24 @@ static meg6_status residual(meg6_grid* g, const double* U) {
     in.stats = g->stats_on ? g->stats : nullptr;
     in.first = (d == 0);
     const bool V = g->p.viscous != 0;
-    if (d == 0) {
+    ProfScope ps(g, 4 + d, 1);
+    if (g->use_tma) {
+      FluxIn2 i2;
+      i2.res = g->res; i2.stats = in.stats; i2.first = in.first; i2.moving = g->p.moving ? 1 : 0;
+      i2.dbg = getenv("MEG6_DBG") ? atoi(getenv("MEG6_DBG")) : 0;
+#define LAUNCH_TMA(D, VV, GRID) k_flux_tma<D, VV><<<GRID, TmaCfg<D, VV>::NT, TmaCfg<D, VV>::SMEM_BYTES, g->stream>>>(c, i2, g->tmaps[D])
+      if (d == 0) {
+        dim3 grid(nblk(c.n[0], TmaCfg<0, false>::TS), nblk(c.n[1], TmaCfg<0, false>::TT), c.n[2]);
+        if (V) LAUNCH_TMA(0, true, grid); else LAUNCH_TMA(0, false, grid);
+      } else if (d == 1) {
+        dim3 grid(nblk(c.n[0], TmaCfg<1, false>::TT), nblk(c.n[1], TmaCfg<1, false>::TS), c.n[2]);
+        if (V) LAUNCH_TMA(1, true, grid); else LAUNCH_TMA(1, false, grid);
+      } else {
+        dim3 grid(nblk(c.n[0], TmaCfg<2, false>::TT), c.n[1], nblk(c.n[2], TmaCfg<2, false>::TS));
+        if (V) LAUNCH_TMA(2, true, grid); else LAUNCH_TMA(2, false, grid);
+      }
+#undef LAUNCH_TMA
+    } else if (d == 0) {
       dim3 grid(nblk(c.n[0], FluxCfg<0, false>::TS), nblk(c.n[1], FluxCfg<0, false>::TT), c.n[2]);
       if (V) k_flux<0, true><<<grid, FluxCfg<0, true>::NT, FluxCfg<0, true>::SMEM_DOUBLES * 8, g->stream>>>(c, in);
       else k_flux<0, false><<<grid, FluxCfg<0, false>::NT, FluxCfg<0, false>::SMEM_DOUBLES * 8, g->stream>>>(c, in);
@@ -244,6 +388,7 @@ static void launch_update(meg6_grid* g, const double* U, double* out, int mode, 
   in.res = g->res; in.rj = g->rj; in.rjt = g->p.moving ? g->rjt : nullptr;
   in.sigma = g->sigma; in.uref = g->uref;
   in.U = U; in.U0 = g->U0; in.out = out; in.a = a; in.b = b; in.dt = dt; in.mode = mode;
+  ProfScope ps(g, 7, 1);
   k_update<<<nblk(g->c.LC.n, 256), 256, 0, g->stream>>>(g->c, in);
 }
 
@@ -260,7 +405,10 @@ meg6_status meg6_rhs(meg6_grid* g, const double* U, double* dUdt) {
 meg6_status meg6_rk3_step(meg6_grid* g, double* U, double t, double dt) {
   if (!g || !U) return fail(MEG6_EINVAL, "rk3_step: null pointer%s");
   if (!g->have_metrics && !g->p.moving) return fail(MEG6_ESTATE, "rk3_step called before metrics_compute%s");
-  CUDA_OK(cudaMemcpyAsync(g->U0, U, sizeof(double) * 5 * (size_t)g->c.LC.n, cudaMemcpyDeviceToDevice, g->stream));
+  {
+    ProfScope ps(g, 8, 0);
+    CUDA_OK(cudaMemcpyAsync(g->U0, U, sizeof(double) * 5 * (size_t)g->c.LC.n, cudaMemcpyDeviceToDevice, g->stream));
+  }
   const double ts[3] = {t, t + dt, t + 0.5 * dt};
   const double aa[3] = {0.0, 3.0 / 4.0, 1.0 / 3.0}, bb[3] = {1.0, 1.0 / 4.0, 2.0 / 3.0};
   for (int s = 0; s < 3; ++s) {
@@ -281,7 +429,7 @@ meg6_status meg6_cfl_dt(meg6_grid* g, const double* U, double cfl, double* dt) {
   for (int q = 0; q < 3; ++q) in.mt[q] = g->mt[q];
   in.rj = g->rj;
   const int nb = (int)((g->c.LC.n + 255) / 256 < CFL_BLOCKS ? (g->c.LC.n + 255) / 256 : CFL_BLOCKS);
-  k_cfl<<<nb, 256, 0, g->stream>>>(g->c, U, in, g->red);
+  { ProfScope ps(g, 9, 1); k_cfl<<<nb, 256, 0, g->stream>>>(g->c, U, in, g->red); }
   static thread_local double host[2 * CFL_BLOCKS];
   CUDA_OK(cudaMemcpyAsync(host, g->red, sizeof(double) * 2 * nb, cudaMemcpyDeviceToHost, g->stream));
   CUDA_OK(cudaStreamSynchronize(g->stream));

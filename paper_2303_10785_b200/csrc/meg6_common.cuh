@@ -1,8 +1,10 @@
 // meg6_common.cuh -- layouts, constants and the grid object of the B200 MEG6 library.
 // Part of the single translation unit meg6.cu.  Shares nothing with oracle/.
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <vector>
 #include "../../include/meg6.h"
 
 namespace meg6 {
@@ -56,14 +58,20 @@ struct Consts {   // per-grid constants passed by value to kernels
   int bc[6];
   double gamma, r_gas, prandtl, mu_ref, t_ref, s_suth, mp_alpha, p_out;
   double kappa_fac;   // gamma r_gas / ((gamma-1) Pr)
-  Lay LX, LP, LG, LC; // coordinates/metrics, primitives, gradients, interior cells
+  Lay LX, LP, LG, LC; // coordinates/metrics, primitives, gradients, interior cells (caller's U layout)
+  Lay LR;             // residual accumulator: interior cells, even row pitch (TMA strides are multiples of 16 B)
   Lay LF[3];          // interface families
+  long long fsP, fsG, fsR, fsM[3];   // distance in doubles between consecutive fields of P, G, res, fmet[d]
 };
 
 }  // namespace meg6
 
+namespace meg6 { struct TmaMaps { CUtensorMap P, M, Mt, G, R; }; }
+
 struct meg6_grid {
   meg6_params p;
+  meg6::TmaMaps tmaps[3];   // per sweep direction
+  int use_tma;
   meg6::Consts c;
   cudaStream_t stream;
   char* ws; size_t ws_bytes;
@@ -86,4 +94,10 @@ struct meg6_grid {
   double* red;                 // reduction scratch
   int stats_on;
   bool have_metrics;
+  // per-kernel timing (meg6_profile_*): event pairs of the launches since the last read
+  int prof_on;
+  std::vector<cudaEvent_t> prof_pool;
+  struct ProfRec { int kind; int launches; size_t e0, e1; };
+  std::vector<ProfRec> prof_recs;
+  size_t prof_used;
 };

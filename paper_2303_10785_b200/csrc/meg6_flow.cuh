@@ -138,12 +138,13 @@ __global__ void __launch_bounds__(256) k_update(Consts c, UpdIn in) {
   if (tid >= N) return;
   const int i = (int)(tid % c.n[0]), j = (int)((tid / c.n[0]) % c.n[1]), k = (int)(tid / ((long long)c.n[0] * c.n[1]));
   const double J = 1.0 / in.rj[c.LX.at(i, j, k)];
+  const long long ar = c.LR.at(i, j, k);
   const double rjt = in.rjt ? in.rjt[tid] : 0.0;
   const double sg = in.sigma ? in.sigma[tid] : 0.0;
 #pragma unroll
   for (int f = 0; f < 5; ++f) {
     const double u = in.U[f * N + tid];
-    double L = J * (in.res[f * N + tid] - rjt * u);
+    double L = J * (in.res[f * c.fsR + ar] - rjt * u);
     if (in.sigma) L -= sg * (u - in.uref[f * N + tid]);
     if (in.mode == 0) in.out[f * N + tid] = L;
     else {

@@ -96,6 +96,112 @@ __device__ __forceinline__ void hllc(const double PL[5], const double PR[5], dou
   }
 }
 
+// O3 steps 1-8 for one interface (Fig. 3).  pP: field 0 of cell i-1; pP1: P' of cell i; pP2: P'' of
+// cell i-1; SS = stride to the next cell along the sweep, FP/F1/F2 = field strides.  Returns the E.1 flags
+// (bit r: left state of component r limited, bit 5+r: right state).
+template <int SS_, int FP, int F1, int F2>
+__device__ __forceinline__ unsigned inviscid_face(const Consts& c, const double* __restrict__ pP, const double* __restrict__ pP1,
+                                                  const double* __restrict__ pP2, double mx, double my, double mz, double mt,
+                                                  double F[5]) {
+  const double g2 = fma(mx, mx, fma(my, my, mz * mz));
+  const double g = sqrt(g2), ig = 1.0 / g;
+  Eig e;
+  e.nx = mx * ig; e.ny = my * ig; e.nz = mz * ig;
+  const double rb = 0.5 * (pP[SS_] + pP[2 * SS_]);
+  const double pb = 0.5 * (pP[4 * FP + SS_] + pP[4 * FP + 2 * SS_]);
+  const double irb = 1.0 / rb;
+  e.a2 = c.gamma * pb * irb;
+  const double a = sqrt(e.a2), ia = 1.0 / a;
+  e.ra = rb * a;
+  const double ia2 = ia * ia, h_ira = 0.5 * irb * ia;
+  double W[4][5], D1[5], D2[5], WL[5], WR[5];
+#pragma unroll
+  for (int cidx = 0; cidx < 4; ++cidx)
+    project(e, pP[cidx * SS_], pP[FP + cidx * SS_], pP[2 * FP + cidx * SS_], pP[3 * FP + cidx * SS_],
+            pP[4 * FP + cidx * SS_], W[cidx]);
+  project(e, pP2[SS_], pP2[F2 + SS_], pP2[2 * F2 + SS_], pP2[3 * F2 + SS_], pP2[4 * F2 + SS_], D1);
+  project(e, pP2[2 * SS_], pP2[F2 + 2 * SS_], pP2[2 * F2 + 2 * SS_], pP2[3 * F2 + 2 * SS_], pP2[4 * F2 + 2 * SS_], D2);
+  {
+    double G0[5], G1[5];
+    project(e, pP1[0], pP1[F1], pP1[2 * F1], pP1[3 * F1], pP1[4 * F1], G0);
+    project(e, pP1[SS_], pP1[F1 + SS_], pP1[2 * F1 + SS_], pP1[3 * F1 + SS_], pP1[4 * F1 + SS_], G1);
+#pragma unroll
+    for (int r = 0; r < 5; ++r) {   // Eq. 21-22
+      WL[r] = W[1][r] + 0.5 * G0[r] + D1[r] / 12.0;
+      WR[r] = W[2][r] - 0.5 * G1[r] + D2[r] / 12.0;
+    }
+  }
+  unsigned fl = 0;
+#pragma unroll
+  for (int r = 0; r < 5; ++r) {
+    if (mp_test(WL[r], W[1][r], W[0][r], W[2][r], c.mp_alpha)) fl |= 1u << r;
+    if (mp_test(WR[r], W[2][r], W[3][r], W[1][r], c.mp_alpha)) fl |= 32u << r;
+  }
+  // warp-uniform early accept of test E.1: the full limiting path runs only if some lane needs it
+  if (__any_sync(__activemask(), fl != 0)) {
+    double D0[5], D3[5];
+    project(e, pP2[0], pP2[F2], pP2[2 * F2], pP2[3 * F2], pP2[4 * F2], D0);
+    project(e, pP2[3 * SS_], pP2[F2 + 3 * SS_], pP2[2 * F2 + 3 * SS_], pP2[3 * F2 + 3 * SS_], pP2[4 * F2 + 3 * SS_], D3);
+#pragma unroll
+    for (int r = 0; r < 5; ++r) {
+      const double dmid = minmod(D1[r], D2[r]);
+      WL[r] = mp_full(WL[r], W[1][r], W[0][r], W[2][r], dmid, minmod(D0[r], D1[r]), c.mp_alpha, (fl >> r) & 1u);
+      WR[r] = mp_full(WR[r], W[2][r], W[3][r], W[1][r], dmid, minmod(D2[r], D3[r]), c.mp_alpha, (fl >> (r + 5)) & 1u);
+    }
+  }
+  double PL[5], PR[5];
+  backproject(e, ia2, h_ira, WL, PL);
+  backproject(e, ia2, h_ira, WR, PR);
+  hllc(PL, PR, mx, my, mz, mt, g, g2, ig * ig, c.gamma, F);
+  return fl;
+}
+
+// O4: alpha-damping viscous flux, Eq. 29-35, subtracted from F (Res = -(F - Fv) differences).
+// pP: field 0 of cell L = i; pP1: P' of cell L; getG(e, f, cell) = stored tangential gradient of field f along e
+// at cell L (0) / R (1); getM(q) = hatted interface metric q (q = 9: 1/J) for the directions other than DIR.
+template <int DIR, int SS_, int FP, int F1, class GetG, class GetM>
+__device__ __forceinline__ void viscous_face(const Consts& c, const double* __restrict__ pP, const double* __restrict__ pP1,
+                                             double mx, double my, double mz, GetG getG, GetM getM, double F[5]) {
+  double val[4], gr[3][4];
+#pragma unroll
+  for (int f = 0; f < 4; ++f) {
+    const int pf = (f < 3) ? f + 1 : 5;
+    const double gL = pP1[pf * F1], gR = pP1[pf * F1 + SS_];
+    const double phL = fma(0.5, gL, pP[pf * FP]);            // Eq. 30 (beta^D = 0)
+    const double phR = fma(-0.5, gR, pP[pf * FP + SS_]);     // Eq. 31
+#pragma unroll
+    for (int e = 0; e < 3; ++e) {
+      if (e == DIR) gr[e][f] = fma(2.0, phR - phL, 0.5 * (gL + gR));   // Eq. 29, alpha^D = 4
+      else gr[e][f] = 0.5 * (getG(e, f, 0) + getG(e, f, 1));           // R11
+    }
+    val[f] = 0.5 * (phL + phR);
+  }
+  const double mu = sutherland(c, val[3]);
+  const double lam = -2.0 / 3.0 * mu, kap = mu * c.kappa_fac;
+  const double irj = 1.0 / getM(9);
+  double mh[9];
+#pragma unroll
+  for (int q = 0; q < 9; ++q) mh[q] = (q / 3 == DIR) ? ((q % 3 == 0) ? mx : (q % 3 == 1) ? my : mz) : getM(q);
+  double dx[3][4];
+#pragma unroll
+  for (int cc = 0; cc < 3; ++cc) {
+    const double k0 = mh[cc] * irj, k1 = mh[3 + cc] * irj, k2 = mh[6 + cc] * irj;   // R12
+#pragma unroll
+    for (int f = 0; f < 4; ++f) dx[cc][f] = fma(k2, gr[2][f], fma(k1, gr[1][f], k0 * gr[0][f]));   // Eq. 32
+  }
+  const double div = dx[0][0] + dx[1][1] + dx[2][2];
+  const double txx = fma(2.0 * mu, dx[0][0], lam * div), tyy = fma(2.0 * mu, dx[1][1], lam * div),
+               tzz = fma(2.0 * mu, dx[2][2], lam * div);
+  const double txy = mu * (dx[1][0] + dx[0][1]), txz = mu * (dx[2][0] + dx[0][2]), tyz = mu * (dx[2][1] + dx[1][2]);
+  const double bx = fma(kap, dx[0][3], fma(val[2], txz, fma(val[1], txy, val[0] * txx)));
+  const double by = fma(kap, dx[1][3], fma(val[2], tyz, fma(val[1], tyy, val[0] * txy)));
+  const double bz = fma(kap, dx[2][3], fma(val[2], tzz, fma(val[1], tyz, val[0] * txz)));
+  F[1] -= fma(mz, txz, fma(my, txy, mx * txx));
+  F[2] -= fma(mz, tyz, fma(my, tyy, mx * txy));
+  F[3] -= fma(mz, tzz, fma(my, tyz, mx * txz));
+  F[4] -= fma(mz, bz, fma(my, by, mx * bx));
+}
+
 template <int DIR, bool VISC>
 struct FluxCfg {
   static constexpr int TS = (DIR == 0) ? 32 : 15;   // cells along the sweep direction per tile
@@ -196,113 +302,25 @@ __global__ void __launch_bounds__(FluxCfg<DIR, VISC>::NT) k_flux(Consts c, FluxI
     const double mt = in.mt ? __ldg(in.mt + af) : 0.0;
     double F[5];
     {
-      const double g2 = fma(mx, mx, fma(my, my, mz * mz));
-      const double g = sqrt(g2), ig = 1.0 / g;
-      Eig e;
-      e.nx = mx * ig; e.ny = my * ig; e.nz = mz * ig;
-      // cells i-1..i+2 = tile cells sI-2..sI+1 -> sP positions sI+4..sI+7
-      const double* pP = sP + sidx<DIR, TT>(0, sI + 4, t, LP);
-      const double* pP1 = sP1 + sidx<DIR, TT>(0, sI, t, L1);
-      const double* pP2 = sP2 + sidx<DIR, TT>(0, sI, t, L2);
       constexpr int FP = (DIR == 0) ? TT * LP : LP * TT;   // field strides
       constexpr int F1 = (DIR == 0) ? TT * L1 : L1 * TT;
       constexpr int F2 = (DIR == 0) ? TT * L2 : L2 * TT;
-      const double rb = 0.5 * (pP[SS_] + pP[2 * SS_]);
-      const double pb = 0.5 * (pP[4 * FP + SS_] + pP[4 * FP + 2 * SS_]);
-      const double irb = 1.0 / rb;
-      e.a2 = c.gamma * pb * irb;
-      const double a = sqrt(e.a2), ia = 1.0 / a;
-      e.ra = rb * a;
-      const double ia2 = ia * ia, h_ira = 0.5 * irb * ia;
-      double W[4][5], D1[5], D2[5], WL[5], WR[5];
-#pragma unroll
-      for (int cidx = 0; cidx < 4; ++cidx)
-        project(e, pP[cidx * SS_], pP[FP + cidx * SS_], pP[2 * FP + cidx * SS_], pP[3 * FP + cidx * SS_],
-                pP[4 * FP + cidx * SS_], W[cidx]);
-      project(e, pP2[SS_], pP2[F2 + SS_], pP2[2 * F2 + SS_], pP2[3 * F2 + SS_], pP2[4 * F2 + SS_], D1);
-      project(e, pP2[2 * SS_], pP2[F2 + 2 * SS_], pP2[2 * F2 + 2 * SS_], pP2[3 * F2 + 2 * SS_], pP2[4 * F2 + 2 * SS_], D2);
-      {
-        double G0[5], G1[5];
-        project(e, pP1[0], pP1[F1], pP1[2 * F1], pP1[3 * F1], pP1[4 * F1], G0);
-        project(e, pP1[SS_], pP1[F1 + SS_], pP1[2 * F1 + SS_], pP1[3 * F1 + SS_], pP1[4 * F1 + SS_], G1);
-#pragma unroll
-        for (int r = 0; r < 5; ++r) {   // Eq. 21-22
-          WL[r] = W[1][r] + 0.5 * G0[r] + D1[r] / 12.0;
-          WR[r] = W[2][r] - 0.5 * G1[r] + D2[r] / 12.0;
-        }
-      }
-      unsigned fl = 0;
-#pragma unroll
-      for (int r = 0; r < 5; ++r) {
-        if (mp_test(WL[r], W[1][r], W[0][r], W[2][r], c.mp_alpha)) fl |= 1u << r;
-        if (mp_test(WR[r], W[2][r], W[3][r], W[1][r], c.mp_alpha)) fl |= 32u << r;
-      }
+      const unsigned fl = inviscid_face<SS_, FP, F1, F2>(c, sP + sidx<DIR, TT>(0, sI + 4, t, LP), sP1 + sidx<DIR, TT>(0, sI, t, L1),
+                                                         sP2 + sidx<DIR, TT>(0, sI, t, L2), mx, my, mz, mt, F);
       if (valid && (sI < TS || s0 + sI == nd)) { nlim += __popc(fl); ntst += 10; }   // tile-shared faces once
-      if (__any_sync(__activemask(), fl != 0)) {
-        double D0[5], D3[5];
-        project(e, pP2[0], pP2[F2], pP2[2 * F2], pP2[3 * F2], pP2[4 * F2], D0);
-        project(e, pP2[3 * SS_], pP2[F2 + 3 * SS_], pP2[2 * F2 + 3 * SS_], pP2[3 * F2 + 3 * SS_], pP2[4 * F2 + 3 * SS_], D3);
-#pragma unroll
-        for (int r = 0; r < 5; ++r) {
-          const double dmid = minmod(D1[r], D2[r]);
-          WL[r] = mp_full(WL[r], W[1][r], W[0][r], W[2][r], dmid, minmod(D0[r], D1[r]), c.mp_alpha, (fl >> r) & 1u);
-          WR[r] = mp_full(WR[r], W[2][r], W[3][r], W[1][r], dmid, minmod(D2[r], D3[r]), c.mp_alpha, (fl >> (r + 5)) & 1u);
-        }
-      }
-      double PL[5], PR[5];
-      backproject(e, ia2, h_ira, WL, PL);
-      backproject(e, ia2, h_ira, WR, PR);
-      hllc(PL, PR, mx, my, mz, mt, g, g2, ig * ig, c.gamma, F);
     }
     if (VISC) {
-      // alpha-damping viscous flux, Eq. 29-35; cells L = sI-1, R = sI
       constexpr int FP = (DIR == 0) ? TT * LP : LP * TT;
       constexpr int F1 = (DIR == 0) ? TT * L1 : L1 * TT;
-      const double* pP = sP + sidx<DIR, TT>(0, sI + 5, t, LP);
-      const double* pP1 = sP1 + sidx<DIR, TT>(0, sI, t, L1);
       const int cl = fs - 1;
       long long agL, agS;
       if (DIR == 0) { agL = c.LG.at(cl, ct, o); agS = 1; }
       else if (DIR == 1) { agL = c.LG.at(ct, cl, o); agS = c.LG.sj; }
       else { agL = c.LG.at(ct, o, cl); agS = c.LG.sk; }
-      double val[4], gr[3][4];
-#pragma unroll
-      for (int f = 0; f < 4; ++f) {
-        const int pf = (f < 3) ? f + 1 : 5;
-        const double gL = pP1[pf * F1], gR = pP1[pf * F1 + SS_];
-        const double phL = fma(0.5, gL, pP[pf * FP]);            // Eq. 30 (beta^D = 0)
-        const double phR = fma(-0.5, gR, pP[pf * FP + SS_]);     // Eq. 31
-#pragma unroll
-        for (int e = 0; e < 3; ++e) {
-          if (e == DIR) gr[e][f] = fma(2.0, phR - phL, 0.5 * (gL + gR));   // Eq. 29, alpha^D = 4
-          else gr[e][f] = 0.5 * (__ldg(in.G[4 * e + f] + agL) + __ldg(in.G[4 * e + f] + agL + agS));   // R11
-        }
-        val[f] = 0.5 * (phL + phR);
-      }
-      const double mu = sutherland(c, val[3]);
-      const double lam = -2.0 / 3.0 * mu, kap = mu * c.kappa_fac;
-      const double irj = 1.0 / __ldg(in.m[9] + af);
-      double mh[9];
-#pragma unroll
-      for (int q = 0; q < 9; ++q) mh[q] = (q / 3 == DIR) ? ((q % 3 == 0) ? mx : (q % 3 == 1) ? my : mz) : __ldg(in.m[q] + af);
-      double dx[3][4];
-#pragma unroll
-      for (int cc = 0; cc < 3; ++cc) {
-        const double k0 = mh[cc] * irj, k1 = mh[3 + cc] * irj, k2 = mh[6 + cc] * irj;   // R12
-#pragma unroll
-        for (int f = 0; f < 4; ++f) dx[cc][f] = fma(k2, gr[2][f], fma(k1, gr[1][f], k0 * gr[0][f]));   // Eq. 32
-      }
-      const double div = dx[0][0] + dx[1][1] + dx[2][2];
-      const double txx = fma(2.0 * mu, dx[0][0], lam * div), tyy = fma(2.0 * mu, dx[1][1], lam * div),
-                   tzz = fma(2.0 * mu, dx[2][2], lam * div);
-      const double txy = mu * (dx[1][0] + dx[0][1]), txz = mu * (dx[2][0] + dx[0][2]), tyz = mu * (dx[2][1] + dx[1][2]);
-      const double bx = fma(kap, dx[0][3], fma(val[2], txz, fma(val[1], txy, val[0] * txx)));
-      const double by = fma(kap, dx[1][3], fma(val[2], tyz, fma(val[1], tyy, val[0] * txy)));
-      const double bz = fma(kap, dx[2][3], fma(val[2], tzz, fma(val[1], tyz, val[0] * txz)));
-      F[1] -= fma(mz, txz, fma(my, txy, mx * txx));   // Res = -(F - Fv) differences (Eq. 8-9)
-      F[2] -= fma(mz, tyz, fma(my, tyy, mx * txy));
-      F[3] -= fma(mz, tzz, fma(my, tyz, mx * txz));
-      F[4] -= fma(mz, bz, fma(my, by, mx * bx));
+      auto getG = [&](int e, int f, int cell) { return __ldg(in.G[4 * e + f] + agL + cell * agS); };
+      auto getM = [&](int q) { return __ldg(in.m[q] + af); };
+      viscous_face<DIR, SS_, FP, F1>(c, sP + sidx<DIR, TT>(0, sI + 5, t, LP), sP1 + sidx<DIR, TT>(0, sI, t, L1),
+                                     mx, my, mz, getG, getM, F);
     }
 #pragma unroll
     for (int f = 0; f < 5; ++f) sF[sidx<DIR, TT>(f, sI, t, LF)] = F[f];
@@ -317,20 +335,19 @@ __global__ void __launch_bounds__(FluxCfg<DIR, VISC>::NT) k_flux(Consts c, FluxI
   }
   __syncthreads();
   // ---- flux difference, Eq. 25: Res_i -= F_{i+1/2} - F_{i-1/2} ----
-  const long long N = c.LC.n;
   for (int item = tid; item < TT * TS; item += NT) {
     int s, t;
     if (DIR == 0) { s = item % TS; t = item / TS; }
     else { t = item % TT; s = item / TT; }
     if (s0 + s >= nd || t0 + t >= nt) continue;
     long long ac;
-    if (DIR == 0) ac = c.LC.at(s0 + s, t0 + t, o);
-    else if (DIR == 1) ac = c.LC.at(t0 + t, s0 + s, o);
-    else ac = c.LC.at(t0 + t, o, s0 + s);
+    if (DIR == 0) ac = c.LR.at(s0 + s, t0 + t, o);
+    else if (DIR == 1) ac = c.LR.at(t0 + t, s0 + s, o);
+    else ac = c.LR.at(t0 + t, o, s0 + s);
 #pragma unroll
     for (int f = 0; f < 5; ++f) {
       const double dF = sF[sidx<DIR, TT>(f, s + 1, t, LF)] - sF[sidx<DIR, TT>(f, s, t, LF)];
-      double* rp = in.res + f * N + ac;
+      double* rp = in.res + f * c.fsR + ac;
       *rp = in.first ? -dF : *rp - dF;
     }
   }
