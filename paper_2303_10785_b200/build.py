@@ -26,6 +26,7 @@ def build(force=False, verbose=False):
     arch = ["-gencode", "arch=compute_100a,code=sm_100a", "-std=c++17", "-O3", "-lineinfo", "-Xcompiler", "-fPIC"]
     if verbose:
         arch.append("-Xptxas=-v")
+    arch += os.environ.get("MEG6_NVCC_FLAGS", "").split()
     objs = []
     # the metric kernels are compiled without FMA contraction (see meg6_geom.cuh); the rest with it
     for src, extra in (("meg6_geom.cu", ["-fmad=false"]), ("meg6.cu", [])):

@@ -37,11 +37,26 @@ __device__ __forceinline__ void tma_load_4d(void* dst, const CUtensorMap* tm, ui
       ::"r"(smem_u32(dst)), "l"((uint64_t)tm), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
 }
 
+// Tile shape (tunable at build time).  Several small CTAs per SM: while one waits on its TMA boxes the others compute.
+#ifndef MEG6_TT_X
+#define MEG6_TT_X 4     // xi sweep: rows (j) per tile
+#endif
+#ifndef MEG6_TT_Y
+#define MEG6_TT_Y 8     // eta/zeta sweep: i-lanes per tile
+#endif
+#ifndef MEG6_MINB_X
+#define MEG6_MINB_X 3
+#endif
+#ifndef MEG6_MINB_Y
+#define MEG6_MINB_Y 4
+#endif
+
 template <int DIR, bool VISC>
 struct TmaCfg {
   static constexpr int TS = (DIR == 0) ? 32 : 15;
-  static constexpr int TT = (DIR == 0) ? 8 : 32;
-  static constexpr int NT = (DIR == 0) ? 288 : 256;
+  static constexpr int TT = (DIR == 0) ? MEG6_TT_X : MEG6_TT_Y;
+  static constexpr int NT = (DIR == 0) ? 36 * MEG6_TT_X : 16 * MEG6_TT_Y;
+  static constexpr int MINB = (DIR == 0) ? MEG6_MINB_X : MEG6_MINB_Y;
   static constexpr int NF = VISC ? 6 : 5;
   static constexpr int NM = VISC ? 10 : 3;
   static constexpr int LP = TS + 12, L1 = TS + 2, L2 = TS + 4;
@@ -66,7 +81,7 @@ struct FluxIn2 {
 };
 
 template <int DIR, bool VISC>
-__global__ void __launch_bounds__(TmaCfg<DIR, VISC>::NT) k_flux_tma(const Consts c, const FluxIn2 in,
+__global__ void __launch_bounds__(TmaCfg<DIR, VISC>::NT, TmaCfg<DIR, VISC>::MINB) k_flux_tma(const Consts c, const FluxIn2 in,
                                                                     const __grid_constant__ TmaMaps tm) {
   using C = TmaCfg<DIR, VISC>;
   constexpr int TS = C::TS, TT = C::TT, NF = C::NF, NM = C::NM, LP = C::LP, L1 = C::L1, L2 = C::L2, LF = C::LF,
@@ -130,8 +145,8 @@ __global__ void __launch_bounds__(TmaCfg<DIR, VISC>::NT) k_flux_tma(const Consts
 
   // thread -> (sweep position, transverse position) without runtime divisions
   int col, row, nrow_step;
-  if (DIR == 0) { col = tid % 36; row = tid / 36; nrow_step = 0; }   // 8 rows x 36 sweep positions
-  else { row = tid & 31; col = tid >> 5; nrow_step = 8; }            // 32 lanes x 8 warps over the sweep
+  if (DIR == 0) { col = tid % 36; row = tid / 36; nrow_step = 0; }   // TT rows x 36 sweep positions
+  else { row = tid % TT; col = tid / TT; nrow_step = C::NT / TT; }    // TT lanes x NT/TT sweep positions
 
   // ---- E6 first gradients (Eq. 17) on cells -1..TS, Eq. 19 second derivatives on cells -2..TS+1 ----
   for (int a = col; a < L2; a += (DIR == 0 ? 36 : nrow_step)) {
