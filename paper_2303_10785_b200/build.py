@@ -5,7 +5,7 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(CSRC, "libmeg6.so")
-SOURCES = ["meg6.cu", "meg6_geom.cu", "meg6_common.cuh", "meg6_geom.cuh", "meg6_flow.cuh", "meg6_flux.cuh"]
+SOURCES = sorted(f for f in os.listdir(CSRC) if f.endswith((".cu", ".cuh")))
 HEADER = os.path.join(HERE, "..", "include", "meg6.h")
 
 

@@ -9,6 +9,7 @@
 #include "meg6_flow.cuh"
 #include "meg6_flux.cuh"
 #include "meg6_flux_tma.cuh"
+#include "meg6_flux3.cuh"
 #include <stdlib.h>
 
 using namespace meg6;
@@ -53,6 +54,8 @@ static Consts make_consts(const meg6_params* p) {
   c.mu_ref = p->mu_ref; c.t_ref = p->t_ref; c.s_suth = p->s_suth;
   c.mp_alpha = p->mp_alpha; c.p_out = p->p_out;
   c.kappa_fac = p->viscous ? p->gamma * p->r_gas / ((p->gamma - 1.0) * p->prandtl) : 0.0;
+  c.igm1 = 1.0 / (p->gamma - 1.0);
+  c.suth_c = (p->viscous && p->s_suth >= 0.0) ? p->mu_ref * (p->t_ref + p->s_suth) / (p->t_ref * sqrt(p->t_ref)) : 0.0;
   c.LX = make_lay(p->ni, p->nj, p->nk, GX, GX, GX);
   // row pitches are even so that every TMA global stride is a multiple of 16 bytes
   c.LP = make_lay(p->ni, p->nj, p->nk, GPI, GPJ, GPK, 2);
@@ -162,6 +165,34 @@ static bool make_maps_dir(EncodeTiledFn fn, meg6_grid* g) {
   return ok;
 }
 
+template <int DIR, bool VISC>
+static bool make_maps3_dir(EncodeTiledFn fn, meg6_grid* g) {
+  using C = Cfg3<DIR, VISC>;
+  const Consts& c = g->c;
+  TmaMaps& t = g->tmaps3[DIR];
+  auto box = [](int sweep, int trans, int nf, int out[4]) {
+    if (DIR == 0) { out[0] = sweep; out[1] = trans; out[2] = 1; }
+    else if (DIR == 1) { out[0] = trans; out[1] = sweep; out[2] = 1; }
+    else { out[0] = trans; out[1] = 1; out[2] = sweep; }
+    out[3] = nf;
+  };
+  int b[4];
+  bool ok = true;
+  box(C::LP, C::TT, C::NF, b);
+  ok = ok && make_map4(fn, &t.P, g->P[0], c.LP, c.fsP, 6, b);
+  box(C::LF, C::TT, C::NM, b);
+  ok = ok && make_map4(fn, &t.M, VISC ? g->fmet[DIR][0] : g->fmet[DIR][3 * DIR], c.LF[DIR], c.fsM[DIR], C::NM, b);
+  if (g->p.moving) {
+    box(C::LF, C::TT, 1, b);
+    ok = ok && make_map4(fn, &t.Mt, g->fmt[DIR], c.LF[DIR], c.fsM[DIR], 1, b);
+  }
+  if (VISC) {
+    box(C::LG, C::TT, 4, b);
+    ok = ok && make_map4(fn, &t.G, g->G[0][0], c.LG, c.fsG, 12, b);
+  }
+  return ok;
+}
+
 static cudaError_t setup_tma(meg6_grid* g) {
   g->use_tma = 0;
   const char* env = getenv("MEG6_FLUX");
@@ -175,13 +206,20 @@ static cudaError_t setup_tma(meg6_grid* g) {
   bool ok;
   if (g->p.viscous) ok = make_maps_dir<0, true>(fn, g) && make_maps_dir<1, true>(fn, g) && make_maps_dir<2, true>(fn, g);
   else ok = make_maps_dir<0, false>(fn, g) && make_maps_dir<1, false>(fn, g) && make_maps_dir<2, false>(fn, g);
+  if (g->p.viscous) ok = ok && make_maps3_dir<0, true>(fn, g) && make_maps3_dir<1, true>(fn, g) && make_maps3_dir<2, true>(fn, g);
+  else ok = ok && make_maps3_dir<0, false>(fn, g) && make_maps3_dir<1, false>(fn, g) && make_maps3_dir<2, false>(fn, g);
   if (!ok) return cudaErrorInvalidValue;
+#define SET_SMEM3(D, V)                                                                                     \
+  if ((e = cudaFuncSetAttribute(k_flux3<D, V>, cudaFuncAttributeMaxDynamicSharedMemorySize,                 \
+                                Cfg3<D, V>::SMEM_BYTES)) != cudaSuccess) return e;
+  SET_SMEM3(0, false) SET_SMEM3(1, false) SET_SMEM3(2, false) SET_SMEM3(0, true) SET_SMEM3(1, true) SET_SMEM3(2, true)
+#undef SET_SMEM3
 #define SET_SMEM(D, V)                                                                                      \
   if ((e = cudaFuncSetAttribute(k_flux_tma<D, V>, cudaFuncAttributeMaxDynamicSharedMemorySize,              \
                                 TmaCfg<D, V>::SMEM_BYTES)) != cudaSuccess) return e;
   SET_SMEM(0, false) SET_SMEM(1, false) SET_SMEM(2, false) SET_SMEM(0, true) SET_SMEM(1, true) SET_SMEM(2, true)
 #undef SET_SMEM
-  g->use_tma = 1;
+  g->use_tma = (env && strcmp(env, "v2") == 0) ? 1 : 2;   // 2: k_flux3 (default); 1: second-generation TMA kernel
   return cudaSuccess;
 }
 
@@ -349,7 +387,22 @@ static meg6_status residual(meg6_grid* g, const double* U) {
     in.first = (d == 0);
     const bool V = g->p.viscous != 0;
     ProfScope ps(g, 4 + d, 1);
-    if (g->use_tma) {
+    if (g->use_tma == 2) {
+      FluxIn3 i3;
+      i3.res = g->res; i3.stats = in.stats; i3.first = in.first; i3.moving = g->p.moving ? 1 : 0;
+#define LAUNCH3(D, VV, GRID) k_flux3<D, VV><<<GRID, Cfg3<D, VV>::NT, Cfg3<D, VV>::SMEM_BYTES, g->stream>>>(c, i3, g->tmaps3[D])
+      if (d == 0) {
+        dim3 grid(nblk(c.n[0], Cfg3<0, false>::TS), nblk(c.n[1], Cfg3<0, false>::TT), c.n[2]);
+        if (V) LAUNCH3(0, true, grid); else LAUNCH3(0, false, grid);
+      } else if (d == 1) {
+        dim3 grid(nblk(c.n[0], Cfg3<1, false>::TT), nblk(c.n[1], Cfg3<1, false>::TS), c.n[2]);
+        if (V) LAUNCH3(1, true, grid); else LAUNCH3(1, false, grid);
+      } else {
+        dim3 grid(nblk(c.n[0], Cfg3<2, false>::TT), c.n[1], nblk(c.n[2], Cfg3<2, false>::TS));
+        if (V) LAUNCH3(2, true, grid); else LAUNCH3(2, false, grid);
+      }
+#undef LAUNCH3
+    } else if (g->use_tma) {
       FluxIn2 i2;
       i2.res = g->res; i2.stats = in.stats; i2.first = in.first; i2.moving = g->p.moving ? 1 : 0;
       i2.dbg = getenv("MEG6_DBG") ? atoi(getenv("MEG6_DBG")) : 0;

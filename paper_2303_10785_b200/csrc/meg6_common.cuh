@@ -58,6 +58,8 @@ struct Consts {   // per-grid constants passed by value to kernels
   int bc[6];
   double gamma, r_gas, prandtl, mu_ref, t_ref, s_suth, mp_alpha, p_out;
   double kappa_fac;   // gamma r_gas / ((gamma-1) Pr)
+  double igm1;        // 1/(gamma-1)
+  double suth_c;      // mu_ref (t_ref + s_suth) / t_ref^1.5: mu = suth_c T sqrt(T)/(T + s_suth)  (R15)
   Lay LX, LP, LG, LC; // coordinates/metrics, primitives, gradients, interior cells (caller's U layout)
   Lay LR;             // residual accumulator: interior cells, even row pitch (TMA strides are multiples of 16 B)
   Lay LF[3];          // interface families
@@ -70,7 +72,8 @@ namespace meg6 { struct TmaMaps { CUtensorMap P, M, Mt, G, R; }; }
 
 struct meg6_grid {
   meg6_params p;
-  meg6::TmaMaps tmaps[3];   // per sweep direction
+  meg6::TmaMaps tmaps[3];   // per sweep direction (second-generation kernel, A/B only)
+  meg6::TmaMaps tmaps3[3];  // per sweep direction (k_flux3)
   int use_tma;
   meg6::Consts c;
   cudaStream_t stream;

@@ -1,0 +1,453 @@
+// meg6_flux3.cuh -- per-direction flux kernel, third generation (sm_100a).
+//
+// Same method as meg6_flux.cuh (Fig. 3 P:204-262 and Fig. 5), reorganised after the first ncu pass
+// (profiles/r1a_*: latency/issue bound at 14 warps per SM, 60 % of the issued instructions not FP64):
+//   * the tile computes, per cell, the two one-sided reconstruction offsets of Eq. 16/21-22
+//        aL = +1/2 P' + P''/12,   aR = -1/2 P' + P''/12        (P' Eq. 17, P'' Eq. 19)
+//     once in shared memory; P'' of a cell is recovered as 6 (aL + aR), P' as aL - aR;
+//   * the characteristic step works on DIFFERENCES (c0 - cm, cp - c0, W_unlimited - c0): every formula of
+//     App. E is invariant under a shift of all its arguments, and the projection is linear (frozen matrix,
+//     Eq. 20), so five projections replace eight and the limited state is P_cell + R (limited offset);
+//   * reciprocals are shared (1/(a b) gives 1/a and 1/b), rsqrt replaces sqrt + divide;
+//   * shared memory is addressed as shared (LDS with immediate offsets), the flux tile aliases the metric tile,
+//     the running residual is read from global memory in the final phase: 5 CTAs of 4 warps per SM.
+// Results differ from the step-by-step order of the oracle at round-off level only.
+#pragma once
+#include <cuda.h>
+#include "meg6_common.cuh"
+
+namespace meg6 {
+
+#ifndef MEG6_MINB3_X
+#define MEG6_MINB3_X 5
+#endif
+#ifndef MEG6_MINB3_Y
+#define MEG6_MINB3_Y 5
+#endif
+
+template <int DIR, bool VISC>
+struct Cfg3 {
+  static constexpr int TS = (DIR == 0) ? 30 : 15;            // cells along the sweep per tile
+  static constexpr int TT = (DIR == 0) ? 4 : 8;              // transverse positions (rows for xi, i-lanes otherwise)
+  static constexpr int NI = TS + 1;                          // interfaces per pencil
+  static constexpr int NT = (DIR == 0) ? 32 * TT : NI * TT;  // threads: one interface each (xi: one warp per row)
+  static constexpr int MINB = (DIR == 0) ? MEG6_MINB3_X : MEG6_MINB3_Y;
+  static constexpr int NF = VISC ? 6 : 5;                    // staged fields (T only for the viscous flux)
+  static constexpr int NM = VISC ? 10 : 3;                   // interface metrics loaded
+  static constexpr int NMF = NM > 5 ? NM : 5;                // the metric region later receives the 5 fluxes
+  static constexpr int LP = TS + 12;                         // P: cells -6 .. TS+5
+  static constexpr int LA = TS + 4;                          // aL/aR: cells -2 .. TS+1
+  static constexpr int LT = TS + 2;                          // T': cells -1 .. TS
+  static constexpr int LF = (DIR == 0) ? TS + 2 : TS + 1;    // interface rows (xi: even length, TMA box bytes % 16)
+  static constexpr int LG = (DIR == 0) ? TS + 4 : TS + 2;    // stored gradients: cells -1..TS (xi: box starts at -2)
+  static constexpr int GOFF = (DIR == 0) ? 1 : 0;
+  static constexpr int nP = NF * LP * TT, nA = 10 * LA * TT, nT1 = VISC ? LT * TT : 0, nM = NMF * LF * TT,
+                       nMt = LF * TT, nG = VISC ? 8 * LG * TT : 0;
+  static constexpr int al(int n) { return (n + 15) / 16 * 16; }   // 128-byte granules (TMA destinations)
+  static constexpr int oP = 0, oM = oP + al(nP), oMt = oM + al(nM), oG = oMt + al(nMt), oA = oG + al(nG),
+                       oT1 = oA + al(nA), oBar = oT1 + al(nT1);
+  static constexpr int SMEM_BYTES = (oBar + 2) * 8;
+};
+
+template <int DIR, int TT>
+__device__ __forceinline__ int sidx3(int f, int a, int t, int LA) {
+  return (DIR == 0) ? (f * TT + t) * LA + a : (f * LA + a) * TT + t;
+}
+
+struct FluxIn3 {
+  double* res;                  // [5] running residual, layout LR, field stride fsR
+  unsigned long long* stats;    // limiter counters or null
+  int first, moving;
+};
+
+__device__ __forceinline__ uint32_t smem_u32_3(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void tma4(void* dst, const CUtensorMap* tm, uint64_t* bar, int c0, int c1, int c2, int c3) {
+  asm volatile(
+      "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"
+      ::"r"(smem_u32_3(dst)), "l"((uint64_t)tm), "r"(smem_u32_3(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
+}
+
+__device__ __forceinline__ double minmod3(double a, double b) {   // E.2
+  const double m = fmin(fabs(a), fabs(b));
+  const bool same = ((__double2hiint(a) ^ __double2hiint(b)) >= 0);
+  return same ? copysign(m, a) : 0.0;
+}
+
+struct Eig3 { double nx, ny, nz, ra, a2; };
+
+// W = Linv * P (A.6a; R6)
+__device__ __forceinline__ void project3(const Eig3& e, double r, double u, double v, double w, double p, double W[5]) {
+  const double un = fma(e.nz, w, fma(e.ny, v, e.nx * u));
+  W[0] = fma(-e.ra, un, p);
+  W[4] = fma(e.ra, un, p);
+  const double q = fma(e.a2, r, -p);
+  W[1] = fma(e.nx, q, fma(e.ny, w, -e.nz * v));
+  W[2] = fma(e.nz, q, fma(e.nx, v, -e.ny * u));
+  W[3] = fma(-e.ny, q, fma(e.nx, w, -e.nz * u));
+}
+
+// P = base + Rmat * W (A.4b; R6)
+__device__ __forceinline__ void backproject3(const Eig3& e, double ia2, double h_ira, const double W[5], const double B[5],
+                                             double P[5]) {
+  const double sp = W[0] + W[4];
+  P[0] = fma(ia2, fma(0.5, sp, fma(e.nx, W[1], fma(e.nz, W[2], -e.ny * W[3]))), B[0]);
+  const double s = h_ira * (W[4] - W[0]);
+  P[1] = B[1] + fma(e.nx, s, -fma(e.ny, W[2], e.nz * W[3]));
+  P[2] = B[2] + fma(e.ny, s, fma(e.nx, W[2], -e.nz * W[1]));
+  P[3] = B[3] + fma(e.nz, s, fma(e.ny, W[1], e.nx * W[3]));
+  P[4] = fma(0.5, sp, B[4]);
+}
+
+// App. E (R7) in offset form (all quantities relative to c0):
+//   e = W_unlimited - c0, dp = cp - c0, dm = c0 - cm; returns the limited offset.
+__device__ __forceinline__ double mp_limit3(double e, double dp, double dm, double dnear, double dfar, double alpha) {
+  const double wmd = 0.5 * (dp - dnear);
+  const double wul = alpha * dm;
+  const double wlc = fma(4.0 / 3.0, dfar, 0.5 * dm);
+  const double wmin = fmax(fmin(fmin(0.0, dp), wmd), fmin(fmin(0.0, wul), wlc));
+  const double wmax = fmin(fmax(fmax(0.0, dp), wmd), fmax(fmax(0.0, wul), wlc));
+  return e + minmod3(wmin - e, wmax - e);   // E.4
+}
+
+// Contravariant HLLC, Eq. 26-27 with the flux of Eq. 2; energy row R9; cascade R10.
+#ifndef MEG6_HLLC_MODE
+#define MEG6_HLLC_MODE 2
+#endif
+__device__ __forceinline__ void hllc3(const double PL[5], const double PR[5], double mx, double my, double mz, double mt,
+                                      double g, double g2, double ig2, double gamma, double igm1, double F[5]) {
+  const double UL = fma(mz, PL[3], fma(my, PL[2], fma(mx, PL[1], mt)));
+  const double UR = fma(mz, PR[3], fma(my, PR[2], fma(mx, PR[1], mt)));
+#if MEG6_HLLC_MODE == 1
+  const double cL = sqrt(gamma * PL[4] / PL[0]) * g, cR = sqrt(gamma * PR[4] / PR[0]) * g;
+#else
+  const double t = 1.0 / (PL[0] * PR[0]);
+  const double irL = PR[0] * t, irR = PL[0] * t;
+  const double cL = sqrt(gamma * PL[4] * irL) * g, cR = sqrt(gamma * PR[4] * irR) * g;
+#endif
+  const double SL = fmin(UL - cL, UR - cR);
+  const double SR = fmax(UL + cL, UR + cR);
+  const double mL = PL[0] * (SL - UL), mR = PR[0] * (SR - UR);
+  const double SS = (fma(mR, UR, -mL * UL) + (PL[4] - PR[4]) * g2) / (mR - mL);
+  const bool left = (SL >= 0.0) || (SS >= 0.0);
+  const bool star = !(SL >= 0.0) && ((SS >= 0.0) || (SR >= 0.0));
+  const double r = left ? PL[0] : PR[0], u = left ? PL[1] : PR[1], v = left ? PL[2] : PR[2];
+  const double w = left ? PL[3] : PR[3], p = left ? PL[4] : PR[4];
+  const double UK = left ? UL : UR, SK = left ? SL : SR;
+  const double E = fma(p, igm1, 0.5 * r * fma(u, u, fma(v, v, w * w)));
+  const double ru = r * UK;
+  F[0] = ru;
+  F[1] = fma(ru, u, mx * p);
+  F[2] = fma(ru, v, my * p);
+  F[3] = fma(ru, w, mz * p);
+  F[4] = fma(E + p, UK, -mt * p);
+  if (star) {
+    const double dS = SK - UK, dK = SK - SS, dSU = SS - UK;
+#if MEG6_HLLC_MODE == 1
+    // the quotients exactly as Eq. 27 states them
+    const double fac = r * dS / dK;
+    const double dU = dSU * ig2;
+    const double q1 = fac * fma(mx, dU, u), q2 = fac * fma(my, dU, v), q3 = fac * fma(mz, dU, w);
+    const double q4 = fac * (E / r + dSU * ((SS - mt) * ig2 + p / (r * dS)));
+    F[0] = fma(SK, fac - r, F[0]);
+    F[1] = fma(SK, q1 - r * u, F[1]);
+    F[2] = fma(SK, q2 - r * v, F[2]);
+    F[3] = fma(SK, q3 - r * w, F[3]);
+    F[4] = fma(SK, q4 - E, F[4]);
+#else
+    // Q*_K - Q_K without cancellation: fac - rho_K = rho_K (S* - U_K)/(S_K - S*), and
+    // fac (S*-U_K) p/(rho_K (S_K-U_K)) = p (S*-U_K)/(S_K-S*)
+    const double idK = 1.0 / dK;
+    const double k = dSU * idK;              // (S* - U_K)/(S_K - S*)
+    const double rk = r * k;                 // fac - rho_K
+    const double fd = (r + rk) * dSU * ig2;  // fac (S* - U_K)/g^2
+    F[0] = fma(SK, rk, F[0]);
+    F[1] = fma(SK, fma(rk, u, fd * mx), F[1]);
+    F[2] = fma(SK, fma(rk, v, fd * my), F[2]);
+    F[3] = fma(SK, fma(rk, w, fd * mz), F[3]);
+    F[4] = fma(SK, fma(k, E + p, fd * (SS - mt)), F[4]);
+#endif
+  }
+}
+
+// One interface: O3 steps 1-8 (inviscid, Fig. 3) and O4 (alpha-damping viscous flux, Fig. 5; subtracted from F).
+//   pP   : field 0 (rho) of cell L-1 in the primitive tile        (cells L-1, L, R, R+1 at +0..3 SS)
+//   pA   : aL field 0 of cell L-1 in the offset tile              (aR fields are 5 FA further)
+//   pT1  : T' of cell L;  pG: stored tangential gradients at cell L;  pM: interface metrics (field stride FM)
+// SS = stride between consecutive cells along the sweep; FP/FA/FG/FM = field strides.
+// Returns the E.1 flags (bit r: left state of component r limited, bit 5+r: right state).
+template <int DIR, bool VISC, int SS, int FP, int FA, int FG, int FM>
+__device__ __forceinline__ unsigned face3(const Consts& c, const double* __restrict__ pP, const double* __restrict__ pA,
+                                          const double* __restrict__ pT1, const double* __restrict__ pG,
+                                          const double* __restrict__ pM, double mt, double F[5]) {
+  constexpr int q0 = VISC ? 3 * DIR : 0;
+  const double mx = pM[q0 * FM], my = pM[(q0 + 1) * FM], mz = pM[(q0 + 2) * FM];
+  const double g2 = fma(mx, mx, fma(my, my, mz * mz));
+  const double ig = rsqrt(g2), g = g2 * ig, ig2 = ig * ig;
+  Eig3 e;
+  e.nx = mx * ig; e.ny = my * ig; e.nz = mz * ig;
+  double BL[5], BR[5];   // cell values L, R
+#pragma unroll
+  for (int f = 0; f < 5; ++f) { BL[f] = pP[f * FP + SS]; BR[f] = pP[f * FP + 2 * SS]; }
+  const double rb = 0.5 * (BL[0] + BR[0]), pb = 0.5 * (BL[4] + BR[4]);   // R5
+  const double irb = 1.0 / rb;
+  e.a2 = c.gamma * pb * irb;
+  const double ia = rsqrt(e.a2), a = e.a2 * ia;
+  e.ra = rb * a;
+  const double ia2 = ia * ia, h_ira = 0.5 * irb * ia;
+  double Wm[5], W0[5], Wp[5], EL[5], ER[5];
+  project3(e, BL[0] - pP[0], BL[1] - pP[FP], BL[2] - pP[2 * FP], BL[3] - pP[3 * FP], BL[4] - pP[4 * FP], Wm);
+  project3(e, BR[0] - BL[0], BR[1] - BL[1], BR[2] - BL[2], BR[3] - BL[3], BR[4] - BL[4], W0);
+  project3(e, pP[3 * SS] - BR[0], pP[FP + 3 * SS] - BR[1], pP[2 * FP + 3 * SS] - BR[2], pP[3 * FP + 3 * SS] - BR[3],
+           pP[4 * FP + 3 * SS] - BR[4], Wp);
+  // Eq. 21-22 as offsets from the cell value
+  project3(e, pA[SS], pA[FA + SS], pA[2 * FA + SS], pA[3 * FA + SS], pA[4 * FA + SS], EL);
+  project3(e, pA[5 * FA + 2 * SS], pA[6 * FA + 2 * SS], pA[7 * FA + 2 * SS], pA[8 * FA + 2 * SS], pA[9 * FA + 2 * SS], ER);
+  unsigned fl = 0;
+#pragma unroll
+  for (int r = 0; r < 5; ++r) {   // E.1: (W - c0)(W - W^MP) <= 1e-20 accepts
+    const double mmL = minmod3(W0[r], c.mp_alpha * Wm[r]);
+    const double mmR = minmod3(W0[r], c.mp_alpha * Wp[r]);
+    if (!(EL[r] * (EL[r] - mmL) <= 1e-20)) fl |= 1u << r;
+    if (!(ER[r] * (ER[r] + mmR) <= 1e-20)) fl |= 32u << r;
+  }
+  // warp-uniform early accept: the full limiting path runs only if some lane needs it
+  if (__any_sync(__activemask(), fl != 0)) {
+    double Dm[5], DL[5], DR[5], Dp[5];   // projected P'' of cells L-1, L, R, R+1;  P'' = 6 (aL + aR)
+#define MEG6_D2(cell, f) (6.0 * (pA[(f) * FA + (cell) * SS] + pA[((f) + 5) * FA + (cell) * SS]))
+    project3(e, MEG6_D2(0, 0), MEG6_D2(0, 1), MEG6_D2(0, 2), MEG6_D2(0, 3), MEG6_D2(0, 4), Dm);
+    project3(e, MEG6_D2(1, 0), MEG6_D2(1, 1), MEG6_D2(1, 2), MEG6_D2(1, 3), MEG6_D2(1, 4), DL);
+    project3(e, MEG6_D2(2, 0), MEG6_D2(2, 1), MEG6_D2(2, 2), MEG6_D2(2, 3), MEG6_D2(2, 4), DR);
+    project3(e, MEG6_D2(3, 0), MEG6_D2(3, 1), MEG6_D2(3, 2), MEG6_D2(3, 3), MEG6_D2(3, 4), Dp);
+#undef MEG6_D2
+#pragma unroll
+    for (int r = 0; r < 5; ++r) {
+      const double dnear = minmod3(DL[r], DR[r]);
+      const double lL = mp_limit3(EL[r], W0[r], Wm[r], dnear, minmod3(Dm[r], DL[r]), c.mp_alpha);
+      const double lR = mp_limit3(ER[r], -W0[r], -Wp[r], dnear, minmod3(DR[r], Dp[r]), c.mp_alpha);
+      EL[r] = ((fl >> r) & 1u) ? lL : EL[r];
+      ER[r] = ((fl >> (r + 5)) & 1u) ? lR : ER[r];
+    }
+  }
+  double PL[5], PR[5];
+  backproject3(e, ia2, h_ira, EL, BL, PL);   // Eq. 23
+  backproject3(e, ia2, h_ira, ER, BR, PR);
+  hllc3(PL, PR, mx, my, mz, mt, g, g2, ig2, c.gamma, c.igm1, F);
+
+  if (VISC) {
+    // O4: Eq. 29-35.  fields (u,v,w,T); normal gradient with alpha^D = 4, beta^D = 0.
+    double val[4], gr[3][4];
+#pragma unroll
+    for (int f = 0; f < 4; ++f) {
+      double cL, cR, gL, gR;
+      if (f < 3) {
+        cL = BL[f + 1]; cR = BR[f + 1];
+        gL = pA[(f + 1) * FA + SS] - pA[(f + 6) * FA + SS];           // P' = aL - aR
+        gR = pA[(f + 1) * FA + 2 * SS] - pA[(f + 6) * FA + 2 * SS];
+      } else {
+        cL = pP[5 * FP + SS]; cR = pP[5 * FP + 2 * SS];
+        gL = pT1[0]; gR = pT1[SS];
+      }
+      const double phL = fma(0.5, gL, cL);            // Eq. 30
+      const double phR = fma(-0.5, gR, cR);           // Eq. 31
+#pragma unroll
+      for (int d = 0; d < 3; ++d) {
+        if (d == DIR) gr[d][f] = fma(2.0, phR - phL, 0.5 * (gL + gR));   // Eq. 29
+        else {
+          const int slot = (DIR == 0) ? d - 1 : (DIR == 1) ? (d == 0 ? 0 : 1) : d;   // tangential directions in order
+          gr[d][f] = 0.5 * (pG[(4 * slot + f) * FG] + pG[(4 * slot + f) * FG + SS]);   // R11
+        }
+      }
+      val[f] = 0.5 * (phL + phR);
+    }
+    // Sutherland (R15) and 1/(1/J) with one division
+    const double rjh = pM[9 * FM];
+    double mu, irj;
+    if (c.s_suth < 0.0) { mu = c.mu_ref; irj = 1.0 / rjh; }
+    else {
+      const double ts = val[3] + c.s_suth;
+      const double t = 1.0 / (rjh * ts);
+      irj = ts * t;
+      mu = c.suth_c * val[3] * sqrt(val[3]) * (rjh * t);
+    }
+    const double lam = -2.0 / 3.0 * mu, kap = mu * c.kappa_fac;
+    double dx[3][4];
+#pragma unroll
+    for (int cc = 0; cc < 3; ++cc) {
+      double k[3];
+#pragma unroll
+      for (int d = 0; d < 3; ++d) k[d] = ((d == DIR) ? ((cc == 0) ? mx : (cc == 1) ? my : mz) : pM[(3 * d + cc) * FM]) * irj;   // R12
+#pragma unroll
+      for (int f = 0; f < 4; ++f) dx[cc][f] = fma(k[2], gr[2][f], fma(k[1], gr[1][f], k[0] * gr[0][f]));   // Eq. 32
+    }
+    const double div = dx[0][0] + dx[1][1] + dx[2][2];
+    const double txx = fma(2.0 * mu, dx[0][0], lam * div), tyy = fma(2.0 * mu, dx[1][1], lam * div),
+                 tzz = fma(2.0 * mu, dx[2][2], lam * div);
+    const double txy = mu * (dx[1][0] + dx[0][1]), txz = mu * (dx[2][0] + dx[0][2]), tyz = mu * (dx[2][1] + dx[1][2]);
+    const double bx = fma(kap, dx[0][3], fma(val[2], txz, fma(val[1], txy, val[0] * txx)));
+    const double by = fma(kap, dx[1][3], fma(val[2], tyz, fma(val[1], tyy, val[0] * txy)));
+    const double bz = fma(kap, dx[2][3], fma(val[2], tzz, fma(val[1], tyz, val[0] * txz)));
+    F[1] -= fma(mz, txz, fma(my, txy, mx * txx));
+    F[2] -= fma(mz, tyz, fma(my, tyy, mx * txy));
+    F[3] -= fma(mz, tzz, fma(my, tyz, mx * txz));
+    F[4] -= fma(mz, bz, fma(my, by, mx * bx));
+  }
+  return fl;
+}
+
+template <int DIR, bool VISC>
+__global__ void __launch_bounds__(Cfg3<DIR, VISC>::NT, Cfg3<DIR, VISC>::MINB) k_flux3(const Consts c, const FluxIn3 in,
+                                                                                     const __grid_constant__ TmaMaps tm) {
+  using C = Cfg3<DIR, VISC>;
+  constexpr int TS = C::TS, TT = C::TT, NT = C::NT, NF = C::NF, LP = C::LP, LA = C::LA, LT = C::LT, LF = C::LF, LG = C::LG;
+  constexpr int SS = (DIR == 0) ? 1 : TT;
+  constexpr int FP = (DIR == 0) ? TT * LP : LP * TT;   // field strides
+  constexpr int FA = (DIR == 0) ? TT * LA : LA * TT;
+  constexpr int FM = (DIR == 0) ? TT * LF : LF * TT;
+  constexpr int FG = (DIR == 0) ? TT * LG : LG * TT;
+  extern __shared__ __align__(1024) double sm3[];
+  double* const sP = sm3 + C::oP;
+  double* const sM = sm3 + C::oM;
+  double* const sMt = sm3 + C::oMt;
+  double* const sG = sm3 + C::oG;
+  double* const sA = sm3 + C::oA;
+  double* const sT1 = sm3 + C::oT1;
+  uint64_t* const bar = (uint64_t*)(sm3 + C::oBar);
+  const int tid = threadIdx.x;
+  int s0, t0, o;
+  if (DIR == 0) { s0 = blockIdx.x * TS; t0 = blockIdx.y * TT; o = blockIdx.z; }
+  else if (DIR == 1) { t0 = blockIdx.x * TT; s0 = blockIdx.y * TS; o = blockIdx.z; }
+  else { t0 = blockIdx.x * TT; o = blockIdx.y; s0 = blockIdx.z * TS; }
+  const int nd = c.n[DIR];
+  const int nt = (DIR == 0) ? c.n[1] : c.n[0];
+
+  if (tid == 0) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32_3(bar)), "r"(1) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    uint32_t bytes = (C::nP + C::NM * LF * TT + C::nG) * 8;
+    if (in.moving) bytes += C::nMt * 8;
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32_3(bar)), "r"(bytes) : "memory");
+    // box coordinates are (i, j, k, field) in the padded layout of each array
+    if (DIR == 0) {
+      tma4(sP, &tm.P, bar, s0 - 6 + GPI, t0 + GPJ, o + GPK, 0);
+      tma4(sM, &tm.M, bar, s0, t0, o, 0);
+      if (in.moving) tma4(sMt, &tm.Mt, bar, s0, t0, o, 0);
+      if (VISC) {
+        tma4(sG, &tm.G, bar, s0 - 2 + GGI, t0 + GGJ, o + GGK, 4);
+        tma4(sG + 4 * FG, &tm.G, bar, s0 - 2 + GGI, t0 + GGJ, o + GGK, 8);
+      }
+    } else if (DIR == 1) {
+      tma4(sP, &tm.P, bar, t0 + GPI, s0 - 6 + GPJ, o + GPK, 0);
+      tma4(sM, &tm.M, bar, t0, s0, o, 0);
+      if (in.moving) tma4(sMt, &tm.Mt, bar, t0, s0, o, 0);
+      if (VISC) {
+        tma4(sG, &tm.G, bar, t0 + GGI, s0 - 1 + GGJ, o + GGK, 0);
+        tma4(sG + 4 * FG, &tm.G, bar, t0 + GGI, s0 - 1 + GGJ, o + GGK, 8);
+      }
+    } else {
+      tma4(sP, &tm.P, bar, t0 + GPI, o + GPJ, s0 - 6 + GPK, 0);
+      tma4(sM, &tm.M, bar, t0, o, s0, 0);
+      if (in.moving) tma4(sMt, &tm.Mt, bar, t0, o, s0, 0);
+      if (VISC) {
+        tma4(sG, &tm.G, bar, t0 + GGI, o + GGJ, s0 - 1 + GGK, 0);
+        tma4(sG + 4 * FG, &tm.G, bar, t0 + GGI, o + GGJ, s0 - 1 + GGK, 4);
+      }
+    }
+  }
+  __syncthreads();   // the barrier is initialised before anyone polls it
+  {
+    uint32_t done = 0;
+    const uint32_t b = smem_u32_3(bar);
+    while (!done) {
+      asm volatile(
+          "{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}\n"
+          : "=r"(done) : "r"(b), "r"(0) : "memory");
+    }
+  }
+
+  // ---- per cell: aL = 1/2 P' + P''/12, aR = -1/2 P' + P''/12 (Eq. 16-17, 19) on cells -2..TS+1; T' on -1..TS ----
+  for (int it = tid; it < 5 * LA * TT; it += NT) {
+    int f, a, t;
+    if (DIR == 0) { a = it % LA; t = (it / LA) % TT; f = it / (LA * TT); }
+    else { t = it % TT; a = (it / TT) % LA; f = it / (TT * LA); }
+    const double* q = sP + sidx3<DIR, TT>(f, a + 4, t, LP);
+    const double c0 = q[0], p1 = q[SS], m1 = q[-SS], p2 = q[2 * SS], m2 = q[-2 * SS], p3 = q[3 * SS], m3 = q[-3 * SS],
+                 p4 = q[4 * SS], m4 = q[-4 * SS];
+    double d1 = CE1 * (p1 - m1);
+    d1 = fma(CE2, p2 - m2, d1);
+    d1 = fma(CE3, p3 - m3, d1);
+    double d2 = CS0 * c0;
+    d2 = fma(CS1, p1 + m1, d2);
+    d2 = fma(CS2, p2 + m2, d2);
+    d2 = fma(CS3, p3 + m3, d2);
+    d2 = fma(CS4, p4 + m4, d2);
+    const double h = 0.5 * d1, d = d2 * (1.0 / 12.0);
+    sA[sidx3<DIR, TT>(f, a, t, LA)] = d + h;
+    sA[sidx3<DIR, TT>(f + 5, a, t, LA)] = d - h;
+  }
+  if (VISC) {
+    for (int it = tid; it < LT * TT; it += NT) {
+      int a, t;
+      if (DIR == 0) { a = it % LT; t = it / LT; }
+      else { t = it % TT; a = it / TT; }
+      const double* q = sP + sidx3<DIR, TT>(5, a + 5, t, LP);
+      double d1 = CE1 * (q[SS] - q[-SS]);
+      d1 = fma(CE2, q[2 * SS] - q[-2 * SS], d1);
+      d1 = fma(CE3, q[3 * SS] - q[-3 * SS], d1);
+      sT1[sidx3<DIR, TT>(0, a, t, LT)] = d1;
+    }
+  }
+  __syncthreads();
+
+  // ---- one interface per thread ----
+  int sI, row;
+  if (DIR == 0) { sI = tid & 31; row = tid >> 5; }
+  else { row = tid % TT; sI = tid / TT; }
+  const bool valid = (sI <= TS) && (s0 + sI <= nd) && (t0 + row < nt);
+  unsigned nlim = 0, ntst = 0;
+  double F[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+  if (valid) {
+    const double mt = in.moving ? sMt[sidx3<DIR, TT>(0, sI, row, LF)] : 0.0;
+    const unsigned fl = face3<DIR, VISC, SS, FP, FA, FG, FM>(
+        c, sP + sidx3<DIR, TT>(0, sI + 4, row, LP), sA + sidx3<DIR, TT>(0, sI, row, LA),
+        sT1 + sidx3<DIR, TT>(0, sI, row, LT), sG + sidx3<DIR, TT>(0, sI + C::GOFF, row, LG),
+        sM + sidx3<DIR, TT>(0, sI, row, LF), mt, F);
+    if (sI < TS || s0 + sI == nd) { nlim = __popc(fl); ntst = 10; }   // tile-shared faces counted once
+  }
+  if (sI <= TS) {
+    // the flux tile aliases the metric tile: slot (sI,row) of every metric field is read only by this thread
+#pragma unroll
+    for (int f = 0; f < 5; ++f) sM[sidx3<DIR, TT>(f, sI, row, LF)] = F[f];
+  }
+  if (in.stats) {
+    for (int off = 16; off > 0; off >>= 1) {
+      nlim += __shfl_down_sync(0xffffffffu, nlim, off);
+      ntst += __shfl_down_sync(0xffffffffu, ntst, off);
+    }
+    if ((tid & 31) == 0 && ntst) { atomicAdd(in.stats, (unsigned long long)nlim); atomicAdd(in.stats + 1, (unsigned long long)ntst); }
+  }
+  __syncthreads();
+  // ---- flux difference, Eq. 25: Res_i -= F_{i+1/2} - F_{i-1/2} ----
+  for (int it = tid; it < TS * TT; it += NT) {
+    int s, t;
+    if (DIR == 0) { s = it % TS; t = it / TS; }
+    else { t = it % TT; s = it / TT; }
+    if (s0 + s >= nd || t0 + t >= nt) continue;
+    long long ac;
+    if (DIR == 0) ac = c.LR.at(s0 + s, t0 + t, o);
+    else if (DIR == 1) ac = c.LR.at(t0 + t, s0 + s, o);
+    else ac = c.LR.at(t0 + t, o, s0 + s);
+    double old[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+    if (!in.first) {
+#pragma unroll
+      for (int f = 0; f < 5; ++f) old[f] = in.res[f * c.fsR + ac];
+    }
+#pragma unroll
+    for (int f = 0; f < 5; ++f) {
+      const double dF = sM[sidx3<DIR, TT>(f, s + 1, t, LF)] - sM[sidx3<DIR, TT>(f, s, t, LF)];
+      in.res[f * c.fsR + ac] = old[f] - dF;
+    }
+  }
+}
+
+}  // namespace meg6
