@@ -2,7 +2,7 @@
 """bench.py -- FP64 MEG6 RHS + SSP-RK3 throughput on B200 (BASELINE.json metric).
 
 One "step" = one rk3_step = three passes of the whole hot path (primitives, ghosts, gradients, three flux
-kernels, assembly + update) over the workload.  value = N_cells * 3 * steps / seconds, in Mcell-updates/s per
+sweeps, the last one fused with residual assembly + RK3 update) over the workload.  value = N_cells * 3 * steps / seconds, in Mcell-updates/s per
 RK stage, summed over all ranks (independent replicas for --gpus > 1: the path is single-GPU).
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c4|c3|c1|c2] [--impl reference]
@@ -55,14 +55,16 @@ def bytes_per_cell_stage(prm, sponge):
     """Compulsory HBM doubles per cell per RK stage of the shipped kernel set."""
     v, m = prm["viscous"], prm["moving"]
     k = {}
-    k["prim"] = 5 + 6
+    k["prim"] = (5 + 6) / 3.0                      # once per step (the caller owns U)
     k["grad"] = (4 + 12) if v else 0
     met = (10 if v else 3) + (1 if m else 0)
-    k["flux_xi"] = (6 if v else 5) + met + (8 if v else 0) + 5
-    k["flux_eta"] = k["flux_xi"] + 5
-    k["flux_zeta"] = k["flux_xi"] + 5
-    k["update"] = 5 + 5 + 10.0 / 3 + 1 + (1 if m else 0) + ((1 + 5) if sponge else 0) + 5
-    k["copy_Un"] = 10.0 / 3
+    base = (6 if v else 5) + met + (8 if v else 0)  # primitive tile, interface metrics, stored gradients
+    k["flux_eta"] = base + 5                        # first sweep: writes the residual
+    k["flux_zeta"] = base + 5 + 5                   # reads and writes it
+    # last sweep, fused with assembly + RK3 stage + primitives of the new state:
+    # reads residual 5, U 5, U0 5 (stages 2-3), 1/J 1 [, (1/J)_t 1] [, sigma 1, Q_ref 5]; writes U 5, U0 5 (stage 1),
+    # P_next 6 (stages 1-2)
+    k["flux_xi"] = base + 5 + 5 + 10.0 / 3 + 1 + (1 if m else 0) + ((1 + 5) if sponge else 0) + 5 + 5.0 / 3 + 4
     k["metrics"] = (6 + 3 + 9 + 9 + 1 + 6 + 3 * met + 1) if m else 0   # nodes+modes, xc, cd, met, rj, xt+mt, faces, rjt
     return {a: 8.0 * b for a, b in k.items()}
 
@@ -254,7 +256,7 @@ def run_ours(args):
     dsec = kernels[dom]["ms_per_stage"] * 1e-3
     ach = bpc[dom] * ncell / dsec / 1e9
     clk = (clocks or {}).get("sm_mhz") or sm_max
-    roof = {"kernel": "k_flux<%s,%s>" % (dom[5:], "visc" if prm["viscous"] else "inv"), "bound": "hbm",
+    roof = {"kernel": "k_flux3<%s,%s>" % (dom[5:], "visc" if prm["viscous"] else "inv"), "bound": "hbm",
             "achieved": ach, "peak": hbm, "unit": "GB/s", "frac": ach / hbm, "traffic": None,
             "peak_source": peak_src, "bytes_per_cell": bpc[dom], "cells_per_launch": ncell,
             "avg_launch_ms": dsec * 1e3,

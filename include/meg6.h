@@ -85,7 +85,8 @@ meg6_status meg6_set_sponge(meg6_grid* g, const double* sigma, const double* U_r
 meg6_status meg6_rhs(meg6_grid* g, const double* U, double* dUdt);
 
 /* One SSP-RK3 step (Eq. B.1) in place on U, from time t to t+dt.  Moving meshes recompute the
- * geometry at the stage times t, t+dt, t+dt/2 (R17) and leave it at t+dt/2. */
+ * geometry at the stage times t, t+dt, t+dt/2 (R17) and leave it at t+dt/2.  U is read and written by the last
+ * sweep of every stage; it must not be touched by other streams while the step is in flight. */
 meg6_status meg6_rk3_step(meg6_grid* g, double* U, double t, double dt);
 
 /* Eq. B.2 / B.3 time step for the state U at the geometry of the last metrics_compute.
@@ -107,9 +108,9 @@ meg6_status meg6_get_array(meg6_grid* g, int kind, int which, double* out);
 /* Per-kernel timing for bench.py: while enabled, every kernel launch of the library is bracketed by CUDA
  * events on the grid's stream.  meg6_profile_read synchronises the stream, adds up the elapsed time and the
  * number of kernel launches per kind since the last read, and clears the record.  HOST pointers, 16 entries
- * each.  Kinds: 0 metric/Jacobian kernels (all of one metrics_compute), 1 primitive conversion, 2 ghost fill,
- * 3 stored E6 gradients, 4/5/6 flux kernel along xi/eta/zeta, 7 residual assembly + RK3 update,
- * 8 copy of U^n (memcpy, not counted as a kernel launch), 9 CFL reduction. */
+ * each.  Kinds: 0 metric/Jacobian kernels (all of one metrics_compute), 1 primitive conversion (once per step),
+ * 2 ghost fill, 3 stored E6 gradients, 4 xi sweep (the last one: fused with residual assembly, the RK3 stage update
+ * and the primitive conversion of the new state), 5 eta sweep (first), 6 zeta sweep, 7-8 unused, 9 CFL reduction. */
 meg6_status meg6_profile_enable(meg6_grid* g, int on);
 meg6_status meg6_profile_read(meg6_grid* g, double* ms_per_kind, unsigned long long* launches_per_kind);
 

@@ -7,8 +7,6 @@
 
 #include "meg6_common.cuh"
 #include "meg6_flow.cuh"
-#include "meg6_flux.cuh"
-#include "meg6_flux_tma.cuh"
 #include "meg6_flux3.cuh"
 #include <stdlib.h>
 
@@ -99,6 +97,7 @@ static size_t carve(const meg6_params* p, const Consts& c, meg6_grid* g, char* b
   }
   G->rjt = p->moving ? take(c.LC.n) : nullptr;
   for (int f = 0; f < 6; ++f) G->P[f] = take(c.LP.n);
+  for (int f = 0; f < 6; ++f) G->Pb[f] = take(c.LP.n);   // ping-pong partner written by the fused last sweep
   for (int e = 0; e < 3; ++e)
     for (int f = 0; f < 4; ++f) G->G[e][f] = p->viscous ? take(c.LG.n) : nullptr;
   G->res = take(c.LR.n);
@@ -136,40 +135,10 @@ static bool make_map4(EncodeTiledFn fn, CUtensorMap* tm, const double* base, con
 }
 
 template <int DIR, bool VISC>
-static bool make_maps_dir(EncodeTiledFn fn, meg6_grid* g) {
-  using C = TmaCfg<DIR, VISC>;
-  const Consts& c = g->c;
-  TmaMaps& t = g->tmaps[DIR];
-  auto box = [](int sweep, int trans, int nf, int out[4]) {
-    if (DIR == 0) { out[0] = sweep; out[1] = trans; out[2] = 1; }
-    else if (DIR == 1) { out[0] = trans; out[1] = sweep; out[2] = 1; }
-    else { out[0] = trans; out[1] = 1; out[2] = sweep; }
-    out[3] = nf;
-  };
-  int b[4];
-  bool ok = true;
-  box(C::LP, C::TT, C::NF, b);
-  ok = ok && make_map4(fn, &t.P, g->P[0], c.LP, c.fsP, 6, b);
-  box(C::LF, C::TT, C::NM, b);
-  ok = ok && make_map4(fn, &t.M, VISC ? g->fmet[DIR][0] : g->fmet[DIR][3 * DIR], c.LF[DIR], c.fsM[DIR], C::NM, b);
-  if (g->p.moving) {
-    box(C::LF, C::TT, 1, b);
-    ok = ok && make_map4(fn, &t.Mt, g->fmt[DIR], c.LF[DIR], c.fsM[DIR], 1, b);
-  }
-  if (VISC) {
-    box(C::LG, C::TT, 4, b);
-    ok = ok && make_map4(fn, &t.G, g->G[0][0], c.LG, c.fsG, 12, b);
-  }
-  box(C::TS, C::TT, 5, b);
-  ok = ok && make_map4(fn, &t.R, g->res, c.LR, c.fsR, 5, b);
-  return ok;
-}
-
-template <int DIR, bool VISC>
-static bool make_maps3_dir(EncodeTiledFn fn, meg6_grid* g) {
+static bool make_maps3_dir(EncodeTiledFn fn, meg6_grid* g, int buf) {
   using C = Cfg3<DIR, VISC>;
   const Consts& c = g->c;
-  TmaMaps& t = g->tmaps3[DIR];
+  TmaMaps& t = g->tmaps3[buf][DIR];
   auto box = [](int sweep, int trans, int nf, int out[4]) {
     if (DIR == 0) { out[0] = sweep; out[1] = trans; out[2] = 1; }
     else if (DIR == 1) { out[0] = trans; out[1] = sweep; out[2] = 1; }
@@ -179,7 +148,7 @@ static bool make_maps3_dir(EncodeTiledFn fn, meg6_grid* g) {
   int b[4];
   bool ok = true;
   box(C::LP, C::TT, C::NF, b);
-  ok = ok && make_map4(fn, &t.P, g->P[0], c.LP, c.fsP, 6, b);
+  ok = ok && make_map4(fn, &t.P, buf ? g->Pb[0] : g->P[0], c.LP, c.fsP, 6, b);
   box(C::LF, C::TT, C::NM, b);
   ok = ok && make_map4(fn, &t.M, VISC ? g->fmet[DIR][0] : g->fmet[DIR][3 * DIR], c.LF[DIR], c.fsM[DIR], C::NM, b);
   if (g->p.moving) {
@@ -194,32 +163,25 @@ static bool make_maps3_dir(EncodeTiledFn fn, meg6_grid* g) {
 }
 
 static cudaError_t setup_tma(meg6_grid* g) {
-  g->use_tma = 0;
-  const char* env = getenv("MEG6_FLUX");
-  if (env && strcmp(env, "v1") == 0) return cudaSuccess;   // A/B switch: plain shared-memory staging kernel
   void* fp = nullptr;
   cudaDriverEntryPointQueryResult qr;
   cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fp, cudaEnableDefault, &qr);
   if (e != cudaSuccess) return e;
   if (!fp || qr != cudaDriverEntryPointSuccess) return cudaErrorNotSupported;
   EncodeTiledFn fn = (EncodeTiledFn)fp;
-  bool ok;
-  if (g->p.viscous) ok = make_maps_dir<0, true>(fn, g) && make_maps_dir<1, true>(fn, g) && make_maps_dir<2, true>(fn, g);
-  else ok = make_maps_dir<0, false>(fn, g) && make_maps_dir<1, false>(fn, g) && make_maps_dir<2, false>(fn, g);
-  if (g->p.viscous) ok = ok && make_maps3_dir<0, true>(fn, g) && make_maps3_dir<1, true>(fn, g) && make_maps3_dir<2, true>(fn, g);
-  else ok = ok && make_maps3_dir<0, false>(fn, g) && make_maps3_dir<1, false>(fn, g) && make_maps3_dir<2, false>(fn, g);
+  bool ok = true;
+  for (int buf = 0; buf < 2 && ok; ++buf) {
+    if (g->p.viscous) ok = make_maps3_dir<0, true>(fn, g, buf) && make_maps3_dir<1, true>(fn, g, buf) && make_maps3_dir<2, true>(fn, g, buf);
+    else ok = make_maps3_dir<0, false>(fn, g, buf) && make_maps3_dir<1, false>(fn, g, buf) && make_maps3_dir<2, false>(fn, g, buf);
+  }
   if (!ok) return cudaErrorInvalidValue;
-#define SET_SMEM3(D, V)                                                                                     \
-  if ((e = cudaFuncSetAttribute(k_flux3<D, V>, cudaFuncAttributeMaxDynamicSharedMemorySize,                 \
+  // opt in to the dynamic shared memory the flux kernels need
+#define SET_SMEM3(D, V, F)                                                                                  \
+  if ((e = cudaFuncSetAttribute(k_flux3<D, V, F>, cudaFuncAttributeMaxDynamicSharedMemorySize,              \
                                 Cfg3<D, V>::SMEM_BYTES)) != cudaSuccess) return e;
-  SET_SMEM3(0, false) SET_SMEM3(1, false) SET_SMEM3(2, false) SET_SMEM3(0, true) SET_SMEM3(1, true) SET_SMEM3(2, true)
+  SET_SMEM3(0, false, true) SET_SMEM3(1, false, false) SET_SMEM3(2, false, false)
+  SET_SMEM3(0, true, true) SET_SMEM3(1, true, false) SET_SMEM3(2, true, false)
 #undef SET_SMEM3
-#define SET_SMEM(D, V)                                                                                      \
-  if ((e = cudaFuncSetAttribute(k_flux_tma<D, V>, cudaFuncAttributeMaxDynamicSharedMemorySize,              \
-                                TmaCfg<D, V>::SMEM_BYTES)) != cudaSuccess) return e;
-  SET_SMEM(0, false) SET_SMEM(1, false) SET_SMEM(2, false) SET_SMEM(0, true) SET_SMEM(1, true) SET_SMEM(2, true)
-#undef SET_SMEM
-  g->use_tma = (env && strcmp(env, "v2") == 0) ? 1 : 2;   // 2: k_flux3 (default); 1: second-generation TMA kernel
   return cudaSuccess;
 }
 
@@ -300,15 +262,6 @@ meg6_status meg6_grid_create(const meg6_params* p, const double* x, const double
     e = cudaMemcpyAsync(g->nodes[q], src[q], nn, cudaMemcpyDeviceToDevice, g->stream);
     if (e == cudaSuccess && p->moving) e = cudaMemcpyAsync(g->modes[q], msrc[q], nn, cudaMemcpyDeviceToDevice, g->stream);
   }
-  if (e == cudaSuccess) {
-    // opt in to the dynamic shared memory the flux kernels need
-    e = cudaFuncSetAttribute(k_flux<0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(FluxCfg<0, false>::SMEM_DOUBLES * 8));
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_flux<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(FluxCfg<1, false>::SMEM_DOUBLES * 8));
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_flux<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(FluxCfg<2, false>::SMEM_DOUBLES * 8));
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_flux<0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(FluxCfg<0, true>::SMEM_DOUBLES * 8));
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_flux<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(FluxCfg<1, true>::SMEM_DOUBLES * 8));
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_flux<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(FluxCfg<2, true>::SMEM_DOUBLES * 8));
-  }
   if (e == cudaSuccess) e = setup_tma(g);
   if (e != cudaSuccess) { delete g; return fail(MEG6_ECUDA, "grid_create: %s", cudaGetErrorString(e)); }
   *out = g;
@@ -350,13 +303,14 @@ meg6_status meg6_set_sponge(meg6_grid* g, const double* sigma, const double* U_r
   return MEG6_OK;
 }
 
-// residual of Eq. 8-9 into g->res for the state U (all kernels of one RK stage but the update)
-static meg6_status residual(meg6_grid* g, const double* U) {
+// One RK stage (or one dQ/dt evaluation) for the state whose primitives are in buffer `buf` (interior cells
+// filled): ghost fill, stored gradients, eta and zeta sweeps into g->res, xi sweep fused with the residual
+// assembly, the stage update and the primitive conversion of the new state (into the other buffer).
+static meg6_status stage(meg6_grid* g, int buf, const Fuse3& fu) {
   const Consts& c = g->c;
+  double* const* Pc = buf ? g->Pb : g->P;
   P6 P;
-  for (int f = 0; f < 6; ++f) P.p[f] = g->P[f];
-  const int T = 256;
-  { ProfScope ps(g, 1, 1); k_prim<<<nblk(c.LC.n, T), T, 0, g->stream>>>(c, U, P); }
+  for (int f = 0; f < 6; ++f) P.p[f] = Pc[f];
   for (int d = 0; d < 3; ++d) {
     int a = (d + 1) % 3, b = (d + 2) % 3;
     if (a > b) { int t = a; a = b; b = t; }
@@ -371,106 +325,79 @@ static meg6_status residual(meg6_grid* g, const double* U) {
     P12 G;
     for (int e = 0; e < 3; ++e)
       for (int f = 0; f < 4; ++f) G.p[4 * e + f] = g->G[e][f];
-    const long long ng = (long long)(c.n[0] + 2) * (c.n[1] + 2) * (c.n[2] + 2);
     ProfScope ps(g, 3, 1);
-    k_grad<<<nblk(ng, T), T, 0, g->stream>>>(c, P, G);
+    k_grad<<<dim3(nblk(c.n[0] + 2, 32), nblk(c.n[1] + 2, 8), nblk(c.n[2] + 2, GRAD_KB)), dim3(32, 8, 1), 0, g->stream>>>(c, P, G);
   }
-  for (int d = 0; d < 3; ++d) {
-    FluxIn in;
-    for (int f = 0; f < 6; ++f) in.P[f] = g->P[f];
-    for (int q = 0; q < 10; ++q) in.m[q] = g->fmet[d][q];
-    in.mt = g->p.moving ? g->fmt[d] : nullptr;
-    for (int e = 0; e < 3; ++e)
-      for (int f = 0; f < 4; ++f) in.G[4 * e + f] = g->G[e][f];
-    in.res = g->res;
-    in.stats = g->stats_on ? g->stats : nullptr;
-    in.first = (d == 0);
-    const bool V = g->p.viscous != 0;
-    ProfScope ps(g, 4 + d, 1);
-    if (g->use_tma == 2) {
-      FluxIn3 i3;
-      i3.res = g->res; i3.stats = in.stats; i3.first = in.first; i3.moving = g->p.moving ? 1 : 0;
-#define LAUNCH3(D, VV, GRID) k_flux3<D, VV><<<GRID, Cfg3<D, VV>::NT, Cfg3<D, VV>::SMEM_BYTES, g->stream>>>(c, i3, g->tmaps3[D])
-      if (d == 0) {
-        dim3 grid(nblk(c.n[0], Cfg3<0, false>::TS), nblk(c.n[1], Cfg3<0, false>::TT), c.n[2]);
-        if (V) LAUNCH3(0, true, grid); else LAUNCH3(0, false, grid);
-      } else if (d == 1) {
-        dim3 grid(nblk(c.n[0], Cfg3<1, false>::TT), nblk(c.n[1], Cfg3<1, false>::TS), c.n[2]);
-        if (V) LAUNCH3(1, true, grid); else LAUNCH3(1, false, grid);
-      } else {
-        dim3 grid(nblk(c.n[0], Cfg3<2, false>::TT), c.n[1], nblk(c.n[2], Cfg3<2, false>::TS));
-        if (V) LAUNCH3(2, true, grid); else LAUNCH3(2, false, grid);
-      }
+  FluxIn3 i3;
+  i3.res = g->res; i3.stats = g->stats_on ? g->stats : nullptr; i3.moving = g->p.moving ? 1 : 0;
+  const bool V = g->p.viscous != 0;
+  const TmaMaps* tm = g->tmaps3[buf];
+#define LAUNCH3(D, VV, FF, GRID) \
+  k_flux3<D, VV, FF><<<GRID, Cfg3<D, VV>::NT, Cfg3<D, VV>::SMEM_BYTES, g->stream>>>(c, i3, tm[D], fu)
+  // sweep order eta, zeta, xi: the fused final phase then works on rows that are contiguous along xi
+  {
+    ProfScope ps(g, 5, 1);
+    i3.first = 1;
+    dim3 grid(nblk(c.n[0], Cfg3<1, false>::TT), nblk(c.n[1], Cfg3<1, false>::TS), c.n[2]);
+    if (V) LAUNCH3(1, true, false, grid); else LAUNCH3(1, false, false, grid);
+  }
+  {
+    ProfScope ps(g, 6, 1);
+    i3.first = 0;
+    dim3 grid(nblk(c.n[0], Cfg3<2, false>::TT), c.n[1], nblk(c.n[2], Cfg3<2, false>::TS));
+    if (V) LAUNCH3(2, true, false, grid); else LAUNCH3(2, false, false, grid);
+  }
+  {
+    ProfScope ps(g, 4, 1);
+    dim3 grid(nblk(c.n[0], Cfg3<0, false>::TS), nblk(c.n[1], Cfg3<0, false>::TT), c.n[2]);
+    if (V) LAUNCH3(0, true, true, grid); else LAUNCH3(0, false, true, grid);
+  }
 #undef LAUNCH3
-    } else if (g->use_tma) {
-      FluxIn2 i2;
-      i2.res = g->res; i2.stats = in.stats; i2.first = in.first; i2.moving = g->p.moving ? 1 : 0;
-      i2.dbg = getenv("MEG6_DBG") ? atoi(getenv("MEG6_DBG")) : 0;
-#define LAUNCH_TMA(D, VV, GRID) k_flux_tma<D, VV><<<GRID, TmaCfg<D, VV>::NT, TmaCfg<D, VV>::SMEM_BYTES, g->stream>>>(c, i2, g->tmaps[D])
-      if (d == 0) {
-        dim3 grid(nblk(c.n[0], TmaCfg<0, false>::TS), nblk(c.n[1], TmaCfg<0, false>::TT), c.n[2]);
-        if (V) LAUNCH_TMA(0, true, grid); else LAUNCH_TMA(0, false, grid);
-      } else if (d == 1) {
-        dim3 grid(nblk(c.n[0], TmaCfg<1, false>::TT), nblk(c.n[1], TmaCfg<1, false>::TS), c.n[2]);
-        if (V) LAUNCH_TMA(1, true, grid); else LAUNCH_TMA(1, false, grid);
-      } else {
-        dim3 grid(nblk(c.n[0], TmaCfg<2, false>::TT), c.n[1], nblk(c.n[2], TmaCfg<2, false>::TS));
-        if (V) LAUNCH_TMA(2, true, grid); else LAUNCH_TMA(2, false, grid);
-      }
-#undef LAUNCH_TMA
-    } else if (d == 0) {
-      dim3 grid(nblk(c.n[0], FluxCfg<0, false>::TS), nblk(c.n[1], FluxCfg<0, false>::TT), c.n[2]);
-      if (V) k_flux<0, true><<<grid, FluxCfg<0, true>::NT, FluxCfg<0, true>::SMEM_DOUBLES * 8, g->stream>>>(c, in);
-      else k_flux<0, false><<<grid, FluxCfg<0, false>::NT, FluxCfg<0, false>::SMEM_DOUBLES * 8, g->stream>>>(c, in);
-    } else if (d == 1) {
-      dim3 grid(nblk(c.n[0], FluxCfg<1, false>::TT), nblk(c.n[1], FluxCfg<1, false>::TS), c.n[2]);
-      if (V) k_flux<1, true><<<grid, FluxCfg<1, true>::NT, FluxCfg<1, true>::SMEM_DOUBLES * 8, g->stream>>>(c, in);
-      else k_flux<1, false><<<grid, FluxCfg<1, false>::NT, FluxCfg<1, false>::SMEM_DOUBLES * 8, g->stream>>>(c, in);
-    } else {
-      dim3 grid(nblk(c.n[0], FluxCfg<2, false>::TT), c.n[1], nblk(c.n[2], FluxCfg<2, false>::TS));
-      if (V) k_flux<2, true><<<grid, FluxCfg<2, true>::NT, FluxCfg<2, true>::SMEM_DOUBLES * 8, g->stream>>>(c, in);
-      else k_flux<2, false><<<grid, FluxCfg<2, false>::NT, FluxCfg<2, false>::SMEM_DOUBLES * 8, g->stream>>>(c, in);
-    }
-  }
   CUDA_OK(cudaGetLastError());
   return MEG6_OK;
 }
 
-static void launch_update(meg6_grid* g, const double* U, double* out, int mode, double a, double b, double dt) {
-  UpdIn in;
-  in.res = g->res; in.rj = g->rj; in.rjt = g->p.moving ? g->rjt : nullptr;
-  in.sigma = g->sigma; in.uref = g->uref;
-  in.U = U; in.U0 = g->U0; in.out = out; in.a = a; in.b = b; in.dt = dt; in.mode = mode;
-  ProfScope ps(g, 7, 1);
-  k_update<<<nblk(g->c.LC.n, 256), 256, 0, g->stream>>>(g->c, in);
+static void launch_prim(meg6_grid* g, const double* U) {
+  P6 P;
+  for (int f = 0; f < 6; ++f) P.p[f] = g->P[f];
+  ProfScope ps(g, 1, 1);
+  k_prim<<<nblk(g->c.LC.n, 256), 256, 0, g->stream>>>(g->c, U, P);
+}
+
+static Fuse3 make_fuse(meg6_grid* g, const double* U, double* out) {
+  Fuse3 fu;
+  memset(&fu, 0, sizeof(fu));
+  fu.U = U; fu.out = out; fu.U0 = g->U0;
+  fu.rj = g->rj; fu.rjt = g->p.moving ? g->rjt : nullptr;
+  fu.sigma = g->sigma; fu.uref = g->uref;
+  return fu;
 }
 
 meg6_status meg6_rhs(meg6_grid* g, const double* U, double* dUdt) {
   if (!g || !U || !dUdt) return fail(MEG6_EINVAL, "rhs: null pointer%s");
   if (!g->have_metrics) return fail(MEG6_ESTATE, "rhs called before metrics_compute%s");
-  meg6_status s = residual(g, U);
-  if (s != MEG6_OK) return s;
-  launch_update(g, U, dUdt, 0, 0.0, 0.0, 0.0);
-  CUDA_OK(cudaGetLastError());
-  return MEG6_OK;
+  launch_prim(g, U);
+  Fuse3 fu = make_fuse(g, U, dUdt);
+  fu.mode = 0;
+  return stage(g, 0, fu);
 }
 
 meg6_status meg6_rk3_step(meg6_grid* g, double* U, double t, double dt) {
   if (!g || !U) return fail(MEG6_EINVAL, "rk3_step: null pointer%s");
   if (!g->have_metrics && !g->p.moving) return fail(MEG6_ESTATE, "rk3_step called before metrics_compute%s");
-  {
-    ProfScope ps(g, 8, 0);
-    CUDA_OK(cudaMemcpyAsync(g->U0, U, sizeof(double) * 5 * (size_t)g->c.LC.n, cudaMemcpyDeviceToDevice, g->stream));
-  }
   const double ts[3] = {t, t + dt, t + 0.5 * dt};
   const double aa[3] = {0.0, 3.0 / 4.0, 1.0 / 3.0}, bb[3] = {1.0, 1.0 / 4.0, 2.0 / 3.0};
+  launch_prim(g, U);   // the caller owns U: its primitives are recomputed at every step
   for (int s = 0; s < 3; ++s) {
     meg6_status st;
     if (g->p.moving && (st = meg6_metrics_compute(g, ts[s])) != MEG6_OK) return st;
-    if ((st = residual(g, U)) != MEG6_OK) return st;
-    launch_update(g, U, U, 1, aa[s], bb[s], dt);
+    const int buf = s & 1;
+    Fuse3 fu = make_fuse(g, U, U);
+    fu.mode = 1; fu.a = aa[s]; fu.b = bb[s]; fu.dt = dt;
+    fu.U0w = (s == 0) ? g->U0 : nullptr;                      // stage 1 saves U^n on the way
+    fu.Pn = (s < 2) ? (buf ? g->P[0] : g->Pb[0]) : nullptr;   // primitives of the next stage's state
+    if ((st = stage(g, buf, fu)) != MEG6_OK) return st;
   }
-  CUDA_OK(cudaGetLastError());
   return MEG6_OK;
 }
 

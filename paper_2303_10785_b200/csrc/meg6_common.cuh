@@ -68,13 +68,11 @@ struct Consts {   // per-grid constants passed by value to kernels
 
 }  // namespace meg6
 
-namespace meg6 { struct TmaMaps { CUtensorMap P, M, Mt, G, R; }; }
+namespace meg6 { struct TmaMaps { CUtensorMap P, M, Mt, G; }; }
 
 struct meg6_grid {
   meg6_params p;
-  meg6::TmaMaps tmaps[3];   // per sweep direction (second-generation kernel, A/B only)
-  meg6::TmaMaps tmaps3[3];  // per sweep direction (k_flux3)
-  int use_tma;
+  meg6::TmaMaps tmaps3[2][3];   // per primitive buffer and sweep direction
   meg6::Consts c;
   cudaStream_t stream;
   char* ws; size_t ws_bytes;
@@ -87,7 +85,8 @@ struct meg6_grid {
   double* fmet[3][10]; double* fmt[3];
   double* rjt;
   // flow
-  double* P[6];
+  double* P[6];       // primitives + T with ghosts, buffer 0
+  double* Pb[6];      // buffer 1 (the fused last sweep writes the next stage's primitives into the other buffer)
   double* G[3][4];    // D1 gradients of (u,v,w,T) along xi,eta,zeta (viscous)
   double* res;        // [5][N]
   double* U0;         // [5][N]

@@ -1,5 +1,5 @@
-// meg6_flow.cuh -- primitive conversion, ghost fill, stored gradients, residual assembly + SSP-RK3 update,
-// CFL reduction.
+// meg6_flow.cuh -- primitive conversion, ghost fill, stored gradients, CFL reduction.
+// Residual assembly and the SSP-RK3 update (rows S, T) are fused into the last sweep, meg6_flux3.cuh.
 #pragma once
 #include "meg6_common.cuh"
 
@@ -105,52 +105,43 @@ __device__ __forceinline__ double d1_op(const double* __restrict__ f, long long 
 
 // G(b): stored gradients of (u,v,w,T) along xi, eta, zeta on cells [-1, n+1)^3 (viscous flux, Fig. 5 P:295;
 // R18: T is differentiated with the same E6 scheme).  G.p[4*e + f].
-__global__ void __launch_bounds__(256) k_grad(Consts c, P6 P, P12 G) {
-  const int ei = c.n[0] + 2, ej = c.n[1] + 2;
-  const long long total = (long long)ei * ej * (c.n[2] + 2);
-  const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (tid >= total) return;
-  const int i = (int)(tid % ei) - 1, j = (int)((tid / ei) % ej) - 1, k = (int)(tid / ((long long)ei * ej)) - 1;
-  const long long ap = c.LP.at(i, j, k), ag = c.LG.at(i, j, k);
+// A block of 32 x 8 threads covers 32 x 8 x GRAD_KB cells: each thread walks GRAD_KB cells along zeta, so the
+// zeta stencil re-uses its loads in registers and the eta stencil of the block re-uses rows in L1
+// (ncu r1c: the one-cell-per-thread version was L1-wavefront bound with a 31 % L1 hit rate).
+#ifndef MEG6_GRAD_KB
+#define MEG6_GRAD_KB 4
+#endif
+#ifndef MEG6_GRAD_MINB
+#define MEG6_GRAD_MINB 3
+#endif
+constexpr int GRAD_KB = MEG6_GRAD_KB;
+__global__ void __launch_bounds__(256, MEG6_GRAD_MINB) k_grad(Consts c, P6 P, P12 G) {
+  const int i = blockIdx.x * 32 + threadIdx.x - 1;
+  const int j = blockIdx.y * 8 + threadIdx.y - 1;
+  const int k0 = blockIdx.z * GRAD_KB - 1;
+  if (i > c.n[0] || j > c.n[1]) return;
+  const long long sj = c.LP.sj, sk = c.LP.sk;
+  const long long ap0 = c.LP.at(i, j, k0), ag0 = c.LG.at(i, j, k0);
 #pragma unroll
-  for (int e = 0; e < 3; ++e) {
-    const long long s = c.LP.stride(e);
+  for (int f = 0; f < 4; ++f) {
+    const double* __restrict__ q = P.p[(f < 3) ? f + 1 : 5] + ap0;
+    double z[GRAD_KB + 6];
 #pragma unroll
-    for (int f = 0; f < 4; ++f) {
-      const int pf = (f < 3) ? f + 1 : 5;
-      G.p[4 * e + f][ag] = d1_op(P.p[pf] + ap, s);
-    }
-  }
-}
-
-// S + T: dQ/dt = J (Res - (1/J)_t Q) - sigma (Q - Q_ref) (Eq. 9, 12, 14; R16) and one SSP-RK3 stage
-// (Eq. B.1):  U <- a U0 + b (U + dt dQ/dt).   mode 0: write dQ/dt to out (meg6_rhs);
-// mode 1: stage update in place on U (a = 0 for stage 1).
-struct UpdIn {
-  const double* res; const double* rj; const double* rjt; const double* sigma; const double* uref;
-  const double* U; const double* U0; double* out;
-  double a, b, dt; int mode;
-};
-
-__global__ void __launch_bounds__(256) k_update(Consts c, UpdIn in) {
-  const long long N = c.LC.n;
-  const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (tid >= N) return;
-  const int i = (int)(tid % c.n[0]), j = (int)((tid / c.n[0]) % c.n[1]), k = (int)(tid / ((long long)c.n[0] * c.n[1]));
-  const double J = 1.0 / in.rj[c.LX.at(i, j, k)];
-  const long long ar = c.LR.at(i, j, k);
-  const double rjt = in.rjt ? in.rjt[tid] : 0.0;
-  const double sg = in.sigma ? in.sigma[tid] : 0.0;
+    for (int m = 0; m < GRAD_KB + 6; ++m) z[m] = (k0 + m - 3 <= c.n[2] + 3) ? q[(m - 3) * sk] : 0.0;
 #pragma unroll
-  for (int f = 0; f < 5; ++f) {
-    const double u = in.U[f * N + tid];
-    double L = J * (in.res[f * c.fsR + ar] - rjt * u);
-    if (in.sigma) L -= sg * (u - in.uref[f * N + tid]);
-    if (in.mode == 0) in.out[f * N + tid] = L;
-    else {
-      double v = u + in.dt * L;
-      if (in.a != 0.0) v = in.a * in.U0[f * N + tid] + in.b * v;
-      in.out[f * N + tid] = v;
+    for (int m = 0; m < GRAD_KB; ++m) {
+      if (k0 + m > c.n[2]) break;
+      const double* __restrict__ qq = q + m * sk;
+      const long long ag = ag0 + m * c.LG.sk;
+      double* __restrict__ gx = G.p[f];
+      double* __restrict__ gy = G.p[4 + f];
+      double* __restrict__ gz = G.p[8 + f];
+      gx[ag] = d1_op(qq, 1);
+      gy[ag] = d1_op(qq, sj);
+      double r = CE1 * (z[m + 4] - z[m + 2]);
+      r = fma(CE2, z[m + 5] - z[m + 1], r);
+      r = fma(CE3, z[m + 6] - z[m], r);
+      gz[ag] = r;
     }
   }
 }

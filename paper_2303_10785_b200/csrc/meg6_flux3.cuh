@@ -24,6 +24,12 @@ namespace meg6 {
 #ifndef MEG6_MINB3_Y
 #define MEG6_MINB3_Y 5
 #endif
+#ifndef MEG6_PF_DIST
+#define MEG6_PF_DIST 0   // L2 prefetch distance in CTAs (0: off; 1024 measured slower on C4, r1)
+#endif
+#ifndef MEG6_RELOAD
+#define MEG6_RELOAD 1
+#endif
 
 template <int DIR, bool VISC>
 struct Cfg3 {
@@ -46,7 +52,7 @@ struct Cfg3 {
   static constexpr int al(int n) { return (n + 15) / 16 * 16; }   // 128-byte granules (TMA destinations)
   static constexpr int oP = 0, oM = oP + al(nP), oMt = oM + al(nM), oG = oMt + al(nMt), oA = oG + al(nG),
                        oT1 = oA + al(nA), oBar = oT1 + al(nT1);
-  static constexpr int SMEM_BYTES = (oBar + 2) * 8;
+  static constexpr int SMEM_BYTES = (oBar + 2) * 8;   // two mbarriers
 };
 
 template <int DIR, int TT>
@@ -60,12 +66,54 @@ struct FluxIn3 {
   int first, moving;
 };
 
+// Residual assembly + SSP-RK3 stage + primitive conversion fused into the final phase of the LAST sweep
+// (SURVEY 8(a) rows S, T and the first half of G): the complete residual of a cell is in registers there, so
+//   dQ/dt = J (Res - (1/J)_t Q) - sigma (Q - Q_ref)            (Eq. 9, 12, 14; R16)
+//   mode 0: out = dQ/dt                                          (meg6_rhs)
+//   mode 1: out = a U0 + b (U + dt dQ/dt)  (a = 0: stage 1, which also saves U0 = U)   (Eq. B.1)
+// and the primitives of the new state go to the OTHER primitive buffer (the current one is still being read by
+// neighbouring tiles), ready for the ghost fill of the next stage.
+struct Fuse3 {
+  const double* U; const double* U0; double* U0w; double* out;
+  const double* rj; const double* rjt; const double* sigma; const double* uref;
+  double* Pn;                   // next primitive buffer (field 0; stride fsP) or null
+  double a, b, dt;
+  int mode;
+};
+
 __device__ __forceinline__ uint32_t smem_u32_3(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
 __device__ __forceinline__ void tma4(void* dst, const CUtensorMap* tm, uint64_t* bar, int c0, int c1, int c2, int c3) {
   asm volatile(
       "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"
       ::"r"(smem_u32_3(dst)), "l"((uint64_t)tm), "r"(smem_u32_3(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
+}
+
+__device__ __forceinline__ void tma_prefetch4(const CUtensorMap* tm, int c0, int c1, int c2, int c3) {
+  asm volatile("cp.async.bulk.prefetch.tensor.4d.L2.global.tile [%0, {%1, %2, %3, %4}];"
+               ::"l"((uint64_t)tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
+}
+
+__device__ __forceinline__ void mbar_wait3(uint64_t* bar) {   // phase 0 (every barrier is used once per CTA)
+  uint32_t done = 0;
+  const uint32_t b = smem_u32_3(bar);
+  while (!done) {
+    asm volatile(
+        "{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}\n"
+        : "=r"(done) : "r"(b), "r"(0) : "memory");
+  }
+}
+
+// shared-memory load the compiler may not merge with an earlier load of the same address: values that are needed
+// again long after their first use are re-read instead of being kept in registers across the limiter
+__device__ __forceinline__ double lds_again(const double* p) {
+#if MEG6_RELOAD
+  double v;
+  asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(smem_u32_3(p)));
+  return v;
+#else
+  return *p;
+#endif
 }
 
 __device__ __forceinline__ double minmod3(double a, double b) {   // E.2
@@ -230,6 +278,10 @@ __device__ __forceinline__ unsigned face3(const Consts& c, const double* __restr
     }
   }
   double PL[5], PR[5];
+#if MEG6_RELOAD
+#pragma unroll
+  for (int f = 0; f < 5; ++f) { BL[f] = lds_again(pP + f * FP + SS); BR[f] = lds_again(pP + f * FP + 2 * SS); }
+#endif
   backproject3(e, ia2, h_ira, EL, BL, PL);   // Eq. 23
   backproject3(e, ia2, h_ira, ER, BR, PR);
   hllc3(PL, PR, mx, my, mz, mt, g, g2, ig2, c.gamma, c.igm1, F);
@@ -241,7 +293,7 @@ __device__ __forceinline__ unsigned face3(const Consts& c, const double* __restr
     for (int f = 0; f < 4; ++f) {
       double cL, cR, gL, gR;
       if (f < 3) {
-        cL = BL[f + 1]; cR = BR[f + 1];
+        cL = lds_again(pP + (f + 1) * FP + SS); cR = lds_again(pP + (f + 1) * FP + 2 * SS);
         gL = pA[(f + 1) * FA + SS] - pA[(f + 6) * FA + SS];           // P' = aL - aR
         gR = pA[(f + 1) * FA + 2 * SS] - pA[(f + 6) * FA + 2 * SS];
       } else {
@@ -295,9 +347,10 @@ __device__ __forceinline__ unsigned face3(const Consts& c, const double* __restr
   return fl;
 }
 
-template <int DIR, bool VISC>
+template <int DIR, bool VISC, bool FUSE>
 __global__ void __launch_bounds__(Cfg3<DIR, VISC>::NT, Cfg3<DIR, VISC>::MINB) k_flux3(const Consts c, const FluxIn3 in,
-                                                                                     const __grid_constant__ TmaMaps tm) {
+                                                                                     const __grid_constant__ TmaMaps tm,
+                                                                                     const Fuse3 fu) {
   using C = Cfg3<DIR, VISC>;
   constexpr int TS = C::TS, TT = C::TT, NT = C::NT, NF = C::NF, LP = C::LP, LA = C::LA, LT = C::LT, LF = C::LF, LG = C::LG;
   constexpr int SS = (DIR == 0) ? 1 : TT;
@@ -323,53 +376,86 @@ __global__ void __launch_bounds__(Cfg3<DIR, VISC>::NT, Cfg3<DIR, VISC>::MINB) k_
 
   if (tid == 0) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32_3(bar)), "r"(1) : "memory");
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32_3(bar + 1)), "r"(1) : "memory");
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    uint32_t bytes = (C::nP + C::NM * LF * TT + C::nG) * 8;
-    if (in.moving) bytes += C::nMt * 8;
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32_3(bar)), "r"(bytes) : "memory");
-    // box coordinates are (i, j, k, field) in the padded layout of each array
-    if (DIR == 0) {
-      tma4(sP, &tm.P, bar, s0 - 6 + GPI, t0 + GPJ, o + GPK, 0);
-      tma4(sM, &tm.M, bar, s0, t0, o, 0);
-      if (in.moving) tma4(sMt, &tm.Mt, bar, s0, t0, o, 0);
-      if (VISC) {
-        tma4(sG, &tm.G, bar, s0 - 2 + GGI, t0 + GGJ, o + GGK, 4);
-        tma4(sG + 4 * FG, &tm.G, bar, s0 - 2 + GGI, t0 + GGJ, o + GGK, 8);
-      }
-    } else if (DIR == 1) {
-      tma4(sP, &tm.P, bar, t0 + GPI, s0 - 6 + GPJ, o + GPK, 0);
-      tma4(sM, &tm.M, bar, t0, s0, o, 0);
-      if (in.moving) tma4(sMt, &tm.Mt, bar, t0, s0, o, 0);
-      if (VISC) {
-        tma4(sG, &tm.G, bar, t0 + GGI, s0 - 1 + GGJ, o + GGK, 0);
-        tma4(sG + 4 * FG, &tm.G, bar, t0 + GGI, s0 - 1 + GGJ, o + GGK, 8);
-      }
-    } else {
-      tma4(sP, &tm.P, bar, t0 + GPI, o + GPJ, s0 - 6 + GPK, 0);
-      tma4(sM, &tm.M, bar, t0, o, s0, 0);
-      if (in.moving) tma4(sMt, &tm.Mt, bar, t0, o, s0, 0);
-      if (VISC) {
-        tma4(sG, &tm.G, bar, t0 + GGI, o + GGJ, s0 - 1 + GGK, 0);
-        tma4(sG + 4 * FG, &tm.G, bar, t0 + GGI, o + GGJ, s0 - 1 + GGK, 4);
+    uint32_t bytes1 = (C::NM * LF * TT + C::nG) * 8;
+    if (in.moving) bytes1 += C::nMt * 8;
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32_3(bar)), "r"(C::nP * 8) : "memory");
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32_3(bar + 1)), "r"(bytes1) : "memory");
+    // box coordinates are (i, j, k, field) in the padded layout of each array: sweep start, transverse start, other
+    auto coords = [](int s, int t, int oo, int gi, int gj, int gk, int& c0, int& c1, int& c2) {
+      if (DIR == 0) { c0 = s + gi; c1 = t + gj; c2 = oo + gk; }
+      else if (DIR == 1) { c0 = t + gi; c1 = s + gj; c2 = oo + gk; }
+      else { c0 = t + gi; c1 = oo + gj; c2 = s + gk; }
+    };
+    constexpr int G0 = (DIR == 0) ? 4 : 0, G1 = (DIR == 2) ? 4 : 8;      // the two tangential gradient groups
+    constexpr int GS = (DIR == 0) ? -2 : -1;                             // first stored-gradient cell of the box
+    int c0, c1, c2;
+    coords(s0 - 6, t0, o, GPI, GPJ, GPK, c0, c1, c2);
+    tma4(sP, &tm.P, bar, c0, c1, c2, 0);
+    coords(s0, t0, o, 0, 0, 0, c0, c1, c2);
+    tma4(sM, &tm.M, bar + 1, c0, c1, c2, 0);
+    if (in.moving) tma4(sMt, &tm.Mt, bar + 1, c0, c1, c2, 0);
+    if (VISC) {
+      coords(s0 + GS, t0, o, GGI, GGJ, GGK, c0, c1, c2);
+      tma4(sG, &tm.G, bar + 1, c0, c1, c2, G0);
+      tma4(sG + 4 * FG, &tm.G, bar + 1, c0, c1, c2, G1);
+    }
+#if MEG6_PF_DIST > 0
+    {
+      // L2 prefetch of the tile a later CTA will load (blocks are dispatched in linear order): its TMA loads then hit L2
+      const long long lin = (long long)blockIdx.x + (long long)gridDim.x * (blockIdx.y + (long long)gridDim.y * blockIdx.z) +
+                            MEG6_PF_DIST;
+      if (lin < (long long)gridDim.x * gridDim.y * gridDim.z) {
+        const int bx = (int)(lin % gridDim.x), by = (int)((lin / gridDim.x) % gridDim.y), bz = (int)(lin / ((long long)gridDim.x * gridDim.y));
+        int ps, pt, po;
+        if (DIR == 0) { ps = bx * TS; pt = by * TT; po = bz; }
+        else if (DIR == 1) { pt = bx * TT; ps = by * TS; po = bz; }
+        else { pt = bx * TT; po = by; ps = bz * TS; }
+        coords(ps - 6, pt, po, GPI, GPJ, GPK, c0, c1, c2);
+        tma_prefetch4(&tm.P, c0, c1, c2, 0);
+        coords(ps, pt, po, 0, 0, 0, c0, c1, c2);
+        tma_prefetch4(&tm.M, c0, c1, c2, 0);
+        if (in.moving) tma_prefetch4(&tm.Mt, c0, c1, c2, 0);
+        if (VISC) {
+          coords(ps + GS, pt, po, GGI, GGJ, GGK, c0, c1, c2);
+          tma_prefetch4(&tm.G, c0, c1, c2, G0);
+          tma_prefetch4(&tm.G, c0, c1, c2, G1);
+        }
       }
     }
+#endif
   }
-  __syncthreads();   // the barrier is initialised before anyone polls it
-  {
-    uint32_t done = 0;
-    const uint32_t b = smem_u32_3(bar);
-    while (!done) {
-      asm volatile(
-          "{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}\n"
-          : "=r"(done) : "r"(b), "r"(0) : "memory");
+  if (FUSE) {
+    // L2 prefetch of what the final phase will read from global memory (running residual, U, U0, 1/J, sponge):
+    // those loads sit at the tail of the CTA with nothing to overlap them
+    constexpr int SEG = (TS * 8 + 127) / 128 + 1;              // 128-byte lines per tile row (xi sweep)
+    const long long N = c.LC.n;
+    for (int it = tid; it < 22 * TT * SEG; it += NT) {
+      const int arr = it / (TT * SEG), rr = (it / SEG) % TT, sg = it % SEG;
+      int ci, cj, ck;
+      if (DIR == 0) { ci = s0 + sg * 16; cj = t0 + rr; ck = o; if (sg * 16 >= TS + 15) continue; }
+      else if (DIR == 1) { ci = t0; cj = s0 + sg; ck = o; }
+      else { ci = t0; cj = o; ck = s0 + sg; }
+      if (ci >= c.n[0] || cj >= c.n[1] || ck >= c.n[2]) continue;
+      const double* ptr = nullptr;
+      const long long ic = c.LC.at(ci, cj, ck);
+      if (arr < 5) ptr = in.first ? nullptr : in.res + arr * c.fsR + c.LR.at(ci, cj, ck);
+      else if (arr < 10) ptr = fu.U + (arr - 5) * N + ic;
+      else if (arr < 15) ptr = (fu.mode == 1 && fu.a != 0.0) ? fu.U0 + (arr - 10) * N + ic : nullptr;
+      else if (arr < 20) ptr = fu.sigma ? fu.uref + (arr - 15) * N + ic : nullptr;
+      else if (arr == 20) ptr = fu.sigma ? fu.sigma + ic : nullptr;
+      else ptr = fu.rj + c.LX.at(ci, cj, ck);
+      if (ptr) asm volatile("prefetch.global.L2 [%0];" ::"l"(ptr));
     }
   }
+  __syncthreads();   // the barriers are initialised before anyone polls them
+  mbar_wait3(bar);   // primitive tile
 
   // ---- per cell: aL = 1/2 P' + P''/12, aR = -1/2 P' + P''/12 (Eq. 16-17, 19) on cells -2..TS+1; T' on -1..TS ----
-  for (int it = tid; it < 5 * LA * TT; it += NT) {
-    int f, a, t;
-    if (DIR == 0) { a = it % LA; t = (it / LA) % TT; f = it / (LA * TT); }
-    else { t = it % TT; a = (it / TT) % LA; f = it / (TT * LA); }
+  // One (cell, lane) position per thread and pass, all five fields; the positions left over after the full
+  // passes are spread over the threads as (position, field) items so that no warp runs an extra pass alone.
+  auto cell_field = [&](int f, int a, int t) {
     const double* q = sP + sidx3<DIR, TT>(f, a + 4, t, LP);
     const double c0 = q[0], p1 = q[SS], m1 = q[-SS], p2 = q[2 * SS], m2 = q[-2 * SS], p3 = q[3 * SS], m3 = q[-3 * SS],
                  p4 = q[4 * SS], m4 = q[-4 * SS];
@@ -384,9 +470,55 @@ __global__ void __launch_bounds__(Cfg3<DIR, VISC>::NT, Cfg3<DIR, VISC>::MINB) k_
     const double h = 0.5 * d1, d = d2 * (1.0 / 12.0);
     sA[sidx3<DIR, TT>(f, a, t, LA)] = d + h;
     sA[sidx3<DIR, TT>(f + 5, a, t, LA)] = d - h;
+  };
+  if (DIR != 0) {
+    // eta/zeta sweeps: the sweep index is the slow one in shared memory, so one thread takes BLK consecutive cells
+    // of one lane and field: BLK + 8 loads instead of 9 BLK (shared-memory bandwidth was at 55-60 % of peak, r1c)
+    constexpr int BLK = 5, NQ = (LA + BLK - 1) / BLK;
+    for (int it = tid; it < NQ * TT * 5; it += NT) {
+      const int t = it % TT, qd = (it / TT) % NQ, f = it / (TT * NQ);
+      const int a0 = qd * BLK;
+      const double* q = sP + sidx3<DIR, TT>(f, a0, t, LP);
+      double v[BLK + 8];
+#pragma unroll
+      for (int m = 0; m < BLK + 8; ++m) v[m] = (a0 + m < LP) ? q[m * SS] : 0.0;
+#pragma unroll
+      for (int b = 0; b < BLK; ++b) {
+        if (a0 + b < LA) {
+          const double* w = v + b + 4;
+          double d1 = CE1 * (w[1] - w[-1]);
+          d1 = fma(CE2, w[2] - w[-2], d1);
+          d1 = fma(CE3, w[3] - w[-3], d1);
+          double d2 = CS0 * w[0];
+          d2 = fma(CS1, w[1] + w[-1], d2);
+          d2 = fma(CS2, w[2] + w[-2], d2);
+          d2 = fma(CS3, w[3] + w[-3], d2);
+          d2 = fma(CS4, w[4] + w[-4], d2);
+          const double h = 0.5 * d1, d = d2 * (1.0 / 12.0);
+          sA[sidx3<DIR, TT>(f, a0 + b, t, LA)] = d + h;
+          sA[sidx3<DIR, TT>(f + 5, a0 + b, t, LA)] = d - h;
+        }
+      }
+    }
+  } else {
+  constexpr int NPOS = LA * TT, NFULL = NPOS / NT, REM = NPOS - NFULL * NT;
+#pragma unroll
+  for (int k = 0; k < NFULL; ++k) {
+    const int p = tid + k * NT;
+    const int a = (DIR == 0) ? p % LA : p / TT, t = (DIR == 0) ? p / LA : p % TT;
+#pragma unroll
+    for (int f = 0; f < 5; ++f) cell_field(f, a, t);
+  }
+  if (REM > 0) {
+    for (int it = tid; it < REM * 5; it += NT) {
+      const int p = NFULL * NT + it % REM, f = it / REM;
+      const int a = (DIR == 0) ? p % LA : p / TT, t = (DIR == 0) ? p / LA : p % TT;
+      cell_field(f, a, t);
+    }
+  }
   }
   if (VISC) {
-    for (int it = tid; it < LT * TT; it += NT) {
+    for (int it = NT - 1 - tid; it < LT * TT; it += NT) {   // reversed: the leftover items go to the last warp
       int a, t;
       if (DIR == 0) { a = it % LT; t = it / LT; }
       else { t = it % TT; a = it / TT; }
@@ -398,6 +530,7 @@ __global__ void __launch_bounds__(Cfg3<DIR, VISC>::NT, Cfg3<DIR, VISC>::MINB) k_
     }
   }
   __syncthreads();
+  mbar_wait3(bar + 1);   // interface metrics and stored gradients (issued together with the primitive tile)
 
   // ---- one interface per thread ----
   int sI, row;
@@ -442,10 +575,45 @@ __global__ void __launch_bounds__(Cfg3<DIR, VISC>::NT, Cfg3<DIR, VISC>::MINB) k_
 #pragma unroll
       for (int f = 0; f < 5; ++f) old[f] = in.res[f * c.fsR + ac];
     }
+    double R[5];
 #pragma unroll
-    for (int f = 0; f < 5; ++f) {
-      const double dF = sM[sidx3<DIR, TT>(f, s + 1, t, LF)] - sM[sidx3<DIR, TT>(f, s, t, LF)];
-      in.res[f * c.fsR + ac] = old[f] - dF;
+    for (int f = 0; f < 5; ++f) R[f] = old[f] - (sM[sidx3<DIR, TT>(f, s + 1, t, LF)] - sM[sidx3<DIR, TT>(f, s, t, LF)]);
+    if (!FUSE) {
+#pragma unroll
+      for (int f = 0; f < 5; ++f) in.res[f * c.fsR + ac] = R[f];
+    } else {
+      int ci, cj, ck;
+      if (DIR == 0) { ci = s0 + s; cj = t0 + t; ck = o; }
+      else if (DIR == 1) { ci = t0 + t; cj = s0 + s; ck = o; }
+      else { ci = t0 + t; cj = o; ck = s0 + s; }
+      const long long N = c.LC.n, ic = c.LC.at(ci, cj, ck);
+      const double J = 1.0 / fu.rj[c.LX.at(ci, cj, ck)];
+      const double rjt = fu.rjt ? fu.rjt[ic] : 0.0;
+      const double sg = fu.sigma ? fu.sigma[ic] : 0.0;
+      double Q[5];
+#pragma unroll
+      for (int f = 0; f < 5; ++f) {
+        const double u = fu.U[f * N + ic];
+        double L = J * (R[f] - rjt * u);
+        if (fu.sigma) L -= sg * (u - fu.uref[f * N + ic]);
+        if (fu.mode == 0) Q[f] = L;
+        else {
+          double v = u + fu.dt * L;
+          if (fu.a != 0.0) v = fu.a * fu.U0[f * N + ic] + fu.b * v;
+          else if (fu.U0w) fu.U0w[f * N + ic] = u;
+          Q[f] = v;
+        }
+      }
+#pragma unroll
+      for (int f = 0; f < 5; ++f) fu.out[f * N + ic] = Q[f];
+      if (fu.Pn) {   // Q -> P of the new state (Eq. 5, P:83 inverted; T = p/(rho R)), as k_prim
+        const double r = Q[0], ir = 1.0 / r;
+        const double u = Q[1] * ir, v = Q[2] * ir, w = Q[3] * ir;
+        const double p = (c.gamma - 1.0) * (Q[4] - 0.5 * r * (u * u + v * v + w * w));
+        double* pn = fu.Pn + c.LP.at(ci, cj, ck);
+        pn[0] = r; pn[c.fsP] = u; pn[2 * c.fsP] = v; pn[3 * c.fsP] = w; pn[4 * c.fsP] = p;
+        pn[5 * c.fsP] = p / (r * c.r_gas);
+      }
     }
   }
 }
