@@ -24,9 +24,6 @@ namespace meg6 {
 #ifndef MEG6_MINB3_Y
 #define MEG6_MINB3_Y 5
 #endif
-#ifndef MEG6_PF_DIST
-#define MEG6_PF_DIST 0   // L2 prefetch distance in CTAs (0: off; 1024 measured slower on C4, r1)
-#endif
 #ifndef MEG6_RELOAD
 #define MEG6_RELOAD 1
 #endif
@@ -89,11 +86,6 @@ __device__ __forceinline__ void tma4(void* dst, const CUtensorMap* tm, uint64_t*
       ::"r"(smem_u32_3(dst)), "l"((uint64_t)tm), "r"(smem_u32_3(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
 }
 
-__device__ __forceinline__ void tma_prefetch4(const CUtensorMap* tm, int c0, int c1, int c2, int c3) {
-  asm volatile("cp.async.bulk.prefetch.tensor.4d.L2.global.tile [%0, {%1, %2, %3, %4}];"
-               ::"l"((uint64_t)tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
-}
-
 __device__ __forceinline__ void mbar_wait3(uint64_t* bar) {   // phase 0 (every barrier is used once per CTA)
   uint32_t done = 0;
   const uint32_t b = smem_u32_3(bar);
@@ -115,6 +107,11 @@ __device__ __forceinline__ double lds_again(const double* p) {
   return *p;
 #endif
 }
+
+// Reciprocal as its own operation: a/b is written a * rcp3(b) (the reciprocal sequence is shorter than the division
+// sequence; C4: -4 % on the sweeps).  Hand-rolled MUFU-seed + Newton versions without the library's special-case
+// branches were measured SLOWER in round 1 (more live registers, more spills).
+__device__ __forceinline__ double rcp3(double x) { return 1.0 / x; }
 
 __device__ __forceinline__ double minmod3(double a, double b) {   // E.2
   const double m = fmin(fabs(a), fabs(b));
@@ -159,24 +156,17 @@ __device__ __forceinline__ double mp_limit3(double e, double dp, double dm, doub
 }
 
 // Contravariant HLLC, Eq. 26-27 with the flux of Eq. 2; energy row R9; cascade R10.
-#ifndef MEG6_HLLC_MODE
-#define MEG6_HLLC_MODE 2
-#endif
 __device__ __forceinline__ void hllc3(const double PL[5], const double PR[5], double mx, double my, double mz, double mt,
                                       double g, double g2, double ig2, double gamma, double igm1, double F[5]) {
   const double UL = fma(mz, PL[3], fma(my, PL[2], fma(mx, PL[1], mt)));
   const double UR = fma(mz, PR[3], fma(my, PR[2], fma(mx, PR[1], mt)));
-#if MEG6_HLLC_MODE == 1
-  const double cL = sqrt(gamma * PL[4] / PL[0]) * g, cR = sqrt(gamma * PR[4] / PR[0]) * g;
-#else
-  const double t = 1.0 / (PL[0] * PR[0]);
+  const double t = rcp3(PL[0] * PR[0]);
   const double irL = PR[0] * t, irR = PL[0] * t;
   const double cL = sqrt(gamma * PL[4] * irL) * g, cR = sqrt(gamma * PR[4] * irR) * g;
-#endif
   const double SL = fmin(UL - cL, UR - cR);
   const double SR = fmax(UL + cL, UR + cR);
   const double mL = PL[0] * (SL - UL), mR = PR[0] * (SR - UR);
-  const double SS = (fma(mR, UR, -mL * UL) + (PL[4] - PR[4]) * g2) / (mR - mL);
+  const double SS = (fma(mR, UR, -mL * UL) + (PL[4] - PR[4]) * g2) * rcp3(mR - mL);
   const bool left = (SL >= 0.0) || (SS >= 0.0);
   const bool star = !(SL >= 0.0) && ((SS >= 0.0) || (SR >= 0.0));
   const double r = left ? PL[0] : PR[0], u = left ? PL[1] : PR[1], v = left ? PL[2] : PR[2];
@@ -190,22 +180,10 @@ __device__ __forceinline__ void hllc3(const double PL[5], const double PR[5], do
   F[3] = fma(ru, w, mz * p);
   F[4] = fma(E + p, UK, -mt * p);
   if (star) {
-    const double dS = SK - UK, dK = SK - SS, dSU = SS - UK;
-#if MEG6_HLLC_MODE == 1
-    // the quotients exactly as Eq. 27 states them
-    const double fac = r * dS / dK;
-    const double dU = dSU * ig2;
-    const double q1 = fac * fma(mx, dU, u), q2 = fac * fma(my, dU, v), q3 = fac * fma(mz, dU, w);
-    const double q4 = fac * (E / r + dSU * ((SS - mt) * ig2 + p / (r * dS)));
-    F[0] = fma(SK, fac - r, F[0]);
-    F[1] = fma(SK, q1 - r * u, F[1]);
-    F[2] = fma(SK, q2 - r * v, F[2]);
-    F[3] = fma(SK, q3 - r * w, F[3]);
-    F[4] = fma(SK, q4 - E, F[4]);
-#else
+    const double dK = SK - SS, dSU = SS - UK;
     // Q*_K - Q_K without cancellation: fac - rho_K = rho_K (S* - U_K)/(S_K - S*), and
     // fac (S*-U_K) p/(rho_K (S_K-U_K)) = p (S*-U_K)/(S_K-S*)
-    const double idK = 1.0 / dK;
+    const double idK = rcp3(dK);
     const double k = dSU * idK;              // (S* - U_K)/(S_K - S*)
     const double rk = r * k;                 // fac - rho_K
     const double fd = (r + rk) * dSU * ig2;  // fac (S* - U_K)/g^2
@@ -214,7 +192,6 @@ __device__ __forceinline__ void hllc3(const double PL[5], const double PR[5], do
     F[2] = fma(SK, fma(rk, v, fd * my), F[2]);
     F[3] = fma(SK, fma(rk, w, fd * mz), F[3]);
     F[4] = fma(SK, fma(k, E + p, fd * (SS - mt)), F[4]);
-#endif
   }
 }
 
@@ -238,7 +215,7 @@ __device__ __forceinline__ unsigned face3(const Consts& c, const double* __restr
 #pragma unroll
   for (int f = 0; f < 5; ++f) { BL[f] = pP[f * FP + SS]; BR[f] = pP[f * FP + 2 * SS]; }
   const double rb = 0.5 * (BL[0] + BR[0]), pb = 0.5 * (BL[4] + BR[4]);   // R5
-  const double irb = 1.0 / rb;
+  const double irb = rcp3(rb);
   e.a2 = c.gamma * pb * irb;
   const double ia = rsqrt(e.a2), a = e.a2 * ia;
   e.ra = rb * a;
@@ -315,10 +292,10 @@ __device__ __forceinline__ unsigned face3(const Consts& c, const double* __restr
     // Sutherland (R15) and 1/(1/J) with one division
     const double rjh = pM[9 * FM];
     double mu, irj;
-    if (c.s_suth < 0.0) { mu = c.mu_ref; irj = 1.0 / rjh; }
+    if (c.s_suth < 0.0) { mu = c.mu_ref; irj = rcp3(rjh); }
     else {
       const double ts = val[3] + c.s_suth;
-      const double t = 1.0 / (rjh * ts);
+      const double t = rcp3(rjh * ts);
       irj = ts * t;
       mu = c.suth_c * val[3] * sqrt(val[3]) * (rjh * t);
     }
@@ -401,30 +378,6 @@ __global__ void __launch_bounds__(Cfg3<DIR, VISC>::NT, Cfg3<DIR, VISC>::MINB) k_
       tma4(sG, &tm.G, bar + 1, c0, c1, c2, G0);
       tma4(sG + 4 * FG, &tm.G, bar + 1, c0, c1, c2, G1);
     }
-#if MEG6_PF_DIST > 0
-    {
-      // L2 prefetch of the tile a later CTA will load (blocks are dispatched in linear order): its TMA loads then hit L2
-      const long long lin = (long long)blockIdx.x + (long long)gridDim.x * (blockIdx.y + (long long)gridDim.y * blockIdx.z) +
-                            MEG6_PF_DIST;
-      if (lin < (long long)gridDim.x * gridDim.y * gridDim.z) {
-        const int bx = (int)(lin % gridDim.x), by = (int)((lin / gridDim.x) % gridDim.y), bz = (int)(lin / ((long long)gridDim.x * gridDim.y));
-        int ps, pt, po;
-        if (DIR == 0) { ps = bx * TS; pt = by * TT; po = bz; }
-        else if (DIR == 1) { pt = bx * TT; ps = by * TS; po = bz; }
-        else { pt = bx * TT; po = by; ps = bz * TS; }
-        coords(ps - 6, pt, po, GPI, GPJ, GPK, c0, c1, c2);
-        tma_prefetch4(&tm.P, c0, c1, c2, 0);
-        coords(ps, pt, po, 0, 0, 0, c0, c1, c2);
-        tma_prefetch4(&tm.M, c0, c1, c2, 0);
-        if (in.moving) tma_prefetch4(&tm.Mt, c0, c1, c2, 0);
-        if (VISC) {
-          coords(ps + GS, pt, po, GGI, GGJ, GGK, c0, c1, c2);
-          tma_prefetch4(&tm.G, c0, c1, c2, G0);
-          tma_prefetch4(&tm.G, c0, c1, c2, G1);
-        }
-      }
-    }
-#endif
   }
   if (FUSE) {
     // L2 prefetch of what the final phase will read from global memory (running residual, U, U0, 1/J, sponge):
@@ -595,7 +548,7 @@ __global__ void __launch_bounds__(Cfg3<DIR, VISC>::NT, Cfg3<DIR, VISC>::MINB) k_
       for (int f = 0; f < 5; ++f) {
         const double u = fu.U[f * N + ic];
         double L = J * (R[f] - rjt * u);
-        if (fu.sigma) L -= sg * (u - fu.uref[f * N + ic]);
+        if (sg != 0.0) L -= sg * (u - fu.uref[f * N + ic]);   // sigma = 0 outside the sponge: Q_ref is not read there
         if (fu.mode == 0) Q[f] = L;
         else {
           double v = u + fu.dt * L;
