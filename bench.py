@@ -154,6 +154,21 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def max_over_ranks(values, dist, device):
+    """Device-side times of one rank -> the maximum over all ranks (the job ends when the slowest rank does)."""
+    import torch
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t]
+
+
+def whole_job_throughput(ncell_per_rank, steps, world, ms):
+    """Mcell-updates/s per RK stage of the whole job: every rank advances its own replica of ncell cells by
+    `steps` RK3 steps (3 stages each) in `ms` milliseconds (max over ranks).  Weak scaling, no data-path collective."""
+    return ncell_per_rank * 3 * steps * world / (ms * 1e-3) / 1e6
+
+
 def run_ours(args):
     import torch
     from paper_2303_10785_b200 import Grid
@@ -227,17 +242,14 @@ def run_ours(args):
     barrier()
     ms_e2e = f0.elapsed_time(f1)
 
-    tms = torch.tensor([ms, ms_e2e], dtype=torch.float64, device=dev)
-    if dist:
-        dist.all_reduce(tms, op=dist.ReduceOp.MAX)
-    ms, ms_e2e = float(tms[0]), float(tms[1])
+    ms, ms_e2e = max_over_ranks([ms, ms_e2e], dist, dev)
     if rank != 0:
         if dist:
             dist.destroy_process_group()
         return
 
-    value = ncell * 3 * args.steps * world / (ms * 1e-3) / 1e6
-    e2e_value = ncell * 3 * args.steps * world / (ms_e2e * 1e-3) / 1e6
+    value = whole_job_throughput(ncell, args.steps, world, ms)
+    e2e_value = whole_job_throughput(ncell, args.steps, world, ms_e2e)
     hbm, sm_max, peak_src = peaks()
     bpc = bytes_per_cell_stage(prm, wl.get("sigma") is not None)
     stage_bytes = sum(bpc.values())

@@ -10,12 +10,16 @@ import subprocess
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_SO = os.path.join(_HERE, "libmeg6_oracle.so")
+# MEG6_ORACLE_SO: load another build of the SAME source (tests/test_oracle_sensitivity.py builds one with FMA
+# contraction switched on to measure how far rounding order alone moves the oracle)
+_SO = os.environ.get("MEG6_ORACLE_SO") or os.path.join(_HERE, "libmeg6_oracle.so")
 _SRC = [os.path.join(_HERE, "meg6_oracle.cpp"), os.path.join(_HERE, "meg6_oracle.h")]
 
 
 def build(force=False):
     """Compile the oracle with the system g++ (-O2 -ffp-contract=off, OpenMP if available)."""
+    if os.environ.get("MEG6_ORACLE_SO"):
+        return _SO
     if not force and os.path.exists(_SO) and all(os.path.getmtime(_SO) >= os.path.getmtime(s) for s in _SRC):
         return _SO
     base = ["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fPIC", "-shared", "-o", _SO, _SRC[0]]

@@ -40,8 +40,9 @@ def rhs_err(a, b, U, gamma=1.4):
     (dQ_c/dt / ref_c, ref = (rho0, rho0 a0, rho0 a0, rho0 a0, rho0 a0^2)) brought back to the units of
     component c.  A component that is physically tiny (the mass equation of the nearly incompressible
     Taylor-Green vortex is 1e-3 of the flux scale) is thereby not normalised by its own cancellation
-    residue; tests/test_oracle_sensitivity.py shows that the oracle itself moves by > 1e-11 in the
-    per-component norm when only its FMA contraction changes.  DESIGN.md, "Tolerances"."""
+    residue.  tests/test_oracle_sensitivity.py measures how far FMA contraction alone moves the oracle on the
+    same case (2.5e-11: more than the tolerance), which is why the metric kernels are bit-exact.
+    DESIGN.md, "Tolerances"."""
     rho = U[0]
     p = (gamma - 1) * (U[4] - 0.5 * (U[1] ** 2 + U[2] ** 2 + U[3] ** 2) / rho)
     rho0, a0 = rho.mean(), np.sqrt(gamma * p / rho).mean()
@@ -213,4 +214,112 @@ def test_sponge_and_rk3_closed_form_on_gpu(mods):
     zz = -0.28
     amp = 1 + zz + zz ** 2 / 2 + zz ** 3 / 6
     assert np.allclose(U.cpu().numpy() - Uref, amp * (U0 - Uref), rtol=1e-12, atol=1e-13)
+    g.close()
+
+
+# ---------------------------------------------------------------------------------------------------------
+# Full sizes of BASELINE.json, in the launch configuration bench.py times.
+
+def test_c1_full_config_10_steps(mods):
+    """Config 1 as BASELINE.json states it: 32^3 wavy mesh, CFL 0.5, 10 RK3 steps, against the oracle."""
+    torch, O, M = mods
+    wl = W.c1_vortex(n=32)
+    og = O.Grid(wl)
+    og.metrics_compute(0.0)
+    dt = wl["dt"] if wl["dt"] else og.cfl_dt(wl["U0"], wl["cfl"])
+    g = M.Grid(wl)
+    g.metrics_compute(0.0)
+    Uo = wl["U0"].copy()
+    U = torch.as_tensor(wl["U0"], device="cuda").contiguous()
+    t = 0.0
+    for s in range(10):
+        og.rk3_step(Uo, t, dt)
+        g.rk3_step(U, t, dt)
+        t += dt
+    e = rel(U.cpu().numpy(), Uo)
+    assert np.all(e <= STEP_TOL), e
+    g.close()
+
+
+def test_c2_full_config_freestream_100_steps(mods):
+    """Config 2 as BASELINE.json states it (64^3 jittered moving mesh, 100 RK3 steps): the residual stays <= 1e-12.
+    A property that holds at any size; no oracle run is needed at this length."""
+    torch, O, M = mods
+    wl = W.c2_dynamic_freestream(n=64)
+    g = M.Grid(wl)
+    g.metrics_compute(0.0)
+    U = torch.as_tensor(wl["U0"], device="cuda").contiguous()
+    dt = wl["dt"] if wl["dt"] else g.cfl_dt(U, wl["cfl"])
+    t = 0.0
+    worst = 0.0
+    for s in range(100):
+        if s % 20 == 0:
+            g.metrics_compute(t)
+            worst = max(worst, float((dt * g.rhs(U)).abs().max()))
+        g.rk3_step(U, t, dt)
+        t += dt
+    Uh = U.cpu().numpy()
+    p = 0.4 * (Uh[4] - 0.5 * (Uh[1] ** 2 + Uh[2] ** 2 + Uh[3] ** 2) / Uh[0])
+    p0 = 1.0 / (1.4 * 0.25)
+    dev = max(np.abs(Uh[0] - 1).max(), np.abs(Uh[1] / Uh[0] - 1).max(), np.abs(Uh[2] / Uh[0]).max(),
+              np.abs(Uh[3] / Uh[0]).max(), np.abs(p - p0).max() / p0)
+    assert worst <= 1e-12 and dev <= 1e-12, (worst, dev)
+    g.close()
+
+
+def test_c4_full_size_rhs_and_step(mods):
+    """The bench workload itself (320 x 200 x 200 jet mesh, inflow/outflow, sponge, viscous): one dQ/dt and one
+    RK3 step of a seeded randomised state against the oracle, every cell compared."""
+    torch, O, M = mods
+    wl = W.c4_jet()
+    rng = np.random.default_rng(44)
+    shape = wl["U0"].shape[1:]
+    rho = 1.0 + 0.2 * rng.uniform(-1, 1, shape)
+    u, v, w = (0.3 * rng.uniform(-1, 1, shape) for _ in range(3))
+    p = (1.0 + 0.2 * rng.uniform(-1, 1, shape)) / 1.4
+    U0 = W.conservative(rho, u, v, w, p)
+    del rho, u, v, w, p
+    og = O.Grid(wl)
+    og.metrics_compute(0.0)
+    ref = og.rhs(U0)
+    g = M.Grid(wl)
+    g.metrics_compute(0.0)
+    U = torch.as_tensor(U0, device="cuda").contiguous()
+    out = g.rhs(U).cpu().numpy()
+    e = rhs_err(out, ref, U0)
+    assert np.all(e <= RHS_TOL), (e, rel(out, ref))
+    del out, ref
+    Uo = U0.copy()
+    og.rk3_step(Uo, 0.0, wl["dt"])
+    g.rk3_step(U, 0.0, wl["dt"])
+    e2 = rel(U.cpu().numpy(), Uo)
+    assert np.all(e2 <= STEP_TOL), e2
+    print("c4 full size: rhs %s, one step %s" % (e, e2))
+    g.close()
+
+
+@pytest.mark.parametrize("shape", [(10, 10, 10), (31, 17, 16), (61, 12, 46)])
+def test_ragged_shapes_non_periodic_viscous(mods, shape):
+    """Tile tails in every direction (xi tiles of 30 cells x 4 rows, eta/zeta tiles of 15 cells x 8 lanes), down to
+    the minimum size, with inflow/outflow ghosts, sponge and viscous terms."""
+    torch, O, M = mods
+    wl = W.c4_jet(ni=shape[0], nj=shape[1], nk=shape[2], steps=2)
+    rng = np.random.default_rng(sum(shape))
+    sh = wl["U0"].shape[1:]
+    wl["U0"] = W.conservative(1.0 + 0.2 * rng.uniform(-1, 1, sh), *(0.3 * rng.uniform(-1, 1, sh) for _ in range(3)),
+                              (1.0 + 0.2 * rng.uniform(-1, 1, sh)) / 1.4)
+    og = O.Grid(wl)
+    og.metrics_compute(0.0)
+    g = M.Grid(wl)
+    g.metrics_compute(0.0)
+    U = torch.as_tensor(wl["U0"], device="cuda").contiguous()
+    e = rhs_err(g.rhs(U).cpu().numpy(), og.rhs(wl["U0"]), wl["U0"])
+    assert np.all(e <= RHS_TOL), e
+    Uo = wl["U0"].copy()
+    t = 0.0
+    for s in range(2):
+        og.rk3_step(Uo, t, wl["dt"])
+        g.rk3_step(U, t, wl["dt"])
+        t += wl["dt"]
+    assert np.all(rel(U.cpu().numpy(), Uo) <= STEP_TOL)
     g.close()
