@@ -319,7 +319,7 @@ static meg6_status stage(meg6_grid* g, int buf, const Fuse3& fu) {
     gin.inflow[0] = g->inflow[2 * d]; gin.inflow[1] = g->inflow[2 * d + 1];
     gin.mx = g->met[3 * d]; gin.my = g->met[3 * d + 1]; gin.mz = g->met[3 * d + 2];
     ProfScope ps(g, 2, 1);
-    k_ghost<<<nblk(ea * eb * 2, 128), 128, 0, g->stream>>>(c, d, P, gin);
+    k_ghost<<<nblk(ea * eb * 12, 256), 256, 0, g->stream>>>(c, d, P, gin);
   }
   if (g->p.viscous) {
     P12 G;

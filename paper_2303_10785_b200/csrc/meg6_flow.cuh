@@ -27,53 +27,50 @@ struct GhostIn { const double* inflow[2]; const double* mx; const double* my; co
 
 // B: ghost layers of direction d (6 deep), after the lower directions have been filled: periodic wrap, fixed
 // inflow ghost = 2 P_in - P_mirror, outflow ghost = last interior cell with p = p_out where the outward normal
-// Mach number is below one (Table 1, R20).  One thread per transverse position and side.
-__global__ void k_ghost(Consts c, int d, P6 P, GhostIn in) {
+// Mach number is below one (Table 1, R20).  One thread per GHOST CELL (all six fields): the twelve ghost
+// cells of a xi line, or the xi-contiguous cells of an eta/zeta ghost layer, go to consecutive threads.
+__global__ void __launch_bounds__(256) k_ghost(Consts c, int d, P6 P, GhostIn in) {
   int a = (d + 1) % 3, b = (d + 2) % 3;
   if (a > b) { int t = a; a = b; b = t; }
-  const int g[3] = {GPJ, GPJ, GPK};   // ghost depth filled per direction (6 everywhere)
+  constexpr int NG = 6;
   // transverse ranges: directions below d are already extended
-  const int loa = (a < d) ? -g[a] : 0, ea = c.n[a] + ((a < d) ? 2 * g[a] : 0);
-  const int lob = (b < d) ? -g[b] : 0, eb = c.n[b] + ((b < d) ? 2 * g[b] : 0);
+  const int loa = (a < d) ? -NG : 0, ea = c.n[a] + ((a < d) ? 2 * NG : 0);
+  const int lob = (b < d) ? -NG : 0, eb = c.n[b] + ((b < d) ? 2 * NG : 0);
   const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (tid >= (long long)ea * eb * 2) return;
-  const int side = (int)(tid / ((long long)ea * eb));
-  const long long r = tid % ((long long)ea * eb);
-  const int ta = loa + (int)(r % ea), tb = lob + (int)(r / ea);
+  if (tid >= (long long)ea * eb * 2 * NG) return;
+  int qs, ta, tb;   // qs = layer + 6 * side
+  if (d == 0) { qs = (int)(tid % (2 * NG)); const long long r = tid / (2 * NG); ta = loa + (int)(r % ea); tb = lob + (int)(r / ea); }
+  else if (d == 1) { ta = loa + (int)(tid % ea); const long long r = tid / ea; qs = (int)(r % (2 * NG)); tb = lob + (int)(r / (2 * NG)); }
+  else { ta = loa + (int)(tid % ea); const long long r = tid / ea; tb = lob + (int)(r % eb); qs = (int)(r / eb); }
+  const int side = qs / NG, q = qs % NG + 1;   // q-th ghost layer, 1 = next to the boundary
   int ix[3];
-  ix[a] = ta; ix[b] = tb;
+  ix[a] = ta; ix[b] = tb; ix[d] = 0;
   const int n = c.n[d];
   const long long s = c.LP.stride(d);
-  ix[d] = 0;
   const long long base = c.LP.at(ix[0], ix[1], ix[2]);   // cell 0 of this line
-  const int NG = 6;
+  const int last = side ? n - 1 : 0, sg = side ? 1 : -1;
+  const long long dst = base + (long long)(last + sg * q) * s;
   if (c.periodic[d]) {
-    for (int q = 1; q <= NG; ++q)
+    const long long src = side ? base + (long long)(q - 1) * s : base + (long long)(n - q) * s;
+    double v[6];
 #pragma unroll
-      for (int f = 0; f < 6; ++f) {
-        if (side == 0) P.p[f][base - q * s] = P.p[f][base + (long long)(n - q) * s];
-        else P.p[f][base + (long long)(n - 1 + q) * s] = P.p[f][base + (long long)(q - 1) * s];
-      }
+    for (int f = 0; f < 6; ++f) v[f] = P.p[f][src];
+#pragma unroll
+    for (int f = 0; f < 6; ++f) P.p[f][dst] = v[f];
     return;
   }
-  const int face = 2 * d + side, bc = c.bc[face];
-  const int last = side ? n - 1 : 0, sg = side ? 1 : -1;
+  const int bc = c.bc[2 * d + side];
   const int ca = min(max(ta, 0), c.n[a] - 1), cb = min(max(tb, 0), c.n[b] - 1);
   if (bc == 1) {
     const long long nf = (long long)c.n[a] * c.n[b];
     const double* pin = in.inflow[side] + (long long)cb * c.n[a] + ca;
-    double pi5[5];
+    const long long mir = base + (long long)(last - sg * (q - 1)) * s;
+    double v[5];
 #pragma unroll
-    for (int f = 0; f < 5; ++f) pi5[f] = pin[f * nf];
-    for (int q = 1; q <= NG; ++q) {
-      double v[5];
+    for (int f = 0; f < 5; ++f) v[f] = 2.0 * pin[f * nf] - P.p[f][mir];
 #pragma unroll
-      for (int f = 0; f < 5; ++f) {
-        v[f] = 2.0 * pi5[f] - P.p[f][base + (long long)(last - sg * (q - 1)) * s];
-        P.p[f][base + (long long)(last + sg * q) * s] = v[f];
-      }
-      P.p[5][base + (long long)(last + sg * q) * s] = v[4] / (v[0] * c.r_gas);
-    }
+    for (int f = 0; f < 5; ++f) P.p[f][dst] = v[f];
+    P.p[5][dst] = v[4] / (v[0] * c.r_gas);
   } else {
     double pv[5];
 #pragma unroll
@@ -86,12 +83,9 @@ __global__ void k_ghost(Consts c, int d, P6 P, GhostIn in) {
     const double cs = sqrt(c.gamma * pv[4] / pv[0]);
     const double mn = sg * (mx * pv[1] + my * pv[2] + mz * pv[3]) / (gm * cs);
     if (mn < 1.0) pv[4] = c.p_out;
-    const double T = pv[4] / (pv[0] * c.r_gas);
-    for (int q = 1; q <= NG; ++q) {
 #pragma unroll
-      for (int f = 0; f < 5; ++f) P.p[f][base + (long long)(last + sg * q) * s] = pv[f];
-      P.p[5][base + (long long)(last + sg * q) * s] = T;
-    }
+    for (int f = 0; f < 5; ++f) P.p[f][dst] = pv[f];
+    P.p[5][dst] = pv[4] / (pv[0] * c.r_gas);
   }
 }
 

@@ -379,26 +379,30 @@ __global__ void __launch_bounds__(Cfg3<DIR, VISC>::NT, Cfg3<DIR, VISC>::MINB) k_
       tma4(sG + 4 * FG, &tm.G, bar + 1, c0, c1, c2, G1);
     }
   }
-  if (FUSE) {
-    // L2 prefetch of what the final phase will read from global memory (running residual, U, U0, 1/J, sponge):
-    // those loads sit at the tail of the CTA with nothing to overlap them
-    constexpr int SEG = (TS * 8 + 127) / 128 + 1;              // 128-byte lines per tile row (xi sweep)
+  if (FUSE || !in.first) {
+    // L2 prefetch of what the final phase will read from global memory (running residual; fused: U, U0, 1/J,
+    // sponge): those loads sit at the tail of the CTA with nothing to overlap them
+    constexpr int NROW = (DIR == 0) ? TT : TS;                  // tile rows that are contiguous in memory
+    constexpr int SEG = (DIR == 0) ? (TS + 15) / 16 + 1 : 1;    // 128-byte lines per row
+    constexpr int NARR = FUSE ? 22 : 5;
     const long long N = c.LC.n;
-    for (int it = tid; it < 22 * TT * SEG; it += NT) {
-      const int arr = it / (TT * SEG), rr = (it / SEG) % TT, sg = it % SEG;
+    for (int it = tid; it < NARR * NROW * SEG; it += NT) {
+      const int arr = it / (NROW * SEG), rr = (it / SEG) % NROW, sg = it % SEG;
       int ci, cj, ck;
       if (DIR == 0) { ci = s0 + sg * 16; cj = t0 + rr; ck = o; if (sg * 16 >= TS + 15) continue; }
-      else if (DIR == 1) { ci = t0; cj = s0 + sg; ck = o; }
-      else { ci = t0; cj = o; ck = s0 + sg; }
+      else if (DIR == 1) { ci = t0; cj = s0 + rr; ck = o; }
+      else { ci = t0; cj = o; ck = s0 + rr; }
       if (ci >= c.n[0] || cj >= c.n[1] || ck >= c.n[2]) continue;
       const double* ptr = nullptr;
-      const long long ic = c.LC.at(ci, cj, ck);
       if (arr < 5) ptr = in.first ? nullptr : in.res + arr * c.fsR + c.LR.at(ci, cj, ck);
-      else if (arr < 10) ptr = fu.U + (arr - 5) * N + ic;
-      else if (arr < 15) ptr = (fu.mode == 1 && fu.a != 0.0) ? fu.U0 + (arr - 10) * N + ic : nullptr;
-      else if (arr < 20) ptr = fu.sigma ? fu.uref + (arr - 15) * N + ic : nullptr;
-      else if (arr == 20) ptr = fu.sigma ? fu.sigma + ic : nullptr;
-      else ptr = fu.rj + c.LX.at(ci, cj, ck);
+      else {
+        const long long ic = c.LC.at(ci, cj, ck);
+        if (arr < 10) ptr = fu.U + (arr - 5) * N + ic;
+        else if (arr < 15) ptr = (fu.mode == 1 && fu.a != 0.0) ? fu.U0 + (arr - 10) * N + ic : nullptr;
+        else if (arr < 20) ptr = fu.sigma ? fu.uref + (arr - 15) * N + ic : nullptr;
+        else if (arr == 20) ptr = fu.sigma ? fu.sigma + ic : nullptr;
+        else ptr = fu.rj + c.LX.at(ci, cj, ck);
+      }
       if (ptr) asm volatile("prefetch.global.L2 [%0];" ::"l"(ptr));
     }
   }
