@@ -344,7 +344,7 @@ static meg6_status stage(meg6_grid* g, int buf, const Fuse3& fu) {
   {
     ProfScope ps(g, 6, 1);
     i3.first = 0;
-    dim3 grid(nblk(c.n[0], Cfg3<2, false>::TT), c.n[1], nblk(c.n[2], Cfg3<2, false>::TS));
+    dim3 grid(nblk(c.n[0], Cfg3<2, false>::TT), nblk(c.n[2], Cfg3<2, false>::TS), c.n[1]);
     if (V) LAUNCH3(2, true, false, grid); else LAUNCH3(2, false, false, grid);
   }
   {

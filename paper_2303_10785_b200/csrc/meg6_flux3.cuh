@@ -347,7 +347,7 @@ __global__ void __launch_bounds__(Cfg3<DIR, VISC>::NT, Cfg3<DIR, VISC>::MINB) k_
   int s0, t0, o;
   if (DIR == 0) { s0 = blockIdx.x * TS; t0 = blockIdx.y * TT; o = blockIdx.z; }
   else if (DIR == 1) { t0 = blockIdx.x * TT; s0 = blockIdx.y * TS; o = blockIdx.z; }
-  else { t0 = blockIdx.x * TT; o = blockIdx.y; s0 = blockIdx.z * TS; }
+  else { t0 = blockIdx.x * TT; s0 = blockIdx.y * TS; o = blockIdx.z; }   // chunks of a line run back to back (halo re-use in L2)
   const int nd = c.n[DIR];
   const int nt = (DIR == 0) ? c.n[1] : c.n[0];
 
@@ -458,26 +458,23 @@ __global__ void __launch_bounds__(Cfg3<DIR, VISC>::NT, Cfg3<DIR, VISC>::MINB) k_
       }
     }
   } else {
-  constexpr int NPOS = LA * TT, NFULL = NPOS / NT, REM = NPOS - NFULL * NT;
+    // xi sweep: one warp per row, and a row needs nothing from the other rows: the warp fills the offsets of its own
+    // row and carries on without a CTA-wide barrier (the warps of a CTA drift apart and overlap each other's tails)
+    const int t = tid >> 5, lane = tid & 31;
+    for (int a = lane; a < LA; a += 32) {
+      if (a < 32) {
 #pragma unroll
-  for (int k = 0; k < NFULL; ++k) {
-    const int p = tid + k * NT;
-    const int a = (DIR == 0) ? p % LA : p / TT, t = (DIR == 0) ? p / LA : p % TT;
-#pragma unroll
-    for (int f = 0; f < 5; ++f) cell_field(f, a, t);
-  }
-  if (REM > 0) {
-    for (int it = tid; it < REM * 5; it += NT) {
-      const int p = NFULL * NT + it % REM, f = it / REM;
-      const int a = (DIR == 0) ? p % LA : p / TT, t = (DIR == 0) ? p / LA : p % TT;
-      cell_field(f, a, t);
+        for (int f = 0; f < 5; ++f) cell_field(f, a, t);
+      }
     }
-  }
+    for (int it = lane; it < (LA - 32) * 5; it += 32) cell_field(it / (LA - 32), 32 + it % (LA - 32), t);
   }
   if (VISC) {
-    for (int it = NT - 1 - tid; it < LT * TT; it += NT) {   // reversed: the leftover items go to the last warp
+    // T' on cells -1..TS.  xi: lane = cell of the warp's own row; eta/zeta: reversed so that the leftover items go to
+    // the last warp
+    for (int it = (DIR == 0) ? (tid & 31) : NT - 1 - tid; it < ((DIR == 0) ? LT : LT * TT); it += (DIR == 0) ? 32 : NT) {
       int a, t;
-      if (DIR == 0) { a = it % LT; t = it / LT; }
+      if (DIR == 0) { a = it; t = tid >> 5; }
       else { t = it % TT; a = it / TT; }
       const double* q = sP + sidx3<DIR, TT>(5, a + 5, t, LP);
       double d1 = CE1 * (q[SS] - q[-SS]);
@@ -486,7 +483,7 @@ __global__ void __launch_bounds__(Cfg3<DIR, VISC>::NT, Cfg3<DIR, VISC>::MINB) k_
       sT1[sidx3<DIR, TT>(0, a, t, LT)] = d1;
     }
   }
-  __syncthreads();
+  if (DIR == 0) __syncwarp(); else __syncthreads();
   mbar_wait3(bar + 1);   // interface metrics and stored gradients (issued together with the primitive tile)
 
   // ---- one interface per thread ----
@@ -504,7 +501,7 @@ __global__ void __launch_bounds__(Cfg3<DIR, VISC>::NT, Cfg3<DIR, VISC>::MINB) k_
         sM + sidx3<DIR, TT>(0, sI, row, LF), mt, F);
     if (sI < TS || s0 + sI == nd) { nlim = __popc(fl); ntst = 10; }   // tile-shared faces counted once
   }
-  if (sI <= TS) {
+  if (DIR != 0 && sI <= TS) {
     // the flux tile aliases the metric tile: slot (sI,row) of every metric field is read only by this thread
 #pragma unroll
     for (int f = 0; f < 5; ++f) sM[sidx3<DIR, TT>(f, sI, row, LF)] = F[f];
@@ -516,13 +513,8 @@ __global__ void __launch_bounds__(Cfg3<DIR, VISC>::NT, Cfg3<DIR, VISC>::MINB) k_
     }
     if ((tid & 31) == 0 && ntst) { atomicAdd(in.stats, (unsigned long long)nlim); atomicAdd(in.stats + 1, (unsigned long long)ntst); }
   }
-  __syncthreads();
-  // ---- flux difference, Eq. 25: Res_i -= F_{i+1/2} - F_{i-1/2} ----
-  for (int it = tid; it < TS * TT; it += NT) {
-    int s, t;
-    if (DIR == 0) { s = it % TS; t = it / TS; }
-    else { t = it % TT; s = it / TT; }
-    if (s0 + s >= nd || t0 + t >= nt) continue;
+  // ---- flux difference, Eq. 25: Res_i -= F_{i+1/2} - F_{i-1/2}, then (last sweep) assembly + update ----
+  auto finish_cell = [&](int s, int t, const double dF[5]) {
     long long ac;
     if (DIR == 0) ac = c.LR.at(s0 + s, t0 + t, o);
     else if (DIR == 1) ac = c.LR.at(t0 + t, s0 + s, o);
@@ -534,7 +526,7 @@ __global__ void __launch_bounds__(Cfg3<DIR, VISC>::NT, Cfg3<DIR, VISC>::MINB) k_
     }
     double R[5];
 #pragma unroll
-    for (int f = 0; f < 5; ++f) R[f] = old[f] - (sM[sidx3<DIR, TT>(f, s + 1, t, LF)] - sM[sidx3<DIR, TT>(f, s, t, LF)]);
+    for (int f = 0; f < 5; ++f) R[f] = old[f] - dF[f];
     if (!FUSE) {
 #pragma unroll
       for (int f = 0; f < 5; ++f) in.res[f * c.fsR + ac] = R[f];
@@ -571,6 +563,23 @@ __global__ void __launch_bounds__(Cfg3<DIR, VISC>::NT, Cfg3<DIR, VISC>::MINB) k_
         pn[0] = r; pn[c.fsP] = u; pn[2 * c.fsP] = v; pn[3 * c.fsP] = w; pn[4 * c.fsP] = p;
         pn[5 * c.fsP] = p / (r * c.r_gas);
       }
+    }
+  };
+  if (DIR == 0) {
+    // the right-hand interface of cell `lane` belongs to the next lane of the same warp: no shared memory, no barrier
+    double dF[5];
+#pragma unroll
+    for (int f = 0; f < 5; ++f) dF[f] = __shfl_down_sync(0xffffffffu, F[f], 1) - F[f];
+    if (sI < TS && s0 + sI < nd && t0 + row < nt) finish_cell(sI, row, dF);
+  } else {
+    __syncthreads();
+    for (int it = tid; it < TS * TT; it += NT) {
+      const int t = it % TT, s = it / TT;
+      if (s0 + s >= nd || t0 + t >= nt) continue;
+      double dF[5];
+#pragma unroll
+      for (int f = 0; f < 5; ++f) dF[f] = sM[sidx3<DIR, TT>(f, s + 1, t, LF)] - sM[sidx3<DIR, TT>(f, s, t, LF)];
+      finish_cell(s, t, dF);
     }
   }
 }
