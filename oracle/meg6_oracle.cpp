@@ -14,7 +14,8 @@
  * fixes the choice; oracle and CUDA path simply share the reading):
  *   - eigenvector averaging state (R5), MP alpha value (R7), tangential viscous gradients (R11),
  *     un-hatted interface metrics (R12), Sutherland constants (R15), sponge form (R16),
- *     per-stage metric recompute (R17), inflow/outflow ghost rules (R20), CFL viscous alpha (R25):
+ *     per-stage metric recompute (R17), inflow/outflow ghost rules (R20), CFL viscous alpha (R25),
+ *     where the IG4 line systems of the MIG4 variant end and how they are closed (R26):
  *     parity unpinned.
  *   - everything else is pinned by tests/test_oracle_*.py (-m "not gpu").
  */
@@ -113,9 +114,45 @@ inline double op_D2(const double* f, const double* f1, ptrdiff_t s) {
 inline double op_Lft(double f, double f1, double f2) { return f + 0.5 * f1 + f2 / 12.0; }
 inline double op_Rgt(double f, double f1, double f2) { return f - 0.5 * f1 + f2 / 12.0; }
 
-/* first gradient of a whole array along dir (scheme 0: E6; scheme 1: IG4 not built yet) */
+/* Eq. 18, implicit fourth-order gradient IG4 (the printed "+" are "-", R2):
+ *     alpha f'_{i-1} + f'_i + alpha f'_{i+1} = (2+alpha)/3 (f_{i+1}-f_{i-1}) + (4 alpha-1)/12 (f_{i+2}-f_{i-2}),
+ * alpha = 5/14, one tridiagonal system along every grid line of the array.  The paper does not say where the
+ * systems end (R26): here a system spans every cell of the padded line whose right-hand side exists, and its
+ * first and last unknowns are given by the explicit fourth-order difference of Eq. D.2 (same reach, same order).
+ * Thomas algorithm, written out: forward  den_i = 1 - alpha c_{i-1}, c_i = alpha/den_i,
+ * d_i = (r_i - alpha d_{i-1})/den_i ;  backward  x_i = d_i - c_i x_{i+1}. */
+const double IG4_ALPHA = 5.0 / 14.0;
+void grad_ig4(const Arr& f, int dir, Arr& out) {
+  out.init(f.n, f.g);
+  for (int a = 0; a < 3; ++a) { out.lo[a] = f.lo[a]; out.hi[a] = f.hi[a]; }
+  out.lo[dir] += 2; out.hi[dir] -= 2;
+  const int m = out.hi[dir] - out.lo[dir];
+  if (m < 3) { out.hi[dir] = out.lo[dir]; return; }
+  const double al = IG4_ALPHA, ca = (2.0 + al) / 3.0, cb = (4.0 * al - 1.0) / 12.0;
+  std::vector<double> cc(m, 0.0), den(m, 1.0);
+  for (int q = 1; q < m - 1; ++q) { den[q] = 1.0 - al * cc[q - 1]; cc[q] = al / den[q]; }
+  const ptrdiff_t s = f.stride(dir);
+  const int a1 = (dir + 1) % 3, a2 = (dir + 2) % 3;
+  OMP_FOR
+  for (int v = out.lo[a2]; v < out.hi[a2]; ++v)
+    for (int u = out.lo[a1]; u < out.hi[a1]; ++u) {
+      int ix[3];
+      ix[a1] = u; ix[a2] = v; ix[dir] = out.lo[dir];
+      const double* pf = &f.d[f.idx(ix[0], ix[1], ix[2])];
+      double* px = &out.d[out.idx(ix[0], ix[1], ix[2])];
+      px[0] = op_C4(pf, s);                                        /* first unknown: explicit */
+      for (int q = 1; q < m - 1; ++q) {
+        const double* c = pf + q * s;
+        const double r = ca * (c[s] - c[-s]) + cb * (c[2 * s] - c[-2 * s]);
+        px[q * s] = (r - al * px[(q - 1) * s]) / den[q];
+      }
+      px[(m - 1) * s] = op_C4(pf + (m - 1) * s, s);                /* last unknown: explicit */
+      for (int q = m - 2; q >= 1; --q) px[q * s] = px[q * s] - cc[q] * px[(q + 1) * s];
+    }
+}
+/* first gradient of a whole array along dir (scheme 0: MEG6 = E6, Eq. 17; scheme 1: MIG4 = IG4, Eq. 18) */
 void grad_dir(const Arr& f, int dir, int scheme, Arr& out) {
-  (void)scheme;
+  if (scheme == 1) { grad_ig4(f, dir, out); return; }
   line_apply(f, dir, 3, 3, out, [](const double* p, ptrdiff_t s) { return op_D1(p, s); });
 }
 void grad_c4(const Arr& f, int dir, Arr& out) {
@@ -259,7 +296,6 @@ meg6o_grid* meg6o_create(const meg6o_params* p, const double* x, const double* y
   size_t nn = (size_t)(p->ni + 1) * (p->nj + 1) * (p->nk + 1);
   G->xn.assign(x, x + nn); G->yn.assign(y, y + nn); G->zn.assign(z, z + nn);
   if (p->moving) { G->dxm.assign(dxm, dxm + nn); G->dym.assign(dym, dym + nn); G->dzm.assign(dzm, dzm + nn); }
-  if (p->scheme != 0) { fprintf(stderr, "meg6o: scheme %d (MIG4) not built\n", p->scheme); }
   return G;
 }
 
@@ -889,6 +925,9 @@ void meg6o_line_op(int op, int n, const double* f, double* out) {
       break;
     }
     case 7: grad_c4(a, 0, r); break;
+    case 8: grad_dir(a, 0, 1, r); break;                       /* IG4 */
+    case 9: delta_dir(a, 0, 1, r); break;                      /* consistent derivative with IG4 gradients */
+    case 10: H_dir(a, 0, 1, false, r); break;
     default: r.init(nn, 0); r.lo[0] = r.hi[0] = 0;
   }
   for (int i = 0; i < n; ++i)

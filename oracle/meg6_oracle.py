@@ -202,7 +202,8 @@ class Grid:
 
 
 # ---- fine-grained pieces ----
-OPS = {"D1": 0, "D2": 1, "Lft": 2, "Rgt": 3, "H": 4, "delta": 5, "alpha_damp": 6, "C4": 7}
+OPS = {"D1": 0, "D2": 1, "Lft": 2, "Rgt": 3, "H": 4, "delta": 5, "alpha_damp": 6, "C4": 7, "IG4": 8,
+       "delta_IG4": 9, "H_IG4": 10}
 
 
 def line_op(op, f):
