@@ -27,7 +27,7 @@ static meg6_status fail(meg6_status s, const char* fmt, const char* a = "") {
 static bool params_ok(const meg6_params* p) {
   if (!p) return false;
   if (p->ni < 10 || p->nj < 10 || p->nk < 10) return false;
-  if (p->scheme != 0) return false;
+  if (p->scheme != 0 && p->scheme != 1) return false;
   if (!(p->gamma > 1.0) || !(p->r_gas > 0.0)) return false;
   for (int d = 0; d < 3; ++d)
     if (!p->periodic[d])
@@ -96,6 +96,12 @@ static size_t carve(const meg6_params* p, const Consts& c, meg6_grid* g, char* b
     G->fmt[d] = p->moving ? take(c.LF[d].n) : nullptr;
   }
   G->rjt = p->moving ? take(c.LC.n) : nullptr;
+  for (int q = 0; q < 6; ++q) G->scr[q] = (p->scheme == 1) ? take(c.LX.n) : nullptr;
+  {
+    const int mx = (p->ni > p->nj ? (p->ni > p->nk ? p->ni : p->nk) : (p->nj > p->nk ? p->nj : p->nk)) + 2 * GX;
+    G->ig4_cc = (p->scheme == 1) ? take(mx) : nullptr;
+    G->ig4_den = (p->scheme == 1) ? take(mx) : nullptr;
+  }
   for (int f = 0; f < 6; ++f) G->P[f] = take(c.LP.n);
   for (int f = 0; f < 6; ++f) G->Pb[f] = take(c.LP.n);   // ping-pong partner written by the fused last sweep
   for (int e = 0; e < 3; ++e)
@@ -262,6 +268,16 @@ meg6_status meg6_grid_create(const meg6_params* p, const double* x, const double
     e = cudaMemcpyAsync(g->nodes[q], src[q], nn, cudaMemcpyDeviceToDevice, g->stream);
     if (e == cudaSuccess && p->moving) e = cudaMemcpyAsync(g->modes[q], msrc[q], nn, cudaMemcpyDeviceToDevice, g->stream);
   }
+  if (e == cudaSuccess && p->scheme == 1) {
+    // Thomas elimination coefficients of the IG4 systems (position-only; R26): den_q = 1 - alpha c_{q-1}, c_q = alpha/den_q
+    const int mx = (p->ni > p->nj ? (p->ni > p->nk ? p->ni : p->nk) : (p->nj > p->nk ? p->nj : p->nk)) + 2 * GX;
+    std::vector<double> cc(mx, 0.0), den(mx, 1.0);
+    const double al = 5.0 / 14.0;
+    for (int q = 1; q < mx; ++q) { den[q] = 1.0 - al * cc[q - 1]; cc[q] = al / den[q]; }
+    e = cudaMemcpyAsync(g->ig4_cc, cc.data(), sizeof(double) * mx, cudaMemcpyHostToDevice, g->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(g->ig4_den, den.data(), sizeof(double) * mx, cudaMemcpyHostToDevice, g->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(g->stream);   // the host vectors go out of scope
+  }
   if (e == cudaSuccess) e = setup_tma(g);
   if (e != cudaSuccess) { delete g; return fail(MEG6_ECUDA, "grid_create: %s", cudaGetErrorString(e)); }
   *out = g;
@@ -308,6 +324,7 @@ meg6_status meg6_set_sponge(meg6_grid* g, const double* sigma, const double* U_r
 // assembly, the stage update and the primitive conversion of the new state (into the other buffer).
 static meg6_status stage(meg6_grid* g, int buf, const Fuse3& fu) {
   const Consts& c = g->c;
+  if (g->p.scheme == 1) return fail(MEG6_EINVAL, "MIG4: only the geometry is built so far%s");
   double* const* Pc = buf ? g->Pb : g->P;
   P6 P;
   for (int f = 0; f < 6; ++f) P.p[f] = Pc[f];

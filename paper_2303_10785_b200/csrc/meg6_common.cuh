@@ -84,6 +84,9 @@ struct meg6_grid {
   double* met[9]; double* rj; double* mt[3];
   double* fmet[3][10]; double* fmt[3];
   double* rjt;
+  // MIG4 (scheme 1): scratch arrays of the pass-based geometry (layout LX), Thomas coefficients, stored gradients
+  double* scr[6];
+  double* ig4_cc; double* ig4_den;
   // flow
   double* P[6];       // primitives + T with ghosts, buffer 0
   double* Pb[6];      // buffer 1 (the fused last sweep writes the next stage's primitives into the other buffer)

@@ -1,10 +1,122 @@
 // meg6_geom.cu -- metric / Jacobian kernels and their launcher.  Compiled with -fmad=false (see meg6_geom.cuh).
 #include <math.h>
 #include "meg6_geom.cuh"
+#include "meg6_ig4.cuh"
 
 namespace meg6 {
 
 static inline unsigned nblk(long long n, int t) { return (unsigned)((n + t - 1) / t); }
+
+// ---- MIG4 (scheme 1): the geometry as whole-array passes, each the operation the discretisation names ----
+static Box box_all(const Consts& c) {
+  Box b;
+  for (int a = 0; a < 3; ++a) { b.lo[a] = -GX; b.hi[a] = c.n[a] + GX; }
+  return b;
+}
+static Box box_and(const Box& a, const Box& b) {
+  Box r;
+  for (int q = 0; q < 3; ++q) { r.lo[q] = a.lo[q] > b.lo[q] ? a.lo[q] : b.lo[q]; r.hi[q] = a.hi[q] < b.hi[q] ? a.hi[q] : b.hi[q]; }
+  return r;
+}
+static long long box_n(const Box& b) { return (long long)(b.hi[0] - b.lo[0]) * (b.hi[1] - b.lo[1]) * (b.hi[2] - b.lo[2]); }
+
+// IG4 gradient of f (valid on fb) along dir into out; returns the valid box of out.  Lay L: layout of both arrays.
+Box launch_ig4(meg6_grid* g, const Lay& L, const double* f, const Box& fb, int dir, double* out) {
+  Box ob = fb;
+  ob.lo[dir] += 2; ob.hi[dir] -= 2;
+  const int a1 = (dir == 0) ? 1 : 0, a2 = (dir == 2) ? 1 : 2;
+  const long long lines = (long long)(ob.hi[a1] - ob.lo[a1]) * (ob.hi[a2] - ob.lo[a2]);
+  if (dir == 0) k_ig4<0><<<nblk(lines, 128), 128, 0, g->stream>>>(L, f, out, ob, g->ig4_cc, g->ig4_den);
+  else if (dir == 1) k_ig4<1><<<nblk(lines, 128), 128, 0, g->stream>>>(L, f, out, ob, g->ig4_cc, g->ig4_den);
+  else k_ig4<2><<<nblk(lines, 128), 128, 0, g->stream>>>(L, f, out, ob, g->ig4_cc, g->ig4_den);
+  return ob;
+}
+
+// H of f along dir into a cell-layout array (index i = interface i+1/2); returns its valid box
+static Box H_pass(meg6_grid* g, const double* f, const Box& fb, int dir, double* f1, double* H) {
+  const Lay& L = g->c.LX;
+  const Box gb = launch_ig4(g, L, f, fb, dir, f1);
+  Box hb = gb;
+  hb.lo[dir] += 1; hb.hi[dir] -= 2;
+  k_H_from<<<nblk(box_n(hb), 256), 256, 0, g->stream>>>(L, L, dir, 0, f, f1, H, hb);
+  return hb;
+}
+// consistent derivative Eq. 37 of f along dir into out
+static Box delta_pass(meg6_grid* g, const double* f, const Box& fb, int dir, double* f1, double* H, double* out) {
+  const Box hb = H_pass(g, f, fb, dir, f1, H);
+  Box db = hb;
+  db.lo[dir] += 1;
+  k_point<<<nblk(box_n(db), 256), 256, 0, g->stream>>>(g->c.LX, 0, dir, H, nullptr, out, db);
+  return db;
+}
+
+static cudaError_t launch_geometry_ig4(meg6_grid* g, const GeomIn& gi) {
+  const Consts& c = g->c;
+  const Lay& L = c.LX;
+  P3 xc, xt;
+  for (int q = 0; q < 3; ++q) { xc.p[q] = g->xc[q]; xt.p[q] = g->xt[q]; }
+  k_centres<<<nblk(L.n, 256), 256, 0, g->stream>>>(c, gi, xc, xt);
+  double* f1 = g->scr[0]; double* H = g->scr[1]; double* t1 = g->scr[2]; double* t2 = g->scr[3];
+  double* d1 = g->scr[4]; double* d2 = g->scr[5];
+  const Box all = box_all(c);
+  Box cdb[9];
+  for (int cc = 0; cc < 3; ++cc)
+    for (int d = 0; d < 3; ++d) cdb[3 * cc + d] = delta_pass(g, g->xc[cc], all, d, f1, H, g->cd[3 * cc + d]);
+  // Thomas-Lombard conservative metrics, Eq. 10: m = delta_b(delta_a(q) s) - delta_a(delta_b(q) s)
+  Box mb[9];
+  for (int r = 0; r < 3; ++r) {
+    const int a = (r + 1) % 3, b = (r + 2) % 3;
+    for (int cc = 0; cc < 3; ++cc) {
+      const int q = (cc + 1) % 3, s = (cc + 2) % 3;
+      const Box b1 = box_and(cdb[3 * q + a], all), b2 = box_and(cdb[3 * q + b], all);
+      k_point<<<nblk(box_n(b1), 256), 256, 0, g->stream>>>(L, 1, 0, g->cd[3 * q + a], g->xc[s], t1, b1);
+      k_point<<<nblk(box_n(b2), 256), 256, 0, g->stream>>>(L, 1, 0, g->cd[3 * q + b], g->xc[s], t2, b2);
+      const Box e1 = delta_pass(g, t1, b1, b, f1, H, d1);
+      const Box e2 = delta_pass(g, t2, b2, a, f1, H, d2);
+      mb[3 * r + cc] = box_and(e1, e2);
+      k_point<<<nblk(box_n(mb[3 * r + cc]), 256), 256, 0, g->stream>>>(L, 2, 0, d1, d2, g->met[3 * r + cc], mb[3 * r + cc]);
+    }
+  }
+  Box rjb = all;
+  for (int q = 0; q < 9; ++q) rjb = box_and(rjb, cdb[q]);
+  {
+    P9c cd;
+    for (int q = 0; q < 9; ++q) cd.p[q] = g->cd[q];
+    k_rj_box<<<nblk(box_n(rjb), 256), 256, 0, g->stream>>>(L, cd, g->rj, rjb);
+  }
+  Box mtb[3];
+  if (g->p.moving) {
+    // the line systems end where the valid range ends (R26): every array keeps exactly the box the passes give it
+    P3c vt;
+    for (int q = 0; q < 3; ++q) vt.p[q] = g->xt[q];
+    for (int r = 0; r < 3; ++r) {
+      mtb[r] = mb[3 * r];
+      k_mt_box<<<nblk(box_n(mtb[r]), 256), 256, 0, g->stream>>>(L, vt, g->met[3 * r], g->met[3 * r + 1], g->met[3 * r + 2],
+                                                                 g->mt[r], mtb[r]);
+    }
+  }
+  // interface metrics: each hatted quantity interpolated as a whole, Eq. 38
+  for (int d = 0; d < 3; ++d) {
+    Box fb;   // interfaces 0..n_d of family d <-> H index -1..n_d-1
+    for (int a = 0; a < 3; ++a) { fb.lo[a] = 0; fb.hi[a] = c.n[a]; }
+    fb.lo[d] = -1;
+    for (int q = 0; q < 11; ++q) {
+      const double* src; Box sb; double* dst;
+      if (q < 9) { src = g->met[q]; sb = mb[q]; dst = g->fmet[d][q]; }
+      else if (q == 9) { src = g->rj; sb = rjb; dst = g->fmet[d][9]; }
+      else { if (!g->p.moving) continue; src = g->mt[d]; sb = mtb[d]; dst = g->fmt[d]; }
+      if (!dst) continue;
+      const Box gb = launch_ig4(g, L, src, sb, d, f1);
+      Box hb = gb;
+      hb.lo[d] += 1; hb.hi[d] -= 2;
+      for (int a = 0; a < 3; ++a)
+        if (hb.lo[a] > fb.lo[a] || hb.hi[a] < fb.hi[a]) return cudaErrorInvalidValue;   // ghost depth too small
+      k_H_from<<<nblk(box_n(fb), 256), 256, 0, g->stream>>>(L, c.LF[d], d, 1, src, f1, dst, fb);
+    }
+  }
+  if (g->p.moving) k_rjt<<<nblk(c.LC.n, 256), 256, 0, g->stream>>>(c, g->fmt[0], g->fmt[1], g->fmt[2], g->rjt);
+  return cudaGetLastError();
+}
 
 cudaError_t launch_geometry(meg6_grid* g, double t) {
   const Consts& c = g->c;
@@ -16,6 +128,7 @@ cudaError_t launch_geometry(meg6_grid* g, double t) {
   P3 xc, xt, mt; P9 cd, met;
   for (int q = 0; q < 3; ++q) { xc.p[q] = g->xc[q]; xt.p[q] = g->xt[q]; mt.p[q] = g->mt[q]; }
   for (int q = 0; q < 9; ++q) { cd.p[q] = g->cd[q]; met.p[q] = g->met[q]; }
+  if (g->p.scheme == 1) return launch_geometry_ig4(g, gi);
   const int T = 256;
   k_centres<<<nblk(c.LX.n, T), T, 0, g->stream>>>(c, gi, xc, xt);
   k_coord_deriv<<<nblk(c.LX.n, T), T, 0, g->stream>>>(c, xc, cd);

@@ -1,0 +1,110 @@
+// meg6_ig4.cuh -- MIG4 variant (scheme = 1): implicit fourth-order gradients IG4, Eq. 18 (R2), and the
+// pass-based geometry that uses them wherever MEG6 uses E6.
+//
+// Reading R26: a tridiagonal system spans every cell of the padded grid line whose right-hand side
+// exists and is closed at both ends with the explicit fourth-order difference of Eq. D.2.  One thread solves one
+// line with the Thomas algorithm; the elimination coefficients depend on the position only and come from the host.
+// Part of meg6_geom.cu (compiled with -fmad=false): the operation order is the one the discretisation states, and
+// the geometry arrays are compared bit for bit with the oracle's.
+#pragma once
+#include "meg6_common.cuh"
+
+namespace meg6 {
+
+struct Box { int lo[3], hi[3]; };   // valid cell range [lo, hi) of an array, per direction
+
+__device__ __forceinline__ double c4_op(const double* __restrict__ f, long long s) {   // Eq. D.2
+  return 2.0 / 3.0 * (f[s] - f[-s]) - 1.0 / 12.0 * (f[2 * s] - f[-2 * s]);
+}
+
+// out = IG4 gradient of f along DIR on `ob` (= the box of f shrunk by 2 at both ends of DIR).
+template <int DIR>
+__global__ void __launch_bounds__(128) k_ig4(Lay L, const double* __restrict__ f, double* __restrict__ out, Box ob,
+                                             const double* __restrict__ cc, const double* __restrict__ den) {
+  constexpr int A1 = (DIR == 0) ? 1 : 0, A2 = (DIR == 2) ? 1 : 2;   // transverse directions, lower index fastest
+  const int n1 = ob.hi[A1] - ob.lo[A1], n2 = ob.hi[A2] - ob.lo[A2];
+  const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (tid >= (long long)n1 * n2) return;
+  int ix[3];
+  ix[A1] = ob.lo[A1] + (int)(tid % n1); ix[A2] = ob.lo[A2] + (int)(tid / n1); ix[DIR] = ob.lo[DIR];
+  const int m = ob.hi[DIR] - ob.lo[DIR];
+  const long long at = L.at(ix[0], ix[1], ix[2]), s = L.stride(DIR);
+  const double* pf = f + at;
+  double* px = out + at;
+  const double al = 5.0 / 14.0, ca = (2.0 + al) / 3.0, cb = (4.0 * al - 1.0) / 12.0;
+  double prev = c4_op(pf, s);                       // first unknown: explicit
+  px[0] = prev;
+  for (int q = 1; q < m - 1; ++q) {
+    const double* c = pf + q * s;
+    const double r = ca * (c[s] - c[-s]) + cb * (c[2 * s] - c[-2 * s]);
+    prev = (r - al * prev) / den[q];
+    px[q * s] = prev;
+  }
+  double nxt = c4_op(pf + (long long)(m - 1) * s, s);   // last unknown: explicit
+  px[(long long)(m - 1) * s] = nxt;
+  for (int q = m - 2; q >= 1; --q) {
+    nxt = px[q * s] - cc[q] * nxt;
+    px[q * s] = nxt;
+  }
+}
+
+// Central interface value Eq. 36/38 from f and its gradient f1: index i of `out` = interface between
+// cells i and i+1 along dir.  The second derivative is Eq. 19.  `out` may have another layout (interface
+// arrays): LO, and an index shift `sh` along dir (interface arrays number the face between cells i-1 and i as i).
+__global__ void __launch_bounds__(256) k_H_from(Lay L, Lay LO, int dir, int sh, const double* __restrict__ f,
+                                                const double* __restrict__ f1, double* __restrict__ out, Box ob) {
+  const int n0 = ob.hi[0] - ob.lo[0], n1 = ob.hi[1] - ob.lo[1], n2 = ob.hi[2] - ob.lo[2];
+  const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (tid >= (long long)n0 * n1 * n2) return;
+  int ix[3] = {ob.lo[0] + (int)(tid % n0), ob.lo[1] + (int)((tid / n0) % n1), ob.lo[2] + (int)(tid / ((long long)n0 * n1))};
+  const long long c = L.at(ix[0], ix[1], ix[2]), s = L.stride(dir);
+  const double* pf = f + c;
+  const double* p1 = f1 + c;
+  const double f2a = 2.0 * (pf[s] - 2.0 * pf[0] + pf[-s]) - 0.5 * (p1[s] - p1[-s]);
+  const double f2b = 2.0 * (pf[2 * s] - 2.0 * pf[s] + pf[0]) - 0.5 * (p1[2 * s] - p1[0]);
+  const double Lv = pf[0] + 0.5 * p1[0] + f2a / 12.0;
+  const double Rv = pf[s] - 0.5 * p1[s] + f2b / 12.0;
+  ix[dir] += sh;
+  out[LO.at(ix[0], ix[1], ix[2])] = 0.5 * (Lv + Rv);
+}
+
+// mode 0: out_i = a_i - a_{i-1 along dir} (Eq. 37);  mode 1: out = a * b;  mode 2: out = a - b
+__global__ void __launch_bounds__(256) k_point(Lay L, int mode, int dir, const double* __restrict__ a,
+                                               const double* __restrict__ b, double* __restrict__ out, Box ob) {
+  const int n0 = ob.hi[0] - ob.lo[0], n1 = ob.hi[1] - ob.lo[1], n2 = ob.hi[2] - ob.lo[2];
+  const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (tid >= (long long)n0 * n1 * n2) return;
+  const int i = ob.lo[0] + (int)(tid % n0), j = ob.lo[1] + (int)((tid / n0) % n1), k = ob.lo[2] + (int)(tid / ((long long)n0 * n1));
+  const long long c = L.at(i, j, k);
+  if (mode == 0) out[c] = a[c] - a[c - L.stride(dir)];
+  else if (mode == 1) out[c] = a[c] * b[c];
+  else out[c] = a[c] - b[c];
+}
+
+struct P9c { const double* p[9]; };
+struct P3c { const double* p[3]; };
+struct P3w { double* p[3]; };
+
+// 1/J = det of the coordinate derivatives, Eq. 13
+__global__ void __launch_bounds__(256) k_rj_box(Lay L, P9c cd, double* __restrict__ rj, Box ob) {
+  const int n0 = ob.hi[0] - ob.lo[0], n1 = ob.hi[1] - ob.lo[1], n2 = ob.hi[2] - ob.lo[2];
+  const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (tid >= (long long)n0 * n1 * n2) return;
+  const long long at = L.at(ob.lo[0] + (int)(tid % n0), ob.lo[1] + (int)((tid / n0) % n1), ob.lo[2] + (int)(tid / ((long long)n0 * n1)));
+  const double xx = cd.p[0][at], xe = cd.p[1][at], xz = cd.p[2][at];
+  const double yx = cd.p[3][at], ye = cd.p[4][at], yz = cd.p[5][at];
+  const double zx = cd.p[6][at], ze = cd.p[7][at], zz = cd.p[8][at];
+  rj[at] = xx * (ye * zz - ze * yz) - yx * (xe * zz - ze * xz) + zx * (xe * yz - ye * xz);
+}
+
+// hatted time metric of direction r, Eq. 11, on the box of that direction's metrics
+__global__ void __launch_bounds__(256) k_mt_box(Lay L, P3c xt, const double* __restrict__ mx, const double* __restrict__ my,
+                                                const double* __restrict__ mz, double* __restrict__ mt, Box ob) {
+  const int n0 = ob.hi[0] - ob.lo[0], n1 = ob.hi[1] - ob.lo[1], n2 = ob.hi[2] - ob.lo[2];
+  const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (tid >= (long long)n0 * n1 * n2) return;
+  const long long at = L.at(ob.lo[0] + (int)(tid % n0), ob.lo[1] + (int)((tid / n0) % n1), ob.lo[2] + (int)(tid / ((long long)n0 * n1)));
+  mt[at] = -(xt.p[0][at] * mx[at] + xt.p[1][at] * my[at] + xt.p[2][at] * mz[at]);
+}
+
+}  // namespace meg6

@@ -323,3 +323,38 @@ def test_ragged_shapes_non_periodic_viscous(mods, shape):
         t += wl["dt"]
     assert np.all(rel(U.cpu().numpy(), Uo) <= STEP_TOL)
     g.close()
+
+
+# ---------------------------------------------------------------------------------------------------------
+# MIG4 variant (scheme = 1, Eq. 18; reading R26)
+
+def mig4_cases():
+    out = {}
+    for name, wl in small_cases().items():
+        wl = dict(wl)
+        wl["params"] = dict(wl["params"], scheme=1)
+        out[name] = wl
+    return out
+
+
+@pytest.mark.parametrize("name", ["c1", "c2", "c3", "c4"])
+def test_mig4_metrics_parity(mods, name):
+    """Geometry of the MIG4 variant (every gradient inside the metric evaluation is the implicit IG4 one): bit for
+    bit, as for MEG6."""
+    torch, O, M = mods
+    wl = mig4_cases()[name]
+    t = 0.13 if wl["params"]["moving"] else 0.0
+    og = O.Grid(wl)
+    og.metrics_compute(t)
+    g = M.Grid(wl)
+    g.metrics_compute(t)
+    checks = [("cell", q, g.get_array(0, q), og.cell(q)) for q in range(10)]
+    for d in range(3):
+        qs = range(10) if wl["params"]["viscous"] else range(3 * d, 3 * d + 3)
+        checks += [("face%d" % d, q, g.get_array(1, 16 * d + q), og.face(d, q)) for q in qs]
+    if wl["params"]["moving"]:
+        checks += [("cell", q, g.get_array(0, q), og.cell(q)) for q in (10, 11, 12, 13)]
+        checks += [("face%d" % d, 10, g.get_array(1, 16 * d + 10), og.face(d, 10)) for d in range(3)]
+    for kind, q, a, b in checks:
+        assert np.array_equal(a, b), (name, kind, q, np.abs(a - b).max() / np.abs(b).max())
+    g.close()
