@@ -39,7 +39,8 @@ typedef struct {
   int ni, nj, nk;     /* interior cells per direction; each >= 10 (periodic wrap of the 10-deep metric halo) */
   int periodic[3];    /* per direction; a periodic direction ignores bc[] of its two faces           */
   double period[3][3];/* period[d] = (dx,dy,dz) added to ghost-cell coordinates across direction d (R14) */
-  int scheme;         /* 0 = MEG6 (E6 gradients, Eq. 17).  1 = MIG4 is not built: MEG6_EINVAL   */
+  int scheme;         /* 0 = MEG6 (E6 gradients, Eq. 17); 1 = MIG4 (implicit IG4 gradients, Eq. 18 P:217,
+                         in reconstruction, viscous flux and metrics; line systems closed per R26)      */
   int viscous;        /* 0: Euler; 1: + alpha-damping viscous flux (Eq. 29-35)            */
   double gamma, r_gas, prandtl; /* T = p/(rho r_gas); kappa = mu gamma r_gas/((gamma-1) Pr)   */
   double mu_ref, t_ref, s_suth; /* mu = mu_ref (T/t_ref)^1.5 (t_ref+s_suth)/(T+s_suth); s_suth<0: mu = mu_ref (R15) */

@@ -97,6 +97,8 @@ static size_t carve(const meg6_params* p, const Consts& c, meg6_grid* g, char* b
   }
   G->rjt = p->moving ? take(c.LC.n) : nullptr;
   for (int q = 0; q < 6; ++q) G->scr[q] = (p->scheme == 1) ? take(c.LX.n) : nullptr;
+  for (int d = 0; d < 3; ++d)
+    for (int f = 0; f < 6; ++f) G->Gi[d][f] = (p->scheme == 1) ? take(c.LP.n) : nullptr;
   {
     const int mx = (p->ni > p->nj ? (p->ni > p->nk ? p->ni : p->nk) : (p->nj > p->nk ? p->nj : p->nk)) + 2 * GX;
     G->ig4_cc = (p->scheme == 1) ? take(mx) : nullptr;
@@ -105,7 +107,7 @@ static size_t carve(const meg6_params* p, const Consts& c, meg6_grid* g, char* b
   for (int f = 0; f < 6; ++f) G->P[f] = take(c.LP.n);
   for (int f = 0; f < 6; ++f) G->Pb[f] = take(c.LP.n);   // ping-pong partner written by the fused last sweep
   for (int e = 0; e < 3; ++e)
-    for (int f = 0; f < 4; ++f) G->G[e][f] = p->viscous ? take(c.LG.n) : nullptr;
+    for (int f = 0; f < 4; ++f) G->G[e][f] = (p->viscous && p->scheme == 0) ? take(c.LG.n) : nullptr;
   G->res = take(c.LR.n);
   for (int f = 1; f < 5; ++f) take(c.LR.n);   // fields c.fsR apart
   G->U0 = take(5 * c.LC.n);
@@ -123,7 +125,10 @@ static size_t carve(const meg6_params* p, const Consts& c, meg6_grid* g, char* b
 }
 
 static inline unsigned nblk(long long n, int t) { return (unsigned)((n + t - 1) / t); }
-namespace meg6 { cudaError_t launch_geometry(meg6_grid* g, double t); }
+namespace meg6 {
+cudaError_t launch_geometry(meg6_grid* g, double t);
+Box launch_ig4(meg6_grid* g, const Lay& L, const double* f, const Box& fb, int dir, double* out);
+}
 
 // ---- TMA descriptors (cuTensorMapEncodeTiled through the runtime's driver entry point: no libcuda link) ----
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
@@ -142,6 +147,40 @@ static bool make_map4(EncodeTiledFn fn, CUtensorMap* tm, const double* base, con
 
 template <int DIR, bool VISC>
 static bool make_maps3_dir(EncodeTiledFn fn, meg6_grid* g, int buf) {
+  if (g->p.scheme == 1) {
+    // MIG4: same tiles, gradients from the line-solve arrays Gi (layout of the primitives)
+    using C = Cfg3<DIR, VISC, true>;
+    const Consts& c = g->c;
+    TmaMaps& t = g->tmaps3[buf][DIR];
+    auto box = [](int sweep, int trans, int nf, int out[4]) {
+      if (DIR == 0) { out[0] = sweep; out[1] = trans; out[2] = 1; }
+      else if (DIR == 1) { out[0] = trans; out[1] = sweep; out[2] = 1; }
+      else { out[0] = trans; out[1] = 1; out[2] = sweep; }
+      out[3] = nf;
+    };
+    int b[4];
+    bool ok = true;
+    box(C::LP, C::TT, C::NF, b);
+    ok = ok && make_map4(fn, &t.P, buf ? g->Pb[0] : g->P[0], c.LP, c.fsP, 6, b);
+    box(C::LF, C::TT, C::NM, b);
+    ok = ok && make_map4(fn, &t.M, VISC ? g->fmet[DIR][0] : g->fmet[DIR][3 * DIR], c.LF[DIR], c.fsM[DIR], C::NM, b);
+    if (g->p.moving) {
+      box(C::LF, C::TT, 1, b);
+      ok = ok && make_map4(fn, &t.Mt, g->fmt[DIR], c.LF[DIR], c.fsM[DIR], 1, b);
+    }
+    box(C::LQ, C::TT, C::NF, b);
+    ok = ok && make_map4(fn, &t.Q, g->Gi[DIR][0], c.LP, c.fsP, 6, b);
+    if (VISC) {
+      int slot = 0;
+      for (int e = 0; e < 3; ++e) {
+        if (e == DIR) continue;
+        box(C::LG, C::TT, 5, b);
+        ok = ok && make_map4(fn, &t.G3[slot], g->Gi[e][0], c.LP, c.fsP, 6, b);
+        ++slot;
+      }
+    }
+    return ok;
+  }
   using C = Cfg3<DIR, VISC>;
   const Consts& c = g->c;
   TmaMaps& t = g->tmaps3[buf][DIR];
@@ -188,6 +227,14 @@ static cudaError_t setup_tma(meg6_grid* g) {
   SET_SMEM3(0, false, true) SET_SMEM3(1, false, false) SET_SMEM3(2, false, false)
   SET_SMEM3(0, true, true) SET_SMEM3(1, true, false) SET_SMEM3(2, true, false)
 #undef SET_SMEM3
+#define SET_SMEM3I(D, V, F)                                                                                 \
+  if ((e = cudaFuncSetAttribute(k_flux3<D, V, F, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,        \
+                                Cfg3<D, V, true>::SMEM_BYTES)) != cudaSuccess) return e;
+  if (g->p.scheme == 1) {
+    SET_SMEM3I(0, false, true) SET_SMEM3I(1, false, false) SET_SMEM3I(2, false, false)
+    SET_SMEM3I(0, true, true) SET_SMEM3I(1, true, false) SET_SMEM3I(2, true, false)
+  }
+#undef SET_SMEM3I
   return cudaSuccess;
 }
 
@@ -324,7 +371,6 @@ meg6_status meg6_set_sponge(meg6_grid* g, const double* sigma, const double* U_r
 // assembly, the stage update and the primitive conversion of the new state (into the other buffer).
 static meg6_status stage(meg6_grid* g, int buf, const Fuse3& fu) {
   const Consts& c = g->c;
-  if (g->p.scheme == 1) return fail(MEG6_EINVAL, "MIG4: only the geometry is built so far%s");
   double* const* Pc = buf ? g->Pb : g->P;
   P6 P;
   for (int f = 0; f < 6; ++f) P.p[f] = Pc[f];
@@ -338,7 +384,15 @@ static meg6_status stage(meg6_grid* g, int buf, const Fuse3& fu) {
     ProfScope ps(g, 2, 1);
     k_ghost<<<nblk(ea * eb * 12, 256), 256, 0, g->stream>>>(c, d, P, gin);
   }
-  if (g->p.viscous) {
+  const bool IG = g->p.scheme == 1;
+  if (IG) {
+    // MIG4: implicit gradients of every staged field along the three directions (Eq. 18), whole grid lines
+    ProfScope ps(g, 3, (g->p.viscous ? 6 : 5) * 3);
+    meg6::Box pb;
+    for (int a = 0; a < 3; ++a) { pb.lo[a] = -6; pb.hi[a] = c.n[a] + 6; }
+    for (int d = 0; d < 3; ++d)
+      for (int f = 0; f < (g->p.viscous ? 6 : 5); ++f) meg6::launch_ig4(g, c.LP, Pc[f], pb, d, g->Gi[d][f]);
+  } else if (g->p.viscous) {
     P12 G;
     for (int e = 0; e < 3; ++e)
       for (int f = 0; f < 4; ++f) G.p[4 * e + f] = g->G[e][f];
@@ -349,8 +403,11 @@ static meg6_status stage(meg6_grid* g, int buf, const Fuse3& fu) {
   i3.res = g->res; i3.stats = g->stats_on ? g->stats : nullptr; i3.moving = g->p.moving ? 1 : 0;
   const bool V = g->p.viscous != 0;
   const TmaMaps* tm = g->tmaps3[buf];
-#define LAUNCH3(D, VV, FF, GRID) \
-  k_flux3<D, VV, FF><<<GRID, Cfg3<D, VV>::NT, Cfg3<D, VV>::SMEM_BYTES, g->stream>>>(c, i3, tm[D], fu)
+#define LAUNCH3(D, VV, FF, GRID)                                                                                        \
+  do {                                                                                                                  \
+    if (IG) k_flux3<D, VV, FF, true><<<GRID, Cfg3<D, VV, true>::NT, Cfg3<D, VV, true>::SMEM_BYTES, g->stream>>>(c, i3, tm[D], fu); \
+    else k_flux3<D, VV, FF><<<GRID, Cfg3<D, VV>::NT, Cfg3<D, VV>::SMEM_BYTES, g->stream>>>(c, i3, tm[D], fu);           \
+  } while (0)
   // sweep order eta, zeta, xi: the fused final phase then works on rows that are contiguous along xi
   {
     ProfScope ps(g, 5, 1);

@@ -50,6 +50,8 @@ inline Lay make_lay(int ni, int nj, int nk, int gi, int gj, int gk, int align_i 
   return L;
 }
 
+struct Box { int lo[3], hi[3]; };   // valid cell range [lo, hi) of an array, per direction (MIG4 passes)
+
 struct Consts {   // per-grid constants passed by value to kernels
   int n[3];
   int periodic[3];
@@ -68,7 +70,9 @@ struct Consts {   // per-grid constants passed by value to kernels
 
 }  // namespace meg6
 
-namespace meg6 { struct TmaMaps { CUtensorMap P, M, Mt, G; }; }
+// P primitives, M interface metrics, Mt time metric, G stored tangential gradients (MEG6); MIG4: Q = implicit
+// gradients along the sweep, G3[s] = gradients (u,v,w,p,T) of tangential direction s
+namespace meg6 { struct TmaMaps { CUtensorMap P, M, Mt, G, Q, G3[2]; }; }
 
 struct meg6_grid {
   meg6_params p;
@@ -86,6 +90,7 @@ struct meg6_grid {
   double* rjt;
   // MIG4 (scheme 1): scratch arrays of the pass-based geometry (layout LX), Thomas coefficients, stored gradients
   double* scr[6];
+  double* Gi[3][6];   // IG4 gradients of the six primitive fields along xi, eta, zeta (layout LP, field stride fsP)
   double* ig4_cc; double* ig4_den;
   // flow
   double* P[6];       // primitives + T with ghosts, buffer 0

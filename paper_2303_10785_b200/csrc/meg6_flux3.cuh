@@ -28,13 +28,15 @@ namespace meg6 {
 #define MEG6_RELOAD 1
 #endif
 
-template <int DIR, bool VISC>
+// IG4 = MIG4 variant (scheme 1): the sweep-direction gradients P' are not E6 stencils of the tile but solutions of
+// the implicit systems of Eq. 18, computed beforehand for whole grid lines and loaded like the primitives.
+template <int DIR, bool VISC, bool IG4 = false>
 struct Cfg3 {
   static constexpr int TS = (DIR == 0) ? 30 : 15;            // cells along the sweep per tile
   static constexpr int TT = (DIR == 0) ? 4 : 8;              // transverse positions (rows for xi, i-lanes otherwise)
   static constexpr int NI = TS + 1;                          // interfaces per pencil
   static constexpr int NT = (DIR == 0) ? 32 * TT : NI * TT;  // threads: one interface each (xi: one warp per row)
-  static constexpr int MINB = (DIR == 0) ? MEG6_MINB3_X : MEG6_MINB3_Y;
+  static constexpr int MINB = IG4 ? 4 : (DIR == 0) ? MEG6_MINB3_X : MEG6_MINB3_Y;
   static constexpr int NF = VISC ? 6 : 5;                    // staged fields (T only for the viscous flux)
   static constexpr int NM = VISC ? 10 : 3;                   // interface metrics loaded
   static constexpr int NMF = NM > 5 ? NM : 5;                // the metric region later receives the 5 fluxes
@@ -44,10 +46,17 @@ struct Cfg3 {
   static constexpr int LF = (DIR == 0) ? TS + 2 : TS + 1;    // interface rows (xi: even length, TMA box bytes % 16)
   static constexpr int LG = (DIR == 0) ? TS + 4 : TS + 2;    // stored gradients: cells -1..TS (xi: box starts at -2)
   static constexpr int GOFF = (DIR == 0) ? 1 : 0;
-  static constexpr int nP = NF * LP * TT, nA = 10 * LA * TT, nT1 = VISC ? LT * TT : 0, nM = NMF * LF * TT,
-                       nMt = LF * TT, nG = VISC ? 8 * LG * TT : 0;
+  static constexpr int LQ = (DIR == 0) ? TS + 8 : TS + 6;    // IG4: P' cells -3..TS+2 (xi: box starts at -4)
+  static constexpr int QOFF = (DIR == 0) ? 1 : 0;
   static constexpr int al(int n) { return (n + 15) / 16 * 16; }   // 128-byte granules (TMA destinations)
-  static constexpr int oP = 0, oM = oP + al(nP), oMt = oM + al(nM), oG = oMt + al(nMt), oA = oG + al(nG),
+  // stored tangential gradients: two groups (the two tangential directions).  MEG6: 4 fields (u,v,w,T) each, one
+  // box per group out of the 12-field array; MIG4: one 5-field box (u,v,w,p,T of the line-solve arrays) per group,
+  // the second group starting on the next 128-byte boundary
+  static constexpr int GFLD = IG4 ? 5 : 4, GSLOT = IG4 ? al(5 * LG * TT) : 4 * LG * TT;
+  static constexpr int nP = NF * LP * TT, nA = 10 * LA * TT, nT1 = (VISC && !IG4) ? LT * TT : 0, nM = NMF * LF * TT,
+                       nMt = LF * TT, nG = VISC ? GSLOT + GFLD * LG * TT : 0, nGtx = VISC ? 2 * GFLD * LG * TT : 0,
+                       nQ = IG4 ? NF * LQ * TT : 0;
+  static constexpr int oP = 0, oM = oP + al(nP), oMt = oM + al(nM), oG = oMt + al(nMt), oQ = oG + al(nG), oA = oQ + al(nQ),
                        oT1 = oA + al(nA), oBar = oT1 + al(nT1);
   static constexpr int SMEM_BYTES = (oBar + 2) * 8;   // two mbarriers
 };
@@ -201,7 +210,7 @@ __device__ __forceinline__ void hllc3(const double PL[5], const double PR[5], do
 //   pT1  : T' of cell L;  pG: stored tangential gradients at cell L;  pM: interface metrics (field stride FM)
 // SS = stride between consecutive cells along the sweep; FP/FA/FG/FM = field strides.
 // Returns the E.1 flags (bit r: left state of component r limited, bit 5+r: right state).
-template <int DIR, bool VISC, int SS, int FP, int FA, int FG, int FM>
+template <int DIR, bool VISC, int SS, int FP, int FA, int FG, int FM, int GSLOT, bool IG4>
 __device__ __forceinline__ unsigned face3(const Consts& c, const double* __restrict__ pP, const double* __restrict__ pA,
                                           const double* __restrict__ pT1, const double* __restrict__ pG,
                                           const double* __restrict__ pM, double mt, double F[5]) {
@@ -284,7 +293,8 @@ __device__ __forceinline__ unsigned face3(const Consts& c, const double* __restr
         if (d == DIR) gr[d][f] = fma(2.0, phR - phL, 0.5 * (gL + gR));   // Eq. 29
         else {
           const int slot = (DIR == 0) ? d - 1 : (DIR == 1) ? (d == 0 ? 0 : 1) : d;   // tangential directions in order
-          gr[d][f] = 0.5 * (pG[(4 * slot + f) * FG] + pG[(4 * slot + f) * FG + SS]);   // R11
+          const int gf = slot * GSLOT + ((IG4 && f == 3) ? 4 : f) * FG;   // MIG4 group: (u,v,w,p,T)
+          gr[d][f] = 0.5 * (pG[gf] + pG[gf + SS]);   // R11
         }
       }
       val[f] = 0.5 * (phL + phR);
@@ -324,11 +334,11 @@ __device__ __forceinline__ unsigned face3(const Consts& c, const double* __restr
   return fl;
 }
 
-template <int DIR, bool VISC, bool FUSE>
-__global__ void __launch_bounds__(Cfg3<DIR, VISC>::NT, Cfg3<DIR, VISC>::MINB) k_flux3(const Consts c, const FluxIn3 in,
-                                                                                     const __grid_constant__ TmaMaps tm,
-                                                                                     const Fuse3 fu) {
-  using C = Cfg3<DIR, VISC>;
+template <int DIR, bool VISC, bool FUSE, bool IG4 = false>
+__global__ void __launch_bounds__(Cfg3<DIR, VISC, IG4>::NT, Cfg3<DIR, VISC, IG4>::MINB)
+k_flux3(const Consts c, const FluxIn3 in, const __grid_constant__ TmaMaps tm, const Fuse3 fu) {
+  using C = Cfg3<DIR, VISC, IG4>;
+  constexpr int LQ = C::LQ;
   constexpr int TS = C::TS, TT = C::TT, NT = C::NT, NF = C::NF, LP = C::LP, LA = C::LA, LT = C::LT, LF = C::LF, LG = C::LG;
   constexpr int SS = (DIR == 0) ? 1 : TT;
   constexpr int FP = (DIR == 0) ? TT * LP : LP * TT;   // field strides
@@ -341,6 +351,7 @@ __global__ void __launch_bounds__(Cfg3<DIR, VISC>::NT, Cfg3<DIR, VISC>::MINB) k_
   double* const sMt = sm3 + C::oMt;
   double* const sG = sm3 + C::oG;
   double* const sA = sm3 + C::oA;
+  double* const sQ = sm3 + C::oQ;   // IG4: P' of the sweep direction
   double* const sT1 = sm3 + C::oT1;
   uint64_t* const bar = (uint64_t*)(sm3 + C::oBar);
   const int tid = threadIdx.x;
@@ -355,9 +366,9 @@ __global__ void __launch_bounds__(Cfg3<DIR, VISC>::NT, Cfg3<DIR, VISC>::MINB) k_
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32_3(bar)), "r"(1) : "memory");
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32_3(bar + 1)), "r"(1) : "memory");
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    uint32_t bytes1 = (C::NM * LF * TT + C::nG) * 8;
+    uint32_t bytes1 = (C::NM * LF * TT + C::nGtx) * 8;
     if (in.moving) bytes1 += C::nMt * 8;
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32_3(bar)), "r"(C::nP * 8) : "memory");
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32_3(bar)), "r"((C::nP + C::nQ) * 8) : "memory");
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32_3(bar + 1)), "r"(bytes1) : "memory");
     // box coordinates are (i, j, k, field) in the padded layout of each array: sweep start, transverse start, other
     auto coords = [](int s, int t, int oo, int gi, int gj, int gk, int& c0, int& c1, int& c2) {
@@ -370,13 +381,24 @@ __global__ void __launch_bounds__(Cfg3<DIR, VISC>::NT, Cfg3<DIR, VISC>::MINB) k_
     int c0, c1, c2;
     coords(s0 - 6, t0, o, GPI, GPJ, GPK, c0, c1, c2);
     tma4(sP, &tm.P, bar, c0, c1, c2, 0);
+    if (IG4) {
+      coords(s0 - 3 - C::QOFF, t0, o, GPI, GPJ, GPK, c0, c1, c2);
+      tma4(sQ, &tm.Q, bar, c0, c1, c2, 0);
+    }
     coords(s0, t0, o, 0, 0, 0, c0, c1, c2);
     tma4(sM, &tm.M, bar + 1, c0, c1, c2, 0);
     if (in.moving) tma4(sMt, &tm.Mt, bar + 1, c0, c1, c2, 0);
     if (VISC) {
       coords(s0 + GS, t0, o, GGI, GGJ, GGK, c0, c1, c2);
-      tma4(sG, &tm.G, bar + 1, c0, c1, c2, G0);
-      tma4(sG + 4 * FG, &tm.G, bar + 1, c0, c1, c2, G1);
+      if (!IG4) {
+        tma4(sG, &tm.G, bar + 1, c0, c1, c2, G0);
+        tma4(sG + 4 * FG, &tm.G, bar + 1, c0, c1, c2, G1);
+      } else {
+        // tangential gradients = the implicit gradients of the two other directions (fields u,v,w and T of each)
+        coords(s0 + GS, t0, o, GPI, GPJ, GPK, c0, c1, c2);
+        tma4(sG, &tm.G3[0], bar + 1, c0, c1, c2, 1);
+        tma4(sG + C::GSLOT, &tm.G3[1], bar + 1, c0, c1, c2, 1);
+      }
     }
   }
   if (FUSE || !in.first) {
@@ -428,7 +450,25 @@ __global__ void __launch_bounds__(Cfg3<DIR, VISC>::NT, Cfg3<DIR, VISC>::MINB) k_
     sA[sidx3<DIR, TT>(f, a, t, LA)] = d + h;
     sA[sidx3<DIR, TT>(f + 5, a, t, LA)] = d - h;
   };
-  if (DIR != 0) {
+  // MIG4: P' comes from the line solves; P'' by Eq. 19 from P and P'
+  auto cell_field_ig4 = [&](int f, int a, int t) {
+    const double* q = sP + sidx3<DIR, TT>(f, a + 4, t, LP);
+    const double* g1 = sQ + sidx3<DIR, TT>(f, a + 1 + C::QOFF, t, LQ);
+    const double d2 = 2.0 * (q[SS] - 2.0 * q[0] + q[-SS]) - 0.5 * (g1[SS] - g1[-SS]);
+    const double h = 0.5 * g1[0], d = d2 * (1.0 / 12.0);
+    sA[sidx3<DIR, TT>(f, a, t, LA)] = d + h;
+    sA[sidx3<DIR, TT>(f + 5, a, t, LA)] = d - h;
+  };
+  if (IG4) {
+    if (DIR == 0) {
+      const int t = tid >> 5, lane = tid & 31;
+#pragma unroll
+      for (int f = 0; f < 5; ++f) cell_field_ig4(f, lane, t);
+      for (int it = lane; it < (LA - 32) * 5; it += 32) cell_field_ig4(it / (LA - 32), 32 + it % (LA - 32), t);
+    } else {
+      for (int it = tid; it < 5 * LA * TT; it += NT) cell_field_ig4(it / (LA * TT), (it / TT) % LA, it % TT);
+    }
+  } else if (DIR != 0) {
     // eta/zeta sweeps: the sweep index is the slow one in shared memory, so one thread takes BLK consecutive cells
     // of one lane and field: BLK + 8 loads instead of 9 BLK (shared-memory bandwidth was at 55-60 % of peak, r1c)
     constexpr int BLK = 5, NQ = (LA + BLK - 1) / BLK;
@@ -469,7 +509,7 @@ __global__ void __launch_bounds__(Cfg3<DIR, VISC>::NT, Cfg3<DIR, VISC>::MINB) k_
     }
     for (int it = lane; it < (LA - 32) * 5; it += 32) cell_field(it / (LA - 32), 32 + it % (LA - 32), t);
   }
-  if (VISC) {
+  if (VISC && !IG4) {
     // T' on cells -1..TS.  xi: lane = cell of the warp's own row; eta/zeta: reversed so that the leftover items go to
     // the last warp
     for (int it = (DIR == 0) ? (tid & 31) : NT - 1 - tid; it < ((DIR == 0) ? LT : LT * TT); it += (DIR == 0) ? 32 : NT) {
@@ -495,9 +535,10 @@ __global__ void __launch_bounds__(Cfg3<DIR, VISC>::NT, Cfg3<DIR, VISC>::MINB) k_
   double F[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
   if (valid) {
     const double mt = in.moving ? sMt[sidx3<DIR, TT>(0, sI, row, LF)] : 0.0;
-    const unsigned fl = face3<DIR, VISC, SS, FP, FA, FG, FM>(
+    const unsigned fl = face3<DIR, VISC, SS, FP, FA, FG, FM, C::GSLOT, IG4>(
         c, sP + sidx3<DIR, TT>(0, sI + 4, row, LP), sA + sidx3<DIR, TT>(0, sI, row, LA),
-        sT1 + sidx3<DIR, TT>(0, sI, row, LT), sG + sidx3<DIR, TT>(0, sI + C::GOFF, row, LG),
+        IG4 ? sQ + sidx3<DIR, TT>(5, sI + 2 + C::QOFF, row, LQ) : sT1 + sidx3<DIR, TT>(0, sI, row, LT),
+        sG + sidx3<DIR, TT>(0, sI + C::GOFF, row, LG),
         sM + sidx3<DIR, TT>(0, sI, row, LF), mt, F);
     if (sI < TS || s0 + sI == nd) { nlim = __popc(fl); ntst = 10; }   // tile-shared faces counted once
   }

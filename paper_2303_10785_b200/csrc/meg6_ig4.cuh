@@ -11,8 +11,6 @@
 
 namespace meg6 {
 
-struct Box { int lo[3], hi[3]; };   // valid cell range [lo, hi) of an array, per direction
-
 __device__ __forceinline__ double c4_op(const double* __restrict__ f, long long s) {   // Eq. D.2
   return 2.0 / 3.0 * (f[s] - f[-s]) - 1.0 / 12.0 * (f[2 * s] - f[-2 * s]);
 }

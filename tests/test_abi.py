@@ -40,7 +40,8 @@ def test_workspace_bytes_and_validation():
     assert L.meg6_workspace_bytes(C.byref(bad)) == 0
     assert b"invalid" in L.meg6_last_error()
     mig4 = B.make_params(dict(wl["params"], scheme=1))
-    assert L.meg6_workspace_bytes(C.byref(mig4)) == 0
+    assert L.meg6_workspace_bytes(C.byref(mig4)) > nb          # MIG4: line-solve arrays and pass scratch on top
+    assert L.meg6_workspace_bytes(C.byref(B.make_params(dict(wl["params"], scheme=2)))) == 0
 
 
 def test_no_silent_cpu_fallback():

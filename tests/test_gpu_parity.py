@@ -358,3 +358,38 @@ def test_mig4_metrics_parity(mods, name):
     for kind, q, a, b in checks:
         assert np.array_equal(a, b), (name, kind, q, np.abs(a - b).max() / np.abs(b).max())
     g.close()
+
+
+@pytest.mark.parametrize("name", ["c1", "c2", "c3", "c4"])
+def test_mig4_rhs_and_steps_parity(mods, name):
+    """dQ/dt and a few RK3 steps of the MIG4 variant against the oracle: implicit gradients in the reconstruction,
+    in the viscous flux (normal and tangential) and in the metrics."""
+    torch, O, M = mods
+    wl = mig4_cases()[name]
+    t = 0.13 if wl["params"]["moving"] else 0.0
+    og = O.Grid(wl)
+    og.metrics_compute(t)
+    ref = og.rhs(wl["U0"])
+    g = M.Grid(wl)
+    g.metrics_compute(t)
+    g.limiter_stats_enable(True)
+    U = torch.as_tensor(wl["U0"], device="cuda").contiguous()
+    out = g.rhs(U).cpu().numpy()
+    e = rhs_err(out, ref, wl["U0"])
+    assert np.all(e <= RHS_TOL), (name, e, rel(out, ref))
+    lim_o, tst_o = og.limiter_stats()
+    lim_g, tst_g = g.limiter_stats()
+    assert tst_g == tst_o and abs(lim_g - lim_o) <= max(5, 1e-3 * lim_o), (lim_g, lim_o, tst_g, tst_o)
+    og.metrics_compute(0.0)
+    g.metrics_compute(0.0)
+    dt = wl["dt"] if wl["dt"] else og.cfl_dt(wl["U0"], wl["cfl"])
+    Uo = wl["U0"].copy()
+    tt = 0.0
+    for s in range(3):
+        og.rk3_step(Uo, tt, dt)
+        g.rk3_step(U, tt, dt)
+        tt += dt
+    e2 = rel(U.cpu().numpy(), Uo)
+    assert np.all(e2 <= STEP_TOL), (name, e2)
+    print("mig4 %s: rhs %s steps %s limited %d/%d" % (name, e, e2, lim_g, tst_g))
+    g.close()
