@@ -45,6 +45,12 @@ def make_workload(name):
         return W.c1_vortex(n=32)
     if name == "c2":
         return W.c2_dynamic_freestream(n=64)
+    if name == "c5":
+        return W.c5_tgv_mig4(n=384)
+    if name.startswith("c5_"):                       # large-grid sweep of config 5: c5_128 ... c5_384
+        return W.c5_tgv_mig4(n=int(name[3:]))
+    if name.startswith("c3_"):                       # same sweep with MEG6
+        return W.c3_tgv(n=int(name[3:]))
     raise SystemExit("unknown workload " + name)
 
 
@@ -59,12 +65,18 @@ def peaks():
 
 def bytes_per_cell_stage(prm, sponge):
     """Compulsory HBM doubles per cell per RK stage of the shipped kernel set."""
-    v, m = prm["viscous"], prm["moving"]
+    v, m, ig = prm["viscous"], prm["moving"], prm.get("scheme", 0) == 1
     k = {}
+    nf = 6 if v else 5
     k["prim"] = (5 + 6) / 3.0                      # once per step (the caller owns U)
-    k["grad"] = (4 + 12) if v else 0
     met = (10 if v else 3) + (1 if m else 0)
-    base = (6 if v else 5) + met + (8 if v else 0)  # primitive tile, interface metrics, stored gradients
+    if ig:
+        # MIG4: 3 nf line solves (read f, write d, read d, write x) ; sweeps read P, P' and two 5-field gradient groups
+        k["grad"] = 3 * nf * 4
+        base = nf + nf + met + (10 if v else 0)
+    else:
+        k["grad"] = (4 + 12) if v else 0
+        base = nf + met + (8 if v else 0)           # primitive tile, interface metrics, stored gradients
     k["flux_eta"] = base + 5                        # first sweep: writes the residual
     k["flux_zeta"] = base + 5 + 5                   # reads and writes it
     # last sweep, fused with assembly + RK3 stage + primitives of the new state:
@@ -286,6 +298,7 @@ def run_ours(args):
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": wl["name"], "cells": ncell, "viscous": prm["viscous"], "moving": prm["moving"],
+                       "scheme": "MIG4" if prm.get("scheme", 0) == 1 else "MEG6",
                        "dt": dt, "parallelism": "replicas x%d" % world,
                        "l2": "working set %.1f GB per stage >> 126 MB L2 (no flush needed)" % (stage_bytes * ncell / 1e9)},
             "clocks": clocks, "gpu_launches": int(launches), "finite": finite,
