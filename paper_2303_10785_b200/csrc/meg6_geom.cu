@@ -26,7 +26,7 @@ Box launch_ig4(meg6_grid* g, const Lay& L, const double* f, const Box& fb, int d
   ob.lo[dir] += 2; ob.hi[dir] -= 2;
   const int a1 = (dir == 0) ? 1 : 0, a2 = (dir == 2) ? 1 : 2;
   const long long lines = (long long)(ob.hi[a1] - ob.lo[a1]) * (ob.hi[a2] - ob.lo[a2]);
-  if (dir == 0) k_ig4<0><<<nblk(lines, 128), 128, 0, g->stream>>>(L, f, out, ob, g->ig4_cc, g->ig4_den);
+  if (dir == 0) k_ig4x<<<nblk(lines, 128), 128, 0, g->stream>>>(L, f, out, ob, g->ig4_cc, g->ig4_den);
   else if (dir == 1) k_ig4<1><<<nblk(lines, 128), 128, 0, g->stream>>>(L, f, out, ob, g->ig4_cc, g->ig4_den);
   else k_ig4<2><<<nblk(lines, 128), 128, 0, g->stream>>>(L, f, out, ob, g->ig4_cc, g->ig4_den);
   return ob;

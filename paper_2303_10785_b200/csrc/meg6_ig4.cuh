@@ -73,6 +73,75 @@ __global__ void __launch_bounds__(128) k_ig4(Lay L, const double* __restrict__ f
   }
 }
 
+// The same solve for lines along xi (unit stride): a thread walking along its own row would touch 32 different rows
+// per warp instruction.  Here a warp owns 32 rows and moves along xi in chunks of 32 columns: the chunk is loaded
+// row by row with full-width coalesced accesses into a shared-memory tile, every lane runs the recurrence of its own
+// row out of the tile (row pitch 37: conflict-free), and the results leave the same way.  Operations and their order
+// per cell are those of k_ig4.
+__global__ void __launch_bounds__(128) k_ig4x(Lay L, const double* __restrict__ f, double* out, Box ob,
+                                              const double* __restrict__ cc, const double* __restrict__ den) {
+  __shared__ double tile[4][32][37];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  double (*T)[37] = tile[warp];
+  const int n1 = ob.hi[1] - ob.lo[1], n2 = ob.hi[2] - ob.lo[2];
+  const long long nl = (long long)n1 * n2, lid = ((long long)blockIdx.x * 4 + warp) * 32 + lane;
+  const bool active = lid < nl;
+  const long long lc = active ? lid : 0;
+  const long long at = L.at(ob.lo[0], ob.lo[1] + (int)(lc % n1), ob.lo[2] + (int)(lc / n1));
+  const int m = ob.hi[0] - ob.lo[0];
+  const double al = 5.0 / 14.0, ca = (2.0 + al) / 3.0, cb = (4.0 * al - 1.0) / 12.0;
+  double prev = c4_op(f + at, 1);                   // first unknown: explicit
+  if (active) out[at] = prev;
+  for (int q0 = 1; q0 < m - 1; q0 += 32) {
+    for (int r = 0; r < 32; ++r) {                  // window columns q0-2 .. q0+33 of row r
+      const long long ar = __shfl_sync(0xffffffffu, at, r);
+      T[r][lane] = f[ar + min(q0 - 2 + lane, m + 1)];
+      if (lane < 4) T[r][32 + lane] = f[ar + min(q0 + 30 + lane, m + 1)];
+    }
+    __syncwarp();
+    for (int u = 0; u < 32; ++u) {
+      const int q = q0 + u;
+      if (q < m - 1) {
+        const double r = ca * (T[lane][u + 3] - T[lane][u + 1]) + cb * (T[lane][u + 4] - T[lane][u]);
+        prev = (r - al * prev) / den[q];
+        T[lane][u] = prev;                          // column u is not read again
+      }
+    }
+    __syncwarp();
+    for (int r = 0; r < 32; ++r) {
+      const long long ar = __shfl_sync(0xffffffffu, at, r);
+      const bool actr = __shfl_sync(0xffffffffu, (int)active, r) != 0;
+      if (actr && q0 + lane < m - 1) out[ar + q0 + lane] = T[r][lane];
+    }
+    __syncwarp();
+  }
+  double nxt = c4_op(f + at + (m - 1), 1);          // last unknown: explicit
+  if (active) out[at + (m - 1)] = nxt;
+  __syncwarp();
+  for (int q0 = m - 2; q0 >= 1; q0 -= 32) {
+    const int lo = q0 - 31;                         // chunk columns lo .. q0
+    for (int r = 0; r < 32; ++r) {
+      const long long ar = __shfl_sync(0xffffffffu, at, r);
+      T[r][lane] = out[ar + max(lo + lane, 1)];
+    }
+    __syncwarp();
+    for (int u = 0; u < 32; ++u) {
+      const int q = q0 - u;
+      if (q >= 1) {
+        nxt = T[lane][q - lo] - cc[q] * nxt;
+        T[lane][q - lo] = nxt;
+      }
+    }
+    __syncwarp();
+    for (int r = 0; r < 32; ++r) {
+      const long long ar = __shfl_sync(0xffffffffu, at, r);
+      const bool actr = __shfl_sync(0xffffffffu, (int)active, r) != 0;
+      if (actr && lo + lane >= 1) out[ar + lo + lane] = T[r][lane];
+    }
+    __syncwarp();
+  }
+}
+
 // Central interface value Eq. 36/38 from f and its gradient f1: index i of `out` = interface between
 // cells i and i+1 along dir.  The second derivative is Eq. 19.  `out` may have another layout (interface
 // arrays): LO, and an index shift `sh` along dir (interface arrays number the face between cells i-1 and i as i).
