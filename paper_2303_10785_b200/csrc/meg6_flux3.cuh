@@ -18,11 +18,13 @@
 
 namespace meg6 {
 
+// CTAs per SM the sweeps are compiled for: 4 (128 registers) and 5 (96 registers, more spills) are equal on the
+// mostly smooth C4 start-up flow; with the full limiting path in every warp (C3/C5) 4 is 7 % faster.
 #ifndef MEG6_MINB3_X
-#define MEG6_MINB3_X 5
+#define MEG6_MINB3_X 4
 #endif
 #ifndef MEG6_MINB3_Y
-#define MEG6_MINB3_Y 5
+#define MEG6_MINB3_Y 4
 #endif
 #ifndef MEG6_RELOAD
 #define MEG6_RELOAD 1
