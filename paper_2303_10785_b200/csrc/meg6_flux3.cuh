@@ -256,13 +256,22 @@ __device__ __forceinline__ unsigned face3(const Consts& c, const double* __restr
     project3(e, MEG6_D2(2, 0), MEG6_D2(2, 1), MEG6_D2(2, 2), MEG6_D2(2, 3), MEG6_D2(2, 4), DR);
     project3(e, MEG6_D2(3, 0), MEG6_D2(3, 1), MEG6_D2(3, 2), MEG6_D2(3, 3), MEG6_D2(3, 4), Dp);
 #undef MEG6_D2
+    // component by component, side by side: evaluated only where some lane of the warp failed E.1 there (failures
+    // cluster at extrema of one characteristic field, so most of the ten evaluations are skipped in smooth flow)
+    const unsigned wfl = __reduce_or_sync(__activemask(), fl);
 #pragma unroll
     for (int r = 0; r < 5; ++r) {
-      const double dnear = minmod3(DL[r], DR[r]);
-      const double lL = mp_limit3(EL[r], W0[r], Wm[r], dnear, minmod3(Dm[r], DL[r]), c.mp_alpha);
-      const double lR = mp_limit3(ER[r], -W0[r], -Wp[r], dnear, minmod3(DR[r], Dp[r]), c.mp_alpha);
-      EL[r] = ((fl >> r) & 1u) ? lL : EL[r];
-      ER[r] = ((fl >> (r + 5)) & 1u) ? lR : ER[r];
+      if ((wfl >> r) & 33u) {
+        const double dnear = minmod3(DL[r], DR[r]);
+        if ((wfl >> r) & 1u) {
+          const double lL = mp_limit3(EL[r], W0[r], Wm[r], dnear, minmod3(Dm[r], DL[r]), c.mp_alpha);
+          EL[r] = ((fl >> r) & 1u) ? lL : EL[r];
+        }
+        if ((wfl >> r) & 32u) {
+          const double lR = mp_limit3(ER[r], -W0[r], -Wp[r], dnear, minmod3(DR[r], Dp[r]), c.mp_alpha);
+          ER[r] = ((fl >> (r + 5)) & 1u) ? lR : ER[r];
+        }
+      }
     }
   }
   double PL[5], PR[5];
