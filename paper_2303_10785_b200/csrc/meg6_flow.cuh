@@ -110,10 +110,12 @@ __device__ __forceinline__ double d1_op(const double* __restrict__ f, long long 
 #endif
 constexpr int GRAD_KB = MEG6_GRAD_KB;
 __global__ void __launch_bounds__(256, MEG6_GRAD_MINB) k_grad(Consts c, P6 P, P12 G) {
-  const int i = blockIdx.x * 32 + threadIdx.x - 1;
+  // i runs over the whole padded row of G (-GGI .. pitch-GGI): the cells beyond -1 and n are padding nobody reads, but
+  // writing them makes every warp store start and end on a 32-byte sector (no partial-sector fills in L2/DRAM)
+  const int i = blockIdx.x * 32 + threadIdx.x - GGI;
   const int j = blockIdx.y * 8 + threadIdx.y - 1;
   const int k0 = blockIdx.z * GRAD_KB - 1;
-  if (i > c.n[0] || j > c.n[1]) return;
+  if (i >= c.LG.pi - GGI || j > c.n[1]) return;
   const long long sj = c.LP.sj, sk = c.LP.sk;
   const long long ap0 = c.LP.at(i, j, k0), ag0 = c.LG.at(i, j, k0);
 #pragma unroll
