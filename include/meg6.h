@@ -94,6 +94,12 @@ meg6_status meg6_rk3_step(meg6_grid* g, double* U, double t, double dt);
  * Synchronises the stream.  *dt is a HOST pointer. */
 meg6_status meg6_cfl_dt(meg6_grid* g, const double* U, double cfl, double* dt);
 
+/* Volume-averaged kinetic energy and enstrophy of the state U (Eq. 54, written for three dimensions with
+ * dV = 1/J; vorticity from the shared first gradients of the velocity) and the volume, at the geometry of the
+ * last metrics_compute: out[0] = E_k, out[1] = enstrophy, out[2] = sum of 1/J.  out is a HOST pointer (3 doubles);
+ * synchronises the stream.  Overwrites the library's primitive buffer (like meg6_rhs). */
+meg6_status meg6_diagnostics(meg6_grid* g, const double* U, double* out);
+
 /* Counters of interface-components tested / limited by the MP limiter (test E.1 failed) since grid
  * creation, accumulated only while enabled (default off; costs atomics).  HOST pointers; synchronises. */
 meg6_status meg6_limiter_stats_enable(meg6_grid* g, int on);

@@ -871,6 +871,35 @@ double meg6o_cfl_dt(meg6o_grid* G, const double* U, double cfl) {
   return cfl * dt;
 }
 
+/* Volume-averaged kinetic energy and enstrophy, the integrals of Eq. 54 written for three dimensions and
+ * curvilinear cells (dV = 1/J), the vorticity from the SHARED first gradients of the primitives through the
+ * chain rule with the cell-centre metrics (Eq. 32 form):  out = { E_k, enstrophy, volume }. */
+void meg6o_diagnostics(meg6o_grid* G, const double* U, double* out) {
+  const meg6o_params& p = G->p;
+  const int ni = G->n[0], nj = G->n[1], nk = G->n[2];
+  fill_primitives(G, U);
+  Arr g[3][3];   /* g[d][c] = gradient along direction d of velocity component c */
+  for (int d = 0; d < 3; ++d)
+    for (int c = 0; c < 3; ++c) grad_dir(G->P[1 + c], d, p.scheme, g[d][c]);
+  double ke = 0.0, en = 0.0, vol = 0.0;
+  for (int k = 0; k < nk; ++k)
+    for (int j = 0; j < nj; ++j)
+      for (int i = 0; i < ni; ++i) {
+        const double rj = G->rj(i, j, k), J = 1.0 / rj;
+        double dv[3][3];   /* dv[c][x] = d(velocity c)/d(coordinate x) */
+        for (int c = 0; c < 3; ++c)
+          for (int x = 0; x < 3; ++x)
+            dv[c][x] = J * (G->met[x](i, j, k) * g[0][c](i, j, k) + G->met[3 + x](i, j, k) * g[1][c](i, j, k) +
+                            G->met[6 + x](i, j, k) * g[2][c](i, j, k));
+        const double ox = dv[2][1] - dv[1][2], oy = dv[0][2] - dv[2][0], oz = dv[1][0] - dv[0][1];
+        const double r = G->P[0](i, j, k), u = G->P[1](i, j, k), v = G->P[2](i, j, k), w = G->P[3](i, j, k);
+        ke += r * 0.5 * (u * u + v * v + w * w) * rj;
+        en += r * 0.5 * (ox * ox + oy * oy + oz * oz) * rj;
+        vol += rj;
+      }
+  out[0] = ke / vol; out[1] = en / vol; out[2] = vol;
+}
+
 void meg6o_limiter_stats(meg6o_grid* G, unsigned long long* n_limited, unsigned long long* n_tested) {
   *n_limited = G->n_limited; *n_tested = G->n_tested;
 }

@@ -50,6 +50,8 @@ void meg6o_set_sponge(meg6o_grid* g, const double* sigma, const double* U_ref);
 void meg6o_rhs(meg6o_grid* g, const double* U, double* dUdt);
 void meg6o_rk3_step(meg6o_grid* g, double* U, double t, double dt);
 double meg6o_cfl_dt(meg6o_grid* g, const double* U, double cfl);
+/* volume-averaged kinetic energy, enstrophy (Eq. 54, in 3-D with dV = 1/J) and the volume: out[3] */
+void meg6o_diagnostics(meg6o_grid* g, const double* U, double* out);
 void meg6o_limiter_stats(meg6o_grid* g, unsigned long long* n_limited, unsigned long long* n_tested);
 
 /* inspection (tests): which = 0..8 hatted metrics (xi_x..zeta_z), 9 = 1/J, 10..12 = xi_t,eta_t,zeta_t

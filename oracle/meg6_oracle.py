@@ -63,6 +63,7 @@ def lib():
         L.meg6o_rk3_step.argtypes = [C.c_void_p, _dp, C.c_double, C.c_double]
         L.meg6o_cfl_dt.restype = C.c_double
         L.meg6o_cfl_dt.argtypes = [C.c_void_p, _dp, C.c_double]
+        L.meg6o_diagnostics.argtypes = [C.c_void_p, _dp, _dp]
         L.meg6o_limiter_stats.argtypes = [C.c_void_p, C.POINTER(C.c_ulonglong), C.POINTER(C.c_ulonglong)]
         L.meg6o_get_cell.argtypes = [C.c_void_p, C.c_int, _dp]
         L.meg6o_get_face.argtypes = [C.c_void_p, C.c_int, C.c_int, _dp]
@@ -168,6 +169,13 @@ class Grid:
         """In place on a contiguous float64 array."""
         assert U.flags.c_contiguous and U.dtype == np.float64
         lib().meg6o_rk3_step(self.h, _p(U), float(t), float(dt))
+
+    def diagnostics(self, U):
+        """(kinetic energy, enstrophy, volume), Eq. 54"""
+        U = _c(U)
+        out = np.empty(3)
+        lib().meg6o_diagnostics(self.h, _p(U), _p(out))
+        return out
 
     def cfl_dt(self, U, cfl):
         U = _c(U)

@@ -8,7 +8,7 @@ import os
 from . import build as _build
 
 EXPORTS = ["meg6_workspace_bytes", "meg6_grid_create", "meg6_grid_destroy", "meg6_metrics_compute",
-           "meg6_set_inflow", "meg6_set_sponge", "meg6_rhs", "meg6_rk3_step", "meg6_cfl_dt",
+           "meg6_set_inflow", "meg6_set_sponge", "meg6_rhs", "meg6_rk3_step", "meg6_cfl_dt", "meg6_diagnostics",
            "meg6_limiter_stats_enable", "meg6_limiter_stats", "meg6_get_array", "meg6_profile_enable",
            "meg6_profile_read", "meg6_last_error",
            "meg6_version"]
@@ -81,6 +81,8 @@ def lib():
         L.meg6_rhs.argtypes = [_vp, _vp, _vp]
         L.meg6_rk3_step.restype = C.c_int
         L.meg6_rk3_step.argtypes = [_vp, _vp, C.c_double, C.c_double]
+        L.meg6_diagnostics.restype = C.c_int
+        L.meg6_diagnostics.argtypes = [_vp, _vp, C.POINTER(C.c_double)]
         L.meg6_cfl_dt.restype = C.c_int
         L.meg6_cfl_dt.argtypes = [_vp, _vp, C.c_double, C.POINTER(C.c_double)]
         L.meg6_limiter_stats_enable.restype = C.c_int
@@ -172,6 +174,12 @@ class Grid:
     def rk3_step(self, U, t, dt):
         self._chk_state(U)
         _check(lib().meg6_rk3_step(self.h, U.data_ptr(), float(t), float(dt)), "meg6_rk3_step")
+
+    def diagnostics(self, U):
+        """(kinetic energy, enstrophy, volume) of the state U, Eq. 54"""
+        out = (C.c_double * 3)()
+        _check(lib().meg6_diagnostics(self.h, U.data_ptr(), out), "meg6_diagnostics")
+        return [out[0], out[1], out[2]]
 
     def cfl_dt(self, U, cfl):
         self._chk_state(U)

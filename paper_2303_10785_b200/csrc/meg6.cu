@@ -120,7 +120,7 @@ static size_t carve(const meg6_params* p, const Consts& c, meg6_grid* g, char* b
     }
   }
   G->stats = (unsigned long long*)take(2);
-  G->red = take(2 * CFL_BLOCKS);
+  G->red = take(4 * CFL_BLOCKS);
   return off;
 }
 
@@ -366,14 +366,8 @@ meg6_status meg6_set_sponge(meg6_grid* g, const double* sigma, const double* U_r
   return MEG6_OK;
 }
 
-// One RK stage (or one dQ/dt evaluation) for the state whose primitives are in buffer `buf` (interior cells
-// filled): ghost fill, stored gradients, eta and zeta sweeps into g->res, xi sweep fused with the residual
-// assembly, the stage update and the primitive conversion of the new state (into the other buffer).
-static meg6_status stage(meg6_grid* g, int buf, const Fuse3& fu) {
+static void fill_ghosts(meg6_grid* g, const P6& P) {
   const Consts& c = g->c;
-  double* const* Pc = buf ? g->Pb : g->P;
-  P6 P;
-  for (int f = 0; f < 6; ++f) P.p[f] = Pc[f];
   for (int d = 0; d < 3; ++d) {
     int a = (d + 1) % 3, b = (d + 2) % 3;
     if (a > b) { int t = a; a = b; b = t; }
@@ -384,6 +378,17 @@ static meg6_status stage(meg6_grid* g, int buf, const Fuse3& fu) {
     ProfScope ps(g, 2, 1);
     k_ghost<<<nblk(ea * eb * 12, 256), 256, 0, g->stream>>>(c, d, P, gin);
   }
+}
+
+// One RK stage (or one dQ/dt evaluation) for the state whose primitives are in buffer `buf` (interior cells
+// filled): ghost fill, stored gradients, eta and zeta sweeps into g->res, xi sweep fused with the residual
+// assembly, the stage update and the primitive conversion of the new state (into the other buffer).
+static meg6_status stage(meg6_grid* g, int buf, const Fuse3& fu) {
+  const Consts& c = g->c;
+  double* const* Pc = buf ? g->Pb : g->P;
+  P6 P;
+  for (int f = 0; f < 6; ++f) P.p[f] = Pc[f];
+  fill_ghosts(g, P);
   const bool IG = g->p.scheme == 1;
   if (IG) {
     // MIG4: implicit gradients of every staged field along the three directions (Eq. 18), whole grid lines
@@ -492,6 +497,41 @@ meg6_status meg6_cfl_dt(meg6_grid* g, const double* U, double cfl, double* dt) {
   double r = a;
   if (g->p.viscous) r = fmin(r, b / 4.0);   // R25: the alpha of Eq. B.3 read as alpha^D = 4
   *dt = cfl * r;
+  return MEG6_OK;
+}
+
+meg6_status meg6_diagnostics(meg6_grid* g, const double* U, double* out) {
+  if (!g || !U || !out) return fail(MEG6_EINVAL, "diagnostics: null pointer%s");
+  if (!g->have_metrics) return fail(MEG6_ESTATE, "diagnostics called before metrics_compute%s");
+  const Consts& c = g->c;
+  launch_prim(g, U);
+  P6 P;
+  for (int f = 0; f < 6; ++f) P.p[f] = g->P[f];
+  fill_ghosts(g, P);
+  DiagIn in;
+  memset(&in, 0, sizeof(in));
+  for (int q = 0; q < 9; ++q) in.met[q] = g->met[q];
+  in.rj = g->rj;
+  for (int f = 0; f < 4; ++f) in.P[f] = g->P[f];
+  in.ig4 = g->p.scheme == 1;
+  if (in.ig4) {
+    meg6::Box pb;
+    for (int a = 0; a < 3; ++a) { pb.lo[a] = -6; pb.hi[a] = c.n[a] + 6; }
+    for (int d = 0; d < 3; ++d)
+      for (int cc = 0; cc < 3; ++cc) {
+        meg6::launch_ig4(g, c.LP, g->P[1 + cc], pb, d, g->Gi[d][1 + cc]);
+        in.g[3 * d + cc] = g->Gi[d][1 + cc];
+      }
+  }
+  const int nb = (int)((c.LC.n + 255) / 256 < CFL_BLOCKS ? (c.LC.n + 255) / 256 : CFL_BLOCKS);
+  k_diag<<<nb, 256, 0, g->stream>>>(c, in, g->red);
+  CUDA_OK(cudaGetLastError());
+  static thread_local double host[3 * CFL_BLOCKS];
+  CUDA_OK(cudaMemcpyAsync(host, g->red, sizeof(double) * 3 * nb, cudaMemcpyDeviceToHost, g->stream));
+  CUDA_OK(cudaStreamSynchronize(g->stream));
+  double ke = 0.0, en = 0.0, vol = 0.0;
+  for (int q = 0; q < nb; ++q) { ke += host[3 * q]; en += host[3 * q + 1]; vol += host[3 * q + 2]; }
+  out[0] = ke / vol; out[1] = en / vol; out[2] = vol;
   return MEG6_OK;
 }
 

@@ -186,4 +186,47 @@ __global__ void __launch_bounds__(256) k_cfl(Consts c, const double* __restrict_
   if (threadIdx.x == 0) { red[2 * blockIdx.x] = sa[0]; red[2 * blockIdx.x + 1] = sb[0]; }
 }
 
+// Volume-averaged kinetic energy and enstrophy (Eq. 54, in three dimensions with dV = 1/J): per-block sums
+// of rho |u|^2/2 dV, rho |omega|^2/2 dV and dV.  The vorticity comes from the shared first gradients of the velocity
+// -- E6 stencils of the primitive arrays, or the stored IG4 gradients for MIG4 -- through the chain rule with
+// the cell-centre metrics.  red[3*b + {0,1,2}]; the host finishes the sums.
+struct DiagIn { const double* met[9]; const double* rj; const double* P[4]; const double* g[9]; int ig4; };
+
+__global__ void __launch_bounds__(256) k_diag(Consts c, DiagIn in, double* __restrict__ red) {
+  const long long N = c.LC.n;
+  double ke = 0.0, en = 0.0, vol = 0.0;
+  for (long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x; tid < N; tid += (long long)gridDim.x * blockDim.x) {
+    const int i = (int)(tid % c.n[0]), j = (int)((tid / c.n[0]) % c.n[1]), k = (int)(tid / ((long long)c.n[0] * c.n[1]));
+    const long long ax = c.LX.at(i, j, k), ap = c.LP.at(i, j, k);
+    const double rj = in.rj[ax], J = 1.0 / rj;
+    double gq[3][3];   // gq[d][comp]
+#pragma unroll
+    for (int d = 0; d < 3; ++d)
+#pragma unroll
+      for (int cc = 0; cc < 3; ++cc)
+        gq[d][cc] = in.ig4 ? in.g[3 * d + cc][ap] : d1_op(in.P[1 + cc] + ap, c.LP.stride(d));
+    double dv[3][3];   // dv[comp][x]
+#pragma unroll
+    for (int cc = 0; cc < 3; ++cc)
+#pragma unroll
+      for (int x = 0; x < 3; ++x)
+        dv[cc][x] = J * (in.met[x][ax] * gq[0][cc] + in.met[3 + x][ax] * gq[1][cc] + in.met[6 + x][ax] * gq[2][cc]);
+    const double ox = dv[2][1] - dv[1][2], oy = dv[0][2] - dv[2][0], oz = dv[1][0] - dv[0][1];
+    const double r = in.P[0][ap], u = in.P[1][ap], v = in.P[2][ap], w = in.P[3][ap];
+    ke += r * 0.5 * (u * u + v * v + w * w) * rj;
+    en += r * 0.5 * (ox * ox + oy * oy + oz * oz) * rj;
+    vol += rj;
+  }
+  __shared__ double sa[256], sb[256], sc[256];
+  sa[threadIdx.x] = ke; sb[threadIdx.x] = en; sc[threadIdx.x] = vol;
+  __syncthreads();
+  for (int o = 128; o > 0; o >>= 1) {
+    if ((int)threadIdx.x < o) {
+      sa[threadIdx.x] += sa[threadIdx.x + o]; sb[threadIdx.x] += sb[threadIdx.x + o]; sc[threadIdx.x] += sc[threadIdx.x + o];
+    }
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) { red[3 * blockIdx.x] = sa[0]; red[3 * blockIdx.x + 1] = sb[0]; red[3 * blockIdx.x + 2] = sc[0]; }
+}
+
 }  // namespace meg6

@@ -415,3 +415,21 @@ def test_mig4_freestream_static_and_dynamic_on_gpu(mods):
         Uh = U.cpu().numpy()
         assert max(np.abs(Uh[0] - 1).max(), np.abs(Uh[2] / Uh[0]).max(), np.abs(Uh[3] / Uh[0]).max()) <= 1e-12
         g.close()
+
+
+@pytest.mark.parametrize("scheme", [0, 1])
+def test_diagnostics_parity(mods, scheme):
+    """Kinetic energy / enstrophy / volume (Eq. 54) on the viscous TGV and on the moving jittered mesh: sums of ~1e5
+    positive terms in a different order on the two sides, hence 1e-12 relative."""
+    torch, O, M = mods
+    cases = mig4_cases() if scheme else small_cases()
+    for name in ("c1", "c2", "c3"):
+        wl = cases[name]
+        og = O.Grid(wl)
+        og.metrics_compute(0.05)
+        g = M.Grid(wl)
+        g.metrics_compute(0.05)
+        U = torch.as_tensor(wl["U0"], device="cuda").contiguous()
+        a, b = np.array(g.diagnostics(U)), og.diagnostics(wl["U0"])
+        assert np.all(np.abs(a - b) <= 1e-12 * np.abs(b)), (name, a, b)
+        g.close()
