@@ -45,6 +45,8 @@ def make_workload(name):
         return W.c1_vortex(n=32)
     if name == "c2":
         return W.c2_dynamic_freestream(n=64)
+    if name.startswith("c2_"):                       # moving-mesh freestream at other sizes
+        return W.c2_dynamic_freestream(n=int(name[3:]))
     if name == "c5":
         return W.c5_tgv_mig4(n=384)
     if name.startswith("c5_"):                       # large-grid sweep of config 5: c5_128 ... c5_384

@@ -7,6 +7,18 @@ namespace meg6 {
 
 static inline unsigned nblk(long long n, int t) { return (unsigned)((n + t - 1) / t); }
 
+// cell centres of the interior, then ghost layers direction by direction (xi, eta over the xi-extended array, zeta)
+static void launch_centres(meg6_grid* g, const GeomIn& gi, P3 xc, P3 xt) {
+  const Consts& c = g->c;
+  k_centres<<<nblk(c.LC.n, 256), 256, 0, g->stream>>>(c, gi, xc, xt);
+  for (int d = 0; d < 3; ++d) {
+    int a = (d + 1) % 3, b = (d + 2) % 3;
+    if (a > b) { int t = a; a = b; b = t; }
+    const long long ea = c.n[a] + ((a < d) ? 2 * GX : 0), eb = c.n[b] + ((b < d) ? 2 * GX : 0);
+    k_extend<<<nblk(ea * eb * 2 * GX, 256), 256, 0, g->stream>>>(c, d, xc, xt);
+  }
+}
+
 // ---- MIG4 (scheme 1): the geometry as whole-array passes, each the operation the discretisation names ----
 static Box box_all(const Consts& c) {
   Box b;
@@ -55,7 +67,7 @@ static cudaError_t launch_geometry_ig4(meg6_grid* g, const GeomIn& gi) {
   const Lay& L = c.LX;
   P3 xc, xt;
   for (int q = 0; q < 3; ++q) { xc.p[q] = g->xc[q]; xt.p[q] = g->xt[q]; }
-  k_centres<<<nblk(L.n, 256), 256, 0, g->stream>>>(c, gi, xc, xt);
+  launch_centres(g, gi, xc, xt);
   double* f1 = g->scr[0]; double* H = g->scr[1]; double* t1 = g->scr[2]; double* t2 = g->scr[3];
   double* d1 = g->scr[4]; double* d2 = g->scr[5];
   const Box all = box_all(c);
@@ -130,7 +142,7 @@ cudaError_t launch_geometry(meg6_grid* g, double t) {
   for (int q = 0; q < 9; ++q) { cd.p[q] = g->cd[q]; met.p[q] = g->met[q]; }
   if (g->p.scheme == 1) return launch_geometry_ig4(g, gi);
   const int T = 256;
-  k_centres<<<nblk(c.LX.n, T), T, 0, g->stream>>>(c, gi, xc, xt);
+  launch_centres(g, gi, xc, xt);
   k_coord_deriv<<<nblk(c.LX.n, T), T, 0, g->stream>>>(c, xc, cd);
   const long long nm = (long long)(c.n[0] + 10) * (c.n[1] + 10) * (c.n[2] + 10);
   k_metrics<<<nblk(nm, 128), 128, 0, g->stream>>>(c, xc, xt, cd, met, g->rj, mt);

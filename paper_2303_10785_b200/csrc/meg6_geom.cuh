@@ -29,49 +29,60 @@ __device__ __forceinline__ double cell_mean(const Consts& c, const GeomIn& g, in
   return acc / 8.0;
 }
 
-// Ghost-cell coordinates (R13, R14), direction by direction: xi first, then eta over the xi-extended
-// array, then zeta.  Periodic: image -/+ period; otherwise linear extrapolation of the last spacing.
-template <int D>
-__device__ double ext_val(const Consts& c, const GeomIn& g, int comp, bool vel, int i, int j, int k) {
-  if constexpr (D < 0) {
-    return cell_mean(c, g, comp, vel, i, j, k);
-  } else {
-    int idx[3] = {i, j, k};
-    const int a = idx[D], n = c.n[D];
-    if (a >= 0 && a < n) return ext_val<D - 1>(c, g, comp, vel, i, j, k);
-    if (c.periodic[D]) {
-      const double off = vel ? 0.0 : c.period[D][comp];
-      if (a < 0) { idx[D] = a + n; return ext_val<D - 1>(c, g, comp, vel, idx[0], idx[1], idx[2]) - off; }
-      idx[D] = a - n;
-      return ext_val<D - 1>(c, g, comp, vel, idx[0], idx[1], idx[2]) + off;
-    }
-    if (a < 0) {
-      idx[D] = 0; const double v0 = ext_val<D - 1>(c, g, comp, vel, idx[0], idx[1], idx[2]);
-      idx[D] = 1; const double v1 = ext_val<D - 1>(c, g, comp, vel, idx[0], idx[1], idx[2]);
-      return v0 - (double)(-a) * (v1 - v0);
-    }
-    idx[D] = n - 1; const double v0 = ext_val<D - 1>(c, g, comp, vel, idx[0], idx[1], idx[2]);
-    idx[D] = n - 2; const double v1 = ext_val<D - 1>(c, g, comp, vel, idx[0], idx[1], idx[2]);
-    return v0 + (double)(a - (n - 1)) * (v0 - v1);
-  }
-}
-
 struct P3 { double* p[3]; };
 struct P9 { double* p[9]; };
 
-// M1: cell-centre coordinates (and grid velocities) on the whole padded box.
-__global__ void k_centres(Consts c, GeomIn g, P3 xc, P3 xt) {
+// M1a: cell-centre coordinates (and grid velocities) of the interior cells: 8-vertex mean.
+__global__ void __launch_bounds__(256) k_centres(Consts c, GeomIn g, P3 xc, P3 xt) {
   const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (tid >= c.LX.n) return;
-  const int pi = (int)(tid % c.LX.pi);
-  const int pj = (int)((tid / c.LX.pi) % c.LX.pj);
-  const int pk = (int)(tid / c.LX.sk);
-  const int i = pi - GX, j = pj - GX, k = pk - GX;
-  if (i >= c.n[0] + GX) return;   // alignment padding
+  if (tid >= c.LC.n) return;
+  const int i = (int)(tid % c.n[0]), j = (int)((tid / c.n[0]) % c.n[1]), k = (int)(tid / ((long long)c.n[0] * c.n[1]));
+  const long long at = c.LX.at(i, j, k);
 #pragma unroll
   for (int comp = 0; comp < 3; ++comp) {
-    xc.p[comp][tid] = ext_val<2>(c, g, comp, false, i, j, k);
-    if (c.moving) xt.p[comp][tid] = ext_val<2>(c, g, comp, true, i, j, k);
+    xc.p[comp][at] = cell_mean(c, g, comp, false, i, j, k);
+    if (c.moving) xt.p[comp][at] = cell_mean(c, g, comp, true, i, j, k);
+  }
+}
+
+// M1b: ghost layers of direction d (R13, R14), after the lower directions: periodic -> image -/+ period (velocities:
+// plain copy); otherwise linear extrapolation of the last spacing.  The same values, operation by operation, as the
+// recursive definition ext_val (xi innermost, zeta outermost).  One thread per ghost cell.
+__global__ void __launch_bounds__(256) k_extend(Consts c, int d, P3 xc, P3 xt) {
+  int a = (d + 1) % 3, b = (d + 2) % 3;
+  if (a > b) { int t = a; a = b; b = t; }
+  const int loa = (a < d) ? -GX : 0, ea = c.n[a] + ((a < d) ? 2 * GX : 0);
+  const int lob = (b < d) ? -GX : 0, eb = c.n[b] + ((b < d) ? 2 * GX : 0);
+  const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (tid >= (long long)ea * eb * 2 * GX) return;
+  int qs, ta, tb;
+  if (d == 0) { qs = (int)(tid % (2 * GX)); const long long r = tid / (2 * GX); ta = loa + (int)(r % ea); tb = lob + (int)(r / ea); }
+  else if (d == 1) { ta = loa + (int)(tid % ea); const long long r = tid / ea; qs = (int)(r % (2 * GX)); tb = lob + (int)(r / (2 * GX)); }
+  else { ta = loa + (int)(tid % ea); const long long r = tid / ea; tb = lob + (int)(r % eb); qs = (int)(r / eb); }
+  const int side = qs / GX, q = qs % GX + 1;
+  const int n = c.n[d];
+  const int ai = side ? n - 1 + q : -q;          // ghost index along d
+  int ix[3];
+  ix[a] = ta; ix[b] = tb; ix[d] = 0;
+  const long long base = c.LX.at(ix[0], ix[1], ix[2]), s = c.LX.stride(d);
+  const long long dst = base + (long long)ai * s;
+#pragma unroll
+  for (int comp = 0; comp < 3; ++comp) {
+#pragma unroll
+    for (int vel = 0; vel < 2; ++vel) {
+      if (vel && !c.moving) continue;
+      double* f = vel ? xt.p[comp] : xc.p[comp];
+      if (c.periodic[d]) {
+        const double off = vel ? 0.0 : c.period[d][comp];
+        f[dst] = side ? f[base + (long long)(ai - n) * s] + off : f[base + (long long)(ai + n) * s] - off;
+      } else if (!side) {
+        const double v0 = f[base], v1 = f[base + s];
+        f[dst] = v0 - (double)(-ai) * (v1 - v0);
+      } else {
+        const double v0 = f[base + (long long)(n - 1) * s], v1 = f[base + (long long)(n - 2) * s];
+        f[dst] = v0 + (double)(ai - (n - 1)) * (v0 - v1);
+      }
+    }
   }
 }
 
@@ -147,7 +158,15 @@ __device__ __forceinline__ double delta_prod(const double* __restrict__ a, const
 
 // M3: Thomas-Lombard conservative metrics Eq. 10, 1/J Eq. 13, hatted time metrics
 // Eq. 11, on cells [-5, n+5)^3.
-__global__ void k_metrics(Consts c, P3 xc, P3 xt, P9 cd, P9 met, double* __restrict__ rj, P3 mt) {
+// k_metrics: the row loop is kept rolled (112 registers, 4 CTAs/SM) -- fully unrolled it needs 224 registers and is
+// 25 % slower on a 256^3 moving mesh (the kernel is bound by its ~400 L1 loads per cell, i.e. by occupancy)
+#ifndef MEG6_KM_MINB
+#define MEG6_KM_MINB 4
+#endif
+#ifndef MEG6_KM_UNROLL
+#define MEG6_KM_UNROLL 0
+#endif
+__global__ void __launch_bounds__(128, MEG6_KM_MINB) k_metrics(Consts c, P3 xc, P3 xt, P9 cd, P9 met, double* __restrict__ rj, P3 mt) {
   const int ei = c.n[0] + 10, ej = c.n[1] + 10;
   const long long total = (long long)ei * ej * (c.n[2] + 10);
   const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -155,7 +174,11 @@ __global__ void k_metrics(Consts c, P3 xc, P3 xt, P9 cd, P9 met, double* __restr
   const int i = (int)(tid % ei) - 5, j = (int)((tid / ei) % ej) - 5, k = (int)(tid / ((long long)ei * ej)) - 5;
   const long long at = c.LX.at(i, j, k);
   double m[9];
+#if MEG6_KM_UNROLL
 #pragma unroll
+#else
+#pragma unroll 1
+#endif
   for (int r = 0; r < 3; ++r) {
     const int a = (r + 1) % 3, b = (r + 2) % 3;
     const long long sa = c.LX.stride(a), sb = c.LX.stride(b);
