@@ -433,3 +433,39 @@ def test_diagnostics_parity(mods, scheme):
         a, b = np.array(g.diagnostics(U)), og.diagnostics(wl["U0"])
         assert np.all(np.abs(a - b) <= 1e-12 * np.abs(b)), (name, a, b)
         g.close()
+
+
+def test_abi_error_paths_on_device(mods):
+    """Error behaviour the header promises: status codes, no exceptions, no partial handles."""
+    import ctypes as C
+    torch, O, M = mods
+    from paper_2303_10785_b200 import binding as B
+    L = B.lib()
+    wl = W.c1_vortex(n=12)
+    p = B.make_params(wl["params"])
+    nb = L.meg6_workspace_bytes(C.byref(p))
+    ws = torch.empty(nb + 512, dtype=torch.uint8, device="cuda")
+    base = (ws.data_ptr() + 255) // 256 * 256
+    x, y, z = (torch.as_tensor(wl[k], device="cuda").contiguous() for k in ("x", "y", "z"))
+    h = C.c_void_p()
+    args = lambda wsp, n: (C.byref(p), C.c_void_p(x.data_ptr()), C.c_void_p(y.data_ptr()), C.c_void_p(z.data_ptr()),
+                           None, None, None, C.c_void_p(wsp), C.c_size_t(n), None, C.byref(h))
+    saved = L.meg6_grid_create.argtypes
+    L.meg6_grid_create.argtypes = None           # raw calls with deliberately wrong arguments; restored below
+    assert L.meg6_grid_create(*args(base, nb - 1)) == 2 and not h.value        # MEG6_ENOMEM: workspace too small
+    assert L.meg6_grid_create(*args(base + 8, nb)) == 1 and not h.value        # MEG6_EINVAL: misaligned workspace
+    assert L.meg6_grid_create(C.byref(p), None, None, None, None, None, None, C.c_void_p(base), C.c_size_t(nb), None,
+                              C.byref(h)) == 1                                  # null node arrays
+    assert L.meg6_grid_create(*args(base, nb)) == 0 and h.value
+    U = torch.as_tensor(wl["U0"], device="cuda").contiguous()
+    out = torch.empty_like(U)
+    assert L.meg6_rhs(h, C.c_void_p(U.data_ptr()), C.c_void_p(out.data_ptr())) == 4       # MEG6_ESTATE
+    assert b"metrics_compute" in L.meg6_last_error()
+    assert L.meg6_rhs(h, None, C.c_void_p(out.data_ptr())) == 1
+    assert L.meg6_metrics_compute(h, C.c_double(0.0)) == 0
+    assert L.meg6_rhs(h, C.c_void_p(U.data_ptr()), C.c_void_p(out.data_ptr())) == 0
+    assert L.meg6_set_inflow(h, 0, C.c_void_p(U.data_ptr())) == 1               # periodic face: not an inflow face
+    torch.cuda.synchronize()
+    assert bool(torch.isfinite(out).all())
+    L.meg6_grid_destroy(h)
+    L.meg6_grid_create.argtypes = saved
