@@ -143,9 +143,13 @@ cudaError_t launch_geometry(meg6_grid* g, double t) {
   if (g->p.scheme == 1) return launch_geometry_ig4(g, gi);
   const int T = 256;
   launch_centres(g, gi, xc, xt);
-  k_coord_deriv<<<nblk(c.LX.n, T), T, 0, g->stream>>>(c, xc, cd);
-  const long long nm = (long long)(c.n[0] + 10) * (c.n[1] + 10) * (c.n[2] + 10);
-  k_metrics<<<nblk(nm, 128), 128, 0, g->stream>>>(c, xc, xt, cd, met, g->rj, mt);
+  k_coord_deriv<<<nblk(c.LX.n, T), T, 0, g->stream>>>(c, xc, cd, g->rj);
+  {
+    const int e0 = c.n[0] + 10, e1 = c.n[1] + 10, e2 = c.n[2] + 10;
+    k_met_dir<0><<<dim3(nblk(e0, MetCfg<0>::TS), nblk(e1, MetCfg<0>::TW), e2), 256, 0, g->stream>>>(c, xc, xt, cd, met, mt);
+    k_met_dir<1><<<dim3(nblk(e0, MetCfg<1>::TW), nblk(e1, MetCfg<1>::TS), e2), 256, 0, g->stream>>>(c, xc, xt, cd, met, mt);
+    k_met_dir<2><<<dim3(nblk(e0, MetCfg<2>::TW), e1, nblk(e2, MetCfg<2>::TS)), 256, 0, g->stream>>>(c, xc, xt, cd, met, mt);
+  }
   for (int d = 0; d < 3; ++d) {
     FaceJob job;
     job.n = 0;

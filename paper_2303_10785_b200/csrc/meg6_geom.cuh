@@ -130,7 +130,7 @@ __device__ __forceinline__ double delta_op(const double* __restrict__ f, long lo
 }
 
 // M2: cd[3*comp + d] = delta_d(x_comp) wherever the 11-point stencil fits inside the padded box.
-__global__ void k_coord_deriv(Consts c, P3 xc, P9 cd) {
+__global__ void k_coord_deriv(Consts c, P3 xc, P9 cd, double* __restrict__ rj) {
   const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (tid >= c.LX.n) return;
   const int pi = (int)(tid % c.LX.pi);
@@ -139,67 +139,102 @@ __global__ void k_coord_deriv(Consts c, P3 xc, P9 cd) {
   const int pos[3] = {pi, pj, pk};
   const int ext[3] = {c.n[0] + 2 * GX, c.n[1] + 2 * GX, c.n[2] + 2 * GX};
   if (pi >= ext[0]) return;
+  double v[9];
+  bool all = true;
 #pragma unroll
   for (int d = 0; d < 3; ++d) {
-    if (pos[d] < 5 || pos[d] >= ext[d] - 5) continue;
+    if (pos[d] < 5 || pos[d] >= ext[d] - 5) { all = false; continue; }
     const long long s = c.LX.stride(d);
 #pragma unroll
-    for (int comp = 0; comp < 3; ++comp) cd.p[3 * comp + d][tid] = delta_op(xc.p[comp] + tid, s);
-  }
-}
-
-// delta along the direction with stride s of the (rounded) product a*b
-__device__ __forceinline__ double delta_prod(const double* __restrict__ a, const double* __restrict__ b, long long s) {
-  double v[11];
-#pragma unroll
-  for (int m = 0; m < 11; ++m) v[m] = a[(m - 5) * s] * b[(m - 5) * s];
-  return delta_vals(v);
-}
-
-// M3: Thomas-Lombard conservative metrics Eq. 10, 1/J Eq. 13, hatted time metrics
-// Eq. 11, on cells [-5, n+5)^3.
-// k_metrics: the row loop is kept rolled (112 registers, 4 CTAs/SM) -- fully unrolled it needs 224 registers and is
-// 25 % slower on a 256^3 moving mesh (the kernel is bound by its ~400 L1 loads per cell, i.e. by occupancy)
-#ifndef MEG6_KM_MINB
-#define MEG6_KM_MINB 4
-#endif
-#ifndef MEG6_KM_UNROLL
-#define MEG6_KM_UNROLL 0
-#endif
-__global__ void __launch_bounds__(128, MEG6_KM_MINB) k_metrics(Consts c, P3 xc, P3 xt, P9 cd, P9 met, double* __restrict__ rj, P3 mt) {
-  const int ei = c.n[0] + 10, ej = c.n[1] + 10;
-  const long long total = (long long)ei * ej * (c.n[2] + 10);
-  const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (tid >= total) return;
-  const int i = (int)(tid % ei) - 5, j = (int)((tid / ei) % ej) - 5, k = (int)(tid / ((long long)ei * ej)) - 5;
-  const long long at = c.LX.at(i, j, k);
-  double m[9];
-#if MEG6_KM_UNROLL
-#pragma unroll
-#else
-#pragma unroll 1
-#endif
-  for (int r = 0; r < 3; ++r) {
-    const int a = (r + 1) % 3, b = (r + 2) % 3;
-    const long long sa = c.LX.stride(a), sb = c.LX.stride(b);
-#pragma unroll
-    for (int cc = 0; cc < 3; ++cc) {
-      const int q = (cc + 1) % 3, s = (cc + 2) % 3;
-      // m = delta_b( delta_a(q) * s ) - delta_a( delta_b(q) * s )
-      const double t1 = delta_prod(cd.p[3 * q + a] + at, xc.p[s] + at, sb);
-      const double t2 = delta_prod(cd.p[3 * q + b] + at, xc.p[s] + at, sa);
-      m[3 * r + cc] = t1 - t2;
-      met.p[3 * r + cc][at] = m[3 * r + cc];
+    for (int comp = 0; comp < 3; ++comp) {
+      v[3 * comp + d] = delta_op(xc.p[comp] + tid, s);
+      cd.p[3 * comp + d][tid] = v[3 * comp + d];
     }
   }
-  const double xx = cd.p[0][at], xe = cd.p[1][at], xz = cd.p[2][at];
-  const double yx = cd.p[3][at], ye = cd.p[4][at], yz = cd.p[5][at];
-  const double zx = cd.p[6][at], ze = cd.p[7][at], zz = cd.p[8][at];
-  rj[at] = xx * (ye * zz - ze * yz) - yx * (xe * zz - ze * xz) + zx * (xe * yz - ye * xz);
-  if (c.moving) {
-    const double vx = xt.p[0][at], vy = xt.p[1][at], vz = xt.p[2][at];
+  if (all) {   // 1/J = det of the coordinate derivatives, Eq. 13, on cells [-5, n+5)^3
+    const double xx = v[0], xe = v[1], xz = v[2], yx = v[3], ye = v[4], yz = v[5], zx = v[6], ze = v[7], zz = v[8];
+    rj[tid] = xx * (ye * zz - ze * yz) - yx * (xe * zz - ze * xz) + zx * (xe * yz - ye * xz);
+  }
+}
+
+// M3 (tiled): the Thomas-Lombard metrics, Eq. 10, one sweep per direction D.  Every metric is
+//     m[r][c] = delta_b( delta_a(q) s ) - delta_a( delta_b(q) s ),  (a,b) = (r+1,r+2), (q,s) = (c+1,c+2) mod 3,
+// so direction D carries six consistent derivatives: the FIRST terms of row (D+1)%3 and the SECOND terms of row
+// (D+2)%3.  A CTA forms the six products on a pencil tile (5-cell halo along D) in shared memory once, each thread
+// then differentiates them for its cell (delta_vals: the operation order of Eq. 17/19/16/36-37, bit for bit the
+// oracle's).  Sweeps run in the order D = 0, 1, 2; the second term to arrive completes the metric with the one
+// subtraction of Eq. 10 (the first to arrive is parked in the metric array itself).  The last sweep also forms the
+// hatted time metrics, Eq. 11.  (ncu r1: the one-thread-per-cell version read ~400 values per cell through
+// L1 and took 60 % of a moving-mesh RK stage.  The same tiling applied to the coordinate derivatives and the
+// interface metrics -- one array at a time through shared memory -- was measured SLOWER than their L1 versions.)
+template <int D>
+struct MetCfg {
+  static constexpr int TS = (D == 0) ? 64 : 8;     // cells along D per tile
+  static constexpr int TW = (D == 0) ? 4 : 32;     // transverse extent: rows j (D = 0) or xi lanes (D != 0)
+  static constexpr int LS = TS + 10;
+};
+
+template <int D>
+__global__ void __launch_bounds__(256) k_met_dir(Consts c, P3 xc, P3 xt, P9 cd, P9 met, P3 mt) {
+  using C = MetCfg<D>;
+  constexpr int TS = C::TS, TW = C::TW, LS = C::LS;
+  __shared__ double sp[6 * LS * TW];
+  auto sidx = [](int p, int pos, int t) { return (D == 0) ? (p * TW + t) * LS + pos : (p * LS + pos) * TW + t; };
+  // tile origin (cells); outputs cover [-5, n+5) in every direction
+  int o[3];
+  if (D == 0) { o[0] = -5 + blockIdx.x * TS; o[1] = -5 + blockIdx.y * TW; o[2] = -5 + blockIdx.z; }
+  else if (D == 1) { o[0] = -5 + blockIdx.x * TW; o[1] = -5 + blockIdx.y * TS; o[2] = -5 + blockIdx.z; }
+  else { o[0] = -5 + blockIdx.x * TW; o[1] = -5 + blockIdx.y; o[2] = -5 + blockIdx.z * TS; }
+  constexpr int TD = (D == 0) ? 1 : 0;             // the transverse direction inside the tile
+  constexpr int A_RB = (D + 2) % 3, B_RA = (D + 1) % 3;
+  const int tid = threadIdx.x;
+  // ---- the six products on the tile, positions -5 .. TS+4 along D (clamped inside the padded arrays) ----
+  for (int it = tid; it < LS * TW; it += 256) {
+    int pos, t;
+    if (D == 0) { pos = it % LS; t = it / LS; } else { t = it % TW; pos = it / TW; }
+    int ix[3] = {o[0], o[1], o[2]};
+    ix[D] = min(o[D] + pos - 5, c.n[D] + GX - 1);
+    ix[TD] = min(o[TD] + t, c.n[TD] + GX - 1);
+    const long long at = c.LX.at(ix[0], ix[1], ix[2]);
 #pragma unroll
-    for (int r = 0; r < 3; ++r) mt.p[r][at] = -(vx * m[3 * r] + vy * m[3 * r + 1] + vz * m[3 * r + 2]);
+    for (int cc = 0; cc < 3; ++cc) {
+      const int q = (cc + 1) % 3, sc = (cc + 2) % 3;
+      const double xs = xc.p[sc][at];
+      sp[sidx(cc, pos, t)] = cd.p[3 * q + A_RB][at] * xs;        // first terms of row (D+1)%3
+      sp[sidx(3 + cc, pos, t)] = cd.p[3 * q + B_RA][at] * xs;    // second terms of row (D+2)%3
+    }
+  }
+  __syncthreads();
+  int s, t;
+  if (D == 0) { s = tid % TS; t = tid / TS; } else { t = tid % TW; s = tid / TW; }
+  int ix[3] = {o[0], o[1], o[2]};
+  ix[D] += s; ix[TD] += t;
+  if (ix[0] >= c.n[0] + 5 || ix[1] >= c.n[1] + 5 || ix[2] >= c.n[2] + 5) return;
+  const long long at = c.LX.at(ix[0], ix[1], ix[2]);
+  constexpr int RB = (D + 1) % 3, RA = (D + 2) % 3;
+  constexpr int SP = (D == 0) ? 1 : TW;            // shared-memory stride along D
+  double mrb[3], mra[3];
+#pragma unroll
+  for (int cc = 0; cc < 3; ++cc) {
+    double v[11];
+#pragma unroll
+    for (int m = 0; m < 11; ++m) v[m] = sp[sidx(cc, s, t) + m * SP];
+    const double d1 = delta_vals(v);
+#pragma unroll
+    for (int m = 0; m < 11; ++m) v[m] = sp[sidx(3 + cc, s, t) + m * SP];
+    const double d2 = delta_vals(v);
+    // row RB: D is its b; its a = (D+2)%3 has already run iff a < D, i.e. D != 0
+    mrb[cc] = (D == 0) ? d1 : d1 - met.p[3 * RB + cc][at];
+    // row RA: D is its a; its b = (D+1)%3 has already run iff b < D, i.e. D == 2
+    mra[cc] = (D == 2) ? met.p[3 * RA + cc][at] - d2 : d2;
+    met.p[3 * RB + cc][at] = mrb[cc];
+    met.p[3 * RA + cc][at] = mra[cc];
+  }
+  if (D == 2 && c.moving) {   // rows 0 (= RB) and 1 (= RA) are final here, row 2 was finished by the eta sweep
+    const double vx = xt.p[0][at], vy = xt.p[1][at], vz = xt.p[2][at];
+    mt.p[0][at] = -(vx * mrb[0] + vy * mrb[1] + vz * mrb[2]);
+    mt.p[1][at] = -(vx * mra[0] + vy * mra[1] + vz * mra[2]);
+    mt.p[2][at] = -(vx * met.p[6][at] + vy * met.p[7][at] + vz * met.p[8][at]);
   }
 }
 
