@@ -49,7 +49,11 @@ typedef struct {
   double omega;
   int bc[6];          /* faces imin,imax,jmin,jmax,kmin,kmax of non-periodic directions:
                          1 fixed inflow (ghost = 2 P_in - P_mirror), 2 outflow (ghost = last interior cell,
-                         p = p_out where the outward normal Mach number < 1)   (Table 1, R20) */
+                         p = p_out where the outward normal Mach number < 1)   (Table 1, R20),
+                         3 inviscid wall (ghost layer q = rho, p of the q-th interior cell, its velocity reflected
+                         about the unit vector of that cell's own hatted metrics of the direction: u - 2 V k~),
+                         4 adiabatic no-slip wall (rho, p mirrored, velocity negated)   (Table 1, R27);
+                         walls need moving == 0 (MEG6_EINVAL otherwise)                                  */
   double p_out;
 } meg6_params;
 

@@ -15,6 +15,7 @@
  *   - eigenvector averaging state (R5), MP alpha value (R7), tangential viscous gradients (R11),
  *     un-hatted interface metrics (R12), Sutherland constants (R15), sponge form (R16),
  *     per-stage metric recompute (R17), inflow/outflow ghost rules (R20), CFL viscous alpha (R25),
+ *     the cell whose metrics give the wall normal of the inviscid-wall rule (R27),
  *     where the IG4 line systems of the MIG4 variant end and how they are closed (R26):
  *     parity unpinned.
  *   - everything else is pinned by tests/test_oracle_*.py (-m "not gpu").
@@ -290,6 +291,8 @@ int meg6o_get_threads(void) { return g_threads; }
 
 meg6o_grid* meg6o_create(const meg6o_params* p, const double* x, const double* y, const double* z,
                          const double* dxm, const double* dym, const double* dzm) {
+  for (int f = 0; f < 6; ++f)   /* Table 1 gives the wall rules without a wall velocity: static meshes only (R27) */
+    if (p->moving && !p->periodic[f / 2] && (p->bc[f] == 3 || p->bc[f] == 4)) return nullptr;
   meg6o_grid* G = new meg6o_grid();
   G->p = *p;
   G->n[0] = p->ni; G->n[1] = p->nj; G->n[2] = p->nk;
@@ -680,6 +683,28 @@ void fill_primitives(meg6o_grid* G, const double* U) {
             for (int q = 1; q <= GP; ++q)
               for (int f = 0; f < 5; ++f)
                 at(f, last + sg * q) = 2.0 * pin[f * nf + (size_t)cb * n1 + ca] - at(f, last - sg * (q - 1));
+          } else if (bc == 3 || bc == 4) {
+            /* walls, Table 1, R27: ghost layer q takes rho and p of its mirror cell m (the q-th interior
+             * cell counted from the face).  Inviscid wall (bc 3): u_ghost = u_m - (2 V ktilde_x)_m and likewise v, w,
+             * V = u ktilde_x + v ktilde_y + w ktilde_z, ktilde = the unit vector along the hatted metrics of this
+             * direction at cell m (static meshes only: no time metric in V).  Adiabatic wall (bc 4): velocity negated. */
+            for (int q = 1; q <= GP; ++q) {
+              const int m = last - sg * (q - 1);
+              double pv[5];
+              for (int f = 0; f < 5; ++f) pv[f] = at(f, m);
+              if (bc == 3) {
+                int im[3]; im[a] = ca; im[b] = cb; im[d] = m;
+                const double mx = G->met[3 * d](im[0], im[1], im[2]), my = G->met[3 * d + 1](im[0], im[1], im[2]),
+                             mz = G->met[3 * d + 2](im[0], im[1], im[2]);
+                const double gm = std::sqrt(mx * mx + my * my + mz * mz);
+                const double kx = mx / gm, ky = my / gm, kz = mz / gm;
+                const double V = pv[1] * kx + pv[2] * ky + pv[3] * kz;
+                pv[1] = pv[1] - 2.0 * V * kx; pv[2] = pv[2] - 2.0 * V * ky; pv[3] = pv[3] - 2.0 * V * kz;
+              } else {
+                pv[1] = -pv[1]; pv[2] = -pv[2]; pv[3] = -pv[3];
+              }
+              for (int f = 0; f < 5; ++f) at(f, last + sg * q) = pv[f];
+            }
           } else {
             /* outflow, Table 1, R20: copy of the last interior cell; p = p_out where the outward
              * normal Mach number of that cell is below one */

@@ -30,7 +30,7 @@ typedef struct {
   double mp_alpha;          /* MP limiter alpha (App. E), default 4                             */
   int moving;               /* 1: x(t) = x0 + sin(2 pi omega t) dx_mode                         */
   double omega;
-  int bc[6];                /* faces imin,imax,jmin,jmax,kmin,kmax: 0 periodic, 1 inflow, 2 outflow */
+  int bc[6];                /* faces imin,imax,jmin,jmax,kmin,kmax: 0 periodic, 1 inflow, 2 outflow, 3 inviscid wall, 4 adiabatic wall */
   double p_out;             /* outflow reference pressure                                       */
   int metric_form;          /* ORACLE ONLY: 0 = conservative Eq. 10 + consistent delta/H (Sec. 7),
                                1 = non-conservative App. D (negative control for freestream)    */

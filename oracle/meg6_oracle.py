@@ -139,6 +139,8 @@ class Grid:
             self.h = L.meg6o_create(C.byref(self.p), _p(x), _p(y), _p(z), _p(m[0]), _p(m[1]), _p(m[2]))
         else:
             self.h = L.meg6o_create(C.byref(self.p), _p(x), _p(y), _p(z), None, None, None)
+        if not self.h:
+            raise ValueError("meg6o_create rejected the parameters (walls need a static mesh)")
         for face, pin in wl.get("inflow", {}).items():
             pin = _c(pin)
             L.meg6o_set_inflow(self.h, int(face), _p(pin))

@@ -32,7 +32,11 @@ static bool params_ok(const meg6_params* p) {
   for (int d = 0; d < 3; ++d)
     if (!p->periodic[d])
       for (int s = 0; s < 2; ++s)
-        if (p->bc[2 * d + s] != 1 && p->bc[2 * d + s] != 2) return false;
+      {
+        const int bc = p->bc[2 * d + s];
+        if (bc < 1 || bc > 4) return false;
+        if (bc >= 3 && p->moving) return false;   // Table 1 gives the wall rules without a wall velocity (R27)
+      }
   if (p->viscous && !(p->prandtl > 0.0)) return false;
   return true;
 }

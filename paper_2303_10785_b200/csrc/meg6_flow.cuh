@@ -71,6 +71,29 @@ __global__ void __launch_bounds__(256) k_ghost(Consts c, int d, P6 P, GhostIn in
 #pragma unroll
     for (int f = 0; f < 5; ++f) P.p[f][dst] = v[f];
     P.p[5][dst] = v[4] / (v[0] * c.r_gas);
+  } else if (bc == 3 || bc == 4) {
+    // walls (Table 1, R27): rho and p of the mirror cell m; inviscid wall: velocity minus twice its
+    // component along the unit vector of m's own hatted metrics of this direction; adiabatic wall: velocity negated
+    const int m = last - sg * (q - 1);
+    const long long mir = base + (long long)m * s;
+    double pv[5];
+#pragma unroll
+    for (int f = 0; f < 5; ++f) pv[f] = P.p[f][mir];
+    if (bc == 3) {
+      int im[3];
+      im[a] = ca; im[b] = cb; im[d] = m;
+      const long long am = c.LX.at(im[0], im[1], im[2]);
+      const double mx = in.mx[am], my = in.my[am], mz = in.mz[am];
+      const double gm = sqrt(mx * mx + my * my + mz * mz);
+      const double kx = mx / gm, ky = my / gm, kz = mz / gm;
+      const double V = pv[1] * kx + pv[2] * ky + pv[3] * kz;
+      pv[1] = pv[1] - 2.0 * V * kx; pv[2] = pv[2] - 2.0 * V * ky; pv[3] = pv[3] - 2.0 * V * kz;
+    } else {
+      pv[1] = -pv[1]; pv[2] = -pv[2]; pv[3] = -pv[3];
+    }
+#pragma unroll
+    for (int f = 0; f < 5; ++f) P.p[f][dst] = pv[f];
+    P.p[5][dst] = pv[4] / (pv[0] * c.r_gas);
   } else {
     double pv[5];
 #pragma unroll

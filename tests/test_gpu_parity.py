@@ -469,3 +469,59 @@ def test_abi_error_paths_on_device(mods):
     assert bool(torch.isfinite(out).all())
     L.meg6_grid_destroy(h)
     L.meg6_grid_create.argtypes = saved
+
+
+# ------------------------------------------------------------------ walls (Table 1, R27)
+def wall_cases():
+    return {
+        "channel_inviscid_wall": W.wall_channel(ni=37, nj=21, nk=26, wall=3, viscous=0, curved=True),
+        "channel_slip_viscous": W.wall_channel(ni=24, nj=33, nk=20, wall=3, viscous=1, curved=True),
+        "channel_adiabatic": W.wall_channel(ni=37, nj=21, nk=26, wall=4, viscous=1, curved=True),
+        "box_mixed_walls": W.wall_box(),
+        "box_mixed_walls_mig4": W.wall_box(ni=20, nj=23, nk=18, scheme=1),
+        "channel_adiabatic_mig4": W.wall_channel(ni=24, nj=18, nk=20, wall=4, viscous=1, curved=True, scheme=1),
+    }
+
+
+@pytest.mark.parametrize("name", list(wall_cases()))
+def test_wall_ghosts_rhs_and_steps_parity(mods, name):
+    """Inviscid and adiabatic no-slip walls (bc 3 / 4): ghost primitives, one dQ/dt and three RK3 steps against the
+    oracle; curved walls, ragged sizes, edges and corners of a closed box with walls of both kinds, MEG6 and MIG4."""
+    torch, O, M = mods
+    wl = wall_cases()[name]
+    og = O.Grid(wl)
+    og.metrics_compute(0.0)
+    ref = og.rhs(wl["U0"])
+    g = M.Grid(wl)
+    g.metrics_compute(0.0)
+    g.limiter_stats_enable(True)
+    U = torch.as_tensor(wl["U0"], device="cuda").contiguous()
+    out = g.rhs(U).cpu().numpy()
+    for f in range(6):
+        a, b = g.get_array(2, f), og.prim(f)
+        assert np.abs(a - b).max() <= 1e-14 * np.abs(b).max()
+    e = rhs_err(out, ref, wl["U0"])
+    assert np.all(e <= RHS_TOL), (name, e, rel(out, ref))
+    lim_o, tst_o = og.limiter_stats()
+    lim_g, tst_g = g.limiter_stats()
+    assert tst_g == tst_o
+    assert abs(lim_g - lim_o) <= max(5, 1e-3 * lim_o), (lim_g, lim_o)
+    dt = og.cfl_dt(wl["U0"], wl["cfl"])
+    assert g.cfl_dt(U, wl["cfl"]) == pytest.approx(dt, rel=1e-12)
+    Uo = wl["U0"].copy()
+    t = 0.0
+    for s in range(3):
+        og.rk3_step(Uo, t, dt)
+        g.rk3_step(U, t, dt)
+        t += dt
+    e = rel(U.cpu().numpy(), Uo)
+    assert np.all(e <= STEP_TOL), (name, e)
+    g.close()
+
+
+def test_walls_on_a_moving_mesh_are_einval(mods):
+    torch, O, M = mods
+    wl = W.c2_dynamic_freestream(n=12, steps=1)
+    wl["params"] = dict(wl["params"], periodic=[1, 0, 1], bc=[0, 0, 4, 4, 0, 0])
+    with pytest.raises(Exception):
+        M.Grid(wl)

@@ -253,3 +253,58 @@ def c4_jet(ni=320, nj=200, nk=200, steps=500, seed=135, re=1.0e4):
 
 def c5_tgv_mig4(n=384, steps=50):
     return c3_tgv(n=n, steps=steps, scheme=1)
+
+
+# --------------------------------------------------------------------------------------------------
+# Walls (Table 1).  Synthetic channel / closed-box inputs; no paper grid is reproduced.
+def _smooth_state(xc, yc, zc, L, seed, mach=0.3, amp=0.05, gamma=GAMMA):
+    """(rho,u,v,w,p): Mach `mach` stream along x plus seeded smooth perturbations of every primitive variable."""
+    rng = np.random.default_rng(seed)
+    ph = rng.uniform(0.0, 2.0 * np.pi, size=(5, 3))
+    kx, ky, kz = 2.0 * np.pi / L[0], 2.0 * np.pi / L[1], 2.0 * np.pi / L[2]
+    f = lambda q: np.sin(kx * xc + ph[q, 0]) * np.cos(ky * yc + ph[q, 1]) * np.sin(kz * zc + ph[q, 2])
+    a0 = 1.0
+    rho = 1.0 + amp * f(0)
+    u = mach * a0 * (1.0 + 2.0 * amp * f(1))
+    v = mach * a0 * 2.0 * amp * f(2)
+    w = mach * a0 * 2.0 * amp * f(3)
+    p = (1.0 / gamma) * (1.0 + amp * f(4))
+    return rho, u, v, w, p
+
+
+def wall_channel(ni=24, nj=16, nk=20, wall=3, viscous=0, scheme=0, seed=4242, curved=True, amp=0.05):
+    """Channel between two eta walls (bc 3 inviscid / 4 adiabatic no-slip), periodic in xi and zeta.
+    curved=False: y = eta with spacing 2/nj (a power of two for nj = 16, 32), x and z wavy in (xi, zeta) only --
+    the mesh of the reflection-principle pin; curved=True: the walls themselves are wavy (non-trivial normals)."""
+    L = (4.0, 2.0, 3.0)
+    X, E, Z = _comp_coords((ni, nj, nk), L)
+    s = lambda a, l: np.sin(2.0 * np.pi * a / l)
+    x = X + 0.08 * s(Z, L[2])
+    z = Z + 0.06 * s(X, L[0])
+    y = E + (0.05 * s(X, L[0]) * np.cos(2.0 * np.pi * Z / L[2]) * (1.0 + 0.5 * E) if curved else 0.0)
+    x, y, z = (np.ascontiguousarray(a) for a in (x, y, z))
+    rho, u, v, w, p = _smooth_state(cell_centres(x), cell_centres(y), cell_centres(z), L, seed, amp=amp)
+    prm = _base_params(ni, nj, nk, periodic=[1, 0, 1], period=[[L[0], 0, 0], [0, 0, 0], [0, 0, L[2]]], scheme=scheme,
+                       viscous=viscous, bc=[0, 0, wall, wall, 0, 0], p_out=1.0 / GAMMA)
+    if viscous:
+        prm.update(mu_ref=0.3 * 1.0 / 200.0, t_ref=1.0 / GAMMA, s_suth=0.4 / GAMMA)   # Re ~ 200 on the unit length
+    return dict(name="wall_channel_%dx%dx%d_bc%d%s" % (ni, nj, nk, wall, "" if curved else "_flat"), params=prm,
+                x=x, y=y, z=z, U0=conservative(rho, u, v, w, p), dt=None, cfl=0.4, steps=3, t0=0.0)
+
+
+def wall_box(ni=22, nj=19, nk=17, bc=(3, 4, 3, 3, 4, 3), viscous=1, scheme=0, seed=515):
+    """Closed box, walls of mixed kind on all six faces of a smoothly distorted non-periodic mesh (edges and
+    corners: ghost cells of ghost cells)."""
+    L = (2.0, 1.5, 1.0)
+    X, E, Z = _comp_coords((ni, nj, nk), L)
+    s = lambda a, l: np.sin(2.0 * np.pi * a / l)
+    x = X + 0.04 * s(E, L[1]) * s(Z, L[2])
+    y = E + 0.03 * s(Z, L[2]) * s(X, L[0])
+    z = Z + 0.02 * s(X, L[0]) * s(E, L[1])
+    x, y, z = (np.ascontiguousarray(a) for a in (x, y, z))
+    rho, u, v, w, p = _smooth_state(cell_centres(x), cell_centres(y), cell_centres(z), L, seed)
+    prm = _base_params(ni, nj, nk, periodic=[0, 0, 0], scheme=scheme, viscous=viscous, bc=list(bc), p_out=1.0 / GAMMA)
+    if viscous:
+        prm.update(mu_ref=0.3 * 1.0 / 200.0, t_ref=1.0 / GAMMA, s_suth=0.4 / GAMMA)
+    return dict(name="wall_box_%dx%dx%d" % (ni, nj, nk), params=prm, x=x, y=y, z=z,
+                U0=conservative(rho, u, v, w, p), dt=None, cfl=0.4, steps=3, t0=0.0)
