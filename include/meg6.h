@@ -52,7 +52,8 @@ typedef struct {
                          p = p_out where the outward normal Mach number < 1)   (Table 1, R20),
                          3 inviscid wall (ghost layer q = rho, p of the q-th interior cell, its velocity reflected
                          about the unit vector of that cell's own hatted metrics of the direction: u - 2 V k~),
-                         4 adiabatic no-slip wall (rho, p mirrored, velocity negated)   (Table 1, R27);
+                         4 adiabatic no-slip wall (rho, p mirrored, velocity negated)   (Table 1, R27),
+                         5 block interface (ghost = neighbour block's interior, meg6_link_blocks; R28);
                          walls need moving == 0 (MEG6_EINVAL otherwise)                                  */
   double p_out;
 } meg6_params;
@@ -93,6 +94,22 @@ meg6_status meg6_rhs(meg6_grid* g, const double* U, double* dUdt);
  * geometry at the stage times t, t+dt, t+dt/2 (R17) and leave it at t+dt/2.  U is read and written by the last
  * sweep of every stage; it must not be touched by other streams while the step is in flight. */
 meg6_status meg6_rk3_step(meg6_grid* g, double* U, double t, double dt);
+
+/* Multi-block (Sec. 6; Table 1 last column P:354-362; reading R28).  A face with bc == 5 is a block
+ * interface: its six ghost layers of primitives are copies of the interior cells of the neighbour block next to the
+ * neighbour's OPPOSITE face (face ^ 1), same transverse indices -- aligned blocks: the three computational axes of
+ * the two blocks point the same way and the transverse cell counts and periodicity agree (MEG6_EINVAL otherwise).
+ * Geometry is per block (ghost coordinates by R13, as at every non-periodic face; the paper: "metric terms are
+ * non-existent" in ghost cells).  A block may be linked to itself (wrap-around).  Both grids must use one
+ * stream; the link is a pointer: the neighbour must outlive the home grid's last call.
+ * meg6_rhs_blocks / meg6_rk3_step_blocks advance n blocks together: primitives of all blocks, then the ghost
+ * exchange direction by direction over all blocks (edge and corner ghosts come from diagonal neighbours in two
+ * steps), then the sweeps of each block; per block the semantics of meg6_rhs / meg6_rk3_step.  g, U, dUdt: HOST
+ * arrays of n pointers (grids; DEVICE state arrays).  Every neighbour of a listed block must be listed.  The
+ * single-grid calls return MEG6_ESTATE on a grid that has an interface to another block or an unlinked one. */
+meg6_status meg6_link_blocks(meg6_grid* home, int face, meg6_grid* neighbour);
+meg6_status meg6_rhs_blocks(int n, meg6_grid* const* g, const double* const* U, double* const* dUdt);
+meg6_status meg6_rk3_step_blocks(int n, meg6_grid* const* g, double* const* U, double t, double dt);
 
 /* Eq. B.2 / B.3 time step for the state U at the geometry of the last metrics_compute.
  * Synchronises the stream.  *dt is a HOST pointer. */

@@ -16,6 +16,7 @@
  *     un-hatted interface metrics (R12), Sutherland constants (R15), sponge form (R16),
  *     per-stage metric recompute (R17), inflow/outflow ghost rules (R20), CFL viscous alpha (R25),
  *     the cell whose metrics give the wall normal of the inviscid-wall rule (R27),
+ *     (block interfaces, R28, are pinned: cut domain == uncut domain on Cartesian meshes)
  *     where the IG4 line systems of the MIG4 variant end and how they are closed (R26):
  *     parity unpinned.
  *   - everything else is pinned by tests/test_oracle_*.py (-m "not gpu").
@@ -231,6 +232,7 @@ struct meg6o_grid {
   std::vector<double> inflow[6];
   std::vector<double> sigma, uref;
   unsigned long long n_limited = 0, n_tested = 0;
+  meg6o_grid* link[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};   /* bc 5: neighbour block per face */
 };
 
 namespace {
@@ -640,7 +642,7 @@ void meg6o_viscous_face(int d, const double phi[2][4], const double g[2][3][4], 
 /* ----------------------------------- O2 primitives + ghosts -------------------------------- */
 namespace {
 
-void fill_primitives(meg6o_grid* G, const double* U) {
+void prim_interior(meg6o_grid* G, const double* U) {
   const meg6o_params& p = G->p;
   const int ni = G->n[0], nj = G->n[1], nk = G->n[2];
   const size_t N = (size_t)ni * nj * nk;
@@ -655,9 +657,15 @@ void fill_primitives(meg6o_grid* G, const double* U) {
         const double pp = (p.gamma - 1.0) * (U[4 * N + c] - 0.5 * r * (u * u + v * v + w * w));
         G->P[0](i, j, k) = r; G->P[1](i, j, k) = u; G->P[2](i, j, k) = v; G->P[3](i, j, k) = w; G->P[4](i, j, k) = pp;
       }
-  /* ghost fill direction by direction: xi over interior (j,k); eta over all filled i; zeta over all (i,j) */
-  int lo[3] = {0, 0, 0}, hi[3] = {ni, nj, nk};
-  for (int d = 0; d < 3; ++d) {
+}
+
+/* ghost fill of direction d, after the lower directions: xi over interior (j,k); eta over all filled i; zeta over
+ * all (i,j).  With several blocks, direction d is filled in every block before direction d+1 in any. */
+void ghost_dir(meg6o_grid* G, int d) {
+  const meg6o_params& p = G->p;
+  int lo[3] = {0, 0, 0}, hi[3] = {G->n[0], G->n[1], G->n[2]};
+  for (int e = 0; e < d; ++e) { lo[e] = -GP; hi[e] = G->n[e] + GP; }
+  {
     const int n = G->n[d];
     int a = (d + 1) % 3, b = (d + 2) % 3;
     if (a > b) std::swap(a, b);   /* a < b: the transverse directions in storage order */
@@ -676,7 +684,16 @@ void fill_primitives(meg6o_grid* G, const double* U) {
           const int last = side ? n - 1 : 0, sg = side ? 1 : -1;
           /* transverse position clamped to the interior for the lookups of face data / metrics */
           const int ca = std::min(std::max(ta, 0), G->n[a] - 1), cb = std::min(std::max(tb, 0), G->n[b] - 1);
-          if (bc == 1) {
+          if (bc == 5) {
+            /* block interface, Table 1 last column, R28: ghost layer q = the q-th interior cell of the
+             * neighbour block counted from its opposite face, same transverse index (aligned blocks) */
+            const meg6o_grid* nb = G->link[face];
+            const int nn = nb->n[d];
+            for (int q = 1; q <= GP; ++q) {
+              int is[3]; is[a] = ta; is[b] = tb; is[d] = side ? q - 1 : nn - q;
+              for (int f = 0; f < 5; ++f) at(f, last + sg * q) = nb->P[f](is[0], is[1], is[2]);
+            }
+          } else if (bc == 1) {
             /* fixed inflow, Table 1, R20: ghost = 2 P_in - P_mirror */
             const size_t n1 = G->n[a], nf = (size_t)G->n[a] * G->n[b];
             const double* pin = G->inflow[face].data();
@@ -722,23 +739,48 @@ void fill_primitives(meg6o_grid* G, const double* U) {
           }
         }
       }
-    lo[d] = -GP; hi[d] = n + GP;
   }
+}
+
+void finish_primitives(meg6o_grid* G) {
+  const meg6o_params& p = G->p;
   for (int f = 0; f < 5; ++f) G->P[f].valid_all();
   /* T = p / (rho R) everywhere, ghosts included (R18) */
   G->P[5].valid_all();
   for (size_t q = 0; q < G->P[5].d.size(); ++q) G->P[5].d[q] = G->P[4].d[q] / (G->P[0].d[q] * p.r_gas);
 }
 
+void fill_primitives(meg6o_grid* G, const double* U) {   /* single block */
+  prim_interior(G, U);
+  for (int d = 0; d < 3; ++d) ghost_dir(G, d);
+  finish_primitives(G);
+}
+
+void rhs_from_primitives(meg6o_grid* G, const double* U, double* dUdt);
+
 }  // namespace
 
 /* --------------------------------------- O2-O5 RHS ---------------------------------------- */
-void meg6o_rhs(meg6o_grid* G, const double* U, double* dUdt) {
+void meg6o_rhs_blocks(int nb, meg6o_grid* const* G, const double* const* U, double* const* dUdt) {
+  for (int b = 0; b < nb; ++b) {
+    if (!G[b]->have_metrics) { fprintf(stderr, "meg6o_rhs before metrics_compute\n"); abort(); }
+    for (int f = 0; f < 6; ++f)
+      if (!G[b]->p.periodic[f / 2] && G[b]->p.bc[f] == 5 && !G[b]->link[f]) { fprintf(stderr, "meg6o_rhs: unlinked block interface\n"); abort(); }
+    prim_interior(G[b], U[b]);
+  }
+  for (int d = 0; d < 3; ++d)
+    for (int b = 0; b < nb; ++b) ghost_dir(G[b], d);
+  for (int b = 0; b < nb; ++b) finish_primitives(G[b]);
+  for (int b = 0; b < nb; ++b) rhs_from_primitives(G[b], U[b], dUdt[b]);
+}
+
+void meg6o_rhs(meg6o_grid* G, const double* U, double* dUdt) { meg6o_rhs_blocks(1, &G, &U, &dUdt); }
+
+namespace {
+void rhs_from_primitives(meg6o_grid* G, const double* U, double* dUdt) {
   const meg6o_params& p = G->p;
   const int ni = G->n[0], nj = G->n[1], nk = G->n[2];
   const size_t N = (size_t)ni * nj * nk;
-  if (!G->have_metrics) { fprintf(stderr, "meg6o_rhs before metrics_compute\n"); abort(); }
-  fill_primitives(G, U);
   /* O2: first gradients of rho,u,v,w,p (and T if viscous) along the three directions, Eq. 17 */
   const int nf = p.viscous ? 6 : 5;
   for (int d = 0; d < 3; ++d)
@@ -852,21 +894,49 @@ void meg6o_rhs(meg6o_grid* G, const double* U, double* dUdt) {
         }
       }
 }
+}  // namespace
 
 /* O6: SSP/TVD-RK3, Eq. B.1; stage times t, t+dt, t+dt/2; moving meshes recompute the
  * geometry at each stage time (R17). */
-void meg6o_rk3_step(meg6o_grid* G, double* U, double t, double dt) {
-  const size_t M = (size_t)5 * G->n[0] * G->n[1] * G->n[2];
-  std::vector<double> U0(U, U + M), L(M);
-  if (G->p.moving) meg6o_metrics_compute(G, t);
-  meg6o_rhs(G, U, L.data());
-  for (size_t q = 0; q < M; ++q) U[q] = U0[q] + dt * L[q];
-  if (G->p.moving) meg6o_metrics_compute(G, t + dt);
-  meg6o_rhs(G, U, L.data());
-  for (size_t q = 0; q < M; ++q) U[q] = 3.0 / 4.0 * U0[q] + 1.0 / 4.0 * (U[q] + dt * L[q]);
-  if (G->p.moving) meg6o_metrics_compute(G, t + 0.5 * dt);
-  meg6o_rhs(G, U, L.data());
-  for (size_t q = 0; q < M; ++q) U[q] = 1.0 / 3.0 * U0[q] + 2.0 / 3.0 * (U[q] + dt * L[q]);
+void meg6o_rk3_step_blocks(int nb, meg6o_grid* const* G, double* const* U, double t, double dt) {
+  std::vector<std::vector<double>> U0(nb), L(nb);
+  std::vector<double*> Lp(nb);
+  std::vector<const double*> Uc(nb);
+  for (int b = 0; b < nb; ++b) {
+    const size_t M = (size_t)5 * G[b]->n[0] * G[b]->n[1] * G[b]->n[2];
+    U0[b].assign(U[b], U[b] + M); L[b].resize(M); Lp[b] = L[b].data(); Uc[b] = U[b];
+  }
+  const double ts[3] = {t, t + dt, t + 0.5 * dt};
+  for (int s = 0; s < 3; ++s) {
+    for (int b = 0; b < nb; ++b)
+      if (G[b]->p.moving) meg6o_metrics_compute(G[b], ts[s]);
+    meg6o_rhs_blocks(nb, G, Uc.data(), Lp.data());
+    for (int b = 0; b < nb; ++b) {
+      double* u = U[b];
+      const double* u0 = U0[b].data();
+      const double* l = L[b].data();
+      const size_t M = U0[b].size();
+      if (s == 0) for (size_t q = 0; q < M; ++q) u[q] = u0[q] + dt * l[q];
+      else if (s == 1) for (size_t q = 0; q < M; ++q) u[q] = 3.0 / 4.0 * u0[q] + 1.0 / 4.0 * (u[q] + dt * l[q]);
+      else for (size_t q = 0; q < M; ++q) u[q] = 1.0 / 3.0 * u0[q] + 2.0 / 3.0 * (u[q] + dt * l[q]);
+    }
+  }
+}
+
+void meg6o_rk3_step(meg6o_grid* G, double* U, double t, double dt) { meg6o_rk3_step_blocks(1, &G, &U, t, dt); }
+
+/* Block interface (Sec. 6; Table 1 last column): face `face` of `home` (bc 5) takes its ghost primitives
+ * from the interior cells of `nb` next to nb's opposite face.  Aligned blocks only (same orientation of the three
+ * computational axes, equal transverse cell counts): R28.  Returns 0 on success. */
+int meg6o_link_blocks(meg6o_grid* home, int face, meg6o_grid* nb) {
+  if (!home || !nb || face < 0 || face > 5) return 1;
+  const int d = face / 2;
+  if (home->p.periodic[d] || home->p.bc[face] != 5) return 1;
+  if (nb->p.periodic[d] || nb->n[d] < GP) return 1;
+  for (int e = 0; e < 3; ++e)
+    if (e != d && (nb->n[e] != home->n[e] || nb->p.periodic[e] != home->p.periodic[e])) return 1;
+  home->link[face] = nb;
+  return 0;
 }
 
 /* Eq. B.2 / B.3: un-hatted metrics = hatted * J; viscous alpha read as alpha^D = 4 (R25) */

@@ -30,7 +30,7 @@ typedef struct {
   double mp_alpha;          /* MP limiter alpha (App. E), default 4                             */
   int moving;               /* 1: x(t) = x0 + sin(2 pi omega t) dx_mode                         */
   double omega;
-  int bc[6];                /* faces imin,imax,jmin,jmax,kmin,kmax: 0 periodic, 1 inflow, 2 outflow, 3 inviscid wall, 4 adiabatic wall */
+  int bc[6];                /* faces imin,imax,jmin,jmax,kmin,kmax: 0 periodic, 1 inflow, 2 outflow, 3 inviscid wall, 4 adiabatic wall, 5 block interface */
   double p_out;             /* outflow reference pressure                                       */
   int metric_form;          /* ORACLE ONLY: 0 = conservative Eq. 10 + consistent delta/H (Sec. 7),
                                1 = non-conservative App. D (negative control for freestream)    */
@@ -49,6 +49,12 @@ void meg6o_set_inflow(meg6o_grid* g, int face, const double* P_in);   /* [5][n2]
 void meg6o_set_sponge(meg6o_grid* g, const double* sigma, const double* U_ref);
 void meg6o_rhs(meg6o_grid* g, const double* U, double* dUdt);
 void meg6o_rk3_step(meg6o_grid* g, double* U, double t, double dt);
+/* Multi-block (Sec. 6; Table 1 last column; R28): face `face` (bc 5) of `home` takes its ghost primitives
+ * from the interior cells of `nb` next to nb's opposite face; aligned blocks, equal transverse sizes.  Returns 0 if ok.
+ * The *_blocks calls advance all blocks together (ghost exchange before every right-hand side). */
+int meg6o_link_blocks(meg6o_grid* home, int face, meg6o_grid* nb);
+void meg6o_rhs_blocks(int nb, meg6o_grid* const* g, const double* const* U, double* const* dUdt);
+void meg6o_rk3_step_blocks(int nb, meg6o_grid* const* g, double* const* U, double t, double dt);
 double meg6o_cfl_dt(meg6o_grid* g, const double* U, double cfl);
 /* volume-averaged kinetic energy, enstrophy (Eq. 54, in 3-D with dV = 1/J) and the volume: out[3] */
 void meg6o_diagnostics(meg6o_grid* g, const double* U, double* out);

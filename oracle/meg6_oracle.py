@@ -61,6 +61,10 @@ def lib():
         L.meg6o_set_sponge.argtypes = [C.c_void_p, _dp, _dp]
         L.meg6o_rhs.argtypes = [C.c_void_p, _dp, _dp]
         L.meg6o_rk3_step.argtypes = [C.c_void_p, _dp, C.c_double, C.c_double]
+        L.meg6o_link_blocks.restype = C.c_int
+        L.meg6o_link_blocks.argtypes = [C.c_void_p, C.c_int, C.c_void_p]
+        L.meg6o_rhs_blocks.argtypes = [C.c_int, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p), C.POINTER(C.c_void_p)]
+        L.meg6o_rk3_step_blocks.argtypes = [C.c_int, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p), C.c_double, C.c_double]
         L.meg6o_cfl_dt.restype = C.c_double
         L.meg6o_cfl_dt.argtypes = [C.c_void_p, _dp, C.c_double]
         L.meg6o_diagnostics.argtypes = [C.c_void_p, _dp, _dp]
@@ -172,6 +176,11 @@ class Grid:
         assert U.flags.c_contiguous and U.dtype == np.float64
         lib().meg6o_rk3_step(self.h, _p(U), float(t), float(dt))
 
+    def link(self, face, neighbour):
+        if lib().meg6o_link_blocks(self.h, int(face), neighbour.h) != 0:
+            raise ValueError("meg6o_link_blocks rejected the pair")
+        self._links = getattr(self, "_links", []) + [neighbour]
+
     def diagnostics(self, U):
         """(kinetic energy, enstrophy, volume), Eq. 54"""
         U = _c(U)
@@ -209,6 +218,27 @@ class Grid:
         out = np.empty(self.shape)
         lib().meg6o_get_grad(self.h, d, f, _p(out))
         return out
+
+
+def _vps(ptrs):
+    return (C.c_void_p * len(ptrs))(*ptrs)
+
+
+def rhs_blocks(grids, Us):
+    """dQ/dt of several linked blocks (meg6o_rhs_blocks)"""
+    Us = [_c(U) for U in Us]
+    outs = [np.empty_like(U) for U in Us]
+    lib().meg6o_rhs_blocks(len(grids), _vps([g.h for g in grids]), _vps([U.ctypes.data for U in Us]),
+                           _vps([o.ctypes.data for o in outs]))
+    return outs
+
+
+def rk3_step_blocks(grids, Us, t, dt):
+    """in place; every U must be a contiguous float64 array"""
+    for U in Us:
+        assert U.flags["C_CONTIGUOUS"] and U.dtype == np.float64
+    lib().meg6o_rk3_step_blocks(len(grids), _vps([g.h for g in grids]), _vps([U.ctypes.data for U in Us]),
+                                float(t), float(dt))
 
 
 # ---- fine-grained pieces ----

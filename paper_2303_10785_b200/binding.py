@@ -11,7 +11,7 @@ EXPORTS = ["meg6_workspace_bytes", "meg6_grid_create", "meg6_grid_destroy", "meg
            "meg6_set_inflow", "meg6_set_sponge", "meg6_rhs", "meg6_rk3_step", "meg6_cfl_dt", "meg6_diagnostics",
            "meg6_limiter_stats_enable", "meg6_limiter_stats", "meg6_get_array", "meg6_profile_enable",
            "meg6_profile_read", "meg6_last_error",
-           "meg6_version"]
+           "meg6_version", "meg6_link_blocks", "meg6_rhs_blocks", "meg6_rk3_step_blocks"]
 
 
 class Meg6Error(RuntimeError):
@@ -95,6 +95,12 @@ def lib():
         L.meg6_profile_enable.argtypes = [_vp, C.c_int]
         L.meg6_profile_read.restype = C.c_int
         L.meg6_profile_read.argtypes = [_vp, C.POINTER(C.c_double), C.POINTER(C.c_ulonglong)]
+        L.meg6_link_blocks.restype = C.c_int
+        L.meg6_link_blocks.argtypes = [_vp, C.c_int, _vp]
+        L.meg6_rhs_blocks.restype = C.c_int
+        L.meg6_rhs_blocks.argtypes = [C.c_int, C.POINTER(_vp), C.POINTER(_vp), C.POINTER(_vp)]
+        L.meg6_rk3_step_blocks.restype = C.c_int
+        L.meg6_rk3_step_blocks.argtypes = [C.c_int, C.POINTER(_vp), C.POINTER(_vp), C.c_double, C.c_double]
         L.meg6_last_error.restype = C.c_char_p
         L.meg6_version.restype = C.c_int
         _lib = L
@@ -175,6 +181,11 @@ class Grid:
         self._chk_state(U)
         _check(lib().meg6_rk3_step(self.h, U.data_ptr(), float(t), float(dt)), "meg6_rk3_step")
 
+    def link(self, face, neighbour):
+        """block interface (bc 5): ghost cells of `face` come from `neighbour`'s interior at its opposite face"""
+        _check(lib().meg6_link_blocks(self.h, int(face), neighbour.h), "meg6_link_blocks")
+        self._links = getattr(self, "_links", []) + [neighbour]   # keep the neighbour alive
+
     def diagnostics(self, U):
         """(kinetic energy, enstrophy, volume) of the state U, Eq. 54"""
         out = (C.c_double * 3)()
@@ -216,3 +227,28 @@ class Grid:
         out = np.empty(shp, dtype=np.float64)
         _check(lib().meg6_get_array(self.h, kind, which, out.ctypes.data), "meg6_get_array")
         return out
+
+
+def _ptr_array(ptrs):
+    return (_vp * len(ptrs))(*ptrs)
+
+
+def rhs_blocks(grids, Us, outs=None):
+    """dQ/dt of several linked blocks (meg6_rhs_blocks); returns the list of output tensors"""
+    for g, U in zip(grids, Us):
+        g._chk_state(U)
+    if outs is None:
+        outs = [g.torch.empty_like(U) for g, U in zip(grids, Us)]
+    _check(lib().meg6_rhs_blocks(len(grids), _ptr_array([g.h.value for g in grids]),
+                                 _ptr_array([U.data_ptr() for U in Us]), _ptr_array([o.data_ptr() for o in outs])),
+           "meg6_rhs_blocks")
+    return outs
+
+
+def rk3_step_blocks(grids, Us, t, dt):
+    """one SSP-RK3 step of several linked blocks, in place (meg6_rk3_step_blocks)"""
+    for g, U in zip(grids, Us):
+        g._chk_state(U)
+    _check(lib().meg6_rk3_step_blocks(len(grids), _ptr_array([g.h.value for g in grids]),
+                                      _ptr_array([U.data_ptr() for U in Us]), float(t), float(dt)),
+           "meg6_rk3_step_blocks")

@@ -34,7 +34,7 @@ static bool params_ok(const meg6_params* p) {
       for (int s = 0; s < 2; ++s)
       {
         const int bc = p->bc[2 * d + s];
-        if (bc < 1 || bc > 4) return false;
+        if (bc < 1 || bc > 5) return false;
         if (bc >= 3 && p->moving) return false;   // Table 1 gives the wall rules without a wall velocity (R27)
       }
   if (p->viscous && !(p->prandtl > 0.0)) return false;
@@ -118,6 +118,7 @@ static size_t carve(const meg6_params* p, const Consts& c, meg6_grid* g, char* b
   for (int f = 0; f < 6; ++f) {
     const int d = f / 2;
     G->inflow[f] = nullptr;
+    G->link[f] = nullptr;
     if (!p->periodic[d] && p->bc[f] == 1) {
       int a = (d + 1) % 3, b = (d + 2) % 3;
       G->inflow[f] = take(5LL * c.n[a] * c.n[b]);
@@ -370,29 +371,52 @@ meg6_status meg6_set_sponge(meg6_grid* g, const double* sigma, const double* U_r
   return MEG6_OK;
 }
 
-static void fill_ghosts(meg6_grid* g, const P6& P) {
-  const Consts& c = g->c;
-  for (int d = 0; d < 3; ++d) {
-    int a = (d + 1) % 3, b = (d + 2) % 3;
-    if (a > b) { int t = a; a = b; b = t; }
-    const long long ea = c.n[a] + ((a < d) ? 12 : 0), eb = c.n[b] + ((b < d) ? 12 : 0);
-    GhostIn gin;
-    gin.inflow[0] = g->inflow[2 * d]; gin.inflow[1] = g->inflow[2 * d + 1];
-    gin.mx = g->met[3 * d]; gin.my = g->met[3 * d + 1]; gin.mz = g->met[3 * d + 2];
-    ProfScope ps(g, 2, 1);
-    k_ghost<<<nblk(ea * eb * 12, 256), 256, 0, g->stream>>>(c, d, P, gin);
-  }
-}
-
-// One RK stage (or one dQ/dt evaluation) for the state whose primitives are in buffer `buf` (interior cells
-// filled): ghost fill, stored gradients, eta and zeta sweeps into g->res, xi sweep fused with the residual
-// assembly, the stage update and the primitive conversion of the new state (into the other buffer).
-static meg6_status stage(meg6_grid* g, int buf, const Fuse3& fu) {
+// ghost layers of direction d in primitive buffer `buf` (the lower directions are filled already).  Block interfaces
+// read the SAME buffer of the neighbour block: with several blocks, direction d is filled in every block before
+// direction d+1 in any (edge and corner ghosts then arrive from the diagonal neighbours in two steps).
+static void fill_ghosts_dir(meg6_grid* g, int buf, int d) {
   const Consts& c = g->c;
   double* const* Pc = buf ? g->Pb : g->P;
   P6 P;
   for (int f = 0; f < 6; ++f) P.p[f] = Pc[f];
-  fill_ghosts(g, P);
+  int a = (d + 1) % 3, b = (d + 2) % 3;
+  if (a > b) { int t = a; a = b; b = t; }
+  const long long ea = c.n[a] + ((a < d) ? 12 : 0), eb = c.n[b] + ((b < d) ? 12 : 0);
+  GhostIn gin;
+  memset(&gin, 0, sizeof(gin));
+  gin.inflow[0] = g->inflow[2 * d]; gin.inflow[1] = g->inflow[2 * d + 1];
+  gin.mx = g->met[3 * d]; gin.my = g->met[3 * d + 1]; gin.mz = g->met[3 * d + 2];
+  for (int side = 0; side < 2; ++side) {
+    const meg6_grid* nb = g->link[2 * d + side];
+    if (!nb) continue;
+    gin.nbP[side] = buf ? nb->Pb[0] : nb->P[0];
+    gin.nbL[side] = nb->c.LP; gin.nbfs[side] = nb->c.fsP; gin.nbn[side] = nb->c.n[d];
+  }
+  ProfScope ps(g, 2, 1);
+  k_ghost<<<nblk(ea * eb * 12, 256), 256, 0, g->stream>>>(c, d, P, gin);
+}
+
+static void fill_ghosts(meg6_grid* g, int buf) {
+  for (int d = 0; d < 3; ++d) fill_ghosts_dir(g, buf, d);
+}
+
+static bool links_ok(const meg6_grid* g, bool single) {
+  for (int f = 0; f < 6; ++f)
+    if (!g->p.periodic[f / 2] && g->p.bc[f] == 5) {
+      if (!g->link[f]) return false;
+      if (single && g->link[f] != g) return false;   // a single-grid call may only see itself across an interface
+    }
+  return true;
+}
+
+// One RK stage (or one dQ/dt evaluation) for the state whose primitives are in buffer `buf` (ghosts filled):
+// stored gradients, eta and zeta sweeps into g->res, xi sweep fused with the residual
+// assembly, the stage update and the primitive conversion of the new state (into the other buffer).
+static meg6_status stage_sweeps(meg6_grid* g, int buf, const Fuse3& fu) {
+  const Consts& c = g->c;
+  double* const* Pc = buf ? g->Pb : g->P;
+  P6 P;
+  for (int f = 0; f < 6; ++f) P.p[f] = Pc[f];
   const bool IG = g->p.scheme == 1;
   if (IG) {
     // MIG4: implicit gradients of every staged field along the three directions (Eq. 18), whole grid lines
@@ -440,6 +464,11 @@ static meg6_status stage(meg6_grid* g, int buf, const Fuse3& fu) {
   return MEG6_OK;
 }
 
+static meg6_status stage(meg6_grid* g, int buf, const Fuse3& fu) {
+  fill_ghosts(g, buf);
+  return stage_sweeps(g, buf, fu);
+}
+
 static void launch_prim(meg6_grid* g, const double* U) {
   P6 P;
   for (int f = 0; f < 6; ++f) P.p[f] = g->P[f];
@@ -459,27 +488,106 @@ static Fuse3 make_fuse(meg6_grid* g, const double* U, double* out) {
 meg6_status meg6_rhs(meg6_grid* g, const double* U, double* dUdt) {
   if (!g || !U || !dUdt) return fail(MEG6_EINVAL, "rhs: null pointer%s");
   if (!g->have_metrics) return fail(MEG6_ESTATE, "rhs called before metrics_compute%s");
+  if (!links_ok(g, true)) return fail(MEG6_ESTATE, "rhs: block-interface face without a link, or linked to another block (use meg6_rhs_blocks)%s");
   launch_prim(g, U);
   Fuse3 fu = make_fuse(g, U, dUdt);
   fu.mode = 0;
   return stage(g, 0, fu);
 }
 
+static const double RK_A[3] = {0.0, 3.0 / 4.0, 1.0 / 3.0}, RK_B[3] = {1.0, 1.0 / 4.0, 2.0 / 3.0};
+
+static Fuse3 make_fuse_rk(meg6_grid* g, double* U, int s, double dt) {
+  const int buf = s & 1;
+  Fuse3 fu = make_fuse(g, U, U);
+  fu.mode = 1; fu.a = RK_A[s]; fu.b = RK_B[s]; fu.dt = dt;
+  fu.U0w = (s == 0) ? g->U0 : nullptr;                      // stage 1 saves U^n on the way
+  fu.Pn = (s < 2) ? (buf ? g->P[0] : g->Pb[0]) : nullptr;   // primitives of the next stage's state
+  return fu;
+}
+
 meg6_status meg6_rk3_step(meg6_grid* g, double* U, double t, double dt) {
   if (!g || !U) return fail(MEG6_EINVAL, "rk3_step: null pointer%s");
   if (!g->have_metrics && !g->p.moving) return fail(MEG6_ESTATE, "rk3_step called before metrics_compute%s");
+  if (!links_ok(g, true)) return fail(MEG6_ESTATE, "rk3_step: block-interface face without a link, or linked to another block (use meg6_rk3_step_blocks)%s");
   const double ts[3] = {t, t + dt, t + 0.5 * dt};
-  const double aa[3] = {0.0, 3.0 / 4.0, 1.0 / 3.0}, bb[3] = {1.0, 1.0 / 4.0, 2.0 / 3.0};
   launch_prim(g, U);   // the caller owns U: its primitives are recomputed at every step
   for (int s = 0; s < 3; ++s) {
     meg6_status st;
     if (g->p.moving && (st = meg6_metrics_compute(g, ts[s])) != MEG6_OK) return st;
-    const int buf = s & 1;
-    Fuse3 fu = make_fuse(g, U, U);
-    fu.mode = 1; fu.a = aa[s]; fu.b = bb[s]; fu.dt = dt;
-    fu.U0w = (s == 0) ? g->U0 : nullptr;                      // stage 1 saves U^n on the way
-    fu.Pn = (s < 2) ? (buf ? g->P[0] : g->Pb[0]) : nullptr;   // primitives of the next stage's state
-    if ((st = stage(g, buf, fu)) != MEG6_OK) return st;
+    if ((st = stage(g, s & 1, make_fuse_rk(g, U, s, dt))) != MEG6_OK) return st;
+  }
+  return MEG6_OK;
+}
+
+// ---- multi-block (Sec. 6; Table 1 last column; R28) ----
+meg6_status meg6_link_blocks(meg6_grid* home, int face, meg6_grid* nb) {
+  if (!home || !nb || face < 0 || face > 5) return fail(MEG6_EINVAL, "link_blocks: bad argument%s");
+  const int d = face / 2;
+  if (home->p.periodic[d] || home->p.bc[face] != 5) return fail(MEG6_EINVAL, "link_blocks: face is not a block-interface face (bc 5)%s");
+  if (nb->p.periodic[d]) return fail(MEG6_EINVAL, "link_blocks: the neighbour is periodic in that direction%s");
+  for (int e = 0; e < 3; ++e)
+    if (e != d && (nb->c.n[e] != home->c.n[e] || nb->c.periodic[e] != home->c.periodic[e]))
+      return fail(MEG6_EINVAL, "link_blocks: transverse sizes or periodicity differ%s");
+  if (nb->stream != home->stream) return fail(MEG6_EINVAL, "link_blocks: the blocks must share one stream%s");
+  home->link[face] = nb;
+  return MEG6_OK;
+}
+
+static meg6_status blocks_ok(int n, meg6_grid* const* g, const char* who) {
+  if (n < 1 || !g) return fail(MEG6_EINVAL, "%s: no blocks", who);
+  for (int b = 0; b < n; ++b) {
+    if (!g[b]) return fail(MEG6_EINVAL, "%s: null grid", who);
+    if (g[b]->stream != g[0]->stream) return fail(MEG6_EINVAL, "%s: the blocks must share one stream", who);
+    if (!links_ok(g[b], false)) return fail(MEG6_ESTATE, "%s: block-interface face without a link", who);
+    for (int f = 0; f < 6; ++f) {   // every neighbour must be advanced by the same call
+      const meg6_grid* nb = g[b]->link[f];
+      bool found = nb == nullptr;
+      for (int q = 0; q < n && !found; ++q) found = g[q] == nb;
+      if (!found) return fail(MEG6_EINVAL, "%s: a linked neighbour is not in the block list", who);
+    }
+  }
+  return MEG6_OK;
+}
+
+meg6_status meg6_rhs_blocks(int n, meg6_grid* const* g, const double* const* U, double* const* dUdt) {
+  meg6_status st = blocks_ok(n, g, "rhs_blocks");
+  if (st != MEG6_OK) return st;
+  if (!U || !dUdt) return fail(MEG6_EINVAL, "rhs_blocks: null pointer%s");
+  for (int b = 0; b < n; ++b) {
+    if (!U[b] || !dUdt[b]) return fail(MEG6_EINVAL, "rhs_blocks: null pointer%s");
+    if (!g[b]->have_metrics) return fail(MEG6_ESTATE, "rhs_blocks called before metrics_compute%s");
+    launch_prim(g[b], U[b]);
+  }
+  for (int d = 0; d < 3; ++d)
+    for (int b = 0; b < n; ++b) fill_ghosts_dir(g[b], 0, d);
+  for (int b = 0; b < n; ++b) {
+    Fuse3 fu = make_fuse(g[b], U[b], dUdt[b]);
+    fu.mode = 0;
+    if ((st = stage_sweeps(g[b], 0, fu)) != MEG6_OK) return st;
+  }
+  return MEG6_OK;
+}
+
+meg6_status meg6_rk3_step_blocks(int n, meg6_grid* const* g, double* const* U, double t, double dt) {
+  meg6_status st = blocks_ok(n, g, "rk3_step_blocks");
+  if (st != MEG6_OK) return st;
+  if (!U) return fail(MEG6_EINVAL, "rk3_step_blocks: null pointer%s");
+  for (int b = 0; b < n; ++b) {
+    if (!U[b]) return fail(MEG6_EINVAL, "rk3_step_blocks: null pointer%s");
+    if (!g[b]->have_metrics && !g[b]->p.moving) return fail(MEG6_ESTATE, "rk3_step_blocks called before metrics_compute%s");
+    launch_prim(g[b], U[b]);
+  }
+  const double ts[3] = {t, t + dt, t + 0.5 * dt};
+  for (int s = 0; s < 3; ++s) {
+    // every block writes the primitives of its new state into the buffer NOT read by this stage, so the ghost
+    // exchange of the next stage finds all neighbours' interiors complete
+    for (int b = 0; b < n; ++b)
+      if (g[b]->p.moving && (st = meg6_metrics_compute(g[b], ts[s])) != MEG6_OK) return st;
+    for (int d = 0; d < 3; ++d)
+      for (int b = 0; b < n; ++b) fill_ghosts_dir(g[b], s & 1, d);
+    for (int b = 0; b < n; ++b)
+      if ((st = stage_sweeps(g[b], s & 1, make_fuse_rk(g[b], U[b], s, dt))) != MEG6_OK) return st;
   }
   return MEG6_OK;
 }
@@ -511,7 +619,7 @@ meg6_status meg6_diagnostics(meg6_grid* g, const double* U, double* out) {
   launch_prim(g, U);
   P6 P;
   for (int f = 0; f < 6; ++f) P.p[f] = g->P[f];
-  fill_ghosts(g, P);
+  fill_ghosts(g, 0);
   DiagIn in;
   memset(&in, 0, sizeof(in));
   for (int q = 0; q < 9; ++q) in.met[q] = g->met[q];

@@ -23,11 +23,16 @@ __global__ void __launch_bounds__(256) k_prim(Consts c, const double* __restrict
   P.p[5][at] = p / (r * c.r_gas);
 }
 
-struct GhostIn { const double* inflow[2]; const double* mx; const double* my; const double* mz; };
+struct GhostIn {
+  const double* inflow[2]; const double* mx; const double* my; const double* mz;
+  // block interfaces (bc 5): field 0 of the neighbour's primitive buffer, its layout, field stride and cell count
+  // along this direction, per side
+  const double* nbP[2]; Lay nbL[2]; long long nbfs[2]; int nbn[2];
+};
 
 // B: ghost layers of direction d (6 deep), after the lower directions have been filled: periodic wrap, fixed
 // inflow ghost = 2 P_in - P_mirror, outflow ghost = last interior cell with p = p_out where the outward normal
-// Mach number is below one (Table 1, R20).  One thread per GHOST CELL (all six fields): the twelve ghost
+// Mach number is below one (Table 1, R20), walls (R27), block interfaces (R28).  One thread per GHOST CELL (all six fields): the twelve ghost
 // cells of a xi line, or the xi-contiguous cells of an eta/zeta ghost layer, go to consecutive threads.
 __global__ void __launch_bounds__(256) k_ghost(Consts c, int d, P6 P, GhostIn in) {
   int a = (d + 1) % 3, b = (d + 2) % 3;
@@ -61,7 +66,18 @@ __global__ void __launch_bounds__(256) k_ghost(Consts c, int d, P6 P, GhostIn in
   }
   const int bc = c.bc[2 * d + side];
   const int ca = min(max(ta, 0), c.n[a] - 1), cb = min(max(tb, 0), c.n[b] - 1);
-  if (bc == 1) {
+  if (bc == 5) {
+    // block interface (Table 1 last column; R28): ghost layer q = the q-th interior cell of the neighbour
+    // block counted from its opposite face, same transverse index
+    int is[3];
+    is[a] = ta; is[b] = tb; is[d] = side ? q - 1 : in.nbn[side] - q;
+    const double* src = in.nbP[side] + in.nbL[side].at(is[0], is[1], is[2]);
+    double v[6];
+#pragma unroll
+    for (int f = 0; f < 6; ++f) v[f] = src[f * in.nbfs[side]];
+#pragma unroll
+    for (int f = 0; f < 6; ++f) P.p[f][dst] = v[f];
+  } else if (bc == 1) {
     const long long nf = (long long)c.n[a] * c.n[b];
     const double* pin = in.inflow[side] + (long long)cb * c.n[a] + ca;
     const long long mir = base + (long long)(last - sg * (q - 1)) * s;

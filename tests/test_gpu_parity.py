@@ -525,3 +525,82 @@ def test_walls_on_a_moving_mesh_are_einval(mods):
     wl["params"] = dict(wl["params"], periodic=[1, 0, 1], bc=[0, 0, 4, 4, 0, 0])
     with pytest.raises(Exception):
         M.Grid(wl)
+
+
+# ------------------------------------------------------------------ block interfaces (NEXT-3, Sec. 6, R28)
+def _block_sets():
+    return {
+        "cart_2x2_viscous": (W.cartesian_periodic(viscous=1), ((14, 10), (10, 10), (16,))),
+        "cart_zeta_cut_inviscid": (W.cartesian_periodic(nk=22, viscous=0), ((24,), (20,), (12, 10))),
+        "curved_box_walls_2x2x2": (W.wall_box(ni=26, nj=24, nk=22), ((14, 12), (11, 13), (10, 12))),
+        "curved_box_walls_mig4": (W.wall_box(ni=26, nj=24, nk=22, scheme=1), ((14, 12), (24,), (10, 12))),
+    }
+
+
+@pytest.mark.parametrize("name", list(_block_sets()))
+def test_blocks_rhs_and_steps_parity(mods, name):
+    """meg6_rhs_blocks / meg6_rk3_step_blocks against the oracle's multi-block calls, block by block: Cartesian cuts
+    (where the oracle pins say cut == uncut) and curved blocks with walls of both kinds on the outer faces, edges and
+    corners through diagonal neighbours, MEG6 and MIG4."""
+    torch, O, M = mods
+    wl, cuts = _block_sets()[name]
+    blocks, links = W.split_blocks(wl, cuts)
+    og = [O.Grid(b) for b in blocks]
+    gg = [M.Grid(b) for b in blocks]
+    for home, face, nb in links:
+        og[home].link(face, og[nb])
+        gg[home].link(face, gg[nb])
+    for a, b in zip(og, gg):
+        a.metrics_compute(0.0)
+        b.metrics_compute(0.0)
+    ref = O.rhs_blocks(og, [b["U0"] for b in blocks])
+    Us = [torch.as_tensor(b["U0"], device="cuda").contiguous() for b in blocks]
+    out = M.rhs_blocks(gg, Us)
+    for b, r, o in zip(blocks, ref, out):
+        e = rhs_err(o.cpu().numpy(), r, b["U0"])
+        assert np.all(e <= RHS_TOL), (name, b["name"], e)
+    dt = min(g.cfl_dt(b["U0"], 0.4) for g, b in zip(og, blocks))
+    Uo = [b["U0"].copy() for b in blocks]
+    for s in range(3):
+        O.rk3_step_blocks(og, Uo, s * dt, dt)
+        M.rk3_step_blocks(gg, Us, s * dt, dt)
+    for b, uo, u in zip(blocks, Uo, Us):
+        e = rel(u.cpu().numpy(), uo)
+        assert np.all(e <= STEP_TOL), (name, b["name"], e)
+    if name.startswith("cart"):
+        # and the cut run equals the uncut one on the GPU as well
+        g1 = M.Grid(wl)
+        g1.metrics_compute(0.0)
+        U1 = torch.as_tensor(wl["U0"], device="cuda").contiguous()
+        for s in range(3):
+            g1.rk3_step(U1, s * dt, dt)
+        U1 = U1.cpu().numpy()
+        for b, u in zip(blocks, Us):
+            e = rel(u.cpu().numpy(), U1[(slice(None),) + b["slices"]])
+            assert np.all(e <= 1e-11), (name, b["name"], e)
+        g1.close()
+    for g in gg:
+        g.close()
+
+
+def test_blocks_call_order_errors(mods):
+    torch, O, M = mods
+    wl = W.cartesian_periodic(ni=20, nj=12, nk=12, viscous=0)
+    blocks, links = W.split_blocks(wl, ((10, 10), (12,), (12,)))
+    gg = [M.Grid(b) for b in blocks]
+    Us = [torch.as_tensor(b["U0"], device="cuda").contiguous() for b in blocks]
+    for g in gg:
+        g.metrics_compute(0.0)
+    with pytest.raises(M.Meg6Error):
+        M.rhs_blocks(gg, Us)                       # interfaces not linked yet
+    for home, face, nb in links:
+        gg[home].link(face, gg[nb])
+    with pytest.raises(M.Meg6Error):
+        gg[0].rhs(Us[0])                           # single-grid call on a block with a foreign neighbour
+    with pytest.raises(M.Meg6Error):
+        M.rhs_blocks(gg[:1], Us[:1])               # neighbour missing from the list
+    with pytest.raises(M.Meg6Error):
+        M.Grid(wl).link(0, gg[0])                  # not an interface face
+    M.rhs_blocks(gg, Us)
+    for g in gg:
+        g.close()

@@ -308,3 +308,65 @@ def wall_box(ni=22, nj=19, nk=17, bc=(3, 4, 3, 3, 4, 3), viscous=1, scheme=0, se
         prm.update(mu_ref=0.3 * 1.0 / 200.0, t_ref=1.0 / GAMMA, s_suth=0.4 / GAMMA)
     return dict(name="wall_box_%dx%dx%d" % (ni, nj, nk), params=prm, x=x, y=y, z=z,
                 U0=conservative(rho, u, v, w, p), dt=None, cfl=0.4, steps=3, t0=0.0)
+
+
+# --------------------------------------------------------------------------------------------------
+# Multi-block inputs (Sec. 6): a single-block workload cut into aligned blocks.
+def cartesian_periodic(ni=24, nj=20, nk=16, viscous=1, seed=77, scheme=0):
+    """Uniform Cartesian periodic box (spacing 1/8: exactly representable coordinates) with a seeded smooth state:
+    the mesh on which linearly extrapolated ghost coordinates (R13) equal the neighbour block's true ones."""
+    h = 0.125
+    L = (ni * h, nj * h, nk * h)
+    X, E, Z = _comp_coords((ni, nj, nk), L)
+    x, y, z = (np.ascontiguousarray(a) for a in (X, E, Z))
+    rho, u, v, w, p = _smooth_state(cell_centres(x), cell_centres(y), cell_centres(z), L, seed)
+    prm = _base_params(ni, nj, nk, period=[[L[0], 0, 0], [0, L[1], 0], [0, 0, L[2]]], viscous=viscous, scheme=scheme)
+    if viscous:
+        prm.update(mu_ref=0.3 * 1.0 / 200.0, t_ref=1.0 / GAMMA, s_suth=0.4 / GAMMA)
+    return dict(name="cart_periodic_%dx%dx%d" % (ni, nj, nk), params=prm, x=x, y=y, z=z,
+                U0=conservative(rho, u, v, w, p), dt=None, cfl=0.4, steps=3, t0=0.0)
+
+
+def split_blocks(wl, cuts):
+    """Cuts a static single-block workload into aligned blocks.  cuts = (cells of the xi pieces, eta pieces, zeta
+    pieces), e.g. ((12, 12), (20,), (16,)).  Returns (blocks, links): blocks in storage order (xi piece fastest),
+    links = [(home, face, neighbour)].  Cut directions become non-periodic with bc 5 on the cut faces; a periodic
+    direction that is cut wraps around through links; outer faces of non-periodic directions keep their bc."""
+    prm = wl["params"]
+    assert not prm["moving"] and "inflow" not in wl and wl.get("sigma") is None
+    n = (prm["ni"], prm["nj"], prm["nk"])
+    for d in range(3):
+        assert sum(cuts[d]) == n[d]
+    starts = [np.concatenate([[0], np.cumsum(cuts[d])]) for d in range(3)]
+    nb = [len(cuts[d]) for d in range(3)]
+    idx = lambda a, b, c: (c * nb[1] + b) * nb[0] + a
+    blocks, links = [], []
+    for c in range(nb[2]):
+        for b in range(nb[1]):
+            for a in range(nb[0]):
+                pos = (a, b, c)
+                lo = [int(starts[d][pos[d]]) for d in range(3)]
+                hi = [int(starts[d][pos[d] + 1]) for d in range(3)]
+                p = dict(prm)
+                p["ni"], p["nj"], p["nk"] = (hi[d] - lo[d] for d in range(3))
+                p["periodic"] = list(prm["periodic"])
+                p["bc"] = list(prm["bc"])
+                for d in range(3):
+                    if nb[d] == 1:
+                        continue
+                    p["periodic"][d] = 0
+                    for side in range(2):
+                        q = pos[d] + (1 if side else -1)
+                        if 0 <= q < nb[d] or prm["periodic"][d]:
+                            p["bc"][2 * d + side] = 5
+                            npos = list(pos)
+                            npos[d] = q % nb[d]
+                            links.append((idx(*pos), 2 * d + side, idx(*npos)))
+                sl_n = tuple(slice(lo[d], hi[d] + 1) for d in (2, 1, 0))
+                sl_c = tuple(slice(lo[d], hi[d]) for d in (2, 1, 0))
+                blocks.append(dict(name="%s_block%d" % (wl["name"], idx(*pos)), params=p,
+                                   x=np.ascontiguousarray(wl["x"][sl_n]), y=np.ascontiguousarray(wl["y"][sl_n]),
+                                   z=np.ascontiguousarray(wl["z"][sl_n]),
+                                   U0=np.ascontiguousarray(wl["U0"][(slice(None),) + sl_c]),
+                                   dt=wl.get("dt"), cfl=wl.get("cfl"), steps=wl.get("steps"), t0=0.0, slices=sl_c))
+    return blocks, links
