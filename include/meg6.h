@@ -111,6 +111,29 @@ meg6_status meg6_link_blocks(meg6_grid* home, int face, meg6_grid* neighbour);
 meg6_status meg6_rhs_blocks(int n, meg6_grid* const* g, const double* const* U, double* const* dUdt);
 meg6_status meg6_rk3_step_blocks(int n, meg6_grid* const* g, double* const* U, double t, double dt);
 
+/* Staged stepping: one RK stage as separate calls, for blocks that live on different devices (a slab decomposition:
+ * SURVEY 8(e)) -- the caller moves the interface layers itself between the ghost fill of one direction and the next.
+ * Per SSP-RK3 step (stage s = 0, 1, 2 at times t, t+dt, t+dt/2; moving meshes: meg6_metrics_compute before each):
+ *   s == 0:  meg6_stage_prim(g, U)                       primitives of U (later stages: written by the previous sweeps)
+ *   for d = 0, 1, 2:
+ *       meg6_stage_pack(g, s, face, layers)              for each interface face of direction d: the six cell layers
+ *                                                        next to `face`, all fields, every transverse position of the
+ *                                                        padded array (ghosts of lower directions included, so edge
+ *                                                        and corner ghosts travel with them); meg6_interface_doubles
+ *                                                        doubles.  The caller delivers them to the neighbour, whose
+ *                                                        buffer was registered with meg6_set_interface_buffer(g, face^1
+ *                                                        seen from there, layers) -- pointer kept; replaces a link.
+ *       meg6_stage_ghosts(g, s, d)                       ghost fill of direction d (all boundary kinds)
+ *   meg6_stage_sweeps(g, U, NULL, s, dt)                 gradients + sweeps + fused RK stage update of U
+ * meg6_stage_sweeps(g, U, dUdt, 0, 0) writes dQ/dt instead (after stage_prim and the ghost fills with s = 0).
+ * Identical, kernel for kernel, to what meg6_rk3_step_blocks launches. */
+size_t      meg6_interface_doubles(const meg6_grid* g, int face);
+meg6_status meg6_set_interface_buffer(meg6_grid* g, int face, const double* layers);
+meg6_status meg6_stage_prim(meg6_grid* g, const double* U);
+meg6_status meg6_stage_pack(meg6_grid* g, int s, int face, double* layers);
+meg6_status meg6_stage_ghosts(meg6_grid* g, int s, int d);
+meg6_status meg6_stage_sweeps(meg6_grid* g, double* U, double* dUdt, int s, double dt);
+
 /* Eq. B.2 / B.3 time step for the state U at the geometry of the last metrics_compute.
  * Synchronises the stream.  *dt is a HOST pointer. */
 meg6_status meg6_cfl_dt(meg6_grid* g, const double* U, double cfl, double* dt);

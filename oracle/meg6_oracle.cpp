@@ -233,6 +233,7 @@ struct meg6o_grid {
   std::vector<double> sigma, uref;
   unsigned long long n_limited = 0, n_tested = 0;
   meg6o_grid* link[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};   /* bc 5: neighbour block per face */
+  const double* ibuf[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr}; /* bc 5: or packed neighbour layers */
 };
 
 namespace {
@@ -688,10 +689,22 @@ void ghost_dir(meg6o_grid* G, int d) {
             /* block interface, Table 1 last column, R28: ghost layer q = the q-th interior cell of the
              * neighbour block counted from its opposite face, same transverse index (aligned blocks) */
             const meg6o_grid* nb = G->link[face];
-            const int nn = nb->n[d];
-            for (int q = 1; q <= GP; ++q) {
-              int is[3]; is[a] = ta; is[b] = tb; is[d] = side ? q - 1 : nn - q;
-              for (int f = 0; f < 5; ++f) at(f, last + sg * q) = nb->P[f](is[0], is[1], is[2]);
+            if (nb) {
+              const int nn = nb->n[d];
+              for (int q = 1; q <= GP; ++q) {
+                int is[3]; is[a] = ta; is[b] = tb; is[d] = side ? q - 1 : nn - q;
+                for (int f = 0; f < 5; ++f) at(f, last + sg * q) = nb->P[f](is[0], is[1], is[2]);
+              }
+            } else {
+              /* packed layers of a neighbour that lives elsewhere (meg6o_stage_pack on its side): layer l = 0..5 in
+               * the neighbour's own order along d, [field][tb][ta][l] over the padded transverse ranges */
+              const double* buf = G->ibuf[face];
+              const size_t ea = G->n[a] + 2 * GP, eb = G->n[b] + 2 * GP;
+              for (int q = 1; q <= GP; ++q) {
+                const int l = side ? q - 1 : GP - q;
+                for (int f = 0; f < 5; ++f)
+                  at(f, last + sg * q) = buf[((f * eb + (size_t)(tb + GP)) * ea + (size_t)(ta + GP)) * GP + l];
+              }
             }
           } else if (bc == 1) {
             /* fixed inflow, Table 1, R20: ghost = 2 P_in - P_mirror */
@@ -765,7 +778,7 @@ void meg6o_rhs_blocks(int nb, meg6o_grid* const* G, const double* const* U, doub
   for (int b = 0; b < nb; ++b) {
     if (!G[b]->have_metrics) { fprintf(stderr, "meg6o_rhs before metrics_compute\n"); abort(); }
     for (int f = 0; f < 6; ++f)
-      if (!G[b]->p.periodic[f / 2] && G[b]->p.bc[f] == 5 && !G[b]->link[f]) { fprintf(stderr, "meg6o_rhs: unlinked block interface\n"); abort(); }
+      if (!G[b]->p.periodic[f / 2] && G[b]->p.bc[f] == 5 && !G[b]->link[f] && !G[b]->ibuf[f]) { fprintf(stderr, "meg6o_rhs: unlinked block interface\n"); abort(); }
     prim_interior(G[b], U[b]);
   }
   for (int d = 0; d < 3; ++d)
@@ -924,6 +937,37 @@ void meg6o_rk3_step_blocks(int nb, meg6o_grid* const* G, double* const* U, doubl
 }
 
 void meg6o_rk3_step(meg6o_grid* G, double* U, double t, double dt) { meg6o_rk3_step_blocks(1, &G, &U, t, dt); }
+
+/* Staged evaluation for blocks that live in different processes (the caller carries the packed layers). */
+size_t meg6o_interface_doubles(const meg6o_grid* G, int face) {
+  const int d = face / 2;
+  int a = (d + 1) % 3, b = (d + 2) % 3;
+  return (size_t)5 * GP * (G->n[a] + 2 * GP) * (G->n[b] + 2 * GP);
+}
+void meg6o_set_interface_buffer(meg6o_grid* G, int face, const double* layers) {
+  G->ibuf[face] = layers;
+  if (layers) G->link[face] = nullptr;
+}
+void meg6o_stage_prim(meg6o_grid* G, const double* U) { prim_interior(G, U); }
+void meg6o_stage_ghosts(meg6o_grid* G, int d) { ghost_dir(G, d); }
+void meg6o_stage_pack(meg6o_grid* G, int face, double* layers) {
+  const int d = face / 2, side = face & 1;
+  int a = (d + 1) % 3, b = (d + 2) % 3;
+  if (a > b) std::swap(a, b);
+  const size_t ea = G->n[a] + 2 * GP, eb = G->n[b] + 2 * GP;
+  const int first = side ? G->n[d] - GP : 0;
+  for (int f = 0; f < 5; ++f)
+    for (int tb = -GP; tb < G->n[b] + GP; ++tb)
+      for (int ta = -GP; ta < G->n[a] + GP; ++ta)
+        for (int l = 0; l < GP; ++l) {
+          int is[3]; is[a] = ta; is[b] = tb; is[d] = first + l;
+          layers[((f * eb + (size_t)(tb + GP)) * ea + (size_t)(ta + GP)) * GP + l] = G->P[f].d[G->P[f].idx(is[0], is[1], is[2])];
+        }
+}
+void meg6o_stage_rhs(meg6o_grid* G, const double* U, double* dUdt) {
+  finish_primitives(G);
+  rhs_from_primitives(G, U, dUdt);
+}
 
 /* Block interface (Sec. 6; Table 1 last column): face `face` of `home` (bc 5) takes its ghost primitives
  * from the interior cells of `nb` next to nb's opposite face.  Aligned blocks only (same orientation of the three

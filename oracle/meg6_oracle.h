@@ -53,6 +53,14 @@ void meg6o_rk3_step(meg6o_grid* g, double* U, double t, double dt);
  * from the interior cells of `nb` next to nb's opposite face; aligned blocks, equal transverse sizes.  Returns 0 if ok.
  * The *_blocks calls advance all blocks together (ghost exchange before every right-hand side). */
 int meg6o_link_blocks(meg6o_grid* home, int face, meg6o_grid* nb);
+/* Staged evaluation for blocks in different processes: prim -> for d: [pack / deliver / set_interface_buffer] ghosts(d)
+ * -> stage_rhs.  The packed layers of a face: meg6o_interface_doubles doubles. */
+size_t meg6o_interface_doubles(const meg6o_grid* g, int face);
+void meg6o_set_interface_buffer(meg6o_grid* g, int face, const double* layers);
+void meg6o_stage_prim(meg6o_grid* g, const double* U);
+void meg6o_stage_ghosts(meg6o_grid* g, int d);
+void meg6o_stage_pack(meg6o_grid* g, int face, double* layers);
+void meg6o_stage_rhs(meg6o_grid* g, const double* U, double* dUdt);
 void meg6o_rhs_blocks(int nb, meg6o_grid* const* g, const double* const* U, double* const* dUdt);
 void meg6o_rk3_step_blocks(int nb, meg6o_grid* const* g, double* const* U, double t, double dt);
 double meg6o_cfl_dt(meg6o_grid* g, const double* U, double cfl);

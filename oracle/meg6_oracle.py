@@ -65,6 +65,13 @@ def lib():
         L.meg6o_link_blocks.argtypes = [C.c_void_p, C.c_int, C.c_void_p]
         L.meg6o_rhs_blocks.argtypes = [C.c_int, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p), C.POINTER(C.c_void_p)]
         L.meg6o_rk3_step_blocks.argtypes = [C.c_int, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p), C.c_double, C.c_double]
+        L.meg6o_interface_doubles.restype = C.c_size_t
+        L.meg6o_interface_doubles.argtypes = [C.c_void_p, C.c_int]
+        L.meg6o_set_interface_buffer.argtypes = [C.c_void_p, C.c_int, C.c_void_p]
+        L.meg6o_stage_prim.argtypes = [C.c_void_p, _dp]
+        L.meg6o_stage_ghosts.argtypes = [C.c_void_p, C.c_int]
+        L.meg6o_stage_pack.argtypes = [C.c_void_p, C.c_int, C.c_void_p]
+        L.meg6o_stage_rhs.argtypes = [C.c_void_p, _dp, _dp]
         L.meg6o_cfl_dt.restype = C.c_double
         L.meg6o_cfl_dt.argtypes = [C.c_void_p, _dp, C.c_double]
         L.meg6o_diagnostics.argtypes = [C.c_void_p, _dp, _dp]
@@ -180,6 +187,29 @@ class Grid:
         if lib().meg6o_link_blocks(self.h, int(face), neighbour.h) != 0:
             raise ValueError("meg6o_link_blocks rejected the pair")
         self._links = getattr(self, "_links", []) + [neighbour]
+
+    # staged evaluation (blocks in different processes); `layers` are numpy float64 arrays kept alive by the caller
+    def interface_doubles(self, face):
+        return int(lib().meg6o_interface_doubles(self.h, int(face)))
+
+    def set_interface_buffer(self, face, layers):
+        assert layers.dtype == np.float64 and layers.flags["C_CONTIGUOUS"]
+        lib().meg6o_set_interface_buffer(self.h, int(face), layers.ctypes.data)
+
+    def stage_prim(self, U):
+        lib().meg6o_stage_prim(self.h, _p(U))
+
+    def stage_ghosts(self, d):
+        lib().meg6o_stage_ghosts(self.h, int(d))
+
+    def stage_pack(self, face, layers):
+        assert layers.dtype == np.float64 and layers.flags["C_CONTIGUOUS"]
+        lib().meg6o_stage_pack(self.h, int(face), layers.ctypes.data)
+
+    def stage_rhs(self, U):
+        out = np.empty_like(U)
+        lib().meg6o_stage_rhs(self.h, _p(U), _p(out))
+        return out
 
     def diagnostics(self, U):
         """(kinetic energy, enstrophy, volume), Eq. 54"""

@@ -11,7 +11,9 @@ EXPORTS = ["meg6_workspace_bytes", "meg6_grid_create", "meg6_grid_destroy", "meg
            "meg6_set_inflow", "meg6_set_sponge", "meg6_rhs", "meg6_rk3_step", "meg6_cfl_dt", "meg6_diagnostics",
            "meg6_limiter_stats_enable", "meg6_limiter_stats", "meg6_get_array", "meg6_profile_enable",
            "meg6_profile_read", "meg6_last_error",
-           "meg6_version", "meg6_link_blocks", "meg6_rhs_blocks", "meg6_rk3_step_blocks"]
+           "meg6_version", "meg6_link_blocks", "meg6_rhs_blocks", "meg6_rk3_step_blocks",
+           "meg6_interface_doubles", "meg6_set_interface_buffer", "meg6_stage_prim", "meg6_stage_pack",
+           "meg6_stage_ghosts", "meg6_stage_sweeps"]
 
 
 class Meg6Error(RuntimeError):
@@ -101,6 +103,18 @@ def lib():
         L.meg6_rhs_blocks.argtypes = [C.c_int, C.POINTER(_vp), C.POINTER(_vp), C.POINTER(_vp)]
         L.meg6_rk3_step_blocks.restype = C.c_int
         L.meg6_rk3_step_blocks.argtypes = [C.c_int, C.POINTER(_vp), C.POINTER(_vp), C.c_double, C.c_double]
+        L.meg6_interface_doubles.restype = C.c_size_t
+        L.meg6_interface_doubles.argtypes = [_vp, C.c_int]
+        L.meg6_set_interface_buffer.restype = C.c_int
+        L.meg6_set_interface_buffer.argtypes = [_vp, C.c_int, _vp]
+        L.meg6_stage_prim.restype = C.c_int
+        L.meg6_stage_prim.argtypes = [_vp, _vp]
+        L.meg6_stage_pack.restype = C.c_int
+        L.meg6_stage_pack.argtypes = [_vp, C.c_int, C.c_int, _vp]
+        L.meg6_stage_ghosts.restype = C.c_int
+        L.meg6_stage_ghosts.argtypes = [_vp, C.c_int, C.c_int]
+        L.meg6_stage_sweeps.restype = C.c_int
+        L.meg6_stage_sweeps.argtypes = [_vp, _vp, _vp, C.c_int, C.c_double]
         L.meg6_last_error.restype = C.c_char_p
         L.meg6_version.restype = C.c_int
         _lib = L
@@ -185,6 +199,33 @@ class Grid:
         """block interface (bc 5): ghost cells of `face` come from `neighbour`'s interior at its opposite face"""
         _check(lib().meg6_link_blocks(self.h, int(face), neighbour.h), "meg6_link_blocks")
         self._links = getattr(self, "_links", []) + [neighbour]   # keep the neighbour alive
+
+    # ---- staged stepping (include/meg6.h "Staged stepping"): the pieces paper_2303_10785_b200.slabs drives ----
+    def new_interface_buffer(self, face):
+        n = lib().meg6_interface_doubles(self.h, int(face))
+        return self.torch.zeros(n, dtype=self.torch.float64, device=self.device)
+
+    def set_interface_buffer(self, face, layers):
+        assert layers.is_cuda and layers.dtype == self.torch.float64 and layers.is_contiguous()
+        _check(lib().meg6_set_interface_buffer(self.h, int(face), layers.data_ptr()), "meg6_set_interface_buffer")
+        if not hasattr(self, "_ibufs"):
+            self._ibufs = {}
+        self._ibufs[int(face)] = layers   # keep it alive
+
+    def stage_prim(self, U):
+        self._chk_state(U)
+        _check(lib().meg6_stage_prim(self.h, U.data_ptr()), "meg6_stage_prim")
+
+    def stage_pack(self, s, face, layers):
+        _check(lib().meg6_stage_pack(self.h, int(s), int(face), layers.data_ptr()), "meg6_stage_pack")
+
+    def stage_ghosts(self, s, d):
+        _check(lib().meg6_stage_ghosts(self.h, int(s), int(d)), "meg6_stage_ghosts")
+
+    def stage_sweeps(self, U, s, dt, out=None):
+        self._chk_state(U)
+        _check(lib().meg6_stage_sweeps(self.h, U.data_ptr(), out.data_ptr() if out is not None else None, int(s),
+                                       float(dt)), "meg6_stage_sweeps")
 
     def diagnostics(self, U):
         """(kinetic energy, enstrophy, volume) of the state U, Eq. 54"""

@@ -119,6 +119,7 @@ static size_t carve(const meg6_params* p, const Consts& c, meg6_grid* g, char* b
     const int d = f / 2;
     G->inflow[f] = nullptr;
     G->link[f] = nullptr;
+    G->ibuf[f] = nullptr;
     if (!p->periodic[d] && p->bc[f] == 1) {
       int a = (d + 1) % 3, b = (d + 2) % 3;
       G->inflow[f] = take(5LL * c.n[a] * c.n[b]);
@@ -388,9 +389,13 @@ static void fill_ghosts_dir(meg6_grid* g, int buf, int d) {
   gin.mx = g->met[3 * d]; gin.my = g->met[3 * d + 1]; gin.mz = g->met[3 * d + 2];
   for (int side = 0; side < 2; ++side) {
     const meg6_grid* nb = g->link[2 * d + side];
-    if (!nb) continue;
-    gin.nbP[side] = buf ? nb->Pb[0] : nb->P[0];
-    gin.nbL[side] = nb->c.LP; gin.nbfs[side] = nb->c.fsP; gin.nbn[side] = nb->c.n[d];
+    if (nb) {
+      gin.nbP[side] = buf ? nb->Pb[0] : nb->P[0];
+      gin.nbL[side] = nb->c.LP; gin.nbfs[side] = nb->c.fsP; gin.nbn[side] = nb->c.n[d];
+    } else if (g->ibuf[2 * d + side]) {   // packed layers of a remote neighbour: a block six cells thick
+      gin.nbP[side] = g->ibuf[2 * d + side];
+      gin.nbL[side] = pack_lay(c.LP, d); gin.nbfs[side] = gin.nbL[side].n; gin.nbn[side] = 6;
+    }
   }
   ProfScope ps(g, 2, 1);
   k_ghost<<<nblk(ea * eb * 12, 256), 256, 0, g->stream>>>(c, d, P, gin);
@@ -403,7 +408,7 @@ static void fill_ghosts(meg6_grid* g, int buf) {
 static bool links_ok(const meg6_grid* g, bool single) {
   for (int f = 0; f < 6; ++f)
     if (!g->p.periodic[f / 2] && g->p.bc[f] == 5) {
-      if (!g->link[f]) return false;
+      if (!g->link[f] && !g->ibuf[f]) return false;
       if (single && g->link[f] != g) return false;   // a single-grid call may only see itself across an interface
     }
   return true;
@@ -590,6 +595,65 @@ meg6_status meg6_rk3_step_blocks(int n, meg6_grid* const* g, double* const* U, d
       if ((st = stage_sweeps(g[b], s & 1, make_fuse_rk(g[b], U[b], s, dt))) != MEG6_OK) return st;
   }
   return MEG6_OK;
+}
+
+// ---- staged stepping: the pieces of one RK stage as separate calls, for callers that exchange interface layers
+// themselves between the ghost fill of one direction and the next (blocks on other devices) ----
+size_t meg6_interface_doubles(const meg6_grid* g, int face) {
+  if (!g || face < 0 || face > 5) return 0;
+  return (size_t)(6 * pack_lay(g->c.LP, face / 2).n);
+}
+
+meg6_status meg6_set_interface_buffer(meg6_grid* g, int face, const double* layers) {
+  if (!g || face < 0 || face > 5) return fail(MEG6_EINVAL, "set_interface_buffer: bad argument%s");
+  if (g->p.periodic[face / 2] || g->p.bc[face] != 5) return fail(MEG6_EINVAL, "set_interface_buffer: face is not a block-interface face (bc 5)%s");
+  g->ibuf[face] = layers;
+  if (layers) g->link[face] = nullptr;
+  return MEG6_OK;
+}
+
+static bool staged_ok(const meg6_grid* g) {
+  for (int f = 0; f < 6; ++f)
+    if (!g->p.periodic[f / 2] && g->p.bc[f] == 5 && !g->link[f] && !g->ibuf[f]) return false;
+  return true;
+}
+
+meg6_status meg6_stage_prim(meg6_grid* g, const double* U) {
+  if (!g || !U) return fail(MEG6_EINVAL, "stage_prim: null pointer%s");
+  launch_prim(g, U);
+  return MEG6_OK;
+}
+
+meg6_status meg6_stage_ghosts(meg6_grid* g, int s, int d) {
+  if (!g || s < 0 || s > 2 || d < 0 || d > 2) return fail(MEG6_EINVAL, "stage_ghosts: bad argument%s");
+  if (!g->have_metrics) return fail(MEG6_ESTATE, "stage_ghosts called before metrics_compute%s");
+  if (!staged_ok(g)) return fail(MEG6_ESTATE, "stage_ghosts: block-interface face without a link or a buffer%s");
+  fill_ghosts_dir(g, s & 1, d);
+  CUDA_OK(cudaGetLastError());
+  return MEG6_OK;
+}
+
+meg6_status meg6_stage_pack(meg6_grid* g, int s, int face, double* layers) {
+  if (!g || !layers || s < 0 || s > 2 || face < 0 || face > 5) return fail(MEG6_EINVAL, "stage_pack: bad argument%s");
+  const int d = face / 2;
+  const Lay LQ = pack_lay(g->c.LP, d);
+  const int first = (face & 1) ? g->c.n[d] - 6 : 0;   // the layers a neighbour beyond this face needs
+  ProfScope ps(g, 2, 1);
+  k_pack<<<nblk(LQ.n, 256), 256, 0, g->stream>>>(g->c.LP, LQ, d, first, g->c.fsP, (s & 1) ? g->Pb[0] : g->P[0], layers);
+  CUDA_OK(cudaGetLastError());
+  return MEG6_OK;
+}
+
+meg6_status meg6_stage_sweeps(meg6_grid* g, double* U, double* dUdt, int s, double dt) {
+  if (!g || !U || s < 0 || s > 2) return fail(MEG6_EINVAL, "stage_sweeps: bad argument%s");
+  if (!g->have_metrics) return fail(MEG6_ESTATE, "stage_sweeps called before metrics_compute%s");
+  if (dUdt) {   // plain right-hand side of the state whose primitives are in buffer 0
+    if (s != 0) return fail(MEG6_EINVAL, "stage_sweeps: dUdt is written at s == 0 only%s");
+    Fuse3 fu = make_fuse(g, U, dUdt);
+    fu.mode = 0;
+    return stage_sweeps(g, 0, fu);
+  }
+  return stage_sweeps(g, s & 1, make_fuse_rk(g, U, s, dt));
 }
 
 meg6_status meg6_cfl_dt(meg6_grid* g, const double* U, double cfl, double* dt) {

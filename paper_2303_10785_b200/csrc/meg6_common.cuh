@@ -100,6 +100,7 @@ struct meg6_grid {
   double* U0;         // [5][N]
   double* inflow[6];
   meg6_grid* link[6];          // bc 5: the neighbour block of each face (meg6_link_blocks)
+  const double* ibuf[6];       // bc 5: or a packed copy of the neighbour's layers (meg6_set_interface_buffer)
   const double* sigma; const double* uref;
   unsigned long long* stats;   // [2] device counters: limited, tested
   double* red;                 // reduction scratch

@@ -128,6 +128,28 @@ __global__ void __launch_bounds__(256) k_ghost(Consts c, int d, P6 P, GhostIn in
   }
 }
 
+// Packed interface layers (meg6_stage_pack): the six cell layers of direction d next to one face, all six fields,
+// every transverse position of the padded primitive array.  The packed array is a padded layout itself: as LP, but
+// with 6 cells and no ghosts along d -- k_ghost reads it like a neighbour block that is six cells thick.
+inline Lay pack_lay(const Lay& LP, int d) {
+  Lay L = LP;
+  if (d == 0) { L.gi = 0; L.pi = 6; } else if (d == 1) { L.gj = 0; L.pj = 6; } else { L.gk = 0; L.pk = 6; }
+  L.sj = L.pi; L.sk = (long long)L.pi * L.pj; L.n = L.sk * L.pk;
+  return L;
+}
+
+__global__ void __launch_bounds__(256) k_pack(Lay LP, Lay LQ, int d, int first, long long fsP, const double* __restrict__ P,
+                                              double* __restrict__ out) {
+  const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (tid >= LQ.n) return;
+  const int pi = (int)(tid % LQ.pi), pj = (int)((tid / LQ.pi) % LQ.pj), pk = (int)(tid / LQ.sk);
+  int ix[3] = {pi - LQ.gi, pj - LQ.gj, pk - LQ.gk};   // cell indices of the packed array
+  ix[d] += first;                                     // ... of the source array
+  const long long src = LP.at(ix[0], ix[1], ix[2]);
+#pragma unroll
+  for (int f = 0; f < 6; ++f) out[f * LQ.n + tid] = P[f * fsP + src];
+}
+
 // E6 gradient, Eq. 17 (R1)
 __device__ __forceinline__ double d1_op(const double* __restrict__ f, long long s) {
   double r = CE1 * (f[s] - f[-s]);

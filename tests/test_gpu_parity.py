@@ -604,3 +604,64 @@ def test_blocks_call_order_errors(mods):
     M.rhs_blocks(gg, Us)
     for g in gg:
         g.close()
+
+
+def test_staged_api_with_packed_layers_equals_linked_blocks(mods):
+    """The staged calls (meg6_stage_prim / _pack / _ghosts / _sweeps with meg6_set_interface_buffer), driven here for
+    two blocks in one process with the packed layers copied by hand, are the path paper_2303_10785_b200.slabs runs
+    between ranks: bit for bit the result of meg6_rk3_step_blocks on linked blocks (same kernels, same data)."""
+    torch, O, M = mods
+    wl = W.wall_box(ni=26, nj=24, nk=22)
+    cuts = ((26,), (11, 13), (10, 12))      # eta and zeta interfaces: edge ghosts travel inside the packed layers
+    blocks, links = W.split_blocks(wl, cuts)
+    ref = [M.Grid(b) for b in blocks]
+    for home, face, nb in links:
+        ref[home].link(face, ref[nb])
+    gg = [M.Grid(b) for b in blocks]
+    send, recv = {}, {}
+    for home, face, nb in links:
+        send[(home, face)] = gg[home].new_interface_buffer(face)
+        recv[(home, face)] = gg[home].new_interface_buffer(face)
+        gg[home].set_interface_buffer(face, recv[(home, face)])
+    for g in ref + gg:
+        g.metrics_compute(0.0)
+    Ur = [torch.as_tensor(b["U0"], device="cuda").contiguous() for b in blocks]
+    Us = [u.clone() for u in Ur]
+    dt = 1.5e-3
+
+    def ghosts(s):
+        for d in range(3):
+            for home, face, nb in links:
+                if face // 2 == d:
+                    gg[home].stage_pack(s, face, send[(home, face)])
+            for home, face, nb in links:
+                if face // 2 == d:
+                    recv[(nb, face ^ 1)].copy_(send[(home, face)])
+            for g in gg:
+                g.stage_ghosts(s, d)
+
+    # right-hand side
+    want = M.rhs_blocks(ref, Ur)
+    got = [torch.empty_like(u) for u in Us]
+    for g, u in zip(gg, Us):
+        g.stage_prim(u)
+    ghosts(0)
+    for g, u, o in zip(gg, Us, got):
+        g.stage_sweeps(u, 0, 0.0, out=o)
+    for a, b in zip(got, want):
+        assert torch.equal(a, b)
+    # two RK3 steps
+    for step in range(2):
+        M.rk3_step_blocks(ref, Ur, step * dt, dt)
+        for s in range(3):
+            if s == 0:
+                for g, u in zip(gg, Us):
+                    g.stage_prim(u)
+            ghosts(s)
+            for g, u in zip(gg, Us):
+                g.stage_sweeps(u, s, dt)
+    for a, b, blk in zip(Us, Ur, blocks):
+        assert torch.equal(a, b)
+        assert (a.cpu().numpy() - blk["U0"]).__abs__().max() > 1e-5
+    for g in ref + gg:
+        g.close()

@@ -333,7 +333,7 @@ def split_blocks(wl, cuts):
     links = [(home, face, neighbour)].  Cut directions become non-periodic with bc 5 on the cut faces; a periodic
     direction that is cut wraps around through links; outer faces of non-periodic directions keep their bc."""
     prm = wl["params"]
-    assert not prm["moving"] and "inflow" not in wl and wl.get("sigma") is None
+    assert not prm["moving"]
     n = (prm["ni"], prm["nj"], prm["nk"])
     for d in range(3):
         assert sum(cuts[d]) == n[d]
@@ -364,7 +364,20 @@ def split_blocks(wl, cuts):
                             links.append((idx(*pos), 2 * d + side, idx(*npos)))
                 sl_n = tuple(slice(lo[d], hi[d] + 1) for d in (2, 1, 0))
                 sl_c = tuple(slice(lo[d], hi[d]) for d in (2, 1, 0))
-                blocks.append(dict(name="%s_block%d" % (wl["name"], idx(*pos)), params=p,
+                extra = {}
+                if wl.get("sigma") is not None:
+                    extra["sigma"] = np.ascontiguousarray(wl["sigma"][sl_c])
+                    extra["U_ref"] = np.ascontiguousarray(wl["U_ref"][(slice(None),) + sl_c])
+                inflow = {}
+                for face, pin in wl.get("inflow", {}).items():   # pin[5][n2][n1], transverse axes in storage order
+                    d = int(face) // 2
+                    if p["bc"][int(face)] != 1:
+                        continue
+                    t1, t2 = [e for e in range(3) if e != d]
+                    inflow[int(face)] = np.ascontiguousarray(pin[:, lo[t2]:hi[t2], lo[t1]:hi[t1]])
+                if inflow:
+                    extra["inflow"] = inflow
+                blocks.append(dict(extra, name="%s_block%d" % (wl["name"], idx(*pos)), params=p,
                                    x=np.ascontiguousarray(wl["x"][sl_n]), y=np.ascontiguousarray(wl["y"][sl_n]),
                                    z=np.ascontiguousarray(wl["z"][sl_n]),
                                    U0=np.ascontiguousarray(wl["U0"][(slice(None),) + sl_c]),
