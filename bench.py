@@ -205,6 +205,20 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=dev)
 
     wl = make_workload(args.workload)
+    wl_name = wl["name"]
+    slabs = args.decomp == "slabs" and world > 1
+    stepper = None
+    if slabs:
+        # strong scaling: the workload cut into `world` zeta slabs, one per rank, six-layer halo exchange of the
+        # primitives per RK stage over NCCL point-to-point (paper_2303_10785_b200/slabs.py)
+        from paper_2303_10785_b200.slabs import SlabStepper, slab_cuts
+        p0 = wl["params"]
+        blocks, links = W.split_blocks(wl, ((p0["ni"],), (p0["nj"],), slab_cuts(p0["nk"], world)))
+        dt_fixed = wl["dt"]
+        wl = blocks[rank]
+        wl["dt"] = dt_fixed
+        remote = {face: nb for home, face, nb in links if home == rank}
+        del blocks
     prm = wl["params"]
     ncell = prm["ni"] * prm["nj"] * prm["nk"]
     g = Grid(wl, device=dev)
@@ -214,6 +228,13 @@ def run_ours(args):
         dt = wl["dt"]
     else:
         dt = g.cfl_dt(U, wl["cfl"])      # on-device Eq. B.2/B.3 (no oracle on the product path)
+        if slabs:                        # one time step for the whole job: the minimum over the slabs
+            tdt = torch.tensor([dt], dtype=torch.float64, device=dev)
+            dist.all_reduce(tdt, op=dist.ReduceOp.MIN)
+            dt = float(tdt.item())
+    if slabs:
+        stepper = SlabStepper(g, remote, moving=bool(prm["moving"]))
+    step = stepper.rk3_step if stepper else g.rk3_step
     stream = torch.cuda.current_stream(dev)
 
     def barrier():
@@ -225,7 +246,7 @@ def run_ours(args):
     # ---------------- device-resident timing ----------------
     t = wl["t0"]
     for _ in range(args.warmup):
-        g.rk3_step(U, t, dt); t += dt
+        step(U, t, dt); t += dt
     g.profile_enable(True)
     g.profile_read()
     sampler = ClockSampler(local)
@@ -235,7 +256,7 @@ def run_ours(args):
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record(stream)
     for _ in range(args.steps):
-        g.rk3_step(U, t, dt); t += dt
+        step(U, t, dt); t += dt
     e1.record(stream)
     barrier()
     ms = e0.elapsed_time(e1)
@@ -249,13 +270,13 @@ def run_ours(args):
     Uh.copy_(U)
     Ud = torch.empty_like(U)
     for _ in range(2):
-        Ud.copy_(Uh, non_blocking=True); g.rk3_step(Ud, t, dt); Uh.copy_(Ud, non_blocking=True)
+        Ud.copy_(Uh, non_blocking=True); step(Ud, t, dt); Uh.copy_(Ud, non_blocking=True)
     barrier()
     f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     f0.record(stream)
     for _ in range(args.steps):
         Ud.copy_(Uh, non_blocking=True)          # host -> device copy of this step's input state
-        g.rk3_step(Ud, t, dt)
+        step(Ud, t, dt)
         Uh.copy_(Ud, non_blocking=True)          # device -> host read of the step's result
         t += dt
     f1.record(stream)
@@ -268,6 +289,8 @@ def run_ours(args):
             dist.destroy_process_group()
         return
 
+    # replicas: every rank advances its own copy; slabs: the ranks share one copy (ncell = this rank's slab; the
+    # slabs differ by at most one plane, rank 0 holds a largest one)
     value = whole_job_throughput(ncell, args.steps, world, ms)
     e2e_value = whole_job_throughput(ncell, args.steps, world, ms_e2e)
     hbm, sm_max, peak_src = peaks()
@@ -297,11 +320,12 @@ def run_ours(args):
             "avg_launch_ms": dsec * 1e3,
             "fp64_pipe_peak_Tinst_s_at_sampled_clock": N_SM * FP64_LANES_PER_SM_CLK * clk * 1e6 / 1e12}
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+            "scaling": "strong" if slabs else "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": wl["name"], "cells": ncell, "viscous": prm["viscous"], "moving": prm["moving"],
+            "config": {"workload": wl_name, "cells": ncell * world if slabs else ncell, "viscous": prm["viscous"], "moving": prm["moving"],
                        "scheme": "MIG4" if prm.get("scheme", 0) == 1 else "MEG6",
-                       "dt": dt, "parallelism": "replicas x%d" % world,
+                       "dt": dt, "parallelism": ("zeta slabs x%d, 6-layer halo exchange per stage" if slabs else "replicas x%d") % world,
                        "l2": "working set %.1f GB per stage >> 126 MB L2 (no flush needed)" % (stage_bytes * ncell / 1e9)},
             "clocks": clocks, "gpu_launches": int(launches), "finite": finite,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(U.numel() * 8),
@@ -327,6 +351,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="c4")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--decomp", default="replicas", choices=["replicas", "slabs"],
+                    help="N > 1: independent replicas (weak scaling, default) or one workload cut into zeta slabs "
+                         "with halo exchange (strong scaling)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3
