@@ -26,6 +26,9 @@ namespace meg6 {
 #ifndef MEG6_MINB3_Y
 #define MEG6_MINB3_Y 4
 #endif
+#ifndef MEG6_TS_Y
+#define MEG6_TS_Y 15
+#endif
 #ifndef MEG6_RELOAD
 #define MEG6_RELOAD 1
 #endif
@@ -34,7 +37,7 @@ namespace meg6 {
 // the implicit systems of Eq. 18, computed beforehand for whole grid lines and loaded like the primitives.
 template <int DIR, bool VISC, bool IG4 = false>
 struct Cfg3 {
-  static constexpr int TS = (DIR == 0) ? 30 : 15;            // cells along the sweep per tile
+  static constexpr int TS = (DIR == 0) ? 30 : MEG6_TS_Y;     // cells along the sweep per tile
   static constexpr int TT = (DIR == 0) ? 4 : 8;              // transverse positions (rows for xi, i-lanes otherwise)
   static constexpr int NI = TS + 1;                          // interfaces per pencil
   static constexpr int NT = (DIR == 0) ? 32 * TT : NI * TT;  // threads: one interface each (xi: one warp per row)
