@@ -148,7 +148,7 @@ cudaError_t launch_geometry(meg6_grid* g, double t) {
     const int e0 = c.n[0] + 10, e1 = c.n[1] + 10, e2 = c.n[2] + 10;
     k_met_dir<0><<<dim3(nblk(e0, MetCfg<0>::TS), nblk(e1, MetCfg<0>::TW), e2), 256, 0, g->stream>>>(c, xc, xt, cd, met, mt);
     k_met_dir<1><<<dim3(nblk(e0, MetCfg<1>::TW), nblk(e1, MetCfg<1>::TS), e2), 256, 0, g->stream>>>(c, xc, xt, cd, met, mt);
-    k_met_dir<2><<<dim3(nblk(e0, MetCfg<2>::TW), e1, nblk(e2, MetCfg<2>::TS)), 256, 0, g->stream>>>(c, xc, xt, cd, met, mt);
+    k_met_dir<2><<<dim3(nblk(e0, MetCfg<2>::TW), nblk(e2, MetCfg<2>::TS), e1), 256, 0, g->stream>>>(c, xc, xt, cd, met, mt);
   }
   for (int d = 0; d < 3; ++d) {
     FaceJob job;

@@ -184,7 +184,7 @@ __global__ void __launch_bounds__(256) k_met_dir(Consts c, P3 xc, P3 xt, P9 cd, 
   int o[3];
   if (D == 0) { o[0] = -5 + (int)blockIdx.x * TS; o[1] = -5 + (int)blockIdx.y * TW; o[2] = -5 + (int)blockIdx.z; }
   else if (D == 1) { o[0] = -5 + (int)blockIdx.x * TW; o[1] = -5 + (int)blockIdx.y * TS; o[2] = -5 + (int)blockIdx.z; }
-  else { o[0] = -5 + (int)blockIdx.x * TW; o[1] = -5 + (int)blockIdx.y; o[2] = -5 + (int)blockIdx.z * TS; }
+  else { o[0] = -5 + (int)blockIdx.x * TW; o[1] = -5 + (int)blockIdx.z; o[2] = -5 + (int)blockIdx.y * TS; }   // zeta tiles of a line back to back: halo planes re-used in L2
   constexpr int TD = (D == 0) ? 1 : 0;             // the transverse direction inside the tile
   constexpr int A_RB = (D + 2) % 3, B_RA = (D + 1) % 3;
   const int tid = threadIdx.x;
