@@ -695,3 +695,28 @@ def test_tgv_kinetic_energy_budget_on_gpu(mods):
     visc = 2.0 / re * h[1:-1, 2]
     assert np.all(np.abs(eps / visc - 1.0) < 0.03), (eps / visc)
     g.close()
+
+
+def test_c3_full_size_conservation_and_symmetry_of_the_step(mods):
+    """Config 3 at BASELINE.json's full size (128^3, the launch configuration bench.py --workload c3 times), checked
+    through properties that hold at any size: the sum over cells of (1/J) dQ/dt telescopes to zero on the periodic
+    mesh (Eq. 8-9), and ten RK3 steps conserve the (1/J)-weighted totals of mass, momentum and energy."""
+    torch, O, M = mods
+    wl = W.c3_tgv(n=128)
+    g = M.Grid(wl)
+    g.metrics_compute(0.0)
+    U = torch.as_tensor(wl["U0"], device="cuda").contiguous()
+    rj = torch.as_tensor(g.get_array(0, 9), device="cuda")
+    r = g.rhs(U)
+    tot = (r * rj).reshape(5, -1).sum(1)
+    scale = (r.abs() * rj).reshape(5, -1).sum(1)
+    assert bool(torch.all(tot.abs() <= 1e-11 * torch.clamp(scale, min=1.0))), (tot, scale)
+    q0 = (U * rj).reshape(5, -1).sum(1)
+    dt = g.cfl_dt(U, wl["cfl"])
+    for s in range(10):
+        g.rk3_step(U, s * dt, dt)
+    q1 = (U * rj).reshape(5, -1).sum(1)
+    ref = (U.abs() * rj).reshape(5, -1).sum(1)
+    assert bool(torch.isfinite(U).all())
+    assert bool(torch.all((q1 - q0).abs() <= 1e-11 * ref)), (q1 - q0, ref)
+    g.close()
