@@ -33,15 +33,21 @@ static Box box_and(const Box& a, const Box& b) {
 static long long box_n(const Box& b) { return (long long)(b.hi[0] - b.lo[0]) * (b.hi[1] - b.lo[1]) * (b.hi[2] - b.lo[2]); }
 
 // IG4 gradient of f (valid on fb) along dir into out; returns the valid box of out.  Lay L: layout of both arrays.
-Box launch_ig4(meg6_grid* g, const Lay& L, const double* f, const Box& fb, int dir, double* out) {
+Box launch_ig4_batch(meg6_grid* g, const Lay& L, const double* f, const Box& fb, int dir, double* out, int nfields,
+                     long long fs_in, long long fs_out) {
   Box ob = fb;
   ob.lo[dir] += 2; ob.hi[dir] -= 2;
   const int a1 = (dir == 0) ? 1 : 0, a2 = (dir == 2) ? 1 : 2;
   const long long lines = (long long)(ob.hi[a1] - ob.lo[a1]) * (ob.hi[a2] - ob.lo[a2]);
-  if (dir == 0) k_ig4x<<<nblk(lines, 128), 128, 0, g->stream>>>(L, f, out, ob, g->ig4_cc, g->ig4_den);
-  else if (dir == 1) k_ig4<1><<<nblk(lines, 128), 128, 0, g->stream>>>(L, f, out, ob, g->ig4_cc, g->ig4_den);
-  else k_ig4<2><<<nblk(lines, 128), 128, 0, g->stream>>>(L, f, out, ob, g->ig4_cc, g->ig4_den);
+  const dim3 grid((unsigned)nblk(lines, 128), (unsigned)nfields);
+  if (dir == 0) k_ig4x<<<grid, 128, 0, g->stream>>>(L, f, out, ob, g->ig4_cc, g->ig4_den, fs_in, fs_out);
+  else if (dir == 1) k_ig4<1><<<grid, 128, 0, g->stream>>>(L, f, out, ob, g->ig4_cc, g->ig4_den, fs_in, fs_out);
+  else k_ig4<2><<<grid, 128, 0, g->stream>>>(L, f, out, ob, g->ig4_cc, g->ig4_den, fs_in, fs_out);
   return ob;
+}
+
+Box launch_ig4(meg6_grid* g, const Lay& L, const double* f, const Box& fb, int dir, double* out) {
+  return launch_ig4_batch(g, L, f, fb, dir, out, 1, 0, 0);
 }
 
 // H of f along dir into a cell-layout array (index i = interface i+1/2); returns its valid box

@@ -18,7 +18,11 @@ __device__ __forceinline__ double c4_op(const double* __restrict__ f, long long 
 // out = IG4 gradient of f along DIR on `ob` (= the box of f shrunk by 2 at both ends of DIR).
 template <int DIR>
 __global__ void __launch_bounds__(128) k_ig4(Lay L, const double* __restrict__ f, double* __restrict__ out, Box ob,
-                                             const double* __restrict__ cc, const double* __restrict__ den) {
+                                             const double* __restrict__ cc, const double* __restrict__ den,
+                                             long long fs_in, long long fs_out) {
+  // blockIdx.y = field of a batch (arrays fs_in / fs_out doubles apart): one launch for all fields keeps the grid many
+  // waves deep -- a thread lives as long as its whole line, so a launch of ~2 waves wastes most of its last one
+  f += blockIdx.y * fs_in; out += blockIdx.y * fs_out;
   constexpr int A1 = (DIR == 0) ? 1 : 0, A2 = (DIR == 2) ? 1 : 2;   // transverse directions, lower index fastest
   const int n1 = ob.hi[A1] - ob.lo[A1], n2 = ob.hi[A2] - ob.lo[A2];
   const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -79,7 +83,9 @@ __global__ void __launch_bounds__(128) k_ig4(Lay L, const double* __restrict__ f
 // row out of the tile (row pitch 37: conflict-free), and the results leave the same way.  Operations and their order
 // per cell are those of k_ig4.
 __global__ void __launch_bounds__(128) k_ig4x(Lay L, const double* __restrict__ f, double* out, Box ob,
-                                              const double* __restrict__ cc, const double* __restrict__ den) {
+                                              const double* __restrict__ cc, const double* __restrict__ den,
+                                              long long fs_in, long long fs_out) {
+  f += blockIdx.y * fs_in; out += blockIdx.y * fs_out;
   __shared__ double tile[4][32][37];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   double (*T)[37] = tile[warp];
