@@ -27,11 +27,11 @@ UNIT = "Mcell-updates/s/stage"
 FP64_LANES_PER_SM_CLK = 64
 N_SM = 148
 # DRAM traffic per launch (dram__bytes_read.sum + dram__bytes_write.sum) and FP64-pipe activity of the sweeps on the
-# C4 workload, from the committed `ncu --set full` capture profiles/r1i_ncu.md (never measured by this script)
+# C4 workload, from the committed `ncu --set full` capture profiles/r1j_ncu.md (never measured by this script)
 NCU = {"c4_jet_320x200x200": {
-    "flux_eta": {"traffic": 3.065686e+09, "fp64_pipe_pct": 53.3},
-    "flux_zeta": {"traffic": 3.577720e+09, "fp64_pipe_pct": 48.2},
-    "flux_xi": {"traffic": 5.884570e+09, "fp64_pipe_pct": 37.9}}}
+    "flux_eta": {"traffic": 3.066528e+09, "fp64_pipe_pct": 53.3},
+    "flux_zeta": {"traffic": 3.577876e+09, "fp64_pipe_pct": 48.1},
+    "flux_xi": {"traffic": 5.886825e+09, "fp64_pipe_pct": 45.0}}}
 
 
 def make_workload(name):
@@ -314,7 +314,7 @@ def run_ours(args):
     roof = {"kernel": "k_flux3<%s,%s>" % (dom[5:], "visc" if prm["viscous"] else "inv"), "bound": "hbm",
             "achieved": ach, "peak": hbm, "unit": "GB/s", "frac": ach / hbm,
             "traffic": NCU.get(wl["name"], {}).get(dom, {}).get("traffic"),
-            "traffic_source": "profiles/r1i_ncu.md" if wl["name"] in NCU else None,
+            "traffic_source": "profiles/r1j_ncu.md" if wl["name"] in NCU else None,
             "fp64_pipe_pct_ncu": NCU.get(wl["name"], {}).get(dom, {}).get("fp64_pipe_pct"),
             "peak_source": peak_src, "bytes_per_cell": bpc[dom], "cells_per_launch": ncell,
             "avg_launch_ms": dsec * 1e3,
