@@ -136,6 +136,8 @@ cudaError_t launch_geometry(meg6_grid* g, double t);
 Box launch_ig4(meg6_grid* g, const Lay& L, const double* f, const Box& fb, int dir, double* out);
 Box launch_ig4_batch(meg6_grid* g, const Lay& L, const double* f, const Box& fb, int dir, double* out, int nfields,
                      long long fs_in, long long fs_out);
+Box launch_ig4_flow(meg6_grid* g, const Lay& L, const double* f, const Box& fb, int dir, double* out, int nfields,
+                    long long fs_in, long long fs_out);
 }
 
 // ---- TMA descriptors (cuTensorMapEncodeTiled through the runtime's driver entry point: no libcuda link) ----
@@ -431,7 +433,7 @@ static meg6_status stage_sweeps(meg6_grid* g, int buf, const Fuse3& fu) {
     meg6::Box pb;
     for (int a = 0; a < 3; ++a) { pb.lo[a] = -6; pb.hi[a] = c.n[a] + 6; }
     // the fields of P and of Gi[d] are fsP doubles apart: one launch per direction for all of them
-    for (int d = 0; d < 3; ++d) meg6::launch_ig4_batch(g, c.LP, Pc[0], pb, d, g->Gi[d][0], g->p.viscous ? 6 : 5, c.fsP, c.fsP);
+    for (int d = 0; d < 3; ++d) meg6::launch_ig4_flow(g, c.LP, Pc[0], pb, d, g->Gi[d][0], g->p.viscous ? 6 : 5, c.fsP, c.fsP);
   } else if (g->p.viscous) {
     P12 G;
     for (int e = 0; e < 3; ++e)

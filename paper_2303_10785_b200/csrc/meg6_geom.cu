@@ -1,6 +1,9 @@
 // meg6_geom.cu -- metric / Jacobian kernels and their launcher.  Compiled with -fmad=false (see meg6_geom.cuh).
 #include <math.h>
 #include "meg6_geom.cuh"
+#ifndef MEG6_IG4_SEGMENTED
+#define MEG6_IG4_SEGMENTED 1
+#endif
 #include "meg6_ig4.cuh"
 
 namespace meg6 {
@@ -48,6 +51,24 @@ Box launch_ig4_batch(meg6_grid* g, const Lay& L, const double* f, const Box& fb,
 
 Box launch_ig4(meg6_grid* g, const Lay& L, const double* f, const Box& fb, int dir, double* out) {
   return launch_ig4_batch(g, L, f, fb, dir, out, 1, 0, 0);
+}
+
+// Flow gradients only (rounding order differs from the plain Thomas loop at segment boundaries): the segmented
+// two-pass solve along eta / zeta where the line fits, the plain kernels otherwise and along xi.
+Box launch_ig4_flow(meg6_grid* g, const Lay& L, const double* f, const Box& fb, int dir, double* out, int nfields,
+                    long long fs_in, long long fs_out) {
+  const int m = fb.hi[dir] - fb.lo[dir] - 4;
+  if (!MEG6_IG4_SEGMENTED || dir == 0 || m - 2 > IG4S_NSEG * IG4S_SEGMAX || m < 3)
+    return launch_ig4_batch(g, L, f, fb, dir, out, nfields, fs_in, fs_out);
+  Box ob = fb;
+  ob.lo[dir] += 2; ob.hi[dir] -= 2;
+  const int od = (dir == 1) ? 2 : 1;
+  const dim3 grid((unsigned)nblk(ob.hi[0] - ob.lo[0], IG4S_LANES), (unsigned)(ob.hi[od] - ob.lo[od]), (unsigned)nfields);
+  const int nseg = (m - 2 + IG4S_SEGMAX - 1) / IG4S_SEGMAX;   // segments of (nearly) full length, fewer threads for short lines
+  const int nthr = IG4S_LANES * ((nseg + 1) / 2 * 2);        // whole warps
+  if (dir == 1) k_ig4s<1><<<grid, nthr, 0, g->stream>>>(L, f, out, ob, g->ig4_cc, fs_in, fs_out);
+  else k_ig4s<2><<<grid, nthr, 0, g->stream>>>(L, f, out, ob, g->ig4_cc, fs_in, fs_out);
+  return ob;
 }
 
 // H of f along dir into a cell-layout array (index i = interface i+1/2); returns its valid box

@@ -148,6 +148,91 @@ __global__ void __launch_bounds__(128) k_ig4x(Lay L, const double* __restrict__ 
   }
 }
 
+// Segmented solve for the FLOW gradients along eta / zeta (not for the geometry: the rounding order differs from the
+// plain Thomas loop at the segment boundaries).  The two sweeps of the Thomas algorithm are first-order linear
+// recurrences, d_q = (r_q - alpha d_{q-1}) / den_q and x_q = d_q - c_q x_{q+1}: a line is cut into NSEG segments, each
+// thread runs its segment once with a zero inflow value (which gives the affine map inflow -> outflow, slope = product
+// of the -c_q, ~0.4^length), the maps are chained through shared memory, and the segment is run again from its true
+// inflow value.  Everything between the two passes stays in registers: f is read once and the gradient written once
+// (the one-thread-per-line kernel writes d and reads it back: four array passes instead of two).
+// CTA = 16 xi-lanes (128-byte rows) x NSEG segments, two CTAs per SM; a line has at most NSEG * SEGMAX + 2 unknowns.
+constexpr int IG4S_NSEG = 32, IG4S_SEGMAX = 13, IG4S_LANES = 16;
+template <int DIR>
+__global__ void __launch_bounds__(IG4S_LANES * IG4S_NSEG, 2) k_ig4s(Lay L, const double* __restrict__ f, double* __restrict__ out,
+                                                                  Box ob, const double* __restrict__ cc, long long fs_in,
+                                                                  long long fs_out) {
+  constexpr int NSEG = IG4S_NSEG, SMAX = IG4S_SEGMAX, NL = IG4S_LANES;
+  constexpr int OD = (DIR == 1) ? 2 : 1;            // the other transverse direction (xi is the lane direction)
+  __shared__ double sA[NSEG][NL], sB[NSEG][NL], sX[2][NL];
+  f += blockIdx.z * fs_in; out += blockIdx.z * fs_out;
+  const int lane = threadIdx.x % NL, seg = threadIdx.x / NL;
+  const int n0 = ob.hi[0] - ob.lo[0];
+  const int i = blockIdx.x * NL + lane;
+  const bool act = i < n0;
+  int ix[3];
+  ix[0] = ob.lo[0] + (act ? i : 0); ix[OD] = ob.lo[OD] + blockIdx.y; ix[DIR] = ob.lo[DIR];
+  const int m = ob.hi[DIR] - ob.lo[DIR];            // unknowns 0 .. m-1; 0 and m-1 explicit
+  const long long at = L.at(ix[0], ix[1], ix[2]), s = L.stride(DIR);
+  const double* pf = f + at;
+  double* px = out + at;
+  const double al = 5.0 / 14.0, ial = 14.0 / 5.0, ca = (2.0 + al) / 3.0, cb = (4.0 * al - 1.0) / 12.0;
+  const int nseg = blockDim.x / NL;                 // segments of this launch (<= NSEG)
+  const int len = (m - 2 + nseg - 1) / nseg;        // interior unknowns per segment (<= SMAX)
+  // a segment multiplies its inflow value by the product of its c_q (< 0.42 each): beyond `reach` segments the
+  // contribution is below 0.42^48 = 1e-18 of the value and is not summed
+  const int reach = (48 + len - 1) / len;
+  const int q0 = 1 + seg * len;                     // first unknown of this segment
+  const int nq = max(0, min(len, m - 1 - q0));      // its unknowns
+  const bool last = nq > 0 && q0 + nq == m - 1;     // the segment next to the explicit last unknown
+  double r[SMAX];
+  {
+    double w[SMAX + 4];
+    const double* pw = pf + (long long)(q0 - 2) * s;   // running pointer: one 64-bit add per load instead of a multiply
+#pragma unroll
+    for (int u = 0; u < SMAX + 4; ++u) { w[u] = (nq > 0 && u < nq + 4) ? *pw : 0.0; pw += s; }
+#pragma unroll
+    for (int u = 0; u < SMAX; ++u) r[u] = fma(cb, w[u + 4] - w[u], ca * (w[u + 3] - w[u + 1]));
+  }
+  if (seg == 0) sX[0][lane] = c4_op(pf, s);                              // first unknown: explicit (R26)
+  if (last) sX[1][lane] = c4_op(pf + (long long)(m - 1) * s, s);         // last unknown: explicit
+  const double* __restrict__ cs = cc + q0;                               // c_q = alpha / den_q, position only
+  // ---- forward sweep: d_q = (r_q - alpha d_{q-1}) / den_q, 1/den_q = c_q / alpha ----
+  {
+    double a = 0.0, b = 1.0;
+#pragma unroll
+    for (int u = 0; u < SMAX; ++u)
+      if (u < nq) { const double c = __ldg(cs + u); a = fma(-al, a, r[u]) * (c * ial); b = -c * b; }
+    sA[seg][lane] = a; sB[seg][lane] = b;
+  }
+  __syncthreads();
+  double din = (seg <= reach) ? sX[0][lane] : 0.0;
+  for (int t = max(0, seg - reach); t < seg; ++t) din = fma(sB[t][lane], din, sA[t][lane]);
+#pragma unroll
+  for (int u = 0; u < SMAX; ++u)
+    if (u < nq) { din = fma(-al, din, r[u]) * (__ldg(cs + u) * ial); r[u] = din; }
+  __syncthreads();
+  // ---- backward sweep: x_q = d_q - c_q x_{q+1} ----
+  {
+    double a = 0.0, b = 1.0;
+#pragma unroll
+    for (int u = SMAX - 1; u >= 0; --u)
+      if (u < nq) { const double c = __ldg(cs + u); a = fma(-c, a, r[u]); b = -c * b; }
+    sA[seg][lane] = a; sB[seg][lane] = b;
+  }
+  __syncthreads();
+  double xin = (seg + reach >= nseg - 1) ? sX[1][lane] : 0.0;
+  for (int t = min(nseg - 1, seg + reach); t > seg; --t) xin = fma(sB[t][lane], xin, sA[t][lane]);
+  if (!act) return;
+  double* po = px + (long long)(q0 + SMAX - 1) * s;
+#pragma unroll
+  for (int u = SMAX - 1; u >= 0; --u) {
+    if (u < nq) { xin = fma(-__ldg(cs + u), xin, r[u]); *po = xin; }
+    po -= s;
+  }
+  if (seg == 0) px[0] = sX[0][lane];
+  if (last) px[(long long)(m - 1) * s] = sX[1][lane];
+}
+
 // Central interface value Eq. 36/38 from f and its gradient f1: index i of `out` = interface between
 // cells i and i+1 along dir.  The second derivative is Eq. 19.  `out` may have another layout (interface
 // arrays): LO, and an index shift `sh` along dir (interface arrays number the face between cells i-1 and i as i).
