@@ -720,3 +720,39 @@ def test_c3_full_size_conservation_and_symmetry_of_the_step(mods):
     assert bool(torch.isfinite(U).all())
     assert bool(torch.all((q1 - q0).abs() <= 1e-11 * ref)), (q1 - q0, ref)
     g.close()
+
+
+def test_full_step_counts_of_configs_3_4_5_stay_finite_and_bounded(mods):
+    """BASELINE.json's step counts at full size on the GPU: config 3 (128^3, 200 RK3 steps), config 4 (320x200x200,
+    500 steps: the jet starts up, shocks form at the nozzle lip, the limiter becomes active) and the MIG4 variant
+    (config 5's flow at 192^3, 50 steps).  The oracle would need hours for these; the checks are properties: finite
+    state, positive density and pressure, kinetic energy of the Taylor-Green vortex decaying."""
+    torch, O, M = mods
+
+    def run(wl, steps, cfl=None):
+        g = M.Grid(wl)
+        g.metrics_compute(0.0)
+        U = torch.as_tensor(wl["U0"], device="cuda").contiguous()
+        dt = wl["dt"] if wl["dt"] else g.cfl_dt(U, cfl or wl["cfl"])
+        ke0 = g.diagnostics(U)[0]
+        for s in range(steps):
+            g.rk3_step(U, s * dt, dt)
+        assert bool(torch.isfinite(U).all())
+        rho = U[0]
+        p = 0.4 * (U[4] - 0.5 * (U[1] ** 2 + U[2] ** 2 + U[3] ** 2) / rho)
+        assert float(rho.min()) > 0.0 and float(p.min()) > 0.0
+        ke1 = g.diagnostics(U)[0]
+        g.limiter_stats_enable(True)
+        g.rk3_step(U, steps * dt, dt)
+        lim, tst = g.limiter_stats()
+        g.close()
+        return ke0, ke1, lim / tst
+
+    ke0, ke1, _ = run(W.c3_tgv(n=128), 200)
+    assert 0.9 * ke0 < ke1 < ke0
+    ke0, ke1, _ = run(W.c5_tgv_mig4(n=192), 50)
+    assert 0.95 * ke0 < ke1 < ke0
+    ke0, ke1, frac = run(W.c4_jet(), 500)
+    assert ke1 > ke0                     # the jet has entered the quiescent domain
+    assert frac > 1e-4                   # and the limiter is at work
+    print("C4 after 500 steps: limited fraction %.4f" % frac)
