@@ -29,12 +29,6 @@ namespace meg6 {
 #ifndef MEG6_PF
 #define MEG6_PF 1
 #endif
-#ifndef MEG6_BULK_PF
-#define MEG6_BULK_PF 0
-#endif
-#ifndef MEG6_TAIL_LOADS_FIRST
-#define MEG6_TAIL_LOADS_FIRST 1
-#endif
 #ifndef MEG6_TS_Y
 #define MEG6_TS_Y 15
 #endif
@@ -424,35 +418,6 @@ k_flux3(const Consts c, const FluxIn3 in, const __grid_constant__ TmaMaps tm, co
       }
     }
   }
-#if MEG6_BULK_PF
-  if (DIR == 0 && FUSE) {
-    // L2 prefetch of what the final phase will read from global memory (running residual, U, U0, 1/J, sponge):
-    // one bulk prefetch per (array, tile row) -- a row is TS contiguous doubles -- issued by one thread each
-    constexpr int NARR = 22;
-    if (tid < NARR * TT) {
-      const int arr = tid / TT, rr = tid % TT;
-      const int ci = s0, cj = t0 + rr, ck = o;
-      if (ci < c.n[0] && cj < c.n[1]) {
-        const long long N = c.LC.n;
-        const double* ptr = nullptr;
-        if (arr < 5) ptr = in.first ? nullptr : in.res + arr * c.fsR + c.LR.at(ci, cj, ck);
-        else {
-          const long long ic = c.LC.at(ci, cj, ck);
-          if (arr < 10) ptr = fu.U + (arr - 5) * N + ic;
-          else if (arr < 15) ptr = (fu.mode == 1 && fu.a != 0.0) ? fu.U0 + (arr - 10) * N + ic : nullptr;
-          else if (arr < 20) ptr = fu.sigma ? fu.uref + (arr - 15) * N + ic : nullptr;
-          else if (arr == 20) ptr = fu.sigma ? fu.sigma + ic : nullptr;
-          else ptr = fu.rj + c.LX.at(ci, cj, ck);
-        }
-        if (ptr) {
-          const int nrow = min(TS, c.n[0] - ci);
-          const unsigned long long a0 = (unsigned long long)ptr & ~15ull, a1 = (unsigned long long)(ptr + nrow) & ~15ull;
-          if (a1 > a0) asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(a0), "r"((unsigned)(a1 - a0)) : "memory");
-        }
-      }
-    }
-  } else
-#endif
   if (MEG6_PF && (FUSE || !in.first)) {
     // L2 prefetch of what the final phase will read from global memory (running residual; fused: U, U0, 1/J,
     // sponge): those loads sit at the tail of the CTA with nothing to overlap them
@@ -629,7 +594,6 @@ k_flux3(const Consts c, const FluxIn3 in, const __grid_constant__ TmaMaps tm, co
       else if (DIR == 1) { ci = t0 + t; cj = s0 + s; ck = o; }
       else { ci = t0 + t; cj = o; ck = s0 + s; }
       const long long N = c.LC.n, ic = c.LC.at(ci, cj, ck);
-#if MEG6_TAIL_LOADS_FIRST
       // every load of the phase before its first store: U, U0w and out may be the same memory as far as the compiler
       // knows, so a store between two loads would chain their latencies one after the other
       const double rjv = fu.rj[c.LX.at(ci, cj, ck)];
@@ -663,27 +627,6 @@ k_flux3(const Consts c, const FluxIn3 in, const __grid_constant__ TmaMaps tm, co
       }
 #pragma unroll
       for (int f = 0; f < 5; ++f) fu.out[f * N + ic] = Q[f];
-#else
-      const double J = 1.0 / fu.rj[c.LX.at(ci, cj, ck)];
-      const double rjt = fu.rjt ? fu.rjt[ic] : 0.0;
-      const double sg = fu.sigma ? fu.sigma[ic] : 0.0;
-      double Q[5];
-#pragma unroll
-      for (int f = 0; f < 5; ++f) {
-        const double u = fu.U[f * N + ic];
-        double L = J * (R[f] - rjt * u);
-        if (sg != 0.0) L -= sg * (u - fu.uref[f * N + ic]);   // sigma = 0 outside the sponge: Q_ref is not read there
-        if (fu.mode == 0) Q[f] = L;
-        else {
-          double v = u + fu.dt * L;
-          if (fu.a != 0.0) v = fu.a * fu.U0[f * N + ic] + fu.b * v;
-          else if (fu.U0w) fu.U0w[f * N + ic] = u;
-          Q[f] = v;
-        }
-      }
-#pragma unroll
-      for (int f = 0; f < 5; ++f) fu.out[f * N + ic] = Q[f];
-#endif
       if (fu.Pn) {   // Q -> P of the new state (Eq. 5, P:83 inverted; T = p/(rho R)), as k_prim
         const double r = Q[0], ir = 1.0 / r;
         const double u = Q[1] * ir, v = Q[2] * ir, w = Q[3] * ir;
