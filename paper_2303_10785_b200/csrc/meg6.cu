@@ -214,6 +214,10 @@ static bool make_maps3_dir(EncodeTiledFn fn, meg6_grid* g, int buf) {
     box(C::LG, C::TT, 4, b);
     ok = ok && make_map4(fn, &t.G, g->G[0][0], c.LG, c.fsG, 12, b);
   }
+  if (C::nR) {   // running residual of the tile, read by the second sweep
+    box(C::TS, C::TT, 5, b);
+    ok = ok && make_map4(fn, &t.R, g->res, c.LR, c.fsR, 5, b);
+  }
   return ok;
 }
 

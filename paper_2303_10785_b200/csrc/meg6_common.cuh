@@ -72,7 +72,7 @@ struct Consts {   // per-grid constants passed by value to kernels
 
 // P primitives, M interface metrics, Mt time metric, G stored tangential gradients (MEG6); MIG4: Q = implicit
 // gradients along the sweep, G3[s] = gradients (u,v,w,p,T) of tangential direction s
-namespace meg6 { struct TmaMaps { CUtensorMap P, M, Mt, G, Q, G3[2]; }; }
+namespace meg6 { struct TmaMaps { CUtensorMap P, M, Mt, G, Q, G3[2], R; }; }   // R: running residual (eta/zeta, MEG6)
 
 struct meg6_grid {
   meg6_params p;

@@ -29,6 +29,9 @@ namespace meg6 {
 #ifndef MEG6_PF
 #define MEG6_PF 1
 #endif
+#ifndef MEG6_RES_TMA
+#define MEG6_RES_TMA 1
+#endif
 #ifndef MEG6_TS_Y
 #define MEG6_TS_Y 15
 #endif
@@ -64,8 +67,11 @@ struct Cfg3 {
   static constexpr int nP = NF * LP * TT, nA = 10 * LA * TT, nT1 = (VISC && !IG4) ? LT * TT : 0, nM = NMF * LF * TT,
                        nMt = LF * TT, nG = VISC ? GSLOT + GFLD * LG * TT : 0, nGtx = VISC ? 2 * GFLD * LG * TT : 0,
                        nQ = IG4 ? NF * LQ * TT : 0;
+  // eta/zeta sweeps, MEG6: the running residual of the tile arrives by TMA with the metrics (it is needed at the very
+  // end of the CTA; as plain loads behind an L2 prefetch it cost the second sweep 0.09 ms against the first)
+  static constexpr int nR = (DIR != 0 && !IG4 && MEG6_RES_TMA) ? 5 * TS * TT : 0;
   static constexpr int oP = 0, oM = oP + al(nP), oMt = oM + al(nM), oG = oMt + al(nMt), oQ = oG + al(nG), oA = oQ + al(nQ),
-                       oT1 = oA + al(nA), oBar = oT1 + al(nT1);
+                       oT1 = oA + al(nA), oR = oT1 + al(nT1), oBar = oR + al(nR);
   static constexpr int SMEM_BYTES = (oBar + 2) * 8;   // two mbarriers
 };
 
@@ -385,6 +391,7 @@ k_flux3(const Consts c, const FluxIn3 in, const __grid_constant__ TmaMaps tm, co
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     uint32_t bytes1 = (C::NM * LF * TT + C::nGtx) * 8;
     if (in.moving) bytes1 += C::nMt * 8;
+    if (C::nR && !in.first) bytes1 += C::nR * 8;
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32_3(bar)), "r"((C::nP + C::nQ) * 8) : "memory");
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32_3(bar + 1)), "r"(bytes1) : "memory");
     // box coordinates are (i, j, k, field) in the padded layout of each array: sweep start, transverse start, other
@@ -405,6 +412,7 @@ k_flux3(const Consts c, const FluxIn3 in, const __grid_constant__ TmaMaps tm, co
     coords(s0, t0, o, 0, 0, 0, c0, c1, c2);
     tma4(sM, &tm.M, bar + 1, c0, c1, c2, 0);
     if (in.moving) tma4(sMt, &tm.Mt, bar + 1, c0, c1, c2, 0);
+    if (C::nR && !in.first) tma4(sm3 + C::oR, &tm.R, bar + 1, c0, c1, c2, 0);   // LR has no ghosts: same coordinates
     if (VISC) {
       coords(s0 + GS, t0, o, GGI, GGJ, GGK, c0, c1, c2);
       if (!IG4) {
@@ -418,7 +426,7 @@ k_flux3(const Consts c, const FluxIn3 in, const __grid_constant__ TmaMaps tm, co
       }
     }
   }
-  if (MEG6_PF && (FUSE || !in.first)) {
+  if (MEG6_PF && (FUSE || (!in.first && !C::nR))) {
     // L2 prefetch of what the final phase will read from global memory (running residual; fused: U, U0, 1/J,
     // sponge): those loads sit at the tail of the CTA with nothing to overlap them
     constexpr int NROW = (DIR == 0) ? TT : TS;                  // tile rows that are contiguous in memory
@@ -580,7 +588,7 @@ k_flux3(const Consts c, const FluxIn3 in, const __grid_constant__ TmaMaps tm, co
     double old[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
     if (!in.first) {
 #pragma unroll
-      for (int f = 0; f < 5; ++f) old[f] = in.res[f * c.fsR + ac];
+      for (int f = 0; f < 5; ++f) old[f] = C::nR ? (sm3 + C::oR)[sidx3<DIR, TT>(f, s, t, TS)] : in.res[f * c.fsR + ac];
     }
     double R[5];
 #pragma unroll
