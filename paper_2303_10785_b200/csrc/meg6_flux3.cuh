@@ -32,6 +32,9 @@ namespace meg6 {
 #ifndef MEG6_RES_TMA
 #define MEG6_RES_TMA 1
 #endif
+#ifndef MEG6_RES_TMA_XI
+#define MEG6_RES_TMA_XI 1
+#endif
 #ifndef MEG6_TS_Y
 #define MEG6_TS_Y 15
 #endif
@@ -69,7 +72,7 @@ struct Cfg3 {
                        nQ = IG4 ? NF * LQ * TT : 0;
   // eta/zeta sweeps, MEG6: the running residual of the tile arrives by TMA with the metrics (it is needed at the very
   // end of the CTA; as plain loads behind an L2 prefetch it cost the second sweep 0.09 ms against the first)
-  static constexpr int nR = (DIR != 0 && !IG4 && MEG6_RES_TMA) ? 5 * TS * TT : 0;
+  static constexpr int nR = (!IG4 && MEG6_RES_TMA && (DIR != 0 || MEG6_RES_TMA_XI)) ? 5 * TS * TT : 0;
   static constexpr int oP = 0, oM = oP + al(nP), oMt = oM + al(nM), oG = oMt + al(nMt), oQ = oG + al(nG), oA = oQ + al(nQ),
                        oT1 = oA + al(nA), oR = oT1 + al(nT1), oBar = oR + al(nR);
   static constexpr int SMEM_BYTES = (oBar + 2) * 8;   // two mbarriers
@@ -441,7 +444,7 @@ k_flux3(const Consts c, const FluxIn3 in, const __grid_constant__ TmaMaps tm, co
       else { ci = t0; cj = o; ck = s0 + rr; }
       if (ci >= c.n[0] || cj >= c.n[1] || ck >= c.n[2]) continue;
       const double* ptr = nullptr;
-      if (arr < 5) ptr = in.first ? nullptr : in.res + arr * c.fsR + c.LR.at(ci, cj, ck);
+      if (arr < 5) ptr = (in.first || C::nR) ? nullptr : in.res + arr * c.fsR + c.LR.at(ci, cj, ck);
       else {
         const long long ic = c.LC.at(ci, cj, ck);
         if (arr < 10) ptr = fu.U + (arr - 5) * N + ic;
