@@ -234,6 +234,15 @@ static cudaError_t setup_tma(meg6_grid* g) {
     else ok = make_maps3_dir<0, false>(fn, g, buf) && make_maps3_dir<1, false>(fn, g, buf) && make_maps3_dir<2, false>(fn, g, buf);
   }
   if (!ok) return cudaErrorInvalidValue;
+  // final phase of the fused xi sweep (MEG6): U^n and 1/J tiles; sigma and the caller's U are encoded when they are known
+  g->encode_fn = (void*)fn;
+  g->mapU_ptr = nullptr; g->mapSg_ptr = nullptr;
+  g->tail_ok = g->p.scheme == 0 && (g->c.n[0] % 2 == 0) && Cfg3<0, true>::nU > 0;
+  if (g->tail_ok) {
+    const int b5[4] = {Cfg3<0, true>::TS, Cfg3<0, true>::TT, 1, 5}, b1[4] = {Cfg3<0, true>::TS, Cfg3<0, true>::TT, 1, 1};
+    g->tail_ok = make_map4(fn, &g->mapU0, g->U0, g->c.LC, g->c.LC.n, 5, b5) &&
+                 make_map4(fn, &g->mapJ, g->rj, g->c.LX, g->c.LX.n, 1, b1);
+  }
   // opt in to the dynamic shared memory the flux kernels need
 #define SET_SMEM3(D, V, F)                                                                                  \
   if ((e = cudaFuncSetAttribute(k_flux3<D, V, F>, cudaFuncAttributeMaxDynamicSharedMemorySize,              \
@@ -448,7 +457,8 @@ static meg6_status stage_sweeps(meg6_grid* g, int buf, const Fuse3& fu) {
   FluxIn3 i3;
   i3.res = g->res; i3.stats = g->stats_on ? g->stats : nullptr; i3.moving = g->p.moving ? 1 : 0;
   const bool V = g->p.viscous != 0;
-  const TmaMaps* tm = g->tmaps3[buf];
+  TmaMaps tm[3] = {g->tmaps3[buf][0], g->tmaps3[buf][1], g->tmaps3[buf][2]};
+  if (fu.tail_tma) { tm[0].U = g->mapU; tm[0].U0 = g->mapU0; tm[0].J = g->mapJ; if (g->sigma) tm[0].Sg = g->mapSg; }
 #define LAUNCH3(D, VV, FF, GRID)                                                                                        \
   do {                                                                                                                  \
     if (IG) k_flux3<D, VV, FF, true><<<GRID, Cfg3<D, VV, true>::NT, Cfg3<D, VV, true>::SMEM_BYTES, g->stream>>>(c, i3, tm[D], fu); \
@@ -495,6 +505,18 @@ static Fuse3 make_fuse(meg6_grid* g, const double* U, double* out) {
   fu.U = U; fu.out = out; fu.U0 = g->U0;
   fu.rj = g->rj; fu.rjt = g->p.moving ? g->rjt : nullptr;
   fu.sigma = g->sigma; fu.uref = g->uref;
+  // tensor maps of the caller's arrays, re-encoded only when a pointer changes
+  fu.tail_tma = 0;
+  if (g->tail_ok && (reinterpret_cast<uintptr_t>(U) & 15) == 0 && (!g->sigma || (reinterpret_cast<uintptr_t>(g->sigma) & 15) == 0)) {
+    EncodeTiledFn fn = (EncodeTiledFn)g->encode_fn;
+    const int b5[4] = {Cfg3<0, true>::TS, Cfg3<0, true>::TT, 1, 5}, b1[4] = {Cfg3<0, true>::TS, Cfg3<0, true>::TT, 1, 1};
+    bool ok = true;
+    if (g->mapU_ptr != U) { ok = make_map4(fn, &g->mapU, U, g->c.LC, g->c.LC.n, 5, b5); g->mapU_ptr = ok ? U : nullptr; }
+    if (ok && g->sigma && g->mapSg_ptr != g->sigma) {
+      ok = make_map4(fn, &g->mapSg, g->sigma, g->c.LC, g->c.LC.n, 1, b1); g->mapSg_ptr = ok ? g->sigma : nullptr;
+    }
+    fu.tail_tma = ok ? 1 : 0;
+  }
   return fu;
 }
 

@@ -72,11 +72,16 @@ struct Consts {   // per-grid constants passed by value to kernels
 
 // P primitives, M interface metrics, Mt time metric, G stored tangential gradients (MEG6); MIG4: Q = implicit
 // gradients along the sweep, G3[s] = gradients (u,v,w,p,T) of tangential direction s
-namespace meg6 { struct TmaMaps { CUtensorMap P, M, Mt, G, Q, G3[2], R; }; }   // R: running residual (eta/zeta, MEG6)
+// R: running residual; U, U0, J, Sg: the caller's state, U^n, 1/J and the sponge coefficient (final phase of the fused xi sweep)
+namespace meg6 { struct TmaMaps { CUtensorMap P, M, Mt, G, Q, G3[2], R, U, U0, J, Sg; }; }
 
 struct meg6_grid {
   meg6_params p;
   meg6::TmaMaps tmaps3[2][3];   // per primitive buffer and sweep direction
+  // tensor maps of the fused final phase: U^n and 1/J (fixed), sigma (set_sponge), the caller's U (re-encoded when the
+  // pointer changes); tail_ok: the layouts allow them (even ni: every global stride a multiple of 16 bytes)
+  void* encode_fn; bool tail_ok;
+  CUtensorMap mapU0, mapJ, mapSg, mapU; const double* mapU_ptr; const double* mapSg_ptr;
   meg6::Consts c;
   cudaStream_t stream;
   char* ws; size_t ws_bytes;

@@ -32,6 +32,9 @@ namespace meg6 {
 #ifndef MEG6_RES_TMA
 #define MEG6_RES_TMA 1
 #endif
+#ifndef MEG6_TAIL_TMA
+#define MEG6_TAIL_TMA 1
+#endif
 #ifndef MEG6_RES_TMA_XI
 #define MEG6_RES_TMA_XI 1
 #endif
@@ -73,8 +76,12 @@ struct Cfg3 {
   // eta/zeta sweeps, MEG6: the running residual of the tile arrives by TMA with the metrics (it is needed at the very
   // end of the CTA; as plain loads behind an L2 prefetch it cost the second sweep 0.09 ms against the first)
   static constexpr int nR = (!IG4 && MEG6_RES_TMA && (DIR != 0 || MEG6_RES_TMA_XI)) ? 5 * TS * TT : 0;
+  // fused xi sweep, MEG6: what the final phase reads besides the residual -- U (5), U^n (5), 1/J, sigma -- as four more
+  // boxes on the same barrier (replaces an L2-prefetch loop of 10 % of the kernel's instructions and 12 late loads)
+  static constexpr int nU = (DIR == 0 && !IG4 && MEG6_TAIL_TMA) ? 5 * TS * TT : 0, n1 = nU ? TS * TT : 0;
   static constexpr int oP = 0, oM = oP + al(nP), oMt = oM + al(nM), oG = oMt + al(nMt), oQ = oG + al(nG), oA = oQ + al(nQ),
-                       oT1 = oA + al(nA), oR = oT1 + al(nT1), oBar = oR + al(nR);
+                       oT1 = oA + al(nA), oR = oT1 + al(nT1), oU = oR + al(nR), oU0 = oU + al(nU), oJ = oU0 + al(nU),
+                       oSg = oJ + al(n1), oBar = oSg + al(n1);
   static constexpr int SMEM_BYTES = (oBar + 2) * 8;   // two mbarriers
 };
 
@@ -102,6 +109,7 @@ struct Fuse3 {
   double* Pn;                   // next primitive buffer (field 0; stride fsP) or null
   double a, b, dt;
   int mode;
+  int tail_tma;                 // U, U0, 1/J, sigma of the tile come by TMA (maps valid)
 };
 
 __device__ __forceinline__ uint32_t smem_u32_3(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -395,6 +403,8 @@ k_flux3(const Consts c, const FluxIn3 in, const __grid_constant__ TmaMaps tm, co
     uint32_t bytes1 = (C::NM * LF * TT + C::nGtx) * 8;
     if (in.moving) bytes1 += C::nMt * 8;
     if (C::nR && !in.first) bytes1 += C::nR * 8;
+    const bool ttma = C::nU && FUSE && fu.tail_tma;
+    if (ttma) bytes1 += (C::nU + C::n1 + ((fu.mode == 1 && fu.a != 0.0) ? C::nU : 0) + (fu.sigma ? C::n1 : 0)) * 8;
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32_3(bar)), "r"((C::nP + C::nQ) * 8) : "memory");
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32_3(bar + 1)), "r"(bytes1) : "memory");
     // box coordinates are (i, j, k, field) in the padded layout of each array: sweep start, transverse start, other
@@ -416,6 +426,12 @@ k_flux3(const Consts c, const FluxIn3 in, const __grid_constant__ TmaMaps tm, co
     tma4(sM, &tm.M, bar + 1, c0, c1, c2, 0);
     if (in.moving) tma4(sMt, &tm.Mt, bar + 1, c0, c1, c2, 0);
     if (C::nR && !in.first) tma4(sm3 + C::oR, &tm.R, bar + 1, c0, c1, c2, 0);   // LR has no ghosts: same coordinates
+    if (ttma) {
+      tma4(sm3 + C::oU, &tm.U, bar + 1, c0, c1, c2, 0);
+      if (fu.mode == 1 && fu.a != 0.0) tma4(sm3 + C::oU0, &tm.U0, bar + 1, c0, c1, c2, 0);
+      if (fu.sigma) tma4(sm3 + C::oSg, &tm.Sg, bar + 1, c0, c1, c2, 0);
+      tma4(sm3 + C::oJ, &tm.J, bar + 1, c0 + GX, c1 + GX, c2 + GX, 0);
+    }
     if (VISC) {
       coords(s0 + GS, t0, o, GGI, GGJ, GGK, c0, c1, c2);
       if (!IG4) {
@@ -429,7 +445,7 @@ k_flux3(const Consts c, const FluxIn3 in, const __grid_constant__ TmaMaps tm, co
       }
     }
   }
-  if (MEG6_PF && (FUSE || (!in.first && !C::nR))) {
+  if (MEG6_PF && ((FUSE && !(C::nU && fu.tail_tma)) || (!FUSE && !in.first && !C::nR))) {
     // L2 prefetch of what the final phase will read from global memory (running residual; fused: U, U0, 1/J,
     // sponge): those loads sit at the tail of the CTA with nothing to overlap them
     constexpr int NROW = (DIR == 0) ? TT : TS;                  // tile rows that are contiguous in memory
@@ -607,15 +623,17 @@ k_flux3(const Consts c, const FluxIn3 in, const __grid_constant__ TmaMaps tm, co
       const long long N = c.LC.n, ic = c.LC.at(ci, cj, ck);
       // every load of the phase before its first store: U, U0w and out may be the same memory as far as the compiler
       // knows, so a store between two loads would chain their latencies one after the other
-      const double rjv = fu.rj[c.LX.at(ci, cj, ck)];
+      const bool tt = C::nU && fu.tail_tma;          // DIR == 0 here: the tile row t, cell s
+      const int st = (C::nU ? t * TS + s : 0);
+      const double rjv = tt ? (sm3 + C::oJ)[st] : fu.rj[c.LX.at(ci, cj, ck)];
       const double rjt = fu.rjt ? fu.rjt[ic] : 0.0;
-      const double sg = fu.sigma ? fu.sigma[ic] : 0.0;
+      const double sg = fu.sigma ? (tt ? (sm3 + C::oSg)[st] : fu.sigma[ic]) : 0.0;
       const bool blend = fu.mode == 1 && fu.a != 0.0;
       double uu[5], ur[5], u0[5];
 #pragma unroll
-      for (int f = 0; f < 5; ++f) uu[f] = fu.U[f * N + ic];
+      for (int f = 0; f < 5; ++f) uu[f] = tt ? (sm3 + C::oU)[f * TT * TS + st] : fu.U[f * N + ic];
 #pragma unroll
-      for (int f = 0; f < 5; ++f) u0[f] = blend ? fu.U0[f * N + ic] : 0.0;
+      for (int f = 0; f < 5; ++f) u0[f] = blend ? (tt ? (sm3 + C::oU0)[f * TT * TS + st] : fu.U0[f * N + ic]) : 0.0;
 #pragma unroll
       for (int f = 0; f < 5; ++f) ur[f] = (sg != 0.0) ? fu.uref[f * N + ic] : 0.0;   // sigma = 0 outside the sponge: Q_ref is not read there
       const double J = 1.0 / rjv;
