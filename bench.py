@@ -27,11 +27,11 @@ UNIT = "Mcell-updates/s/stage"
 FP64_LANES_PER_SM_CLK = 64
 N_SM = 148
 # DRAM traffic per launch (dram__bytes_read.sum + dram__bytes_write.sum) and FP64-pipe activity of the sweeps on the
-# C4 workload, from the committed `ncu --set full` capture profiles/r1j_ncu.md (never measured by this script)
+# C4 workload, from the committed `ncu --set full` capture profiles/r1l_ncu.md (never measured by this script)
 NCU = {"c4_jet_320x200x200": {
-    "flux_eta": {"traffic": 3.066528e+09, "fp64_pipe_pct": 53.3},
-    "flux_zeta": {"traffic": 3.577876e+09, "fp64_pipe_pct": 48.1},
-    "flux_xi": {"traffic": 5.886825e+09, "fp64_pipe_pct": 45.0}}}
+    "flux_eta": {"traffic": 3.068790e+09, "fp64_pipe_pct": 53.5},
+    "flux_zeta": {"traffic": 3.578168e+09, "fp64_pipe_pct": 52.3},
+    "flux_xi": {"traffic": 5.485381e+09, "fp64_pipe_pct": 46.7}}}
 
 
 def make_workload(name):
@@ -331,7 +331,7 @@ def run_ours(args):
     roof = {"kernel": "k_flux3<%s,%s>" % (dom[5:], "visc" if prm["viscous"] else "inv"), "bound": "hbm",
             "achieved": ach, "peak": hbm, "unit": "GB/s", "frac": ach / hbm,
             "traffic": NCU.get(wl["name"], {}).get(dom, {}).get("traffic"),
-            "traffic_source": "profiles/r1j_ncu.md" if wl["name"] in NCU else None,
+            "traffic_source": "profiles/r1l_ncu.md" if wl["name"] in NCU else None,
             "fp64_pipe_pct_ncu": NCU.get(wl["name"], {}).get(dom, {}).get("fp64_pipe_pct"),
             "peak_source": peak_src, "bytes_per_cell": bpc[dom], "cells_per_launch": ncell,
             "avg_launch_ms": dsec * 1e3,
