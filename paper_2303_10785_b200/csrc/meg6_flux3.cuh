@@ -44,16 +44,22 @@ namespace meg6 {
 #ifndef MEG6_RELOAD
 #define MEG6_RELOAD 1
 #endif
+#ifndef MEG6_TT_Y
+#define MEG6_TT_Y 8
+#endif
+#ifndef MEG6_BLK_Y
+#define MEG6_BLK_Y 5
+#endif
 
 // IG4 = MIG4 variant (scheme 1): the sweep-direction gradients P' are not E6 stencils of the tile but solutions of
 // the implicit systems of Eq. 18, computed beforehand for whole grid lines and loaded like the primitives.
 template <int DIR, bool VISC, bool IG4 = false>
 struct Cfg3 {
   static constexpr int TS = (DIR == 0) ? 30 : MEG6_TS_Y;     // cells along the sweep per tile
-  static constexpr int TT = (DIR == 0) ? 4 : 8;              // transverse positions (rows for xi, i-lanes otherwise)
+  static constexpr int TT = (DIR == 0) ? 4 : MEG6_TT_Y;              // transverse positions (rows for xi, i-lanes otherwise)
   static constexpr int NI = TS + 1;                          // interfaces per pencil
   static constexpr int NT = (DIR == 0) ? 32 * TT : NI * TT;  // threads: one interface each (xi: one warp per row)
-  static constexpr int MINB = IG4 ? 4 : (DIR == 0) ? MEG6_MINB3_X : MEG6_MINB3_Y;
+  static constexpr int MINB = (DIR == 0) ? (IG4 ? 4 : MEG6_MINB3_X) : (IG4 ? 4 : MEG6_MINB3_Y) * 8 / MEG6_TT_Y;
   static constexpr int NF = VISC ? 6 : 5;                    // staged fields (T only for the viscous flux)
   static constexpr int NM = VISC ? 10 : 3;                   // interface metrics loaded
   static constexpr int NMF = NM > 5 ? NM : 5;                // the metric region later receives the 5 fluxes
@@ -515,7 +521,7 @@ k_flux3(const Consts c, const FluxIn3 in, const __grid_constant__ TmaMaps tm, co
   } else if (DIR != 0) {
     // eta/zeta sweeps: the sweep index is the slow one in shared memory, so one thread takes BLK consecutive cells
     // of one lane and field: BLK + 8 loads instead of 9 BLK (shared-memory bandwidth was at 55-60 % of peak, r1c)
-    constexpr int BLK = 5, NQ = (LA + BLK - 1) / BLK;
+    constexpr int BLK = MEG6_BLK_Y, NQ = (LA + BLK - 1) / BLK;
     for (int it = tid; it < NQ * TT * 5; it += NT) {
       const int t = it % TT, qd = (it / TT) % NQ, f = it / (TT * NQ);
       const int a0 = qd * BLK;

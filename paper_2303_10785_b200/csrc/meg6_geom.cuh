@@ -90,6 +90,19 @@ __global__ void __launch_bounds__(256) k_extend(Consts c, int d, P3 xc, P3 xt) {
 // the order the discretisation states them.  This translation unit is compiled with -fmad=false: at low Mach
 // number a relative metric perturbation of 1e-15 is amplified by p/(rho u^2 k h) ~ 1e4 in the flux
 // difference, so the metric arithmetic is kept free of contraction-dependent rounding.
+// x / 12, correctly rounded, in three operations instead of the division sequence (the metric kernels are bound by the
+// FP64 pipe, ncu r1m, and delta_vals divides three times).  y = RN(1/12); q = RN(x y) is within 1.5 ulp of x/12;
+// r = x - 12 q is exact (a multiple of 4 ulp(q), at most 18 ulp(q)); q + r y differs from x/12 by less than 2e-16 ulp(q),
+// while x/12 = (x/3)/4 sits on a third of an ulp -- at least 1/6 ulp from every rounding boundary -- so the last
+// rounding gives RN(x/12), the value the oracle's division gives (no overflow or underflow at metric magnitudes;
+// x = 0 gives 0).  The fma is explicit: -fmad=false only forbids contraction.
+__device__ __forceinline__ double div12(double x) {
+  constexpr double y = 1.0 / 12.0;
+  const double q = x * y;
+  const double r = fma(-12.0, q, x);
+  return fma(r, y, q);
+}
+
 __device__ __forceinline__ double e6(const double* v) {   // Eq. 17 (R1) at v[0]
   return 3.0 / 4.0 * (v[1] - v[-1]) - 3.0 / 20.0 * (v[2] - v[-2]) + 1.0 / 60.0 * (v[3] - v[-3]);
 }
@@ -102,10 +115,10 @@ __device__ __forceinline__ double delta_vals(const double* v) {
 #pragma unroll
   for (int j = -1; j <= 1; ++j)   // Eq. 19
     d2[j + 1] = 2.0 * (c[j + 1] - 2.0 * c[j] + c[j - 1]) - 0.5 * (d1[j + 3] - d1[j + 1]);
-  const double Lm = c[-1] + 0.5 * d1[1] + d2[0] / 12.0;   // Eq. 16: left state of face -1/2
-  const double R0 = c[0] - 0.5 * d1[2] + d2[1] / 12.0;    // right state of face -1/2
-  const double L0 = c[0] + 0.5 * d1[2] + d2[1] / 12.0;    // left state of face +1/2
-  const double Rp = c[1] - 0.5 * d1[3] + d2[2] / 12.0;    // right state of face +1/2
+  const double Lm = c[-1] + 0.5 * d1[1] + div12(d2[0]);   // Eq. 16: left state of face -1/2
+  const double R0 = c[0] - 0.5 * d1[2] + div12(d2[1]);    // right state of face -1/2
+  const double L0 = c[0] + 0.5 * d1[2] + div12(d2[1]);    // left state of face +1/2
+  const double Rp = c[1] - 0.5 * d1[3] + div12(d2[2]);    // right state of face +1/2
   const double Hp = 0.5 * (L0 + Rp), Hm = 0.5 * (Lm + R0);   // Eq. 36
   return Hp - Hm;
 }
@@ -117,8 +130,8 @@ __device__ __forceinline__ double H_vals(const double* v) {
 #pragma unroll
   for (int j = 0; j < 2; ++j)
     d2[j] = 2.0 * (v[5 + j] - 2.0 * v[4 + j] + v[3 + j]) - 0.5 * (d1[j + 2] - d1[j]);
-  const double L = v[4] + 0.5 * d1[1] + d2[0] / 12.0;
-  const double R = v[5] - 0.5 * d1[2] + d2[1] / 12.0;
+  const double L = v[4] + 0.5 * d1[1] + div12(d2[0]);
+  const double R = v[5] - 0.5 * d1[2] + div12(d2[1]);
   return 0.5 * (L + R);
 }
 
