@@ -106,6 +106,8 @@ __device__ __forceinline__ double div12(double x) {
 __device__ __forceinline__ double e6(const double* v) {   // Eq. 17 (R1) at v[0]
   return 3.0 / 4.0 * (v[1] - v[-1]) - 3.0 / 20.0 * (v[2] - v[-2]) + 1.0 / 60.0 * (v[3] - v[-3]);
 }
+// Products with 2, -2, 0.5 and -0.5 are exact (no underflow at metric magnitudes), so a * b + c with such an a is
+// written as fma(a, b, c): the same single rounding as the multiply-then-add of the stated formula, one operation less.
 // consistent derivative Eq. 37 at the centre v[5] of 11 consecutive values v[0..10]
 __device__ __forceinline__ double delta_vals(const double* v) {
   const double* c = v + 5;
@@ -114,13 +116,14 @@ __device__ __forceinline__ double delta_vals(const double* v) {
   for (int j = -2; j <= 2; ++j) d1[j + 2] = e6(c + j);
 #pragma unroll
   for (int j = -1; j <= 1; ++j)   // Eq. 19
-    d2[j + 1] = 2.0 * (c[j + 1] - 2.0 * c[j] + c[j - 1]) - 0.5 * (d1[j + 3] - d1[j + 1]);
-  const double Lm = c[-1] + 0.5 * d1[1] + div12(d2[0]);   // Eq. 16: left state of face -1/2
-  const double R0 = c[0] - 0.5 * d1[2] + div12(d2[1]);    // right state of face -1/2
-  const double L0 = c[0] + 0.5 * d1[2] + div12(d2[1]);    // left state of face +1/2
-  const double Rp = c[1] - 0.5 * d1[3] + div12(d2[2]);    // right state of face +1/2
-  const double Hp = 0.5 * (L0 + Rp), Hm = 0.5 * (Lm + R0);   // Eq. 36
-  return Hp - Hm;
+    d2[j + 1] = fma(-0.5, d1[j + 3] - d1[j + 1], 2.0 * (fma(-2.0, c[j], c[j + 1]) + c[j - 1]));
+  const double q0 = div12(d2[0]), q1 = div12(d2[1]), q2 = div12(d2[2]);
+  const double Lm = fma(0.5, d1[1], c[-1]) + q0;    // Eq. 16: left state of face -1/2
+  const double R0 = fma(-0.5, d1[2], c[0]) + q1;    // right state of face -1/2
+  const double L0 = fma(0.5, d1[2], c[0]) + q1;     // left state of face +1/2
+  const double Rp = fma(-0.5, d1[3], c[1]) + q2;    // right state of face +1/2
+  // Eq. 36-37: H+ - H- with H = 0.5 (L + R); the halves are exact, so one scaling of the difference
+  return 0.5 * ((L0 + Rp) - (Lm + R0));
 }
 // central interface value Eq. 38 between v[4] and v[5] of 10 consecutive values v[0..9]
 __device__ __forceinline__ double H_vals(const double* v) {
@@ -129,9 +132,9 @@ __device__ __forceinline__ double H_vals(const double* v) {
   for (int j = 0; j < 4; ++j) d1[j] = e6(v + 3 + j);
 #pragma unroll
   for (int j = 0; j < 2; ++j)
-    d2[j] = 2.0 * (v[5 + j] - 2.0 * v[4 + j] + v[3 + j]) - 0.5 * (d1[j + 2] - d1[j]);
-  const double L = v[4] + 0.5 * d1[1] + div12(d2[0]);
-  const double R = v[5] - 0.5 * d1[2] + div12(d2[1]);
+    d2[j] = fma(-0.5, d1[j + 2] - d1[j], 2.0 * (fma(-2.0, v[4 + j], v[5 + j]) + v[3 + j]));
+  const double L = fma(0.5, d1[1], v[4]) + div12(d2[0]);
+  const double R = fma(-0.5, d1[2], v[5]) + div12(d2[1]);
   return 0.5 * (L + R);
 }
 
