@@ -170,7 +170,11 @@ cudaError_t launch_geometry(meg6_grid* g, double t) {
   if (g->p.scheme == 1) return launch_geometry_ig4(g, gi);
   const int T = 256;
   launch_centres(g, gi, xc, xt);
+#if MEG6_CD_KB > 1
+  k_coord_deriv_blk<MEG6_CD_KB><<<nblk((long long)c.LX.pi * c.LX.pj * nblk(c.n[2] + 2 * GX, MEG6_CD_KB), T), T, 0, g->stream>>>(c, xc, cd, g->rj);
+#else
   k_coord_deriv<<<nblk(c.LX.n, T), T, 0, g->stream>>>(c, xc, cd, g->rj);
+#endif
   {
     const int e0 = c.n[0] + 10, e1 = c.n[1] + 10, e2 = c.n[2] + 10;
     k_met_dir<0><<<dim3(nblk(e0, MetCfg<0>::TS), nblk(e1, MetCfg<0>::TW), e2), 256, 0, g->stream>>>(c, xc, xt, cd, met, mt);
@@ -183,7 +187,12 @@ cudaError_t launch_geometry(meg6_grid* g, double t) {
     for (int q = 0; q < 10; ++q)
       if (g->fmet[d][q]) { job.src[job.n] = (q < 9) ? g->met[q] : g->rj; job.dst[job.n] = g->fmet[d][q]; ++job.n; }
     if (g->p.moving) { job.src[job.n] = g->mt[d]; job.dst[job.n] = g->fmt[d]; ++job.n; }
-    k_face_metrics<<<nblk(c.LF[d].n, T), T, 0, g->stream>>>(c, d, job);
+    if (d == 0) k_face_metrics<<<nblk(c.LF[d].n, T), T, 0, g->stream>>>(c, d, job);
+    else {
+      const Lay& LF = c.LF[d];
+      const long long nthr = (long long)LF.pi * nblk(d == 1 ? LF.pj : LF.pk, MEG6_FACE_KB) * (d == 1 ? LF.pk : LF.pj);
+      k_face_metrics_blk<MEG6_FACE_KB><<<nblk(nthr, T), T, 0, g->stream>>>(c, d, job);
+    }
   }
   if (g->p.moving) k_rjt<<<nblk(c.LC.n, T), T, 0, g->stream>>>(c, g->fmt[0], g->fmt[1], g->fmt[2], g->rjt);
   return cudaGetLastError();

@@ -173,6 +173,70 @@ __global__ void k_coord_deriv(Consts c, P3 xc, P9 cd, double* __restrict__ rj) {
   }
 }
 
+// M2, blocked along zeta: a thread takes KB consecutive cells of a zeta column.  The three zeta derivatives of the
+// block share their E6 gradients, second derivatives, one-sided states and interface values in registers (33 FP64
+// operations per derivative instead of 76 at KB = 6; the kernel is FP64-pipe-bound, ncu r1m); the xi and eta derivatives
+// are formed per cell as before.  Every value goes through the operations of delta_vals in its order (bit-identical).
+#ifndef MEG6_CD_KB
+#define MEG6_CD_KB 6
+#endif
+template <int KB>
+__global__ void __launch_bounds__(256) k_coord_deriv_blk(Consts c, P3 xc, P9 cd, double* __restrict__ rj) {
+  const int ext[3] = {c.n[0] + 2 * GX, c.n[1] + 2 * GX, c.n[2] + 2 * GX};
+  const int nb = (ext[2] + KB - 1) / KB;
+  const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (tid >= (long long)c.LX.pi * c.LX.pj * nb) return;
+  const int pi = (int)(tid % c.LX.pi);
+  const int pj = (int)((tid / c.LX.pi) % c.LX.pj);
+  const int pk0 = (int)(tid / ((long long)c.LX.pi * c.LX.pj)) * KB;
+  if (pi >= ext[0] || pj >= ext[1]) return;
+  const long long a0 = (long long)pk0 * c.LX.sk + (long long)pj * c.LX.sj + pi, sk = c.LX.sk;
+  double dz[3][KB];
+#pragma unroll
+  for (int comp = 0; comp < 3; ++comp) {
+    const double* __restrict__ p = xc.p[comp] + a0;
+    double v[KB + 10], d1[KB + 10], hl[KB + 10], hr[KB + 10], H[KB + 10];   // index m <-> plane pk0 + m - 5
+#pragma unroll
+    for (int m = 0; m < KB + 10; ++m) v[m] = p[(long long)(min(max(pk0 + m - 5, 0), ext[2] - 1) - pk0) * sk];
+#pragma unroll
+    for (int m = 3; m <= KB + 6; ++m) d1[m] = e6(v + m);
+#pragma unroll
+    for (int m = 4; m <= KB + 5; ++m) {
+      const double d2 = fma(-0.5, d1[m + 1] - d1[m - 1], 2.0 * (fma(-2.0, v[m], v[m + 1]) + v[m - 1]));   // Eq. 19
+      const double qd = div12(d2);
+      hl[m] = fma(0.5, d1[m], v[m]) + qd;          // Eq. 16: state of plane m at its face +1/2
+      hr[m] = fma(-0.5, d1[m], v[m]) + qd;         //         and at its face -1/2
+    }
+#pragma unroll
+    for (int m = 4; m <= KB + 4; ++m) H[m] = hl[m] + hr[m + 1];       // twice the interface value of face m+1/2
+#pragma unroll
+    for (int b = 0; b < KB; ++b) dz[comp][b] = 0.5 * (H[b + 5] - H[b + 4]);   // Eq. 36-37 as in delta_vals
+  }
+#pragma unroll
+  for (int b = 0; b < KB; ++b) {
+    const int pk = pk0 + b;
+    if (pk >= ext[2]) break;
+    const long long at = a0 + b * sk;
+    const int pos[3] = {pi, pj, pk};
+    double v[9];
+    bool all = true;
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      if (pos[d] < 5 || pos[d] >= ext[d] - 5) { all = false; continue; }
+      const long long s = c.LX.stride(d);
+#pragma unroll
+      for (int comp = 0; comp < 3; ++comp) {
+        v[3 * comp + d] = (d == 2) ? dz[comp][b] : delta_op(xc.p[comp] + at, s);
+        cd.p[3 * comp + d][at] = v[3 * comp + d];
+      }
+    }
+    if (all) {   // 1/J = det of the coordinate derivatives, Eq. 13, on cells [-5, n+5)^3
+      const double xx = v[0], xe = v[1], xz = v[2], yx = v[3], ye = v[4], yz = v[5], zx = v[6], ze = v[7], zz = v[8];
+      rj[at] = xx * (ye * zz - ze * yz) - yx * (xe * zz - ze * xz) + zx * (xe * yz - ye * xz);
+    }
+  }
+}
+
 // M3 (tiled): the Thomas-Lombard metrics, Eq. 10, one sweep per direction D.  Every metric is
 //     m[r][c] = delta_b( delta_a(q) s ) - delta_a( delta_b(q) s ),  (a,b) = (r+1,r+2), (q,s) = (c+1,c+2) mod 3,
 // so direction D carries six consistent derivatives: the FIRST terms of row (D+1)%3 and the SECOND terms of row
@@ -272,6 +336,47 @@ __global__ void k_face_metrics(Consts c, int d, FaceJob job) {
   const int i = (int)(tid % LF.pi), j = (int)((tid / LF.pi) % LF.pj), k = (int)(tid / LF.sk);
   const long long at = c.LX.at(i, j, k), s = c.LX.stride(d);
   for (int q = 0; q < job.n; ++q) job.dst[q][tid] = H_op(job.src[q] + at, s);
+}
+
+// M4 for the eta and zeta families: a thread forms KB consecutive interfaces of one grid line.  Neighbouring
+// interfaces share the E6 gradients, second derivatives and one-sided states of their cells, which the thread keeps in
+// registers: 30 FP64 operations per interface instead of 56 at KB = 4 (k_face_metrics is FP64-pipe-bound, ncu r1m);
+// the operations on every value are those of H_vals, in its order (bit-identical results).  Lanes run along xi.
+#ifndef MEG6_FACE_KB
+#define MEG6_FACE_KB 6
+#endif
+template <int KB>
+__global__ void __launch_bounds__(256) k_face_metrics_blk(Consts c, int d, FaceJob job) {
+  const Lay& LF = c.LF[d];
+  const int nfd = (d == 1) ? LF.pj : LF.pk, nb = (nfd + KB - 1) / KB, no = (d == 1) ? LF.pk : LF.pj;
+  const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (tid >= (long long)LF.pi * nb * no) return;
+  const int i = (int)(tid % LF.pi);
+  const long long r = tid / LF.pi;
+  int j, k, f0;
+  if (d == 1) { f0 = (int)(r % nb) * KB; j = f0; k = (int)(r / nb); }
+  else { j = (int)(r % LF.pj); f0 = (int)(r / LF.pj) * KB; k = f0; }
+  const long long at = c.LX.at(i, j, k), s = c.LX.stride(d);
+  const long long ao = LF.at(i, j, k), so = LF.stride(d);
+  const int lim = c.n[d] + GX - 1 - f0;            // last cell inside the padded array, relative to f0
+  for (int q = 0; q < job.n; ++q) {
+    const double* __restrict__ p = job.src[q] + at;
+    double v[KB + 9], d1[KB + 9], hl[KB + 9], hr[KB + 9];   // index m <-> cell f0 + m - 5
+#pragma unroll
+    for (int m = 0; m < KB + 9; ++m) v[m] = p[(long long)min(m - 5, lim) * s];
+#pragma unroll
+    for (int m = 3; m <= KB + 5; ++m) d1[m] = e6(v + m);
+#pragma unroll
+    for (int m = 4; m <= KB + 4; ++m) {
+      const double d2 = fma(-0.5, d1[m + 1] - d1[m - 1], 2.0 * (fma(-2.0, v[m], v[m + 1]) + v[m - 1]));   // Eq. 19
+      const double qd = div12(d2);
+      hl[m] = fma(0.5, d1[m], v[m]) + qd;          // Eq. 16: state of cell m at its face +1/2
+      hr[m] = fma(-0.5, d1[m], v[m]) + qd;         //         and at its face -1/2
+    }
+#pragma unroll
+    for (int b = 0; b < KB; ++b)
+      if (f0 + b < nfd) job.dst[q][ao + b * so] = 0.5 * (hl[b + 4] + hr[b + 5]);   // Eq. 38
+  }
 }
 
 // M5: GCL, Eq. 14: (1/J)_t = -sum_d [ (m_t)_{+1/2} - (m_t)_{-1/2} ] of the interface values above.
