@@ -74,7 +74,9 @@ void meg6_grid_destroy(meg6_grid* g);
  * (R13, R14); Thomas-Lombard conservative metrics Eq. 10 with every derivative the consistent
  * central derivative of Eq. 36-37 / 41; 1/J Eq. 13; time metrics Eq. 11; interface values by
  * the central interpolation Eq. 38; (1/J)_t Eq. 14 from the same interface values.
- * Static meshes: t ignored, idempotent.  Moving meshes: geometry at time t. */
+ * Static meshes: t ignored, idempotent.  Moving meshes: geometry at time t.
+ * Environment: MEG6_GEOM_BLOCKED=0|1 forces the one-cell-per-thread or the line-blocked form of the coordinate
+ * derivative and interface-metric kernels (default: blocked from 2^21 cells); both give the same bits. */
 meg6_status meg6_metrics_compute(meg6_grid* g, double t);
 
 /* Inflow data of one bc==1 face: P_in[5][n2][n1] = (rho,u,v,w,p) per face cell, (n1,n2) = the two

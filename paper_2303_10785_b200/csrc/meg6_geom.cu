@@ -1,4 +1,5 @@
 // meg6_geom.cu -- metric / Jacobian kernels and their launcher.  Compiled with -fmad=false (see meg6_geom.cuh).
+#include <cstdlib>
 #include <math.h>
 #include "meg6_geom.cuh"
 #ifndef MEG6_IG4_SEGMENTED
@@ -170,11 +171,16 @@ cudaError_t launch_geometry(meg6_grid* g, double t) {
   if (g->p.scheme == 1) return launch_geometry_ig4(g, gi);
   const int T = 256;
   launch_centres(g, gi, xc, xt);
+  // blocking along the grid line trades threads for shared intermediates: it pays once the grid fills the GPU several
+  // times over (256^3: -7 % per call), not on config 2's 64^3 (+3 %)
+  // MEG6_GEOM_BLOCKED=0/1 in the environment forces the choice (the parity tests run both forms on the same small grids)
+  const char* forced = getenv("MEG6_GEOM_BLOCKED");
+  const bool blocked = forced ? (forced[0] == '1') : (c.LC.n >= (1LL << 21));
 #if MEG6_CD_KB > 1
-  k_coord_deriv_blk<MEG6_CD_KB><<<nblk((long long)c.LX.pi * c.LX.pj * nblk(c.n[2] + 2 * GX, MEG6_CD_KB), T), T, 0, g->stream>>>(c, xc, cd, g->rj);
-#else
-  k_coord_deriv<<<nblk(c.LX.n, T), T, 0, g->stream>>>(c, xc, cd, g->rj);
+  if (blocked) k_coord_deriv_blk<MEG6_CD_KB><<<nblk((long long)c.LX.pi * c.LX.pj * nblk(c.n[2] + 2 * GX, MEG6_CD_KB), T), T, 0, g->stream>>>(c, xc, cd, g->rj);
+  else
 #endif
+  k_coord_deriv<<<nblk(c.LX.n, T), T, 0, g->stream>>>(c, xc, cd, g->rj);
   {
     const int e0 = c.n[0] + 10, e1 = c.n[1] + 10, e2 = c.n[2] + 10;
     k_met_dir<0><<<dim3(nblk(e0, MetCfg<0>::TS), nblk(e1, MetCfg<0>::TW), e2), 256, 0, g->stream>>>(c, xc, xt, cd, met, mt);
@@ -187,7 +193,7 @@ cudaError_t launch_geometry(meg6_grid* g, double t) {
     for (int q = 0; q < 10; ++q)
       if (g->fmet[d][q]) { job.src[job.n] = (q < 9) ? g->met[q] : g->rj; job.dst[job.n] = g->fmet[d][q]; ++job.n; }
     if (g->p.moving) { job.src[job.n] = g->mt[d]; job.dst[job.n] = g->fmt[d]; ++job.n; }
-    if (d == 0) k_face_metrics<<<nblk(c.LF[d].n, T), T, 0, g->stream>>>(c, d, job);
+    if (d == 0 || !blocked) k_face_metrics<<<nblk(c.LF[d].n, T), T, 0, g->stream>>>(c, d, job);
     else {
       const Lay& LF = c.LF[d];
       const long long nthr = (long long)LF.pi * nblk(d == 1 ? LF.pj : LF.pk, MEG6_FACE_KB) * (d == 1 ? LF.pk : LF.pj);

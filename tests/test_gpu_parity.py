@@ -78,10 +78,14 @@ def cases():
     return small_cases()
 
 
+@pytest.mark.parametrize("blocked", ["0", "1"])
 @pytest.mark.parametrize("name", ["c1", "c2", "c3", "c4"])
-def test_metrics_parity(mods, cases, name):
+def test_metrics_parity(mods, cases, name, blocked, monkeypatch):
     torch, O, M = mods
     wl = cases[name]
+    # both forms of the coordinate-derivative / interface-metric kernels (one cell per thread, and blocks of six along the
+    # grid line, which grids of 2 M cells and more take by default): the library reads the switch at every call
+    monkeypatch.setenv("MEG6_GEOM_BLOCKED", blocked)
     t = 0.13 if wl["params"]["moving"] else 0.0
     og = O.Grid(wl)
     og.metrics_compute(t)
