@@ -14,12 +14,15 @@
  * fixes the choice; oracle and CUDA path simply share the reading):
  *   - eigenvector averaging state (R5), MP alpha value (R7), tangential viscous gradients (R11),
  *     un-hatted interface metrics (R12), Sutherland constants (R15), sponge form (R16),
- *     per-stage metric recompute (R17), inflow/outflow ghost rules (R20), CFL viscous alpha (R25),
+ *     inflow/outflow ghost rules (R20), the VALUE of the alpha in Eq. B.3 (R25; the formula around it is pinned),
  *     the cell whose metrics give the wall normal of the inviscid-wall rule (R27),
- *     (block interfaces, R28, are pinned: cut domain == uncut domain on Cartesian meshes)
  *     where the IG4 line systems of the MIG4 variant end and how they are closed (R26):
  *     parity unpinned.
- *   - everything else is pinned by tests/test_oracle_*.py (-m "not gpu").
+ *     (block interfaces, R28, are pinned: cut domain == uncut domain)
+ *   - everything else is pinned by tests/test_oracle_*.py (-m "not gpu"); in particular the grid-velocity path
+ *     (node velocities P:166, time metrics Eq. 11, interface time metric, GCL Eq. 14, stage times of Eq. B.1 / R17) by
+ *     tests/test_oracle_moving.py (rigidly translating mesh in closed form, stationary vortex on a deforming mesh
+ *     P:573-579, third order in time) and meg6o_cfl_dt (Eq. B.2/B.3) by tests/test_oracle_cfl.py (closed forms).
  */
 #include "meg6_oracle.h"
 

@@ -198,6 +198,23 @@ def test_limiter_formulae_on_hand_computed_case():
     assert fl == 1 and v == pytest.approx(1.5, abs=1e-15)
 
 
+def test_limiter_hand_computed_cases_where_WMD_and_WLC_bind():
+    """E.3-E.4 by hand, alpha = 4, chosen so that the median (W^MD) and the large-curvature (W^LC)
+    bounds are the ones that decide -- the first hand-computed case is decided by c_p alone.
+    A: c0=1, cm=0.5, cp=1.2, dM_near=-0.4, dM_far=0.3, w=1.5: WMP = 1 + minmod(0.2, 2) = 1.2, (0.5)(0.3) > 0 -> limit;
+       WMD = 1.1 + 0.2 = 1.3, WUL = 3, WLC = 1.25 + 0.4 = 1.65; Wmin = max(1, 1) = 1, Wmax = min(1.3, 3) = 1.3;
+       result = 1.5 + minmod(-0.5, -0.2) = 1.3                                          (W^MD binds).
+    B: c0=1, cm=1.1, cp=1.5, dM_near=0.1, dM_far=0.15, w=1.4: WMP = 1 + minmod(0.5, -0.4) = 1, (0.4)(0.4) > 0 -> limit;
+       WMD = 1.25 - 0.05 = 1.2, WUL = 0.6, WLC = 0.95 + 4/3 0.15 = 1.15; Wmin = max(1, 0.6) = 1,
+       Wmax = min(1.5, max(1, 0.6, 1.15)) = 1.15; result = 1.4 + minmod(-0.4, -0.25) = 1.15   (W^LC with its 4/3 binds).
+    The limiter is odd: negating every argument negates the result (W^min and W^max swap roles)."""
+    for args, want in (((1.5, 1.0, 0.5, 1.2, -0.4, 0.3), 1.3), ((1.4, 1.0, 1.1, 1.5, 0.1, 0.15), 1.15)):
+        v, fl = O.mp_limit(*args, alpha=4.0)
+        assert fl == 1 and v == pytest.approx(want, abs=1e-15)
+        v, fl = O.mp_limit(*(-a for a in args), alpha=4.0)
+        assert fl == 1 and v == pytest.approx(-want, abs=1e-15)
+
+
 # ------------------------------------------------------------------ full inviscid interface (O3)
 def test_inviscid_face_uniform_state_returns_exact_flux():
     P = np.array([1.2, 0.3, -0.1, 0.2, 0.8])
@@ -206,16 +223,20 @@ def test_inviscid_face_uniform_state_returns_exact_flux():
     assert np.allclose(F, flux_of_state(P, m), rtol=1e-12, atol=1e-13)
 
 
-def test_inviscid_face_mirror_symmetry_L_R():
+@pytest.mark.parametrize("rough", [0, 1, 2, 3, 4, 5])
+def test_inviscid_face_mirror_symmetry_L_R(rough):
     """R8: the right state is the mirror image of the left one: reflecting the data about the interface
     (cells reversed, normal velocity and gradients' sign flipped) must flip mass/energy flux and keep the
-    normal momentum flux."""
-    rng = np.random.default_rng(3)
+    normal momentum flux.  rough > 0: seeded cell-to-cell noise on every field, so that both states are limited with
+    all of d^M_near, d^M_far of E.3 non-zero and different on the two sides."""
+    rng = np.random.default_rng(3 + rough)
     x = np.arange(-6, 6) + 0.5          # cell centres; interface at 0 between index 5 and 6
     P = np.stack([1 + 0.2 * np.sin(0.4 * x + 1), 0.3 + 0.2 * np.cos(0.3 * x), 0.1 * np.sin(0.5 * x),
                   0.05 * x, 1 + 0.1 * np.cos(0.45 * x + 2)], axis=1)
     # add a kink so that the limiter is active on some component
     P[7:, 0] += 0.4
+    if rough:
+        P += 0.08 * rng.standard_normal(P.shape)
 
     def face(Pa):
         g1 = np.stack([O.line_op("D1", Pa[:, f]) for f in range(5)], axis=1)
@@ -287,6 +308,36 @@ def test_viscous_face_damping_term_only_on_normal_direction():
     txx = 2 * 0.01 * ux - 2.0 / 3.0 * 0.01 * ux
     assert Fv[1] == pytest.approx(txx, rel=1e-13)
     assert Fv[4] == pytest.approx(0.05 * txx, rel=1e-13)
+
+
+def test_viscous_face_normal_gradient_is_the_P4_stencil_and_differences_to_D2():
+    """P4 through the function the right-hand side calls (not the line-operator restatement): on unit Cartesian metrics
+    with a velocity u(xi) alone, F_v[1] = (2 mu + lambda) u_xi = 4/3 mu g_{i+1/2}.  The interface gradient of Eq. 29-31
+    (alpha^D = 4, beta^D = 0) has the stencil (1/120, -1/15, 3/10, -13/8, 13/8, -3/10, 1/15, -1/120) on
+    i-3..i+4 and consecutive interface gradients differ by Eq. 19's D2 exactly (fourth order)."""
+    mh = np.eye(3).reshape(9)
+    mu = CFG["mu_ref"]
+
+    def iface_grad(f):
+        d1 = O.line_op("D1", f)
+        out = np.full(f.size, np.nan)
+        for i in range(3, f.size - 4):
+            phi = np.array([[f[i], 0, 0, 1.0], [f[i + 1], 0, 0, 1.0]])
+            g = np.zeros((2, 3, 4))
+            g[0, 0, 0], g[1, 0, 0] = d1[i], d1[i + 1]
+            out[i] = O.viscous_face(0, phi, g, mh, 1.0, CFG)[1] / (4.0 / 3.0 * mu)
+        return out
+    imp = np.zeros(21)
+    imp[10] = 1.0
+    r = iface_grad(imp)
+    want = [1 / 120, -1 / 15, 3 / 10, -13 / 8, 13 / 8, -3 / 10, 1 / 15, -1 / 120]
+    # response at interface i+1/2 to an impulse at cell 10 = stencil weight of offset 10 - i
+    assert np.allclose([r[10 - m] for m in range(-3, 5)], want, atol=1e-14)
+    f = np.random.default_rng(3).standard_normal(40)
+    g = iface_grad(f)
+    d2 = O.line_op("D2", f)
+    for i in range(6, 32):
+        assert g[i] - g[i - 1] == pytest.approx(d2[i], abs=5e-14)
 
 
 def test_sutherland():

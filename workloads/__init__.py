@@ -13,11 +13,9 @@ Every generator returns a dict:
   U0       initial conservative state, shape (5, nk, nj, ni)
   inflow   {face: P_in (5, n2, n1)}       (optional)
   sigma, U_ref                            (optional sponge)
-  dt, steps, name, t0
+  dt (None: CFL-based, from `cfl` by Eq. B.2/B.3 on the solver's side), cfl, steps, name, t0
 """
 import hashlib
-import json
-import os
 
 import numpy as np
 
@@ -59,18 +57,6 @@ def _comp_coords(n, L):
     ze = np.arange(nk + 1) * (L[2] / nk)
     Z, E, X = np.meshgrid(ze, et, xi, indexing="ij")
     return X, E, Z
-
-
-_DT_FILE = os.path.join(os.path.dirname(os.path.abspath(__file__)), "..", "tests", "golden", "dt.json")
-
-
-def stored_dt(name):
-    """Time steps written by tests/golden/make_dt.py (oracle's Eq. B.2/B.3); None if not stored."""
-    try:
-        with open(_DT_FILE) as f:
-            return json.load(f).get(name)
-    except FileNotFoundError:
-        return None
 
 
 # --------------------------------------------------------------------------------------------------
@@ -121,7 +107,7 @@ def c1_vortex(n=32, wavy=True, steps=10):
     rho, u, v, w, p = isentropic_vortex(cell_centres(x), cell_centres(y))
     prm = _base_params(n, n, n, period=[[L, 0, 0], [0, L, 0], [0, 0, L]])
     name = "c1_vortex_%d%s" % (n, "" if wavy else "_cart")
-    return dict(name=name, params=prm, x=x, y=y, z=z, U0=conservative(rho, u, v, w, p), dt=stored_dt(name),
+    return dict(name=name, params=prm, x=x, y=y, z=z, U0=conservative(rho, u, v, w, p), dt=None,
                 cfl=0.5, steps=steps, t0=0.0)
 
 
@@ -163,7 +149,7 @@ def c2_dynamic_freestream(n=64, steps=100, seed=20231):
     U0 = conservative(*freestream_state((n, n, n)))
     name = "c2_dynfree_%d" % n
     return dict(name=name, params=prm, x=xj, y=yj, z=zj, dx_mode=dxm, dy_mode=dym, dz_mode=dzm, U0=U0,
-                dt=stored_dt(name), cfl=0.2, steps=steps, t0=0.0)
+                dt=None, cfl=0.2, steps=steps, t0=0.0)
 
 
 def tgv_state(xc, yc, zc, mach=0.1, gamma=GAMMA):
@@ -192,7 +178,7 @@ def c3_tgv(n=128, steps=200, seed=1600, amp=0.05, scheme=0, re=1600.0):
                        mu_ref=1.0 / re, t_ref=1.0, s_suth=110.4 / 293.0, scheme=scheme)
     rho, u, v, w, p = tgv_state(cell_centres(x), cell_centres(y), cell_centres(z), mach)
     name = "c%d_tgv_%d" % (5 if scheme else 3, n)
-    return dict(name=name, params=prm, x=x, y=y, z=z, U0=conservative(rho, u, v, w, p), dt=stored_dt(name),
+    return dict(name=name, params=prm, x=x, y=y, z=z, U0=conservative(rho, u, v, w, p), dt=None,
                 cfl=0.2, steps=steps, t0=0.0)
 
 
