@@ -23,15 +23,19 @@ import workloads as W  # noqa: E402
 
 METRIC = "FP64 MEG6 RHS Mcell-updates/s per RK stage"
 UNIT = "Mcell-updates/s/stage"
-# FP64 (DFMA-pipe) warp-instruction peak: 148 SMs x 64 lanes/clk x clock
+# Nominal FP64 (DFMA-pipe) thread-instruction rate: 148 SMs x 64 lanes/clk x clock; the roof bench.py
+# reports is MEASURED by the library's DFMA micro-benchmark (meg6_fp64_peak), this is printed beside it
 FP64_LANES_PER_SM_CLK = 64
 N_SM = 148
-# DRAM traffic per launch (dram__bytes_read.sum + dram__bytes_write.sum) and FP64-pipe activity of the sweeps on the
-# C4 workload, from the committed `ncu --set full` capture profiles/r1l_ncu.md (never measured by this script)
-NCU = {"c4_jet_320x200x200": {
-    "flux_eta": {"traffic": 3.068790e+09, "fp64_pipe_pct": 53.5},
-    "flux_zeta": {"traffic": 3.578168e+09, "fp64_pipe_pct": 52.3},
-    "flux_xi": {"traffic": 5.485381e+09, "fp64_pipe_pct": 46.7}}}
+# DRAM traffic per launch (dram__bytes_read.sum + dram__bytes_write.sum) and FP64-pipe activity of the sweeps from the
+# committed `ncu --set full` captures (never measured by this script: a run under ncu is not a bench run).  `state` says
+# which flow state and clock the capture saw; the timed region of this script is the mid-run, power-capped state.
+NCU = {}
+try:
+    with open(os.path.join(ROOT, "profiles", "ncu_constants.json")) as _f:
+        NCU = json.load(_f)
+except Exception:
+    pass
 
 
 def make_workload(name):
@@ -65,8 +69,9 @@ def peaks():
         return 6650.0, 1965.0, "fallback (B200_PROFILING.md)"
 
 
-def bytes_per_cell_stage(prm, sponge):
-    """Compulsory HBM doubles per cell per RK stage of the shipped kernel set."""
+def bytes_per_cell_stage(prm, sponge_frac):
+    """Compulsory HBM doubles per cell per RK stage of the shipped kernel set.
+    sponge_frac: None without a sponge, else the fraction of cells with sigma != 0 (Q_ref is read only there)."""
     v, m, ig = prm["viscous"], prm["moving"], prm.get("scheme", 0) == 1
     k = {}
     nf = 6 if v else 5
@@ -77,16 +82,51 @@ def bytes_per_cell_stage(prm, sponge):
         k["grad"] = 3 * nf * 4
         base = nf + nf + met + (10 if v else 0)
     else:
-        k["grad"] = (4 + 12) if v else 0
-        base = nf + met + (8 if v else 0)           # primitive tile, interface metrics, stored gradients
+        k["grad"] = GRAD_DOUBLES if v else 0
+        base = nf + met + (SWEEP_GRAD_DOUBLES if v else 0)   # primitive tile, interface metrics, stored gradients
     k["flux_eta"] = base + 5                        # first sweep: writes the residual
     k["flux_zeta"] = base + 5 + 5                   # reads and writes it
     # last sweep, fused with assembly + RK3 stage + primitives of the new state:
-    # reads residual 5, U 5, U0 5 (stages 2-3), 1/J 1 [, (1/J)_t 1] [, sigma 1, Q_ref 5]; writes U 5, U0 5 (stage 1),
-    # P_next 6 (stages 1-2)
-    k["flux_xi"] = base + 5 + 5 + 10.0 / 3 + 1 + (1 if m else 0) + ((1 + 5) if sponge else 0) + 5 + 5.0 / 3 + 4
+    # reads residual 5, U 5, U0 5 (stages 2-3), 1/J 1 [, (1/J)_t 1] [, sigma 1, Q_ref 5 where sigma != 0]; writes U 5,
+    # U0 5 (stage 1), P_next 6 (stages 1-2)
+    sp = 0.0 if sponge_frac is None else 1.0 + 5.0 * sponge_frac
+    k["flux_xi"] = base + 5 + 5 + 10.0 / 3 + 1 + (1 if m else 0) + sp + 5 + 5.0 / 3 + 4
     k["metrics"] = (6 + 3 + 9 + 9 + 1 + 6 + 3 * met + 1) if m else 0   # nodes+modes, xc, cd, met, rj, xt+mt, faces, rjt
     return {a: 8.0 * b for a, b in k.items()}
+
+
+# stored tangential gradients of the viscous flux (MEG6): k_grad reads (u,v,w,T) and writes 12 arrays; each sweep reads
+# the 8 arrays of its two tangential directions
+GRAD_DOUBLES = 4 + 12
+SWEEP_GRAD_DOUBLES = 8
+
+
+def sponge_fraction(wl):
+    sg = wl.get("sigma")
+    return None if sg is None else float(np.count_nonzero(sg)) / sg.size
+
+
+def input_hashes(wl):
+    """SHA-256 of the generated arrays (oracle and GPU provably see the same bits)"""
+    h = {"nodes": W.sha256(wl["x"], wl["y"], wl["z"]), "U0": W.sha256(wl["U0"])}
+    if wl.get("dx_mode") is not None:
+        h["modes"] = W.sha256(wl["dx_mode"], wl["dy_mode"], wl["dz_mode"])
+    if wl.get("sigma") is not None:
+        h["sponge"] = W.sha256(wl["sigma"], wl["U_ref"])
+    for f, pin in sorted(wl.get("inflow", {}).items()):
+        h["inflow%d" % int(f)] = W.sha256(pin)
+    return h
+
+
+def cpu_model():
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.startswith("model name"):
+                    return line.split(":", 1)[1].strip()
+    except Exception:
+        pass
+    return "unknown"
 
 
 class ClockSampler:
@@ -135,21 +175,40 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def oracle_sample(threads=None):
-    """The CPU oracle as it stands, timed on a bounded sample of the C4 workload (1/8 of the cells)."""
+SAMPLE = dict(ni=160, nj=100, nk=100)
+
+
+def oracle_sample(threads=None, grid=None):
+    """The CPU oracle as it stands, timed on a bounded sample of the C4 workload (1/8 of the cells): one RK3 step.
+    Returns (record, seconds, (grid, workload)) -- the grid can be reused for another thread count (static mesh)."""
     from oracle import meg6_oracle as O
     nthr = threads or (os.cpu_count() or 1)
+    if grid is None:
+        O.set_threads(os.cpu_count() or 1)
+        wl = W.c4_jet(**SAMPLE)
+        g = O.Grid(wl)
+        g.metrics_compute(0.0)
+    else:
+        g, wl = grid
     O.set_threads(nthr)
-    wl = W.c4_jet(ni=160, nj=100, nk=100)
-    g = O.Grid(wl)
-    g.metrics_compute(0.0)
     U = wl["U0"].copy()
     t0 = time.perf_counter()
     g.rk3_step(U, 0.0, wl["dt"])
     dt = time.perf_counter() - t0
     n = U[0].size
-    return {"value": n * 3 / dt / 1e6, "unit": UNIT, "cores": O.get_threads(), "kind": "oracle",
-            "sample": "c4_jet 160x100x100 (1.6 M cells, 1/8 of the workload), 1 RK3 step, %.1f s" % dt}, dt
+    rec = {"value": n * 3 / dt / 1e6, "unit": UNIT, "cores": O.get_threads(), "kind": "oracle",
+           "sample": "c4_jet %dx%dx%d (%.1f M cells, 1/8 of the workload), 1 RK3 step, %.1f s"
+                     % (SAMPLE["ni"], SAMPLE["nj"], SAMPLE["nk"], n / 1e6, dt),
+           "cpu_model": cpu_model(), "nproc": os.cpu_count()}
+    return rec, dt, (g, wl)
+
+
+def cpu_baseline():
+    """(b) all host cores and (a) one thread -- the paper's like-for-like is one Xeon Gold 5115 core"""
+    rec, _, grid = oracle_sample()
+    one, dt1, _ = oracle_sample(threads=1, grid=grid)
+    rec["single_thread"] = {"value": one["value"], "unit": UNIT, "cores": 1, "sample": one["sample"]}
+    return rec
 
 
 def run_reference(args):
@@ -158,8 +217,9 @@ def run_reference(args):
         return
     vals = []
     base = None
+    grid = None
     for s in range(args.warmup + args.steps):
-        base, dt = oracle_sample()
+        base, dt, grid = oracle_sample(grid=grid)
         if s >= args.warmup:
             vals.append((base["value"], dt))
     v = float(np.mean([a for a, _ in vals]))
@@ -221,7 +281,14 @@ def run_ours(args):
         del blocks
     prm = wl["params"]
     ncell = prm["ni"] * prm["nj"] * prm["nk"]
+    ncell_job = ncell * world                      # replicas: every rank its own copy
+    if slabs:                                      # slabs: the ranks share one copy; the slabs differ by up to a plane
+        tn = torch.tensor([ncell], dtype=torch.int64, device=dev)
+        dist.all_reduce(tn, op=dist.ReduceOp.SUM)
+        ncell_job = int(tn.item())
     g = Grid(wl, device=dev)
+    if args.metrics_only:
+        return run_metrics_only(args, g, wl, dev)
     g.metrics_compute(wl["t0"])
     U = torch.as_tensor(wl["U0"], device=dev).contiguous()
     if wl["dt"] is not None:
@@ -264,8 +331,7 @@ def run_ours(args):
         startup = max_over_ranks([s0.elapsed_time(s1)], dist, dev)[0]
         for _ in range(max(0, develop - args.steps - args.warmup)):
             step(U, t, dt); t += dt
-    g.profile_enable(True)
-    g.profile_read()
+    # headline: K steps, no per-kernel events inside the timed region
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
@@ -277,6 +343,18 @@ def run_ours(args):
     e1.record(stream)
     barrier()
     ms = e0.elapsed_time(e1)
+    # per-kernel breakdown: a second pass of K steps of the same (still developed, still warm) run with one CUDA event
+    # pair around every kernel launch on the launching stream; its own wall time is reported as `profiled_ms_per_step`
+    g.profile_enable(True)
+    g.profile_read()
+    barrier()
+    p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    p0.record(stream)
+    for _ in range(args.steps):
+        step(U, t, dt); t += dt
+    p1.record(stream)
+    barrier()
+    ms_prof = p0.elapsed_time(p1)
     clocks = sampler.stop() if rank == 0 else None
     prof = g.profile_read()
     g.profile_enable(False)
@@ -306,14 +384,12 @@ def run_ours(args):
             dist.destroy_process_group()
         return
 
-    # replicas: every rank advances its own copy; slabs: the ranks share one copy (ncell = this rank's slab; the
-    # slabs differ by at most one plane, rank 0 holds a largest one)
-    value = whole_job_throughput(ncell, args.steps, world, ms)
-    e2e_value = whole_job_throughput(ncell, args.steps, world, ms_e2e)
+    value = whole_job_throughput(ncell_job / world, args.steps, world, ms)
+    e2e_value = whole_job_throughput(ncell_job / world, args.steps, world, ms_e2e)
     hbm, sm_max, peak_src = peaks()
-    bpc = bytes_per_cell_stage(prm, wl.get("sigma") is not None)
+    bpc = bytes_per_cell_stage(prm, sponge_fraction(wl))
     stage_bytes = sum(bpc.values())
-    # per-kernel breakdown measured live with CUDA events on the launching stream
+    # per-kernel breakdown measured live with CUDA events on the launching stream (the profiled pass)
     tot_prof = sum(v[0] for v in prof.values())
     kernels = {}
     launches = 0
@@ -328,42 +404,80 @@ def run_ours(args):
     dsec = kernels[dom]["ms_per_stage"] * 1e-3
     ach = bpc[dom] * ncell / dsec / 1e9
     clk = (clocks or {}).get("sm_mhz") or sm_max
+    from paper_2303_10785_b200 import fp64_peak
+    dfma = fp64_peak(dev)                      # measured right after the timed steps: the clock the steps ended with
+    ncu = NCU.get(wl["name"], {}).get(dom, {})
     roof = {"kernel": "k_flux3<%s,%s>" % (dom[5:], "visc" if prm["viscous"] else "inv"), "bound": "hbm",
             "achieved": ach, "peak": hbm, "unit": "GB/s", "frac": ach / hbm,
-            "traffic": NCU.get(wl["name"], {}).get(dom, {}).get("traffic"),
-            "traffic_source": "profiles/r1l_ncu.md" if wl["name"] in NCU else None,
-            "fp64_pipe_pct_ncu": NCU.get(wl["name"], {}).get(dom, {}).get("fp64_pipe_pct"),
+            "traffic": ncu.get("traffic"), "traffic_source": ncu.get("source"), "traffic_state": ncu.get("state"),
+            "fp64_pipe_pct_ncu": ncu.get("fp64_pipe_pct"),
             "peak_source": peak_src, "bytes_per_cell": bpc[dom], "cells_per_launch": ncell,
             "avg_launch_ms": dsec * 1e3,
-            "fp64_pipe_peak_Tinst_s_at_sampled_clock": N_SM * FP64_LANES_PER_SM_CLK * clk * 1e6 / 1e12}
+            "fp64_roof": {"measured_Tdfma_s": dfma / 1e12,
+                          "how": "meg6_fp64_peak: register-resident DFMA loop on every SM, best of 3, run after the "
+                                 "timed steps",
+                          "nominal_Tdfma_s_at_sampled_clock": N_SM * FP64_LANES_PER_SM_CLK * clk * 1e6 / 1e12}}
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
             "scaling": "strong" if slabs else "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": wl_name, "cells": ncell * world if slabs else ncell, "viscous": prm["viscous"], "moving": prm["moving"],
+            "config": {"workload": wl_name, "cells": ncell_job if slabs else ncell, "viscous": prm["viscous"], "moving": prm["moving"],
                        "scheme": "MIG4" if prm.get("scheme", 0) == 1 else "MEG6",
                        "dt": dt, "parallelism": ("zeta slabs x%d, 6-layer halo exchange per stage" if slabs else "replicas x%d") % world,
                        "l2": "working set %.1f GB per stage >> 126 MB L2 (no flush needed)" % (stage_bytes * ncell / 1e9)},
             "clocks": clocks, "gpu_launches": int(launches), "finite": finite,
+            "profiled_ms_per_step": ms_prof / args.steps, "inputs_sha256": input_hashes(wl),
+            "sponge_cell_fraction": sponge_fraction(wl),
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(U.numel() * 8),
                     "d2h_bytes_per_step": int(U.numel() * 8), "ms_per_step": ms_e2e / args.steps},
             "roofline": roof,
             "hbm_roofline_step": {"bytes_per_cell_stage": stage_bytes,
-                                  "achieved_GBps": stage_bytes * ncell * 3 * args.steps / (ms * 1e-3) / 1e9,
-                                  "frac": stage_bytes * ncell * 3 * args.steps / (ms * 1e-3) / 1e9 / hbm,
+                                  "achieved_GBps": stage_bytes * ncell_job * 3 * args.steps / (ms * 1e-3) / 1e9 / world,
+                                  "frac": stage_bytes * ncell_job * 3 * args.steps / (ms * 1e-3) / 1e9 / world / hbm,
                                   "peak": hbm, "peak_source": peak_src},
             "kernels": kernels}
     line["config"]["state"] = "timed after %d untimed steps of the config's %s-step run (warm-up included)" % (
         max(develop, args.warmup), wl.get("steps"))
     if startup is not None:
-        line["startup"] = {"value": whole_job_throughput(ncell, args.steps, world, startup), "unit": UNIT,
+        line["startup"] = {"value": whole_job_throughput(ncell_job / world, args.steps, world, startup), "unit": UNIT,
                            "ms_per_step": startup / args.steps,
                            "state": "the %d steps right after the %d warm-up steps from the initial state" % (args.steps, args.warmup)}
     if world == 1 and not args.no_cpu_baseline:
-        line["cpu_baseline"], _ = oracle_sample()
+        line["cpu_baseline"] = cpu_baseline()
     print(json.dumps(line))
     if dist:
         dist.destroy_process_group()
+
+
+def run_metrics_only(args, g, wl, dev):
+    """--metrics-only: times meg6_metrics_compute(t) alone (every RK stage on a moving mesh) --
+    the command the geometry profiles under profiles/ are taken with."""
+    import torch
+    stream = torch.cuda.current_stream(dev)
+    for r in range(max(3, args.warmup)):
+        g.metrics_compute(0.01 * (r + 1))
+    torch.cuda.synchronize(dev)
+    g.profile_enable(True)
+    g.profile_read()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for r in range(args.steps):
+        g.metrics_compute(0.1 + 0.01 * r)
+    e1.record(stream)
+    torch.cuda.synchronize(dev)
+    ms = e0.elapsed_time(e1) / args.steps
+    prof = g.profile_read()
+    prm = wl["params"]
+    ncell = prm["ni"] * prm["nj"] * prm["nk"]
+    bpc = bytes_per_cell_stage(prm, sponge_fraction(wl))["metrics"]
+    hbm, _, peak_src = peaks()
+    print(json.dumps({"metric": "meg6_metrics_compute ms per call", "value": ms, "unit": "ms", "higher_is_better": False,
+                      "calls": args.steps, "dtype": "f64", "data": "synthetic",
+                      "config": {"workload": wl["name"], "cells": ncell, "moving": prm["moving"],
+                                 "scheme": "MIG4" if prm.get("scheme", 0) == 1 else "MEG6"},
+                      "gpu_launches": int(prof["metrics"][1]),
+                      "algorithmic_GBps": (bpc * ncell / (ms * 1e-3) / 1e9) if bpc else None, "hbm_peak": hbm,
+                      "peak_source": peak_src}))
 
 
 def main():
@@ -377,6 +491,8 @@ def main():
     ap.add_argument("--develop", type=int, default=None,
                     help="untimed steps that advance the flow before the timed ones (default: half of the config's step "
                          "count for c4, 0 otherwise)")
+    ap.add_argument("--metrics-only", action="store_true",
+                    help="time meg6_metrics_compute alone (moving-mesh workloads c2, c2_N): `--steps` calls")
     ap.add_argument("--decomp", default="replicas", choices=["replicas", "slabs"],
                     help="N > 1: independent replicas (weak scaling, default) or one workload cut into zeta slabs "
                          "with halo exchange (strong scaling)")

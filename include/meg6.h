@@ -151,6 +151,17 @@ meg6_status meg6_diagnostics(meg6_grid* g, const double* U, double* out);
 meg6_status meg6_limiter_stats_enable(meg6_grid* g, int on);
 meg6_status meg6_limiter_stats(meg6_grid* g, unsigned long long* n_limited, unsigned long long* n_tested);
 
+/* Per-interface branch record (north_star: "any cell where an MP-limiter branch flips is reported separately").  While a
+ * pointer is set, every right-hand side (each stage of rk3_step) overwrites it with one 16-bit word per interface of that
+ * family -- (ni+1) nj nk words for xi, ni (nj+1) nk for eta, ni nj (nk+1) for zeta, index along the family's direction
+ * running over n_d + 1, i fastest:
+ *   bit r (0..4)  the LEFT state of characteristic component r failed test E.1 and went through E.2-E.4,
+ *   bit 5 + r     the same for the RIGHT state (R8),
+ *   bits 10-11    the branch of Eq. 26 (cascade R10) the HLLC flux took: 0 F_L, 1 F*_L, 2 F*_R, 3 F_R.
+ * DEVICE pointers owned by the caller, each may be NULL (that family is not recorded); the decisions are taken in FP64
+ * as in the flux itself.  Costs one 2-byte store per interface while set. */
+meg6_status meg6_set_branch_masks(meg6_grid* g, unsigned short* xi, unsigned short* eta, unsigned short* zeta);
+
 /* Inspection for tests: copies an internal array to HOST memory `out` (interior cells, [nk][nj][ni], or
  * for interface arrays n_d+1 entries along d).  kind 0: cell array `which` = 0..8 hatted metrics
  * (xi_x..zeta_z), 9 = 1/J, 10..12 = hatted time metrics, 13 = (1/J)_t, 14..16 = cell-centre x,y,z;
@@ -166,6 +177,12 @@ meg6_status meg6_get_array(meg6_grid* g, int kind, int which, double* out);
  * and the primitive conversion of the new state), 5 eta sweep (first), 6 zeta sweep, 7-8 unused, 9 CFL reduction. */
 meg6_status meg6_profile_enable(meg6_grid* g, int on);
 meg6_status meg6_profile_read(meg6_grid* g, double* ms_per_kind, unsigned long long* launches_per_kind);
+
+/* FP64-pipe roof of the device by measurement (bench.py prints it beside the HBM roof): runs a
+ * register-resident loop of independent DFMA chains that fills every SM (4 launches, ~10 ms) and returns the best rate
+ * in DFMA thread-instructions per second (x 2 = flop/s).  scratch: DEVICE pointer to one double (never written in
+ * practice); dfma_per_second: HOST pointer.  Synchronises the stream.  Needs no grid. */
+meg6_status meg6_fp64_peak(void* cuda_stream, double* scratch, double* dfma_per_second);
 
 const char* meg6_last_error(void);
 /* Library/ABI version: 1000*major + minor. */

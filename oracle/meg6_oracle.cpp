@@ -235,6 +235,11 @@ struct meg6o_grid {
   std::vector<double> inflow[6];
   std::vector<double> sigma, uref;
   unsigned long long n_limited = 0, n_tested = 0;
+  /* branch record of the last right-hand side (tests: which interfaces took which branch), per interface family:
+   * bit r (0..4) = left state of characteristic component r failed E.1, bit 5+r = right state, bits 10-11 = branch
+   * 0..3 of Eq. 26.  Interface index along d runs over n_d + 1, i fastest. */
+  bool want_masks = false;
+  std::vector<unsigned short> mask[3];
   meg6o_grid* link[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};   /* bc 5: neighbour block per face */
   const double* ibuf[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr}; /* bc 5: or packed neighbour layers */
 };
@@ -539,7 +544,7 @@ int meg6o_hllc(const double PL[5], const double PR[5], const double m[4], double
 }
 
 namespace {
-struct FaceStats { unsigned long long limited = 0, tested = 0; };
+struct FaceStats { unsigned long long limited = 0, tested = 0; unsigned mask = 0; };
 
 /* O3 steps 1-8 for one interface */
 void inviscid_face_impl(const double Pc[4][5], const double P1[2][5], const double P2[4][5],
@@ -577,7 +582,7 @@ void inviscid_face_impl(const double Pc[4][5], const double P1[2][5], const doub
     const double dm_mid = minmod(D[1][r], D[2][r]);
     WL[r] = meg6o_mp_limit(wl, W[1][r], W[0][r], W[2][r], dm_mid, minmod(D[0][r], D[1][r]), alpha, &fl);
     WR[r] = meg6o_mp_limit(wr, W[2][r], W[3][r], W[1][r], dm_mid, minmod(D[2][r], D[3][r]), alpha, &fr);
-    if (st) { st->tested += 2; st->limited += fl + fr; }
+    if (st) { st->tested += 2; st->limited += fl + fr; st->mask |= ((unsigned)fl << r) | ((unsigned)fr << (5 + r)); }
   }
   /* step 7: Eq. 23 */
   double PL[5], PR[5];
@@ -587,7 +592,24 @@ void inviscid_face_impl(const double Pc[4][5], const double P1[2][5], const doub
     PL[r] = s; PR[r] = t;
   }
   /* step 8 */
-  meg6o_hllc(PL, PR, m, gamma, F);
+  const int branch = meg6o_hllc(PL, PR, m, gamma, F);
+  if (st) {
+    st->mask |= (unsigned)branch << 10;
+    /* tie flag for the branch record (tests): a wave speed the cascade of Eq. 26 actually tested lies within 1e-10 of
+     * zero relative to the fastest wave -- R10: both sides of such a tie give the same flux up to round-off, and which
+     * side is taken depends on the rounding order (fluid at rest: S* = +-1e-17) */
+    const double mx = m[0], my = m[1], mz = m[2], mt = m[3], gg = std::sqrt(mx * mx + my * my + mz * mz);
+    const double UL = mt + mx * PL[1] + my * PL[2] + mz * PL[3], UR = mt + mx * PR[1] + my * PR[2] + mz * PR[3];
+    const double cL = std::sqrt(gamma * PL[4] / PL[0]), cR = std::sqrt(gamma * PR[4] / PR[0]);
+    const double SL = std::min(UL - cL * gg, UR - cR * gg), SR = std::max(UL + cL * gg, UR + cR * gg);
+    const double SS = (PR[0] * UR * (SR - UR) - PL[0] * UL * (SL - UL) + (PL[4] - PR[4]) * gg * gg) /
+                      (PR[0] * (SR - UR) - PL[0] * (SL - UL));
+    const double tol = 1e-10 * std::max(std::fabs(SL), std::fabs(SR));
+    bool tie = std::fabs(SL) <= tol;
+    if (SL < 0.0) tie = tie || std::fabs(SS) <= tol;
+    if (SL < 0.0 && SS < 0.0) tie = tie || std::fabs(SR) <= tol;
+    if (tie) st->mask |= 1u << 12;
+  }
 }
 }  // namespace
 
@@ -814,6 +836,7 @@ void rhs_from_primitives(meg6o_grid* G, const double* U, double* dUdt) {
     fn[d] += 1;
     std::vector<double> flux((size_t)5 * fn[0] * fn[1] * fn[2]);
     const size_t FN = (size_t)fn[0] * fn[1] * fn[2];
+    if (G->want_masks) G->mask[d].assign(FN, 0);
 #ifdef _OPENMP
 #pragma omp parallel for schedule(static) num_threads(g_threads) reduction(+ : lim, tst)
 #endif
@@ -840,6 +863,7 @@ void rhs_from_primitives(meg6o_grid* G, const double* U, double* dUdt) {
           lim += st.limited; tst += st.tested;
           const size_t fi = ((size_t)k * fn[1] + j) * fn[0] + i;
           for (int f = 0; f < 5; ++f) flux[f * FN + fi] = F[f];
+          if (G->want_masks) G->mask[d][fi] = (unsigned short)st.mask;
         }
     /* Eq. 25, Eq. 8-9: Res_i -= F_{i+1/2} - F_{i-1/2} */
     const size_t fs = (d == 0) ? 1 : (d == 1) ? (size_t)fn[0] : (size_t)fn[0] * fn[1];
@@ -1044,6 +1068,16 @@ void meg6o_diagnostics(meg6o_grid* G, const double* U, double* out) {
 
 void meg6o_limiter_stats(meg6o_grid* G, unsigned long long* n_limited, unsigned long long* n_tested) {
   *n_limited = G->n_limited; *n_tested = G->n_tested;
+}
+
+void meg6o_branch_masks_enable(meg6o_grid* G, int on) {
+  G->want_masks = on != 0;
+  if (!on) for (int d = 0; d < 3; ++d) std::vector<unsigned short>().swap(G->mask[d]);
+}
+size_t meg6o_get_branch_mask(meg6o_grid* G, int d, unsigned short* out) {
+  if (d < 0 || d > 2) return 0;
+  if (out) std::copy(G->mask[d].begin(), G->mask[d].end(), out);
+  return G->mask[d].size();
 }
 
 /* -------------------------------------- inspection ---------------------------------------- */

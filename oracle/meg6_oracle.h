@@ -67,6 +67,15 @@ double meg6o_cfl_dt(meg6o_grid* g, const double* U, double cfl);
 /* volume-averaged kinetic energy, enstrophy (Eq. 54, in 3-D with dV = 1/J) and the volume: out[3] */
 void meg6o_diagnostics(meg6o_grid* g, const double* U, double* out);
 void meg6o_limiter_stats(meg6o_grid* g, unsigned long long* n_limited, unsigned long long* n_tested);
+/* Branch record of the LAST right-hand side (last stage of the last rk3_step), kept while enabled: one 16-bit word per
+ * interface of family d (n_d + 1 interfaces along d, interior extents along the others, i fastest, as meg6o_get_face):
+ * bit r (0..4): the left state of characteristic component r failed test E.1 and was limited; bit 5+r: the
+ * right state; bits 10-11: the branch 0..3 of Eq. 26 (cascade R10) the HLLC flux took; bit 12 (oracle only):
+ * that branch was a tie -- a wave speed the cascade tested lies within 1e-10 of zero relative to the fastest wave, so
+ * either neighbouring branch gives the same flux up to round-off (R10).
+ * get returns the number of words (out may be NULL). */
+void meg6o_branch_masks_enable(meg6o_grid* g, int on);
+size_t meg6o_get_branch_mask(meg6o_grid* g, int d, unsigned short* out);
 
 /* inspection (tests): which = 0..8 hatted metrics (xi_x..zeta_z), 9 = 1/J, 10..12 = xi_t,eta_t,zeta_t
  * (hatted), 13 = (1/J)_t, 14..16 = cell-centre x,y,z.   out[nk][nj][ni]                          */

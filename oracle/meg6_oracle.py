@@ -76,6 +76,9 @@ def lib():
         L.meg6o_cfl_dt.argtypes = [C.c_void_p, _dp, C.c_double]
         L.meg6o_diagnostics.argtypes = [C.c_void_p, _dp, _dp]
         L.meg6o_limiter_stats.argtypes = [C.c_void_p, C.POINTER(C.c_ulonglong), C.POINTER(C.c_ulonglong)]
+        L.meg6o_branch_masks_enable.argtypes = [C.c_void_p, C.c_int]
+        L.meg6o_get_branch_mask.restype = C.c_size_t
+        L.meg6o_get_branch_mask.argtypes = [C.c_void_p, C.c_int, C.c_void_p]
         L.meg6o_get_cell.argtypes = [C.c_void_p, C.c_int, _dp]
         L.meg6o_get_face.argtypes = [C.c_void_p, C.c_int, C.c_int, _dp]
         L.meg6o_get_prim.argtypes = [C.c_void_p, C.c_int, _dp]
@@ -226,6 +229,19 @@ class Grid:
         a, b = C.c_ulonglong(), C.c_ulonglong()
         lib().meg6o_limiter_stats(self.h, C.byref(a), C.byref(b))
         return a.value, b.value
+
+    def branch_masks_enable(self, on=True):
+        lib().meg6o_branch_masks_enable(self.h, int(on))
+
+    def branch_mask(self, d):
+        """uint16 per interface of family d after the last rhs: bits 0-4 / 5-9 E.1 failed (left / right state of the
+        five characteristic components), bits 10-11 branch of Eq. 26; shape as face(d, .)"""
+        shp = list(self.shape)
+        shp[2 - d] += 1
+        out = np.empty(shp, dtype=np.uint16)
+        n = lib().meg6o_get_branch_mask(self.h, int(d), out.ctypes.data)
+        assert n == out.size, (n, out.size)
+        return out
 
     def cell(self, which):
         out = np.empty(self.shape)

@@ -9,8 +9,8 @@ from . import build as _build
 
 EXPORTS = ["meg6_workspace_bytes", "meg6_grid_create", "meg6_grid_destroy", "meg6_metrics_compute",
            "meg6_set_inflow", "meg6_set_sponge", "meg6_rhs", "meg6_rk3_step", "meg6_cfl_dt", "meg6_diagnostics",
-           "meg6_limiter_stats_enable", "meg6_limiter_stats", "meg6_get_array", "meg6_profile_enable",
-           "meg6_profile_read", "meg6_last_error",
+           "meg6_limiter_stats_enable", "meg6_limiter_stats", "meg6_set_branch_masks", "meg6_get_array", "meg6_profile_enable",
+           "meg6_profile_read", "meg6_fp64_peak", "meg6_last_error",
            "meg6_version", "meg6_link_blocks", "meg6_rhs_blocks", "meg6_rk3_step_blocks",
            "meg6_interface_doubles", "meg6_set_interface_buffer", "meg6_stage_prim", "meg6_stage_pack",
            "meg6_stage_ghosts", "meg6_stage_sweeps"]
@@ -91,6 +91,8 @@ def lib():
         L.meg6_limiter_stats_enable.argtypes = [_vp, C.c_int]
         L.meg6_limiter_stats.restype = C.c_int
         L.meg6_limiter_stats.argtypes = [_vp, C.POINTER(C.c_ulonglong), C.POINTER(C.c_ulonglong)]
+        L.meg6_set_branch_masks.restype = C.c_int
+        L.meg6_set_branch_masks.argtypes = [_vp, _vp, _vp, _vp]
         L.meg6_get_array.restype = C.c_int
         L.meg6_get_array.argtypes = [_vp, C.c_int, C.c_int, _vp]
         L.meg6_profile_enable.restype = C.c_int
@@ -115,6 +117,8 @@ def lib():
         L.meg6_stage_ghosts.argtypes = [_vp, C.c_int, C.c_int]
         L.meg6_stage_sweeps.restype = C.c_int
         L.meg6_stage_sweeps.argtypes = [_vp, _vp, _vp, C.c_int, C.c_double]
+        L.meg6_fp64_peak.restype = C.c_int
+        L.meg6_fp64_peak.argtypes = [_vp, _vp, C.POINTER(C.c_double)]
         L.meg6_last_error.restype = C.c_char_p
         L.meg6_version.restype = C.c_int
         _lib = L
@@ -247,6 +251,24 @@ class Grid:
         _check(lib().meg6_limiter_stats(self.h, C.byref(a), C.byref(b)), "meg6_limiter_stats")
         return a.value, b.value
 
+    def branch_masks_enable(self, on=True):
+        """allocates (or drops) the three per-interface branch-record arrays and hands them to the library"""
+        if on:
+            t = self.torch
+            nk, nj, ni = self.shape
+            self.branch_mask = [t.zeros((nk, nj, ni + 1), dtype=t.int16, device=self.device),
+                                t.zeros((nk, nj + 1, ni), dtype=t.int16, device=self.device),
+                                t.zeros((nk + 1, nj, ni), dtype=t.int16, device=self.device)]
+            ptrs = [m.data_ptr() for m in self.branch_mask]
+        else:
+            self.branch_mask, ptrs = None, [None, None, None]
+        _check(lib().meg6_set_branch_masks(self.h, *ptrs), "meg6_set_branch_masks")
+
+    def branch_mask_host(self, d):
+        """numpy uint16 copy of the record of family d (bits: include/meg6.h)"""
+        import numpy as np
+        return self.branch_mask[d].cpu().numpy().view(np.uint16)
+
     PROFILE_KINDS = ["metrics", "prim", "ghost", "grad", "flux_xi", "flux_eta", "flux_zeta", "update",
                      "copy_Un", "cfl"]
 
@@ -268,6 +290,18 @@ class Grid:
         out = np.empty(shp, dtype=np.float64)
         _check(lib().meg6_get_array(self.h, kind, which, out.ctypes.data), "meg6_get_array")
         return out
+
+
+def fp64_peak(device="cuda:0"):
+    """measured FP64-pipe roof of the device in DFMA thread-instructions per second (meg6_fp64_peak)"""
+    import torch
+    dev = torch.device(device)
+    with torch.cuda.device(dev):
+        scratch = torch.zeros(1, dtype=torch.float64, device=dev)
+        r = C.c_double()
+        _check(lib().meg6_fp64_peak(torch.cuda.current_stream(dev).cuda_stream, scratch.data_ptr(), C.byref(r)),
+               "meg6_fp64_peak")
+    return r.value
 
 
 def _ptr_array(ptrs):

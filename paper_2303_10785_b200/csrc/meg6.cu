@@ -8,6 +8,7 @@
 #include "meg6_common.cuh"
 #include "meg6_flow.cuh"
 #include "meg6_flux3.cuh"
+#include "meg6_probe.cuh"
 #include <stdlib.h>
 
 using namespace meg6;
@@ -278,6 +279,7 @@ struct ProfScope {
     g->prof_recs.push_back(r);
     rec = g->prof_recs.size() - 1;
   }
+  void set_launches(int n) { if (rec != (size_t)-1) g->prof_recs[rec].launches = n; }
   ~ProfScope() {
     if (rec != (size_t)-1) cudaEventRecord(g->prof_pool[g->prof_recs[rec].e1], g->stream);
   }
@@ -328,6 +330,10 @@ meg6_status meg6_grid_create(const meg6_params* p, const double* x, const double
   g->c = make_consts(p);
   g->stream = (cudaStream_t)cuda_stream;
   g->ws = (char*)workspace; g->ws_bytes = workspace_bytes;
+  {
+    const char* forced = getenv("MEG6_GEOM_BLOCKED");   // read once, here: which form of the geometry kernels (tests)
+    g->geom_blocked = forced ? (forced[0] == '1' ? 1 : 0) : -1;
+  }
   const size_t need = carve(p, g->c, g, g->ws);
   if (need > workspace_bytes) { delete g; return fail(MEG6_ENOMEM, "workspace too small%s"); }
   const size_t nn = (size_t)(p->ni + 1) * (p->nj + 1) * (p->nk + 1) * sizeof(double);
@@ -365,8 +371,10 @@ meg6_status meg6_metrics_compute(meg6_grid* g, double t) {
   if (g->have_metrics && !g->p.moving) return MEG6_OK;   // static: idempotent
   cudaError_t e;
   {
-    ProfScope ps(g, 0, 3 + 3 + (g->p.moving ? 1 : 0));
+    ProfScope ps(g, 0, 0);
+    g->geom_launches = 0;
     e = meg6::launch_geometry(g, t);                      // meg6_geom.cu (compiled with -fmad=false)
+    ps.set_launches(g->geom_launches);
   }
   if (e != cudaSuccess) return fail(MEG6_ECUDA, "metrics_compute: %s", cudaGetErrorString(e));
   g->have_metrics = true;
@@ -392,7 +400,7 @@ meg6_status meg6_set_sponge(meg6_grid* g, const double* sigma, const double* U_r
 // ghost layers of direction d in primitive buffer `buf` (the lower directions are filled already).  Block interfaces
 // read the SAME buffer of the neighbour block: with several blocks, direction d is filled in every block before
 // direction d+1 in any (edge and corner ghosts then arrive from the diagonal neighbours in two steps).
-static void fill_ghosts_dir(meg6_grid* g, int buf, int d) {
+static cudaError_t fill_ghosts_dir(meg6_grid* g, int buf, int d) {
   const Consts& c = g->c;
   double* const* Pc = buf ? g->Pb : g->P;
   P6 P;
@@ -416,10 +424,15 @@ static void fill_ghosts_dir(meg6_grid* g, int buf, int d) {
   }
   ProfScope ps(g, 2, 1);
   k_ghost<<<nblk(ea * eb * 12, 256), 256, 0, g->stream>>>(c, d, P, gin);
+  return cudaGetLastError();
 }
 
-static void fill_ghosts(meg6_grid* g, int buf) {
-  for (int d = 0; d < 3; ++d) fill_ghosts_dir(g, buf, d);
+static cudaError_t fill_ghosts(meg6_grid* g, int buf) {
+  for (int d = 0; d < 3; ++d) {
+    const cudaError_t e = fill_ghosts_dir(g, buf, d);
+    if (e != cudaSuccess) return e;
+  }
+  return cudaSuccess;
 }
 
 static bool links_ok(const meg6_grid* g, bool single) {
@@ -454,8 +467,9 @@ static meg6_status stage_sweeps(meg6_grid* g, int buf, const Fuse3& fu) {
     ProfScope ps(g, 3, 1);
     k_grad<<<dim3(nblk(c.LG.pi, 32), nblk(c.n[1] + 2, 8), nblk(c.n[2] + 2, GRAD_KB)), dim3(32, 8, 1), 0, g->stream>>>(c, P, G);
   }
+  CUDA_OK(cudaGetLastError());
   FluxIn3 i3;
-  i3.res = g->res; i3.stats = g->stats_on ? g->stats : nullptr; i3.moving = g->p.moving ? 1 : 0;
+  i3.res = g->res; i3.stats = g->stats_on ? g->stats : nullptr; i3.moving = g->p.moving ? 1 : 0; i3.mask = nullptr;
   const bool V = g->p.viscous != 0;
   TmaMaps tm[3] = {g->tmaps3[buf][0], g->tmaps3[buf][1], g->tmaps3[buf][2]};
   if (fu.tail_tma) { tm[0].U = g->mapU; tm[0].U0 = g->mapU0; tm[0].J = g->mapJ; if (g->sigma) tm[0].Sg = g->mapSg; }
@@ -467,18 +481,19 @@ static meg6_status stage_sweeps(meg6_grid* g, int buf, const Fuse3& fu) {
   // sweep order eta, zeta, xi: the fused final phase then works on rows that are contiguous along xi
   {
     ProfScope ps(g, 5, 1);
-    i3.first = 1;
+    i3.first = 1; i3.mask = g->bmask[1];
     dim3 grid(nblk(c.n[0], Cfg3<1, false>::TT), nblk(c.n[1], Cfg3<1, false>::TS), c.n[2]);
     if (V) LAUNCH3(1, true, false, grid); else LAUNCH3(1, false, false, grid);
   }
   {
     ProfScope ps(g, 6, 1);
-    i3.first = 0;
+    i3.first = 0; i3.mask = g->bmask[2];
     dim3 grid(nblk(c.n[0], Cfg3<2, false>::TT), nblk(c.n[2], Cfg3<2, false>::TS), c.n[1]);
     if (V) LAUNCH3(2, true, false, grid); else LAUNCH3(2, false, false, grid);
   }
   {
     ProfScope ps(g, 4, 1);
+    i3.mask = g->bmask[0];
     dim3 grid(nblk(c.n[0], Cfg3<0, false>::TS), nblk(c.n[1], Cfg3<0, false>::TT), c.n[2]);
     if (V) LAUNCH3(0, true, true, grid); else LAUNCH3(0, false, true, grid);
   }
@@ -488,15 +503,16 @@ static meg6_status stage_sweeps(meg6_grid* g, int buf, const Fuse3& fu) {
 }
 
 static meg6_status stage(meg6_grid* g, int buf, const Fuse3& fu) {
-  fill_ghosts(g, buf);
+  CUDA_OK(fill_ghosts(g, buf));
   return stage_sweeps(g, buf, fu);
 }
 
-static void launch_prim(meg6_grid* g, const double* U) {
+static cudaError_t launch_prim(meg6_grid* g, const double* U) {
   P6 P;
   for (int f = 0; f < 6; ++f) P.p[f] = g->P[f];
   ProfScope ps(g, 1, 1);
   k_prim<<<nblk(g->c.LC.n, 256), 256, 0, g->stream>>>(g->c, U, P);
+  return cudaGetLastError();
 }
 
 static Fuse3 make_fuse(meg6_grid* g, const double* U, double* out) {
@@ -524,7 +540,7 @@ meg6_status meg6_rhs(meg6_grid* g, const double* U, double* dUdt) {
   if (!g || !U || !dUdt) return fail(MEG6_EINVAL, "rhs: null pointer%s");
   if (!g->have_metrics) return fail(MEG6_ESTATE, "rhs called before metrics_compute%s");
   if (!links_ok(g, true)) return fail(MEG6_ESTATE, "rhs: block-interface face without a link, or linked to another block (use meg6_rhs_blocks)%s");
-  launch_prim(g, U);
+  CUDA_OK(launch_prim(g, U));
   Fuse3 fu = make_fuse(g, U, dUdt);
   fu.mode = 0;
   return stage(g, 0, fu);
@@ -546,7 +562,7 @@ meg6_status meg6_rk3_step(meg6_grid* g, double* U, double t, double dt) {
   if (!g->have_metrics && !g->p.moving) return fail(MEG6_ESTATE, "rk3_step called before metrics_compute%s");
   if (!links_ok(g, true)) return fail(MEG6_ESTATE, "rk3_step: block-interface face without a link, or linked to another block (use meg6_rk3_step_blocks)%s");
   const double ts[3] = {t, t + dt, t + 0.5 * dt};
-  launch_prim(g, U);   // the caller owns U: its primitives are recomputed at every step
+  CUDA_OK(launch_prim(g, U));   // the caller owns U: its primitives are recomputed at every step
   for (int s = 0; s < 3; ++s) {
     meg6_status st;
     if (g->p.moving && (st = meg6_metrics_compute(g, ts[s])) != MEG6_OK) return st;
@@ -592,10 +608,10 @@ meg6_status meg6_rhs_blocks(int n, meg6_grid* const* g, const double* const* U, 
   for (int b = 0; b < n; ++b) {
     if (!U[b] || !dUdt[b]) return fail(MEG6_EINVAL, "rhs_blocks: null pointer%s");
     if (!g[b]->have_metrics) return fail(MEG6_ESTATE, "rhs_blocks called before metrics_compute%s");
-    launch_prim(g[b], U[b]);
+    CUDA_OK(launch_prim(g[b], U[b]));
   }
   for (int d = 0; d < 3; ++d)
-    for (int b = 0; b < n; ++b) fill_ghosts_dir(g[b], 0, d);
+    for (int b = 0; b < n; ++b) CUDA_OK(fill_ghosts_dir(g[b], 0, d));
   for (int b = 0; b < n; ++b) {
     Fuse3 fu = make_fuse(g[b], U[b], dUdt[b]);
     fu.mode = 0;
@@ -611,7 +627,7 @@ meg6_status meg6_rk3_step_blocks(int n, meg6_grid* const* g, double* const* U, d
   for (int b = 0; b < n; ++b) {
     if (!U[b]) return fail(MEG6_EINVAL, "rk3_step_blocks: null pointer%s");
     if (!g[b]->have_metrics && !g[b]->p.moving) return fail(MEG6_ESTATE, "rk3_step_blocks called before metrics_compute%s");
-    launch_prim(g[b], U[b]);
+    CUDA_OK(launch_prim(g[b], U[b]));
   }
   const double ts[3] = {t, t + dt, t + 0.5 * dt};
   for (int s = 0; s < 3; ++s) {
@@ -620,7 +636,7 @@ meg6_status meg6_rk3_step_blocks(int n, meg6_grid* const* g, double* const* U, d
     for (int b = 0; b < n; ++b)
       if (g[b]->p.moving && (st = meg6_metrics_compute(g[b], ts[s])) != MEG6_OK) return st;
     for (int d = 0; d < 3; ++d)
-      for (int b = 0; b < n; ++b) fill_ghosts_dir(g[b], s & 1, d);
+      for (int b = 0; b < n; ++b) CUDA_OK(fill_ghosts_dir(g[b], s & 1, d));
     for (int b = 0; b < n; ++b)
       if ((st = stage_sweeps(g[b], s & 1, make_fuse_rk(g[b], U[b], s, dt))) != MEG6_OK) return st;
   }
@@ -650,7 +666,7 @@ static bool staged_ok(const meg6_grid* g) {
 
 meg6_status meg6_stage_prim(meg6_grid* g, const double* U) {
   if (!g || !U) return fail(MEG6_EINVAL, "stage_prim: null pointer%s");
-  launch_prim(g, U);
+  CUDA_OK(launch_prim(g, U));
   return MEG6_OK;
 }
 
@@ -658,8 +674,7 @@ meg6_status meg6_stage_ghosts(meg6_grid* g, int s, int d) {
   if (!g || s < 0 || s > 2 || d < 0 || d > 2) return fail(MEG6_EINVAL, "stage_ghosts: bad argument%s");
   if (!g->have_metrics) return fail(MEG6_ESTATE, "stage_ghosts called before metrics_compute%s");
   if (!staged_ok(g)) return fail(MEG6_ESTATE, "stage_ghosts: block-interface face without a link or a buffer%s");
-  fill_ghosts_dir(g, s & 1, d);
-  CUDA_OK(cudaGetLastError());
+  CUDA_OK(fill_ghosts_dir(g, s & 1, d));
   return MEG6_OK;
 }
 
@@ -710,10 +725,8 @@ meg6_status meg6_diagnostics(meg6_grid* g, const double* U, double* out) {
   if (!g || !U || !out) return fail(MEG6_EINVAL, "diagnostics: null pointer%s");
   if (!g->have_metrics) return fail(MEG6_ESTATE, "diagnostics called before metrics_compute%s");
   const Consts& c = g->c;
-  launch_prim(g, U);
-  P6 P;
-  for (int f = 0; f < 6; ++f) P.p[f] = g->P[f];
-  fill_ghosts(g, 0);
+  CUDA_OK(launch_prim(g, U));
+  CUDA_OK(fill_ghosts(g, 0));
   DiagIn in;
   memset(&in, 0, sizeof(in));
   for (int q = 0; q < 9; ++q) in.met[q] = g->met[q];
@@ -741,9 +754,42 @@ meg6_status meg6_diagnostics(meg6_grid* g, const double* U, double* out) {
   return MEG6_OK;
 }
 
+meg6_status meg6_fp64_peak(void* cuda_stream, double* scratch, double* dfma_per_second) {
+  if (!scratch || !dfma_per_second) return fail(MEG6_EINVAL, "fp64_peak: null pointer%s");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  int dev = 0, nsm = 0;
+  CUDA_OK(cudaGetDevice(&dev));
+  CUDA_OK(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
+  const int blocks = nsm * 8 * 4;   // four waves of eight 256-thread CTAs per SM
+  cudaEvent_t e0, e1;
+  CUDA_OK(cudaEventCreate(&e0));
+  CUDA_OK(cudaEventCreate(&e1));
+  double best = 0.0;
+  for (int rep = 0; rep < 4; ++rep) {   // the first repetition warms up
+    cudaEventRecord(e0, st);
+    k_dfma_probe<<<blocks, PROBE_THREADS, 0, st>>>(1.0000001, 1e-9, scratch);
+    cudaEventRecord(e1, st);
+    cudaError_t e = cudaEventSynchronize(e1);
+    float ms = 0.f;
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+    if (e != cudaSuccess) { cudaEventDestroy(e0); cudaEventDestroy(e1); return fail(MEG6_ECUDA, "fp64_peak: %s", cudaGetErrorString(e)); }
+    const double rate = (double)blocks * PROBE_THREADS * PROBE_CHAINS * PROBE_ITERS / (ms * 1e-3);
+    if (rep > 0 && rate > best) best = rate;
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  *dfma_per_second = best;
+  return MEG6_OK;
+}
+
 meg6_status meg6_limiter_stats_enable(meg6_grid* g, int on) {
   if (!g) return fail(MEG6_EINVAL, "null grid%s");
   g->stats_on = on ? 1 : 0;
+  return MEG6_OK;
+}
+
+meg6_status meg6_set_branch_masks(meg6_grid* g, unsigned short* xi, unsigned short* eta, unsigned short* zeta) {
+  if (!g) return fail(MEG6_EINVAL, "null grid%s");
+  g->bmask[0] = xi; g->bmask[1] = eta; g->bmask[2] = zeta;
   return MEG6_OK;
 }
 

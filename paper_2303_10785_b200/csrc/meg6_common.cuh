@@ -108,9 +108,12 @@ struct meg6_grid {
   const double* ibuf[6];       // bc 5: or a packed copy of the neighbour's layers (meg6_set_interface_buffer)
   const double* sigma; const double* uref;
   unsigned long long* stats;   // [2] device counters: limited, tested
+  unsigned short* bmask[3];    // caller's branch-record arrays per interface family (meg6_set_branch_masks) or null
   double* red;                 // reduction scratch
   int stats_on;
   bool have_metrics;
+  int geom_blocked;            // -1 by size, 0 / 1 forced (MEG6_GEOM_BLOCKED in the environment at grid_create; tests)
+  int geom_launches;           // kernels launched by the last metrics_compute
   // per-kernel timing (meg6_profile_*): event pairs of the launches since the last read
   int prof_on;
   std::vector<cudaEvent_t> prof_pool;

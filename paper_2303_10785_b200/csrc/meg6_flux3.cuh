@@ -99,6 +99,7 @@ __device__ __forceinline__ int sidx3(int f, int a, int t, int LA) {
 struct FluxIn3 {
   double* res;                  // [5] running residual, layout LR, field stride fsR
   unsigned long long* stats;    // limiter counters or null
+  unsigned short* mask;         // branch record of this family's interfaces (meg6_set_branch_masks) or null
   int first, moving;
 };
 
@@ -153,10 +154,22 @@ __device__ __forceinline__ double lds_again(const double* p) {
 // branches were measured SLOWER in round 1 (more live registers, more spills).
 __device__ __forceinline__ double rcp3(double x) { return 1.0 / x; }
 
+// min / max of two doubles as one compare and one select.  The library fmin / fmax carry IEEE NaN handling and compile
+// to DSETP + SEL + FSEL + LOP3 + three or four register moves each (sm_100a has no FP64 min/max instruction; SASS of the
+// round-1 build: 8 instructions per call, 24 % of the limiting path); a NaN here means the state is lost anyway.  For
+// ordered operands the result is the same value bit for bit (the limiter's own +-0 cases select equal magnitudes).
+// Unordered operands: the forms below are those of std::min / std::max -- the first operand comes back when the
+// second is a NaN -- which is what the step-by-step CPU restatement of the method does at an interface whose limited
+// right state has left the physical range (sound speed of a negative density: the violent inflow interface of the
+// randomised parity case), so such an interface takes the same branch of Eq. 26 on both sides.
+__device__ __forceinline__ double dmin3(double a, double b) { return (b < a) ? b : a; }
+__device__ __forceinline__ double dmax3(double a, double b) { return (a < b) ? b : a; }
+
 __device__ __forceinline__ double minmod3(double a, double b) {   // E.2
-  const double m = fmin(fabs(a), fabs(b));
+  // same sign: the operand of smaller magnitude IS sign * min(|a|, |b|)
+  const double m = (fabs(b) < fabs(a)) ? b : a;
   const bool same = ((__double2hiint(a) ^ __double2hiint(b)) >= 0);
-  return same ? copysign(m, a) : 0.0;
+  return same ? m : 0.0;
 }
 
 struct Eig3 { double nx, ny, nz, ra, a2; };
@@ -190,21 +203,22 @@ __device__ __forceinline__ double mp_limit3(double e, double dp, double dm, doub
   const double wmd = 0.5 * (dp - dnear);
   const double wul = alpha * dm;
   const double wlc = fma(4.0 / 3.0, dfar, 0.5 * dm);
-  const double wmin = fmax(fmin(fmin(0.0, dp), wmd), fmin(fmin(0.0, wul), wlc));
-  const double wmax = fmin(fmax(fmax(0.0, dp), wmd), fmax(fmax(0.0, wul), wlc));
+  const double wmin = dmax3(dmin3(dmin3(0.0, dp), wmd), dmin3(dmin3(0.0, wul), wlc));
+  const double wmax = dmin3(dmax3(dmax3(0.0, dp), wmd), dmax3(dmax3(0.0, wul), wlc));
   return e + minmod3(wmin - e, wmax - e);   // E.4
 }
 
 // Contravariant HLLC, Eq. 26-27 with the flux of Eq. 2; energy row R9; cascade R10.
-__device__ __forceinline__ void hllc3(const double PL[5], const double PR[5], double mx, double my, double mz, double mt,
-                                      double g, double g2, double ig2, double gamma, double igm1, double F[5]) {
+// Returns the branch 0..3 of Eq. 26 taken.
+__device__ __forceinline__ unsigned hllc3(const double PL[5], const double PR[5], double mx, double my, double mz, double mt,
+                                          double g, double g2, double ig2, double gamma, double igm1, double F[5]) {
   const double UL = fma(mz, PL[3], fma(my, PL[2], fma(mx, PL[1], mt)));
   const double UR = fma(mz, PR[3], fma(my, PR[2], fma(mx, PR[1], mt)));
   const double t = rcp3(PL[0] * PR[0]);
   const double irL = PR[0] * t, irR = PL[0] * t;
   const double cL = sqrt(gamma * PL[4] * irL) * g, cR = sqrt(gamma * PR[4] * irR) * g;
-  const double SL = fmin(UL - cL, UR - cR);
-  const double SR = fmax(UL + cL, UR + cR);
+  const double SL = dmin3(UL - cL, UR - cR);
+  const double SR = dmax3(UL + cL, UR + cR);
   const double mL = PL[0] * (SL - UL), mR = PR[0] * (SR - UR);
   const double SS = (fma(mR, UR, -mL * UL) + (PL[4] - PR[4]) * g2) * rcp3(mR - mL);
   const bool left = (SL >= 0.0) || (SS >= 0.0);
@@ -233,6 +247,7 @@ __device__ __forceinline__ void hllc3(const double PL[5], const double PR[5], do
     F[3] = fma(SK, fma(rk, w, fd * mz), F[3]);
     F[4] = fma(SK, fma(k, E + p, fd * (SS - mt)), F[4]);
   }
+  return left ? (star ? 1u : 0u) : (star ? 2u : 3u);
 }
 
 // One interface: O3 steps 1-8 (inviscid, Fig. 3) and O4 (alpha-damping viscous flux, Fig. 5; subtracted from F).
@@ -240,7 +255,8 @@ __device__ __forceinline__ void hllc3(const double PL[5], const double PR[5], do
 //   pA   : aL field 0 of cell L-1 in the offset tile              (aR fields are 5 FA further)
 //   pT1  : T' of cell L;  pG: stored tangential gradients at cell L;  pM: interface metrics (field stride FM)
 // SS = stride between consecutive cells along the sweep; FP/FA/FG/FM = field strides.
-// Returns the E.1 flags (bit r: left state of component r limited, bit 5+r: right state).
+// Returns the E.1 flags (bit r: left state of component r limited, bit 5+r: right state) and, in bits 10-11, the
+// branch of Eq. 26 the HLLC flux took.
 template <int DIR, bool VISC, int SS, int FP, int FA, int FG, int FM, int GSLOT, bool IG4>
 __device__ __forceinline__ unsigned face3(const Consts& c, const double* __restrict__ pP, const double* __restrict__ pA,
                                           const double* __restrict__ pT1, const double* __restrict__ pG,
@@ -310,7 +326,7 @@ __device__ __forceinline__ unsigned face3(const Consts& c, const double* __restr
 #endif
   backproject3(e, ia2, h_ira, EL, BL, PL);   // Eq. 23
   backproject3(e, ia2, h_ira, ER, BR, PR);
-  hllc3(PL, PR, mx, my, mz, mt, g, g2, ig2, c.gamma, c.igm1, F);
+  fl |= hllc3(PL, PR, mx, my, mz, mt, g, g2, ig2, c.gamma, c.igm1, F) << 10;
 
   if (VISC) {
     // O4: Eq. 29-35.  fields (u,v,w,T); normal gradient with alpha^D = 4, beta^D = 0.
@@ -590,7 +606,16 @@ k_flux3(const Consts c, const FluxIn3 in, const __grid_constant__ TmaMaps tm, co
         IG4 ? sQ + sidx3<DIR, TT>(5, sI + 2 + C::QOFF, row, LQ) : sT1 + sidx3<DIR, TT>(0, sI, row, LT),
         sG + sidx3<DIR, TT>(0, sI + C::GOFF, row, LG),
         sM + sidx3<DIR, TT>(0, sI, row, LF), mt, F);
-    if (sI < TS || s0 + sI == nd) { nlim = __popc(fl); ntst = 10; }   // tile-shared faces counted once
+    if (sI < TS || s0 + sI == nd) {   // tile-shared faces counted once
+      nlim = __popc(fl & 1023u); ntst = 10;
+      if (in.mask) {   // interface (s0 + sI) of n_d + 1 along the sweep, interior extents along the others, i fastest
+        long long im;
+        if (DIR == 0) im = ((long long)o * c.n[1] + (t0 + row)) * (c.n[0] + 1) + (s0 + sI);
+        else if (DIR == 1) im = ((long long)o * (c.n[1] + 1) + (s0 + sI)) * c.n[0] + (t0 + row);
+        else im = ((long long)(s0 + sI) * c.n[1] + o) * c.n[0] + (t0 + row);
+        in.mask[im] = (unsigned short)fl;
+      }
+    }
   }
   if (DIR != 0 && sI <= TS) {
     // the flux tile aliases the metric tile: slot (sI,row) of every metric field is read only by this thread

@@ -15,6 +15,7 @@ static inline unsigned nblk(long long n, int t) { return (unsigned)((n + t - 1) 
 static void launch_centres(meg6_grid* g, const GeomIn& gi, P3 xc, P3 xt) {
   const Consts& c = g->c;
   k_centres<<<nblk(c.LC.n, 256), 256, 0, g->stream>>>(c, gi, xc, xt);
+  g->geom_launches += 4;
   for (int d = 0; d < 3; ++d) {
     int a = (d + 1) % 3, b = (d + 2) % 3;
     if (a > b) { int t = a; a = b; b = t; }
@@ -47,6 +48,7 @@ Box launch_ig4_batch(meg6_grid* g, const Lay& L, const double* f, const Box& fb,
   if (dir == 0) k_ig4x<<<grid, 128, 0, g->stream>>>(L, f, out, ob, g->ig4_cc, g->ig4_den, fs_in, fs_out);
   else if (dir == 1) k_ig4<1><<<grid, 128, 0, g->stream>>>(L, f, out, ob, g->ig4_cc, g->ig4_den, fs_in, fs_out);
   else k_ig4<2><<<grid, 128, 0, g->stream>>>(L, f, out, ob, g->ig4_cc, g->ig4_den, fs_in, fs_out);
+  ++g->geom_launches;
   return ob;
 }
 
@@ -79,6 +81,7 @@ static Box H_pass(meg6_grid* g, const double* f, const Box& fb, int dir, double*
   Box hb = gb;
   hb.lo[dir] += 1; hb.hi[dir] -= 2;
   k_H_from<<<nblk(box_n(hb), 256), 256, 0, g->stream>>>(L, L, dir, 0, f, f1, H, hb);
+  ++g->geom_launches;
   return hb;
 }
 // consistent derivative Eq. 37 of f along dir into out
@@ -87,6 +90,7 @@ static Box delta_pass(meg6_grid* g, const double* f, const Box& fb, int dir, dou
   Box db = hb;
   db.lo[dir] += 1;
   k_point<<<nblk(box_n(db), 256), 256, 0, g->stream>>>(g->c.LX, 0, dir, H, nullptr, out, db);
+  ++g->geom_launches;
   return db;
 }
 
@@ -115,6 +119,7 @@ static cudaError_t launch_geometry_ig4(meg6_grid* g, const GeomIn& gi) {
       const Box e2 = delta_pass(g, t2, b2, a, f1, H, d2);
       mb[3 * r + cc] = box_and(e1, e2);
       k_point<<<nblk(box_n(mb[3 * r + cc]), 256), 256, 0, g->stream>>>(L, 2, 0, d1, d2, g->met[3 * r + cc], mb[3 * r + cc]);
+      g->geom_launches += 3;
     }
   }
   Box rjb = all;
@@ -123,6 +128,7 @@ static cudaError_t launch_geometry_ig4(meg6_grid* g, const GeomIn& gi) {
     P9c cd;
     for (int q = 0; q < 9; ++q) cd.p[q] = g->cd[q];
     k_rj_box<<<nblk(box_n(rjb), 256), 256, 0, g->stream>>>(L, cd, g->rj, rjb);
+    ++g->geom_launches;
   }
   Box mtb[3];
   if (g->p.moving) {
@@ -133,6 +139,7 @@ static cudaError_t launch_geometry_ig4(meg6_grid* g, const GeomIn& gi) {
       mtb[r] = mb[3 * r];
       k_mt_box<<<nblk(box_n(mtb[r]), 256), 256, 0, g->stream>>>(L, vt, g->met[3 * r], g->met[3 * r + 1], g->met[3 * r + 2],
                                                                  g->mt[r], mtb[r]);
+      ++g->geom_launches;
     }
   }
   // interface metrics: each hatted quantity interpolated as a whole, Eq. 38
@@ -152,9 +159,10 @@ static cudaError_t launch_geometry_ig4(meg6_grid* g, const GeomIn& gi) {
       for (int a = 0; a < 3; ++a)
         if (hb.lo[a] > fb.lo[a] || hb.hi[a] < fb.hi[a]) return cudaErrorInvalidValue;   // ghost depth too small
       k_H_from<<<nblk(box_n(fb), 256), 256, 0, g->stream>>>(L, c.LF[d], d, 1, src, f1, dst, fb);
+      ++g->geom_launches;
     }
   }
-  if (g->p.moving) k_rjt<<<nblk(c.LC.n, 256), 256, 0, g->stream>>>(c, g->fmt[0], g->fmt[1], g->fmt[2], g->rjt);
+  if (g->p.moving) { k_rjt<<<nblk(c.LC.n, 256), 256, 0, g->stream>>>(c, g->fmt[0], g->fmt[1], g->fmt[2], g->rjt); ++g->geom_launches; }
   return cudaGetLastError();
 }
 
@@ -173,9 +181,10 @@ cudaError_t launch_geometry(meg6_grid* g, double t) {
   launch_centres(g, gi, xc, xt);
   // blocking along the grid line trades threads for shared intermediates: it pays once the grid fills the GPU several
   // times over (256^3: -7 % per call), not on config 2's 64^3 (+3 %)
-  // MEG6_GEOM_BLOCKED=0/1 in the environment forces the choice (the parity tests run both forms on the same small grids)
-  const char* forced = getenv("MEG6_GEOM_BLOCKED");
-  const bool blocked = forced ? (forced[0] == '1') : (c.LC.n >= (1LL << 21));
+  // MEG6_GEOM_BLOCKED=0/1 in the environment at grid_create forces the choice (the parity tests run both forms on the
+  // same small grids)
+  const bool blocked = g->geom_blocked >= 0 ? (g->geom_blocked == 1) : (c.LC.n >= (1LL << 21));
+  g->geom_launches += 1 + 3 + 3 + (g->p.moving ? 1 : 0);   // coordinate derivatives, metric sweeps, interface families, GCL
 #if MEG6_CD_KB > 1
   if (blocked) k_coord_deriv_blk<MEG6_CD_KB><<<nblk((long long)c.LX.pi * c.LX.pj * nblk(c.n[2] + 2 * GX, MEG6_CD_KB), T), T, 0, g->stream>>>(c, xc, cd, g->rj);
   else

@@ -10,6 +10,8 @@ if ROOT not in sys.path:
 
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box)")
+    config.addinivalue_line("markers", "slow: minutes of CPU-oracle time (step-count parity at the configs' own sizes); "
+                                       "part of -m gpu, deselect with -m 'gpu and not slow' while iterating")
 
 
 @pytest.fixture(scope="session", autouse=True)

@@ -12,6 +12,10 @@ pytestmark = pytest.mark.gpu
 
 RHS_TOL = 1e-11
 STEP_TOL = 1e-9
+# the same right-hand sides in the norm of SURVEY 8(d) as written (per component, by that component's own maximum): the
+# 1e-11 bound holds as it stands except for config 3, whose mass equation is 1e-3 of the flux scale at Ma 0.1 (its
+# round-off is that of the fluxes: the bound is loosened by that factor)
+STRICT_RHS_TOL = {"c1": 1e-11, "c2": 1e-11, "c3": 1e-8, "c4": 1e-11}
 
 
 @pytest.fixture(scope="module")
@@ -50,6 +54,44 @@ def rhs_err(a, b, U, gamma=1.4):
     mag = np.abs(b).reshape(5, -1).max(1) / ref
     scale = ref * mag.max()
     return np.abs(a - b).reshape(5, -1).max(1) / scale
+
+
+def strict_rel(a, b):
+    """SURVEY 8(d) as written: per-component max |a-b| / max |b_c|, every component by its own magnitude"""
+    n = a.shape[0]
+    return np.abs(a - b).reshape(n, -1).max(1) / np.maximum(np.abs(b).reshape(n, -1).max(1), 1e-300)
+
+
+def flip_report(g, og, shape):
+    """Branch records of the two sides after the same right-hand side (include/meg6.h: bits 0-9 test E.1 per
+    characteristic component and side, bits 10-11 branch of Eq. 26), compared bit for bit.  Returns
+    (report dict, boolean cell array: cells next to an interface whose record differs)."""
+    nk, nj, ni = shape
+    touched = np.zeros(shape, dtype=bool)
+    rep = {"interfaces": 0, "e1_flips": 0, "hllc_flips": 0, "hllc_flips_at_ties": 0, "ties": 0, "flipped": []}
+    for d in range(3):
+        a, b = g.branch_mask_host(d), og.branch_mask(d)
+        assert a.shape == b.shape
+        rep["interfaces"] += a.size
+        tie = (b >> 12) & 1          # oracle only: the cascade of Eq. 26 tested a wave speed that is zero to 1e-10 (R10)
+        rep["ties"] += int(tie.sum())
+        x = (a ^ b) & 0x0FFF
+        hl = (x >> 10) != 0
+        rep["e1_flips"] += int(sum(((x >> bit) & 1).sum() for bit in range(10)))
+        rep["hllc_flips_at_ties"] += int((hl & (tie == 1)).sum())
+        rep["hllc_flips"] += int((hl & (tie == 0)).sum())
+        # listed and attributed: every differing E.1 decision and every differing DECISIVE branch of Eq. 26; a tie flips
+        # with the rounding order and gives the same flux either way (counted above)
+        idx = np.argwhere(((x & 0x3FF) != 0) | (hl & (tie == 0)))
+        for k, j, i in idx:
+            if len(rep["flipped"]) < 20:
+                rep["flipped"].append((d, int(i), int(j), int(k), int(a[k, j, i]), int(b[k, j, i])))
+            for off in (-1, 0):     # interface s of family d lies between cells s-1 and s
+                c = [k, j, i]
+                c[2 - d] += off
+                if 0 <= c[2 - d] < shape[2 - d]:
+                    touched[c[0], c[1], c[2]] = True
+    return rep, touched
 
 
 def small_cases():
@@ -118,10 +160,12 @@ def test_rhs_parity(mods, cases, name):
     t = 0.13 if wl["params"]["moving"] else 0.0
     og = O.Grid(wl)
     og.metrics_compute(t)
+    og.branch_masks_enable(True)
     ref = og.rhs(wl["U0"])
     g = M.Grid(wl)
     g.metrics_compute(t)
     g.limiter_stats_enable(True)
+    g.branch_masks_enable(True)
     U = torch.as_tensor(wl["U0"], device="cuda").contiguous()
     out = g.rhs(U).cpu().numpy()
     for f in range(6):
@@ -129,14 +173,25 @@ def test_rhs_parity(mods, cases, name):
         assert np.abs(a - b).max() <= 1e-14 * np.abs(b).max()
     e = rhs_err(out, ref, wl["U0"])
     assert np.all(e <= RHS_TOL), (name, e, rel(out, ref))
-    # limiter branch statistics: same interfaces tested; flips reported, must be rare
+    # the norm of SURVEY 8(d) as written (every component by its own magnitude) is recorded and bounded as well: it
+    # differs from the one above only where a component is physically tiny (mass equation of the Ma 0.1 TGV)
+    es = strict_rel(out, ref)
+    assert np.all(es <= STRICT_RHS_TOL[name]), (name, es)
+    # branch decisions, interface by interface: same interfaces tested; every differing E.1 / Eq. 26 decision is listed
     lim_o, tst_o = og.limiter_stats()
     lim_g, tst_g = g.limiter_stats()
     assert tst_g == tst_o
-    assert abs(lim_g - lim_o) <= max(5, 1e-3 * lim_o), (lim_g, lim_o)
-    print("%s: per-component rel Linf %s" % (name, rel(out, ref)))
-    print("%s: rel Linf %s, limited %d/%d (oracle %d), branch-count difference %d"
-          % (name, e, lim_g, tst_g, lim_o, lim_g - lim_o))
+    rep, touched = flip_report(g, og, wl["U0"].shape[1:])
+    assert rep["e1_flips"] >= abs(lim_g - lim_o)
+    assert rep["e1_flips"] + rep["hllc_flips"] <= 1e-5 * rep["interfaces"] + 2, rep
+    if touched.any():   # the tolerance holds on the flipped cells too (the limiter and HLLC are continuous across
+        ef = np.abs(out - ref)[:, touched].max(1) / np.abs(ref).reshape(5, -1).max(1)   # their switches)
+        print("%s: %d cells next to flipped decisions, strict error there %s" % (name, int(touched.sum()), ef))
+    print("%s: strict per-component rel Linf %s" % (name, es))
+    print("%s: rel Linf %s, limited %d/%d (oracle %d); flipped E.1 decisions %d, flipped decisive Eq. 26 branches %d "
+          "(+ %d at the %d ties) of %d interfaces: %s" % (name, e, lim_g, tst_g, lim_o, rep["e1_flips"],
+                                                          rep["hllc_flips"], rep["hllc_flips_at_ties"], rep["ties"],
+                                                          rep["interfaces"], rep["flipped"]))
     # time step formula
     assert g.cfl_dt(U, 0.2) == pytest.approx(og.cfl_dt(wl["U0"], 0.2), rel=1e-12)
     g.close()

@@ -1,0 +1,104 @@
+"""Step-count parity at the configs' own sizes (BASELINE.json north_star: "1e-9 after the config's step count"; SURVEY
+8(d): full step counts on C1-C3, >= 20 steps on C4/C5 where the oracle is too slow for all of them).
+
+The CPU oracle needs minutes for these (config 3: 128^3 x 200 steps ~ 7 min on 16 host cores; config 4: 20 steps of
+12.8 M cells ~ 5 min), hence the extra marker `slow` -- they are part of `-m gpu`.  Every test reports, per step, the
+number of interface-components that failed test E.1 on each side, and after the last right-hand side the branch records
+(E.1 per component and side, branch of Eq. 26) are compared interface by interface: flipped decisions are listed.
+"""
+import time
+
+import numpy as np
+import pytest
+
+import workloads as W
+from test_gpu_parity import STEP_TOL, flip_report, mods, rel, strict_rel  # noqa: F401
+
+pytestmark = [pytest.mark.gpu, pytest.mark.slow]
+
+
+def run_both(torch, O, M, wl, U0, steps, t0=0.0, dt=None, label=""):
+    og = O.Grid(wl)
+    og.metrics_compute(t0)
+    g = M.Grid(wl)
+    g.metrics_compute(t0)
+    U = torch.as_tensor(U0, device="cuda").contiguous()
+    if dt is None:
+        dt = g.cfl_dt(U, wl["cfl"])
+        assert dt == pytest.approx(og.cfl_dt(U0, wl["cfl"]), rel=1e-12)
+    Uo = U0.copy()
+    g.limiter_stats_enable(True)
+    g.branch_masks_enable(True)
+    og.branch_masks_enable(True)
+    hist = []
+    lo0 = lg0 = to0 = tg0 = 0
+    t = t0
+    wall = time.time()
+    for s in range(steps):
+        og.rk3_step(Uo, t, dt)
+        g.rk3_step(U, t, dt)
+        t += dt
+        lo, to = og.limiter_stats()
+        lg, tg = g.limiter_stats()
+        hist.append((lo - lo0, lg - lg0))
+        tested = to - to0
+        assert tg - tg0 == tested
+        lo0, lg0, to0, tg0 = lo, lg, to, tg
+        if s in (0, 1, 4, 9, 19, 49, 99, 199) or s == steps - 1:
+            print("%s step %d: rel %s, limited this step oracle %d gpu %d of %d" % (
+                label, s + 1, rel(U.cpu().numpy(), Uo), hist[-1][0], hist[-1][1], tested))
+    wall = time.time() - wall
+    Ug = U.cpu().numpy()
+    rep, touched = flip_report(g, og, U0.shape[1:])
+    diffs = [a - b for a, b in hist]
+    print("%s: %d steps in %.0f s; per-step limited-count differences (oracle - gpu): min %d max %d, nonzero in %d steps"
+          % (label, steps, wall, min(diffs), max(diffs), sum(1 for d in diffs if d)))
+    print("%s: last right-hand side: %d flipped E.1 decisions, %d flipped decisive Eq. 26 branches (+ %d at the %d ties, "
+          "R10) of %d interfaces; first: %s" % (label, rep["e1_flips"], rep["hllc_flips"], rep["hllc_flips_at_ties"],
+                                                rep["ties"], rep["interfaces"], rep["flipped"]))
+    print("%s: strict per-component rel %s" % (label, strict_rel(Ug, Uo)))
+    g.close()
+    return Ug, Uo, rep, touched, hist
+
+
+def test_c3_128_200_steps(mods):
+    """Config 3 as BASELINE.json states it: 128^3 wavy mesh, viscous TGV, CFL 0.2, all 200 RK3 steps, every cell."""
+    torch, O, M = mods
+    wl = W.c3_tgv(n=128)
+    Ug, Uo, rep, touched, hist = run_both(torch, O, M, wl, wl["U0"], 200, label="c3 128^3")
+    e = rel(Ug, Uo)
+    assert np.all(e <= STEP_TOL), e
+    assert hist[-1][0] > 0.02 * 30 * 128 ** 3 * 3       # 3.4 % of the interface-components are limited in every stage
+    assert rep["e1_flips"] + rep["hllc_flips"] <= 20, rep
+
+
+def test_c4_full_size_20_steps_from_the_developed_state(mods):
+    """Config 4 at full size (320 x 200 x 200), 20 RK3 steps starting from the DEVELOPED jet: the GPU advances the
+    initial state by 250 steps (the middle of the config's 500-step run, the state bench.py times: shocks at the nozzle
+    lip, limiter active), both sides then take the same 20 steps from that state."""
+    torch, O, M = mods
+    wl = W.c4_jet()
+    g = M.Grid(wl)
+    g.metrics_compute(0.0)
+    U = torch.as_tensor(wl["U0"], device="cuda").contiguous()
+    for s in range(250):
+        g.rk3_step(U, s * wl["dt"], wl["dt"])
+    U250 = U.cpu().numpy()
+    g.close()
+    del U, g
+    assert np.isfinite(U250).all()
+    Ug, Uo, rep, touched, hist = run_both(torch, O, M, wl, U250, 20, t0=250 * wl["dt"], dt=wl["dt"], label="c4 developed")
+    e = rel(Ug, Uo)
+    assert np.all(e <= STEP_TOL), e
+    assert hist[-1][0] > 1e-3 * 30 * 12.8e6 * 3           # the limiter is at work in the developed state
+    assert rep["e1_flips"] + rep["hllc_flips"] <= 20, rep
+    assert np.abs(Ug - U250).max() > 1e-3                  # and the 20 steps did something
+
+
+def test_mig4_128_20_steps(mods):
+    """Config 5's scheme (MIG4) and flow at 128^3 (the smallest grid of its sweep), 20 RK3 steps, every cell."""
+    torch, O, M = mods
+    wl = W.c5_tgv_mig4(n=128, steps=20)
+    Ug, Uo, rep, touched, hist = run_both(torch, O, M, wl, wl["U0"], 20, label="c5 mig4 128^3")
+    e = rel(Ug, Uo)
+    assert np.all(e <= STEP_TOL), e

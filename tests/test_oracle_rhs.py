@@ -273,3 +273,41 @@ def test_isentropic_vortex_advection_order(wavy):
     rate = np.log2(errs[0] / errs[1])
     assert rate > 1.9, (errs, rate)
     assert errs[1] < 3e-4
+
+
+# ------------------------------------------------------------------ branch record (per-interface E.1 / Eq. 26 decisions)
+def test_branch_record_matches_counters_and_hllc_regimes():
+    """The per-interface branch record the parity tests compare with the GPU's (bits 0-9: E.1 failed per characteristic
+    component and side, bits 10-11: branch of Eq. 26, bit 12: tie): its population count is the limiter counter; a
+    uniform supersonic stream takes branch 0 (S_L >= 0: F_L) everywhere along +x and branch 3 against it, a subsonic one
+    the star branches 1 / 2 by the sign of S* = the contravariant velocity; fluid at rest is a tie (R10)."""
+    n = 12
+    x, y, z = W.wavy_periodic_grid(n, 6.0, 0.0)
+    prm = W._base_params(n, n, n, period=[[6.0, 0, 0], [0, 6.0, 0], [0, 0, 6.0]])
+    one = np.ones((n, n, n))
+    g = O.Grid(dict(params=prm, x=x, y=y, z=z))
+    g.metrics_compute(0.0)
+    g.branch_masks_enable(True)
+    a = np.sqrt(1.4)
+    for u, want_x, tie in ((2.0 * a, 0, 0), (-2.0 * a, 3, 0), (0.5 * a, 1, 0), (-0.5 * a, 2, 0), (0.0, None, 1)):
+        g.rhs(W.conservative(one, u * one, 0.3 * a * one, 0 * one, one))
+        m = g.branch_mask(0)
+        assert np.all((m & 0x3FF) == 0)                          # uniform state: nothing limited
+        assert np.all(((m >> 12) & 1) == tie)
+        if want_x is not None:
+            assert np.all(((m >> 10) & 3) == want_x), (u, np.unique((m >> 10) & 3))
+        assert np.all(((g.branch_mask(1) >> 10) & 3) == 1)       # v = +0.3 a: subsonic, S* > 0 along eta
+        assert np.all(((g.branch_mask(2) >> 12) & 1) == 1)       # w = 0: tie along zeta
+    # a state with a density step: some components limited; bits = counters
+    wl = W.c1_vortex(n=16)
+    U = wl["U0"].copy()
+    U[0, :, :, 8:] *= 1.5
+    g2 = O.Grid(wl)
+    g2.metrics_compute(0.0)
+    g2.branch_masks_enable(True)
+    l0, t0 = g2.limiter_stats()
+    g2.rhs(U)
+    l1, t1 = g2.limiter_stats()
+    bits = sum(int(((g2.branch_mask(d) >> b) & 1).sum()) for d in range(3) for b in range(10))
+    assert l1 - l0 == bits > 0
+    assert t1 - t0 == 10 * sum(g2.branch_mask(d).size for d in range(3))
