@@ -171,7 +171,7 @@ static bool make_maps3_dir(EncodeTiledFn fn, meg6_grid* g, int buf) {
     };
     int b[4];
     bool ok = true;
-    box(C::LP, C::TT, C::NF, b);
+    box(C::LPT, C::TT, C::NF, b);
     ok = ok && make_map4(fn, &t.P, buf ? g->Pb[0] : g->P[0], c.LP, c.fsP, 6, b);
     box(C::LF, C::TT, C::NM, b);
     ok = ok && make_map4(fn, &t.M, VISC ? g->fmet[DIR][0] : g->fmet[DIR][3 * DIR], c.LF[DIR], c.fsM[DIR], C::NM, b);
@@ -203,7 +203,7 @@ static bool make_maps3_dir(EncodeTiledFn fn, meg6_grid* g, int buf) {
   };
   int b[4];
   bool ok = true;
-  box(C::LP, C::TT, C::NF, b);
+  box(C::LPT, C::TT, C::NF, b);
   ok = ok && make_map4(fn, &t.P, buf ? g->Pb[0] : g->P[0], c.LP, c.fsP, 6, b);
   box(C::LF, C::TT, C::NM, b);
   ok = ok && make_map4(fn, &t.M, VISC ? g->fmet[DIR][0] : g->fmet[DIR][3 * DIR], c.LF[DIR], c.fsM[DIR], C::NM, b);
@@ -482,13 +482,13 @@ static meg6_status stage_sweeps(meg6_grid* g, int buf, const Fuse3& fu) {
   {
     ProfScope ps(g, 5, 1);
     i3.first = 1; i3.mask = g->bmask[1];
-    dim3 grid(nblk(c.n[0], Cfg3<1, false>::TT), nblk(c.n[1], Cfg3<1, false>::TS), c.n[2]);
+    dim3 grid(nblk(c.n[0], Cfg3<1, false>::TT), nblk(c.n[1], Cfg3<1, false>::TS * (IG ? 1 : Cfg3<1, false>::NSUB)), c.n[2]);
     if (V) LAUNCH3(1, true, false, grid); else LAUNCH3(1, false, false, grid);
   }
   {
     ProfScope ps(g, 6, 1);
     i3.first = 0; i3.mask = g->bmask[2];
-    dim3 grid(nblk(c.n[0], Cfg3<2, false>::TT), nblk(c.n[2], Cfg3<2, false>::TS), c.n[1]);
+    dim3 grid(nblk(c.n[0], Cfg3<2, false>::TT), nblk(c.n[2], Cfg3<2, false>::TS * (IG ? 1 : Cfg3<2, false>::NSUB)), c.n[1]);
     if (V) LAUNCH3(2, true, false, grid); else LAUNCH3(2, false, false, grid);
   }
   {

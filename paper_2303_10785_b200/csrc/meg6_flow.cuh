@@ -163,17 +163,8 @@ __device__ __forceinline__ double d1_op(const double* __restrict__ f, long long 
 // A block of 32 x 8 threads covers 32 x 8 x GRAD_KB cells: each thread walks GRAD_KB cells along zeta, so the
 // zeta stencil re-uses its loads in registers and the eta stencil of the block re-uses rows in L1
 // (ncu r1c: the one-cell-per-thread version was L1-wavefront bound with a 31 % L1 hit rate).
-#ifndef MEG6_GRAD_NOBREAK
-#define MEG6_GRAD_NOBREAK 1
-#endif
-#ifndef MEG6_GRAD_KB
-#define MEG6_GRAD_KB 4
-#endif
-#ifndef MEG6_GRAD_MINB
-#define MEG6_GRAD_MINB 4
-#endif
-constexpr int GRAD_KB = MEG6_GRAD_KB;
-__global__ void __launch_bounds__(256, MEG6_GRAD_MINB) k_grad(Consts c, P6 P, P12 G) {
+constexpr int GRAD_KB = 4;   // cells per thread along zeta (2 and 8: +10 %, r2c)
+__global__ void __launch_bounds__(256, 4) k_grad(Consts c, P6 P, P12 G) {
   // i runs over the whole padded row of G (-GGI .. pitch-GGI): the cells beyond -1 and n are padding nobody reads, but
   // writing them makes every warp store start and end on a 32-byte sector (no partial-sector fills in L2/DRAM)
   const int i = blockIdx.x * 32 + threadIdx.x - GGI;
@@ -190,15 +181,10 @@ __global__ void __launch_bounds__(256, MEG6_GRAD_MINB) k_grad(Consts c, P6 P, P1
     for (int m = 0; m < GRAD_KB + 6; ++m) z[m] = (k0 + m - 3 <= c.n[2] + 3) ? q[(m - 3) * sk] : 0.0;
 #pragma unroll
     for (int m = 0; m < GRAD_KB; ++m) {
-#if MEG6_GRAD_NOBREAK
       // no early exit: the planes beyond n+1 are inside the 6-deep ghost padding of P, only the stores are guarded, so
       // the loads of the next cells can be issued before the stores of this one (the kernel was a chain of 16
       // load-wait-store rounds per thread)
       const bool ok = k0 + m <= c.n[2];
-#else
-      if (k0 + m > c.n[2]) break;
-      const bool ok = true;
-#endif
       const double* __restrict__ qq = q + m * sk;
       const long long ag = ag0 + m * c.LG.sk;
       double* __restrict__ gx = G.p[f];

@@ -18,52 +18,31 @@
 
 namespace meg6 {
 
-// CTAs per SM the sweeps are compiled for: 4 (128 registers) and 5 (96 registers, more spills) are equal on the
-// mostly smooth C4 start-up flow; with the full limiting path in every warp (C3/C5) 4 is 7 % faster.
-#ifndef MEG6_MINB3_X
-#define MEG6_MINB3_X 4
-#endif
-#ifndef MEG6_MINB3_Y
-#define MEG6_MINB3_Y 4
-#endif
-#ifndef MEG6_PF
-#define MEG6_PF 1
-#endif
-#ifndef MEG6_RES_TMA
-#define MEG6_RES_TMA 1
-#endif
-#ifndef MEG6_TAIL_TMA
-#define MEG6_TAIL_TMA 1
-#endif
-#ifndef MEG6_RES_TMA_XI
-#define MEG6_RES_TMA_XI 1
-#endif
-#ifndef MEG6_TS_Y
-#define MEG6_TS_Y 15
-#endif
-#ifndef MEG6_RELOAD
-#define MEG6_RELOAD 1
-#endif
-#ifndef MEG6_TT_Y
-#define MEG6_TT_Y 8
-#endif
-#ifndef MEG6_BLK_Y
-#define MEG6_BLK_Y 5
-#endif
+// Build parameters of the sweeps, fixed after the measurements recorded in DESIGN.md section 6 ("tried and rejected"):
+// 4 CTAs per SM (128 registers; 5 CTAs at 96-100 registers: -6 % eta/zeta, -10 % all three on C4, r2c), eta/zeta tiles
+// of 15 cells x 8 xi-lanes (11, 19, 23, 31 cells and 16 lanes all slower), 5 cells per thread in the offset phase.
+constexpr int SWEEP_MINB = 4, TS_Y = 15, TT_Y = 8, BLK_Y = 5, NSUB_Y = 2;
 
 // IG4 = MIG4 variant (scheme 1): the sweep-direction gradients P' are not E6 stencils of the tile but solutions of
 // the implicit systems of Eq. 18, computed beforehand for whole grid lines and loaded like the primitives.
 template <int DIR, bool VISC, bool IG4 = false>
 struct Cfg3 {
-  static constexpr int TS = (DIR == 0) ? 30 : MEG6_TS_Y;     // cells along the sweep per tile
-  static constexpr int TT = (DIR == 0) ? 4 : MEG6_TT_Y;              // transverse positions (rows for xi, i-lanes otherwise)
+  static constexpr int TS = (DIR == 0) ? 30 : TS_Y;     // cells along the sweep per tile
+  static constexpr int TT = (DIR == 0) ? 4 : TT_Y; // transverse positions (rows for xi, i-lanes otherwise)
   static constexpr int NI = TS + 1;                          // interfaces per pencil
   static constexpr int NT = (DIR == 0) ? 32 * TT : NI * TT;  // threads: one interface each (xi: one warp per row)
-  static constexpr int MINB = (DIR == 0) ? (IG4 ? 4 : MEG6_MINB3_X) : (IG4 ? 4 : MEG6_MINB3_Y) * 8 / MEG6_TT_Y;
+  static constexpr int MINB = SWEEP_MINB;
   static constexpr int NF = VISC ? 6 : 5;                    // staged fields (T only for the viscous flux)
   static constexpr int NM = VISC ? 10 : 3;                   // interface metrics loaded
   static constexpr int NMF = NM > 5 ? NM : 5;                // the metric region later receives the 5 fluxes
-  static constexpr int LP = TS + 12;                         // P: cells -6 .. TS+5
+  // eta/zeta sweeps (MEG6): a CTA works through NSUB consecutive sub-tiles of TS cells along the sweep out of ONE
+  // primitive window of NSUB TS + 12 cells, loaded by one TMA box at the start: the wait for the primitives (DRAM
+  // latency at the head of every CTA, 15 % of the warp samples of the one-tile kernel, ncu r2c) is paid once per NSUB
+  // sub-tiles, and the 12-cell halo is shared; the metric / gradient / residual boxes of sub-tile h+1 are issued when
+  // sub-tile h is finished and arrive while its offsets (phase 1) are formed
+  static constexpr int NSUB = (DIR != 0 && !IG4) ? NSUB_Y : 1;
+  static constexpr int LP = TS + 12;                         // P of one sub-tile: cells -6 .. TS+5
+  static constexpr int LPT = TS * NSUB + 12;                 // the primitive window of the CTA
   static constexpr int LA = TS + 4;                          // aL/aR: cells -2 .. TS+1
   static constexpr int LT = TS + 2;                          // T': cells -1 .. TS
   static constexpr int LF = (DIR == 0) ? TS + 2 : TS + 1;    // interface rows (xi: even length, TMA box bytes % 16)
@@ -76,15 +55,15 @@ struct Cfg3 {
   // box per group out of the 12-field array; MIG4: one 5-field box (u,v,w,p,T of the line-solve arrays) per group,
   // the second group starting on the next 128-byte boundary
   static constexpr int GFLD = IG4 ? 5 : 4, GSLOT = IG4 ? al(5 * LG * TT) : 4 * LG * TT;
-  static constexpr int nP = NF * LP * TT, nA = 10 * LA * TT, nT1 = (VISC && !IG4) ? LT * TT : 0, nM = NMF * LF * TT,
+  static constexpr int nP = NF * LPT * TT, nA = 10 * LA * TT, nT1 = (VISC && !IG4) ? LT * TT : 0, nM = NMF * LF * TT,
                        nMt = LF * TT, nG = VISC ? GSLOT + GFLD * LG * TT : 0, nGtx = VISC ? 2 * GFLD * LG * TT : 0,
                        nQ = IG4 ? NF * LQ * TT : 0;
   // eta/zeta sweeps, MEG6: the running residual of the tile arrives by TMA with the metrics (it is needed at the very
   // end of the CTA; as plain loads behind an L2 prefetch it cost the second sweep 0.09 ms against the first)
-  static constexpr int nR = (!IG4 && MEG6_RES_TMA && (DIR != 0 || MEG6_RES_TMA_XI)) ? 5 * TS * TT : 0;
+  static constexpr int nR = !IG4 ? 5 * TS * TT : 0;
   // fused xi sweep, MEG6: what the final phase reads besides the residual -- U (5), U^n (5), 1/J, sigma -- as four more
   // boxes on the same barrier (replaces an L2-prefetch loop of 10 % of the kernel's instructions and 12 late loads)
-  static constexpr int nU = (DIR == 0 && !IG4 && MEG6_TAIL_TMA) ? 5 * TS * TT : 0, n1 = nU ? TS * TT : 0;
+  static constexpr int nU = (DIR == 0 && !IG4) ? 5 * TS * TT : 0, n1 = nU ? TS * TT : 0;
   static constexpr int oP = 0, oM = oP + al(nP), oMt = oM + al(nM), oG = oMt + al(nMt), oQ = oG + al(nG), oA = oQ + al(nQ),
                        oT1 = oA + al(nA), oR = oT1 + al(nT1), oU = oR + al(nR), oU0 = oU + al(nU), oJ = oU0 + al(nU),
                        oSg = oJ + al(n1), oBar = oSg + al(n1);
@@ -127,26 +106,22 @@ __device__ __forceinline__ void tma4(void* dst, const CUtensorMap* tm, uint64_t*
       ::"r"(smem_u32_3(dst)), "l"((uint64_t)tm), "r"(smem_u32_3(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
 }
 
-__device__ __forceinline__ void mbar_wait3(uint64_t* bar) {   // phase 0 (every barrier is used once per CTA)
+__device__ __forceinline__ void mbar_wait3(uint64_t* bar, uint32_t parity = 0) {   // phase `parity` of the barrier
   uint32_t done = 0;
   const uint32_t b = smem_u32_3(bar);
   while (!done) {
     asm volatile(
         "{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}\n"
-        : "=r"(done) : "r"(b), "r"(0) : "memory");
+        : "=r"(done) : "r"(b), "r"(parity) : "memory");
   }
 }
 
 // shared-memory load the compiler may not merge with an earlier load of the same address: values that are needed
 // again long after their first use are re-read instead of being kept in registers across the limiter
 __device__ __forceinline__ double lds_again(const double* p) {
-#if MEG6_RELOAD
   double v;
   asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(smem_u32_3(p)));
   return v;
-#else
-  return *p;
-#endif
 }
 
 // Reciprocal as its own operation: a/b is written a * rcp3(b) (the reciprocal sequence is shorter than the division
@@ -320,10 +295,8 @@ __device__ __forceinline__ unsigned face3(const Consts& c, const double* __restr
     }
   }
   double PL[5], PR[5];
-#if MEG6_RELOAD
 #pragma unroll
   for (int f = 0; f < 5; ++f) { BL[f] = lds_again(pP + f * FP + SS); BR[f] = lds_again(pP + f * FP + 2 * SS); }
-#endif
   backproject3(e, ia2, h_ira, EL, BL, PL);   // Eq. 23
   backproject3(e, ia2, h_ira, ER, BR, PR);
   fl |= hllc3(PL, PR, mx, my, mz, mt, g, g2, ig2, c.gamma, c.igm1, F) << 10;
@@ -396,8 +369,9 @@ k_flux3(const Consts c, const FluxIn3 in, const __grid_constant__ TmaMaps tm, co
   using C = Cfg3<DIR, VISC, IG4>;
   constexpr int LQ = C::LQ;
   constexpr int TS = C::TS, TT = C::TT, NT = C::NT, NF = C::NF, LP = C::LP, LA = C::LA, LT = C::LT, LF = C::LF, LG = C::LG;
+  constexpr int NSUB = C::NSUB, LPT = C::LPT;          // sub-tiles per CTA, length of the primitive window
   constexpr int SS = (DIR == 0) ? 1 : TT;
-  constexpr int FP = (DIR == 0) ? TT * LP : LP * TT;   // field strides
+  constexpr int FP = (DIR == 0) ? TT * LPT : LPT * TT;   // field strides
   constexpr int FA = (DIR == 0) ? TT * LA : LA * TT;
   constexpr int FM = (DIR == 0) ? TT * LF : LF * TT;
   constexpr int FG = (DIR == 0) ? TT * LG : LG * TT;
@@ -413,38 +387,29 @@ k_flux3(const Consts c, const FluxIn3 in, const __grid_constant__ TmaMaps tm, co
   const int tid = threadIdx.x;
   int s0, t0, o;
   if (DIR == 0) { s0 = blockIdx.x * TS; t0 = blockIdx.y * TT; o = blockIdx.z; }
-  else if (DIR == 1) { t0 = blockIdx.x * TT; s0 = blockIdx.y * TS; o = blockIdx.z; }
-  else { t0 = blockIdx.x * TT; s0 = blockIdx.y * TS; o = blockIdx.z; }   // chunks of a line run back to back (halo re-use in L2)
+  else if (DIR == 1) { t0 = blockIdx.x * TT; s0 = blockIdx.y * (TS * NSUB); o = blockIdx.z; }
+  else { t0 = blockIdx.x * TT; s0 = blockIdx.y * (TS * NSUB); o = blockIdx.z; }   // chunks of a line run back to back (halo re-use in L2)
   const int nd = c.n[DIR];
   const int nt = (DIR == 0) ? c.n[1] : c.n[0];
 
-  if (tid == 0) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32_3(bar)), "r"(1) : "memory");
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32_3(bar + 1)), "r"(1) : "memory");
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  // box coordinates are (i, j, k, field) in the padded layout of each array: sweep start, transverse start, other
+  auto coords = [](int s, int t, int oo, int gi, int gj, int gk, int& c0, int& c1, int& c2) {
+    if (DIR == 0) { c0 = s + gi; c1 = t + gj; c2 = oo + gk; }
+    else if (DIR == 1) { c0 = t + gi; c1 = s + gj; c2 = oo + gk; }
+    else { c0 = t + gi; c1 = oo + gj; c2 = s + gk; }
+  };
+  // what a sub-tile starting at cell s needs besides the primitives, on the second barrier (thread 0 only)
+  auto issue_tile = [&](int s) {
     uint32_t bytes1 = (C::NM * LF * TT + C::nGtx) * 8;
     if (in.moving) bytes1 += C::nMt * 8;
     if (C::nR && !in.first) bytes1 += C::nR * 8;
     const bool ttma = C::nU && FUSE && fu.tail_tma;
     if (ttma) bytes1 += (C::nU + C::n1 + ((fu.mode == 1 && fu.a != 0.0) ? C::nU : 0) + (fu.sigma ? C::n1 : 0)) * 8;
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32_3(bar)), "r"((C::nP + C::nQ) * 8) : "memory");
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32_3(bar + 1)), "r"(bytes1) : "memory");
-    // box coordinates are (i, j, k, field) in the padded layout of each array: sweep start, transverse start, other
-    auto coords = [](int s, int t, int oo, int gi, int gj, int gk, int& c0, int& c1, int& c2) {
-      if (DIR == 0) { c0 = s + gi; c1 = t + gj; c2 = oo + gk; }
-      else if (DIR == 1) { c0 = t + gi; c1 = s + gj; c2 = oo + gk; }
-      else { c0 = t + gi; c1 = oo + gj; c2 = s + gk; }
-    };
     constexpr int G0 = (DIR == 0) ? 4 : 0, G1 = (DIR == 2) ? 4 : 8;      // the two tangential gradient groups
     constexpr int GS = (DIR == 0) ? -2 : -1;                             // first stored-gradient cell of the box
     int c0, c1, c2;
-    coords(s0 - 6, t0, o, GPI, GPJ, GPK, c0, c1, c2);
-    tma4(sP, &tm.P, bar, c0, c1, c2, 0);
-    if (IG4) {
-      coords(s0 - 3 - C::QOFF, t0, o, GPI, GPJ, GPK, c0, c1, c2);
-      tma4(sQ, &tm.Q, bar, c0, c1, c2, 0);
-    }
-    coords(s0, t0, o, 0, 0, 0, c0, c1, c2);
+    coords(s, t0, o, 0, 0, 0, c0, c1, c2);
     tma4(sM, &tm.M, bar + 1, c0, c1, c2, 0);
     if (in.moving) tma4(sMt, &tm.Mt, bar + 1, c0, c1, c2, 0);
     if (C::nR && !in.first) tma4(sm3 + C::oR, &tm.R, bar + 1, c0, c1, c2, 0);   // LR has no ghosts: same coordinates
@@ -455,19 +420,33 @@ k_flux3(const Consts c, const FluxIn3 in, const __grid_constant__ TmaMaps tm, co
       tma4(sm3 + C::oJ, &tm.J, bar + 1, c0 + GX, c1 + GX, c2 + GX, 0);
     }
     if (VISC) {
-      coords(s0 + GS, t0, o, GGI, GGJ, GGK, c0, c1, c2);
+      coords(s + GS, t0, o, GGI, GGJ, GGK, c0, c1, c2);
       if (!IG4) {
         tma4(sG, &tm.G, bar + 1, c0, c1, c2, G0);
         tma4(sG + 4 * FG, &tm.G, bar + 1, c0, c1, c2, G1);
       } else {
         // tangential gradients = the implicit gradients of the two other directions (fields u,v,w and T of each)
-        coords(s0 + GS, t0, o, GPI, GPJ, GPK, c0, c1, c2);
+        coords(s + GS, t0, o, GPI, GPJ, GPK, c0, c1, c2);
         tma4(sG, &tm.G3[0], bar + 1, c0, c1, c2, 1);
         tma4(sG + C::GSLOT, &tm.G3[1], bar + 1, c0, c1, c2, 1);
       }
     }
+  };
+  if (tid == 0) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32_3(bar)), "r"(1) : "memory");
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32_3(bar + 1)), "r"(1) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32_3(bar)), "r"((C::nP + C::nQ) * 8) : "memory");
+    int c0, c1, c2;
+    coords(s0 - 6, t0, o, GPI, GPJ, GPK, c0, c1, c2);
+    tma4(sP, &tm.P, bar, c0, c1, c2, 0);   // the whole primitive window of the CTA
+    if (IG4) {
+      coords(s0 - 3 - C::QOFF, t0, o, GPI, GPJ, GPK, c0, c1, c2);
+      tma4(sQ, &tm.Q, bar, c0, c1, c2, 0);
+    }
+    issue_tile(s0);
   }
-  if (MEG6_PF && ((FUSE && !(C::nU && fu.tail_tma)) || (!FUSE && !in.first && !C::nR))) {
+  if ((FUSE && !(C::nU && fu.tail_tma)) || (!FUSE && !in.first && !C::nR)) {
     // L2 prefetch of what the final phase will read from global memory (running residual; fused: U, U0, 1/J,
     // sponge): those loads sit at the tail of the CTA with nothing to overlap them
     constexpr int NROW = (DIR == 0) ? TT : TS;                  // tile rows that are contiguous in memory
@@ -495,13 +474,15 @@ k_flux3(const Consts c, const FluxIn3 in, const __grid_constant__ TmaMaps tm, co
     }
   }
   __syncthreads();   // the barriers are initialised before anyone polls them
-  mbar_wait3(bar);   // primitive tile
+  mbar_wait3(bar);   // primitive window
+  int s0h = s0;                 // first cell of the current sub-tile
+  const double* sPh = sP;       // its cell -6 in the primitive window
 
   // ---- per cell: aL = 1/2 P' + P''/12, aR = -1/2 P' + P''/12 (Eq. 16-17, 19) on cells -2..TS+1; T' on -1..TS ----
   // One (cell, lane) position per thread and pass, all five fields; the positions left over after the full
   // passes are spread over the threads as (position, field) items so that no warp runs an extra pass alone.
   auto cell_field = [&](int f, int a, int t) {
-    const double* q = sP + sidx3<DIR, TT>(f, a + 4, t, LP);
+    const double* q = sPh + sidx3<DIR, TT>(f, a + 4, t, LPT);
     const double c0 = q[0], p1 = q[SS], m1 = q[-SS], p2 = q[2 * SS], m2 = q[-2 * SS], p3 = q[3 * SS], m3 = q[-3 * SS],
                  p4 = q[4 * SS], m4 = q[-4 * SS];
     double d1 = CE1 * (p1 - m1);
@@ -518,200 +499,216 @@ k_flux3(const Consts c, const FluxIn3 in, const __grid_constant__ TmaMaps tm, co
   };
   // MIG4: P' comes from the line solves; P'' by Eq. 19 from P and P'
   auto cell_field_ig4 = [&](int f, int a, int t) {
-    const double* q = sP + sidx3<DIR, TT>(f, a + 4, t, LP);
+    const double* q = sPh + sidx3<DIR, TT>(f, a + 4, t, LPT);
     const double* g1 = sQ + sidx3<DIR, TT>(f, a + 1 + C::QOFF, t, LQ);
     const double d2 = 2.0 * (q[SS] - 2.0 * q[0] + q[-SS]) - 0.5 * (g1[SS] - g1[-SS]);
     const double h = 0.5 * g1[0], d = d2 * (1.0 / 12.0);
     sA[sidx3<DIR, TT>(f, a, t, LA)] = d + h;
     sA[sidx3<DIR, TT>(f + 5, a, t, LA)] = d - h;
   };
-  if (IG4) {
-    if (DIR == 0) {
+  // ---- the sub-tiles of the CTA, one after the other (NSUB = 1: the body below runs once) ----
+#pragma unroll 1
+  for (int h = 0; h < NSUB; ++h) {
+    if (h > 0) {
+      s0h = s0 + h * TS;
+      if (s0h >= nd) break;                 // ragged end of the line (uniform over the CTA)
+      sPh = sP + h * TS * SS;
+      __syncthreads();                      // every thread is through the final phase of the previous sub-tile
+      if (tid == 0) {
+        // the metric / gradient / residual buffers were read and written through the generic proxy: order those
+        // accesses before the asynchronous-proxy writes of the new boxes
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        issue_tile(s0h);
+      }
+    }
+    if (IG4) {
+      if (DIR == 0) {
+        const int t = tid >> 5, lane = tid & 31;
+#pragma unroll
+        for (int f = 0; f < 5; ++f) cell_field_ig4(f, lane, t);
+        for (int it = lane; it < (LA - 32) * 5; it += 32) cell_field_ig4(it / (LA - 32), 32 + it % (LA - 32), t);
+      } else {
+        for (int it = tid; it < 5 * LA * TT; it += NT) cell_field_ig4(it / (LA * TT), (it / TT) % LA, it % TT);
+      }
+    } else if (DIR != 0) {
+      // eta/zeta sweeps: the sweep index is the slow one in shared memory, so one thread takes BLK consecutive cells
+      // of one lane and field: BLK + 8 loads instead of 9 BLK (shared-memory bandwidth was at 55-60 % of peak, r1c)
+      constexpr int BLK = BLK_Y, NQ = (LA + BLK - 1) / BLK;
+      for (int it = tid; it < NQ * TT * 5; it += NT) {
+        const int t = it % TT, qd = (it / TT) % NQ, f = it / (TT * NQ);
+        const int a0 = qd * BLK;
+        const double* q = sPh + sidx3<DIR, TT>(f, a0, t, LPT);
+        double v[BLK + 8];
+#pragma unroll
+        for (int m = 0; m < BLK + 8; ++m) v[m] = (a0 + m < LP) ? q[m * SS] : 0.0;
+#pragma unroll
+        for (int b = 0; b < BLK; ++b) {
+          if (a0 + b < LA) {
+            const double* w = v + b + 4;
+            double d1 = CE1 * (w[1] - w[-1]);
+            d1 = fma(CE2, w[2] - w[-2], d1);
+            d1 = fma(CE3, w[3] - w[-3], d1);
+            double d2 = CS0 * w[0];
+            d2 = fma(CS1, w[1] + w[-1], d2);
+            d2 = fma(CS2, w[2] + w[-2], d2);
+            d2 = fma(CS3, w[3] + w[-3], d2);
+            d2 = fma(CS4, w[4] + w[-4], d2);
+            const double h = 0.5 * d1, d = d2 * (1.0 / 12.0);
+            sA[sidx3<DIR, TT>(f, a0 + b, t, LA)] = d + h;
+            sA[sidx3<DIR, TT>(f + 5, a0 + b, t, LA)] = d - h;
+          }
+        }
+      }
+    } else {
+      // xi sweep: one warp per row, and a row needs nothing from the other rows: the warp fills the offsets of its own
+      // row and carries on without a CTA-wide barrier (the warps of a CTA drift apart and overlap each other's tails)
       const int t = tid >> 5, lane = tid & 31;
+      for (int a = lane; a < LA; a += 32) {
+        if (a < 32) {
 #pragma unroll
-      for (int f = 0; f < 5; ++f) cell_field_ig4(f, lane, t);
-      for (int it = lane; it < (LA - 32) * 5; it += 32) cell_field_ig4(it / (LA - 32), 32 + it % (LA - 32), t);
-    } else {
-      for (int it = tid; it < 5 * LA * TT; it += NT) cell_field_ig4(it / (LA * TT), (it / TT) % LA, it % TT);
-    }
-  } else if (DIR != 0) {
-    // eta/zeta sweeps: the sweep index is the slow one in shared memory, so one thread takes BLK consecutive cells
-    // of one lane and field: BLK + 8 loads instead of 9 BLK (shared-memory bandwidth was at 55-60 % of peak, r1c)
-    constexpr int BLK = MEG6_BLK_Y, NQ = (LA + BLK - 1) / BLK;
-    for (int it = tid; it < NQ * TT * 5; it += NT) {
-      const int t = it % TT, qd = (it / TT) % NQ, f = it / (TT * NQ);
-      const int a0 = qd * BLK;
-      const double* q = sP + sidx3<DIR, TT>(f, a0, t, LP);
-      double v[BLK + 8];
-#pragma unroll
-      for (int m = 0; m < BLK + 8; ++m) v[m] = (a0 + m < LP) ? q[m * SS] : 0.0;
-#pragma unroll
-      for (int b = 0; b < BLK; ++b) {
-        if (a0 + b < LA) {
-          const double* w = v + b + 4;
-          double d1 = CE1 * (w[1] - w[-1]);
-          d1 = fma(CE2, w[2] - w[-2], d1);
-          d1 = fma(CE3, w[3] - w[-3], d1);
-          double d2 = CS0 * w[0];
-          d2 = fma(CS1, w[1] + w[-1], d2);
-          d2 = fma(CS2, w[2] + w[-2], d2);
-          d2 = fma(CS3, w[3] + w[-3], d2);
-          d2 = fma(CS4, w[4] + w[-4], d2);
-          const double h = 0.5 * d1, d = d2 * (1.0 / 12.0);
-          sA[sidx3<DIR, TT>(f, a0 + b, t, LA)] = d + h;
-          sA[sidx3<DIR, TT>(f + 5, a0 + b, t, LA)] = d - h;
+          for (int f = 0; f < 5; ++f) cell_field(f, a, t);
         }
       }
+      for (int it = lane; it < (LA - 32) * 5; it += 32) cell_field(it / (LA - 32), 32 + it % (LA - 32), t);
     }
-  } else {
-    // xi sweep: one warp per row, and a row needs nothing from the other rows: the warp fills the offsets of its own
-    // row and carries on without a CTA-wide barrier (the warps of a CTA drift apart and overlap each other's tails)
-    const int t = tid >> 5, lane = tid & 31;
-    for (int a = lane; a < LA; a += 32) {
-      if (a < 32) {
-#pragma unroll
-        for (int f = 0; f < 5; ++f) cell_field(f, a, t);
+    if (VISC && !IG4) {
+      // T' on cells -1..TS.  xi: lane = cell of the warp's own row; eta/zeta: reversed so that the leftover items go to
+      // the last warp
+      for (int it = (DIR == 0) ? (tid & 31) : NT - 1 - tid; it < ((DIR == 0) ? LT : LT * TT); it += (DIR == 0) ? 32 : NT) {
+        int a, t;
+        if (DIR == 0) { a = it; t = tid >> 5; }
+        else { t = it % TT; a = it / TT; }
+        const double* q = sPh + sidx3<DIR, TT>(5, a + 5, t, LPT);
+        double d1 = CE1 * (q[SS] - q[-SS]);
+        d1 = fma(CE2, q[2 * SS] - q[-2 * SS], d1);
+        d1 = fma(CE3, q[3 * SS] - q[-3 * SS], d1);
+        sT1[sidx3<DIR, TT>(0, a, t, LT)] = d1;
       }
     }
-    for (int it = lane; it < (LA - 32) * 5; it += 32) cell_field(it / (LA - 32), 32 + it % (LA - 32), t);
-  }
-  if (VISC && !IG4) {
-    // T' on cells -1..TS.  xi: lane = cell of the warp's own row; eta/zeta: reversed so that the leftover items go to
-    // the last warp
-    for (int it = (DIR == 0) ? (tid & 31) : NT - 1 - tid; it < ((DIR == 0) ? LT : LT * TT); it += (DIR == 0) ? 32 : NT) {
-      int a, t;
-      if (DIR == 0) { a = it; t = tid >> 5; }
-      else { t = it % TT; a = it / TT; }
-      const double* q = sP + sidx3<DIR, TT>(5, a + 5, t, LP);
-      double d1 = CE1 * (q[SS] - q[-SS]);
-      d1 = fma(CE2, q[2 * SS] - q[-2 * SS], d1);
-      d1 = fma(CE3, q[3 * SS] - q[-3 * SS], d1);
-      sT1[sidx3<DIR, TT>(0, a, t, LT)] = d1;
-    }
-  }
-  if (DIR == 0) __syncwarp(); else __syncthreads();
-  mbar_wait3(bar + 1);   // interface metrics and stored gradients (issued together with the primitive tile)
+    if (DIR == 0) __syncwarp(); else __syncthreads();
+    mbar_wait3(bar + 1, (uint32_t)(h & 1));   // interface metrics and stored gradients (issued together with the primitive tile)
 
-  // ---- one interface per thread ----
-  int sI, row;
-  if (DIR == 0) { sI = tid & 31; row = tid >> 5; }
-  else { row = tid % TT; sI = tid / TT; }
-  const bool valid = (sI <= TS) && (s0 + sI <= nd) && (t0 + row < nt);
-  unsigned nlim = 0, ntst = 0;
-  double F[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
-  if (valid) {
-    const double mt = in.moving ? sMt[sidx3<DIR, TT>(0, sI, row, LF)] : 0.0;
-    const unsigned fl = face3<DIR, VISC, SS, FP, FA, FG, FM, C::GSLOT, IG4>(
-        c, sP + sidx3<DIR, TT>(0, sI + 4, row, LP), sA + sidx3<DIR, TT>(0, sI, row, LA),
-        IG4 ? sQ + sidx3<DIR, TT>(5, sI + 2 + C::QOFF, row, LQ) : sT1 + sidx3<DIR, TT>(0, sI, row, LT),
-        sG + sidx3<DIR, TT>(0, sI + C::GOFF, row, LG),
-        sM + sidx3<DIR, TT>(0, sI, row, LF), mt, F);
-    if (sI < TS || s0 + sI == nd) {   // tile-shared faces counted once
-      nlim = __popc(fl & 1023u); ntst = 10;
-      if (in.mask) {   // interface (s0 + sI) of n_d + 1 along the sweep, interior extents along the others, i fastest
-        long long im;
-        if (DIR == 0) im = ((long long)o * c.n[1] + (t0 + row)) * (c.n[0] + 1) + (s0 + sI);
-        else if (DIR == 1) im = ((long long)o * (c.n[1] + 1) + (s0 + sI)) * c.n[0] + (t0 + row);
-        else im = ((long long)(s0 + sI) * c.n[1] + o) * c.n[0] + (t0 + row);
-        in.mask[im] = (unsigned short)fl;
-      }
-    }
-  }
-  if (DIR != 0 && sI <= TS) {
-    // the flux tile aliases the metric tile: slot (sI,row) of every metric field is read only by this thread
-#pragma unroll
-    for (int f = 0; f < 5; ++f) sM[sidx3<DIR, TT>(f, sI, row, LF)] = F[f];
-  }
-  if (in.stats) {
-    for (int off = 16; off > 0; off >>= 1) {
-      nlim += __shfl_down_sync(0xffffffffu, nlim, off);
-      ntst += __shfl_down_sync(0xffffffffu, ntst, off);
-    }
-    if ((tid & 31) == 0 && ntst) { atomicAdd(in.stats, (unsigned long long)nlim); atomicAdd(in.stats + 1, (unsigned long long)ntst); }
-  }
-  // ---- flux difference, Eq. 25: Res_i -= F_{i+1/2} - F_{i-1/2}, then (last sweep) assembly + update ----
-  auto finish_cell = [&](int s, int t, const double dF[5]) {
-    long long ac;
-    if (DIR == 0) ac = c.LR.at(s0 + s, t0 + t, o);
-    else if (DIR == 1) ac = c.LR.at(t0 + t, s0 + s, o);
-    else ac = c.LR.at(t0 + t, o, s0 + s);
-    double old[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
-    if (!in.first) {
-#pragma unroll
-      for (int f = 0; f < 5; ++f) old[f] = C::nR ? (sm3 + C::oR)[sidx3<DIR, TT>(f, s, t, TS)] : in.res[f * c.fsR + ac];
-    }
-    double R[5];
-#pragma unroll
-    for (int f = 0; f < 5; ++f) R[f] = old[f] - dF[f];
-    if (!FUSE) {
-#pragma unroll
-      for (int f = 0; f < 5; ++f) in.res[f * c.fsR + ac] = R[f];
-    } else {
-      int ci, cj, ck;
-      if (DIR == 0) { ci = s0 + s; cj = t0 + t; ck = o; }
-      else if (DIR == 1) { ci = t0 + t; cj = s0 + s; ck = o; }
-      else { ci = t0 + t; cj = o; ck = s0 + s; }
-      const long long N = c.LC.n, ic = c.LC.at(ci, cj, ck);
-      // every load of the phase before its first store: U, U0w and out may be the same memory as far as the compiler
-      // knows, so a store between two loads would chain their latencies one after the other
-      const bool tt = C::nU && fu.tail_tma;          // DIR == 0 here: the tile row t, cell s
-      const int st = (C::nU ? t * TS + s : 0);
-      const double rjv = tt ? (sm3 + C::oJ)[st] : fu.rj[c.LX.at(ci, cj, ck)];
-      const double rjt = fu.rjt ? fu.rjt[ic] : 0.0;
-      const double sg = fu.sigma ? (tt ? (sm3 + C::oSg)[st] : fu.sigma[ic]) : 0.0;
-      const bool blend = fu.mode == 1 && fu.a != 0.0;
-      double uu[5], ur[5], u0[5];
-#pragma unroll
-      for (int f = 0; f < 5; ++f) uu[f] = tt ? (sm3 + C::oU)[f * TT * TS + st] : fu.U[f * N + ic];
-#pragma unroll
-      for (int f = 0; f < 5; ++f) u0[f] = blend ? (tt ? (sm3 + C::oU0)[f * TT * TS + st] : fu.U0[f * N + ic]) : 0.0;
-#pragma unroll
-      for (int f = 0; f < 5; ++f) ur[f] = (sg != 0.0) ? fu.uref[f * N + ic] : 0.0;   // sigma = 0 outside the sponge: Q_ref is not read there
-      const double J = 1.0 / rjv;
-      double Q[5];
-#pragma unroll
-      for (int f = 0; f < 5; ++f) {
-        const double u = uu[f];
-        double L = J * (R[f] - rjt * u);
-        if (sg != 0.0) L -= sg * (u - ur[f]);
-        if (fu.mode == 0) Q[f] = L;
-        else {
-          double v = u + fu.dt * L;
-          if (fu.a != 0.0) v = fu.a * u0[f] + fu.b * v;
-          Q[f] = v;
+    // ---- one interface per thread ----
+    int sI, row;
+    if (DIR == 0) { sI = tid & 31; row = tid >> 5; }
+    else { row = tid % TT; sI = tid / TT; }
+    const bool valid = (sI <= TS) && (s0h + sI <= nd) && (t0 + row < nt);
+    unsigned nlim = 0, ntst = 0;
+    double F[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+    if (valid) {
+      const double mt = in.moving ? sMt[sidx3<DIR, TT>(0, sI, row, LF)] : 0.0;
+      const unsigned fl = face3<DIR, VISC, SS, FP, FA, FG, FM, C::GSLOT, IG4>(
+          c, sPh + sidx3<DIR, TT>(0, sI + 4, row, LPT), sA + sidx3<DIR, TT>(0, sI, row, LA),
+          IG4 ? sQ + sidx3<DIR, TT>(5, sI + 2 + C::QOFF, row, LQ) : sT1 + sidx3<DIR, TT>(0, sI, row, LT),
+          sG + sidx3<DIR, TT>(0, sI + C::GOFF, row, LG),
+          sM + sidx3<DIR, TT>(0, sI, row, LF), mt, F);
+      if (sI < TS || s0h + sI == nd) {   // tile-shared faces counted once
+        nlim = __popc(fl & 1023u); ntst = 10;
+        if (in.mask) {   // interface (s0h + sI) of n_d + 1 along the sweep, interior extents along the others, i fastest
+          long long im;
+          if (DIR == 0) im = ((long long)o * c.n[1] + (t0 + row)) * (c.n[0] + 1) + (s0h + sI);
+          else if (DIR == 1) im = ((long long)o * (c.n[1] + 1) + (s0h + sI)) * c.n[0] + (t0 + row);
+          else im = ((long long)(s0h + sI) * c.n[1] + o) * c.n[0] + (t0 + row);
+          in.mask[im] = (unsigned short)fl;
         }
       }
-      if (fu.mode == 1 && fu.a == 0.0 && fu.U0w) {
-#pragma unroll
-        for (int f = 0; f < 5; ++f) fu.U0w[f * N + ic] = uu[f];
-      }
-#pragma unroll
-      for (int f = 0; f < 5; ++f) fu.out[f * N + ic] = Q[f];
-      if (fu.Pn) {   // Q -> P of the new state (Eq. 5, P:83 inverted; T = p/(rho R)), as k_prim
-        const double r = Q[0], ir = 1.0 / r;
-        const double u = Q[1] * ir, v = Q[2] * ir, w = Q[3] * ir;
-        const double p = (c.gamma - 1.0) * (Q[4] - 0.5 * r * (u * u + v * v + w * w));
-        double* pn = fu.Pn + c.LP.at(ci, cj, ck);
-        pn[0] = r; pn[c.fsP] = u; pn[2 * c.fsP] = v; pn[3 * c.fsP] = w; pn[4 * c.fsP] = p;
-        pn[5 * c.fsP] = p / (r * c.r_gas);
-      }
     }
-  };
-  if (DIR == 0) {
-    // the right-hand interface of cell `lane` belongs to the next lane of the same warp: no shared memory, no barrier
-    double dF[5];
+    if (DIR != 0 && sI <= TS) {
+      // the flux tile aliases the metric tile: slot (sI,row) of every metric field is read only by this thread
 #pragma unroll
-    for (int f = 0; f < 5; ++f) dF[f] = __shfl_down_sync(0xffffffffu, F[f], 1) - F[f];
-    if (sI < TS && s0 + sI < nd && t0 + row < nt) finish_cell(sI, row, dF);
-  } else {
-    __syncthreads();
-    for (int it = tid; it < TS * TT; it += NT) {
-      const int t = it % TT, s = it / TT;
-      if (s0 + s >= nd || t0 + t >= nt) continue;
+      for (int f = 0; f < 5; ++f) sM[sidx3<DIR, TT>(f, sI, row, LF)] = F[f];
+    }
+    if (in.stats) {
+      for (int off = 16; off > 0; off >>= 1) {
+        nlim += __shfl_down_sync(0xffffffffu, nlim, off);
+        ntst += __shfl_down_sync(0xffffffffu, ntst, off);
+      }
+      if ((tid & 31) == 0 && ntst) { atomicAdd(in.stats, (unsigned long long)nlim); atomicAdd(in.stats + 1, (unsigned long long)ntst); }
+    }
+    // ---- flux difference, Eq. 25: Res_i -= F_{i+1/2} - F_{i-1/2}, then (last sweep) assembly + update ----
+    auto finish_cell = [&](int s, int t, const double dF[5]) {
+      long long ac;
+      if (DIR == 0) ac = c.LR.at(s0h + s, t0 + t, o);
+      else if (DIR == 1) ac = c.LR.at(t0 + t, s0h + s, o);
+      else ac = c.LR.at(t0 + t, o, s0h + s);
+      double old[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+      if (!in.first) {
+#pragma unroll
+        for (int f = 0; f < 5; ++f) old[f] = C::nR ? (sm3 + C::oR)[sidx3<DIR, TT>(f, s, t, TS)] : in.res[f * c.fsR + ac];
+      }
+      double R[5];
+#pragma unroll
+      for (int f = 0; f < 5; ++f) R[f] = old[f] - dF[f];
+      if (!FUSE) {
+#pragma unroll
+        for (int f = 0; f < 5; ++f) in.res[f * c.fsR + ac] = R[f];
+      } else {
+        int ci, cj, ck;
+        if (DIR == 0) { ci = s0h + s; cj = t0 + t; ck = o; }
+        else if (DIR == 1) { ci = t0 + t; cj = s0h + s; ck = o; }
+        else { ci = t0 + t; cj = o; ck = s0h + s; }
+        const long long N = c.LC.n, ic = c.LC.at(ci, cj, ck);
+        // every load of the phase before its first store: U, U0w and out may be the same memory as far as the compiler
+        // knows, so a store between two loads would chain their latencies one after the other
+        const bool tt = C::nU && fu.tail_tma;          // DIR == 0 here: the tile row t, cell s
+        const int st = (C::nU ? t * TS + s : 0);
+        const double rjv = tt ? (sm3 + C::oJ)[st] : fu.rj[c.LX.at(ci, cj, ck)];
+        const double rjt = fu.rjt ? fu.rjt[ic] : 0.0;
+        const double sg = fu.sigma ? (tt ? (sm3 + C::oSg)[st] : fu.sigma[ic]) : 0.0;
+        const bool blend = fu.mode == 1 && fu.a != 0.0;
+        double uu[5], ur[5], u0[5];
+#pragma unroll
+        for (int f = 0; f < 5; ++f) uu[f] = tt ? (sm3 + C::oU)[f * TT * TS + st] : fu.U[f * N + ic];
+#pragma unroll
+        for (int f = 0; f < 5; ++f) u0[f] = blend ? (tt ? (sm3 + C::oU0)[f * TT * TS + st] : fu.U0[f * N + ic]) : 0.0;
+#pragma unroll
+        for (int f = 0; f < 5; ++f) ur[f] = (sg != 0.0) ? fu.uref[f * N + ic] : 0.0;   // sigma = 0 outside the sponge: Q_ref is not read there
+        const double J = 1.0 / rjv;
+        double Q[5];
+#pragma unroll
+        for (int f = 0; f < 5; ++f) {
+          const double u = uu[f];
+          double L = J * (R[f] - rjt * u);
+          if (sg != 0.0) L -= sg * (u - ur[f]);
+          if (fu.mode == 0) Q[f] = L;
+          else {
+            double v = u + fu.dt * L;
+            if (fu.a != 0.0) v = fu.a * u0[f] + fu.b * v;
+            Q[f] = v;
+          }
+        }
+        if (fu.mode == 1 && fu.a == 0.0 && fu.U0w) {
+#pragma unroll
+          for (int f = 0; f < 5; ++f) fu.U0w[f * N + ic] = uu[f];
+        }
+#pragma unroll
+        for (int f = 0; f < 5; ++f) fu.out[f * N + ic] = Q[f];
+        if (fu.Pn) {   // Q -> P of the new state (Eq. 5, P:83 inverted; T = p/(rho R)), as k_prim
+          const double r = Q[0], ir = 1.0 / r;
+          const double u = Q[1] * ir, v = Q[2] * ir, w = Q[3] * ir;
+          const double p = (c.gamma - 1.0) * (Q[4] - 0.5 * r * (u * u + v * v + w * w));
+          double* pn = fu.Pn + c.LP.at(ci, cj, ck);
+          pn[0] = r; pn[c.fsP] = u; pn[2 * c.fsP] = v; pn[3 * c.fsP] = w; pn[4 * c.fsP] = p;
+          pn[5 * c.fsP] = p / (r * c.r_gas);
+        }
+      }
+    };
+    if (DIR == 0) {
+      // the right-hand interface of cell `lane` belongs to the next lane of the same warp: no shared memory, no barrier
       double dF[5];
 #pragma unroll
-      for (int f = 0; f < 5; ++f) dF[f] = sM[sidx3<DIR, TT>(f, s + 1, t, LF)] - sM[sidx3<DIR, TT>(f, s, t, LF)];
-      finish_cell(s, t, dF);
+      for (int f = 0; f < 5; ++f) dF[f] = __shfl_down_sync(0xffffffffu, F[f], 1) - F[f];
+      if (sI < TS && s0h + sI < nd && t0 + row < nt) finish_cell(sI, row, dF);
+    } else {
+      __syncthreads();
+      for (int it = tid; it < TS * TT; it += NT) {
+        const int t = it % TT, s = it / TT;
+        if (s0h + s >= nd || t0 + t >= nt) continue;
+        double dF[5];
+#pragma unroll
+        for (int f = 0; f < 5; ++f) dF[f] = sM[sidx3<DIR, TT>(f, s + 1, t, LF)] - sM[sidx3<DIR, TT>(f, s, t, LF)];
+        finish_cell(s, t, dF);
+      }
     }
   }
 }
