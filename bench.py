@@ -289,7 +289,11 @@ def run_ours(args):
     g = Grid(wl, device=dev)
     if args.metrics_only:
         return run_metrics_only(args, g, wl, dev)
-    g.metrics_compute(wl["t0"])
+    if slabs:   # ghost coordinates of the cut faces come from the neighbour slab: the stepper exchanges them
+        stepper = SlabStepper(g, remote, moving=bool(prm["moving"]), offsets=wl["link_offset"])
+        stepper.metrics_compute(wl["t0"])
+    else:
+        g.metrics_compute(wl["t0"])
     U = torch.as_tensor(wl["U0"], device=dev).contiguous()
     if wl["dt"] is not None:
         dt = wl["dt"]
@@ -299,8 +303,6 @@ def run_ours(args):
             tdt = torch.tensor([dt], dtype=torch.float64, device=dev)
             dist.all_reduce(tdt, op=dist.ReduceOp.MIN)
             dt = float(tdt.item())
-    if slabs:
-        stepper = SlabStepper(g, remote, moving=bool(prm["moving"]))
     step = stepper.rk3_step if stepper else g.rk3_step
     stream = torch.cuda.current_stream(dev)
 

@@ -97,19 +97,34 @@ meg6_status meg6_rhs(meg6_grid* g, const double* U, double* dUdt);
  * sweep of every stage; it must not be touched by other streams while the step is in flight. */
 meg6_status meg6_rk3_step(meg6_grid* g, double* U, double t, double dt);
 
-/* Multi-block (Sec. 6; Table 1 last column P:354-362; reading R28).  A face with bc == 5 is a block
- * interface: its six ghost layers of primitives are copies of the interior cells of the neighbour block next to the
- * neighbour's OPPOSITE face (face ^ 1), same transverse indices -- aligned blocks: the three computational axes of
- * the two blocks point the same way and the transverse cell counts and periodicity agree (MEG6_EINVAL otherwise).
- * Geometry is per block (ghost coordinates by R13, as at every non-periodic face; the paper: "metric terms are
- * non-existent" in ghost cells).  A block may be linked to itself (wrap-around).  Both grids must use one
- * stream; the link is a pointer: the neighbour must outlive the home grid's last call.
- * meg6_rhs_blocks / meg6_rk3_step_blocks advance n blocks together: primitives of all blocks, then the ghost
- * exchange direction by direction over all blocks (edge and corner ghosts come from diagonal neighbours in two
- * steps), then the sweeps of each block; per block the semantics of meg6_rhs / meg6_rk3_step.  g, U, dUdt: HOST
- * arrays of n pointers (grids; DEVICE state arrays).  Every neighbour of a listed block must be listed.  The
- * single-grid calls return MEG6_ESTATE on a grid that has an interface to another block or an unlinked one. */
+/* Multi-block (Sec. 6; Table 1 last column P:354-362; readings R28, R29).  A face with bc == 5 is a block
+ * interface: its ghost CELLS are the neighbour block's cells next to the face the two blocks share -- the six ghost
+ * layers of primitives at every stage, and the ten ghost layers of cell-centre coordinates (and grid velocities) the
+ * metrics are formed from, so that both blocks difference the same coordinates across the interface (the interface
+ * metrics of a cut mesh are those of the uncut one, bit for bit; fluxes across the cut are equal and opposite).
+ * meg6_link_blocks: aligned blocks -- the three computational axes of the two blocks point the same way, the
+ * neighbour's face is face ^ 1, the transverse cell counts and periodicity agree.
+ * meg6_link_blocks_oriented: "each block possesses its own coordinate system" -- home's `face` is the
+ * neighbour's `nb_face`; home's two transverse axes, in storage order (a < b), run along the neighbour's transverse axes
+ * (a' < b') as a -> a', b -> b' (swap 0) or a -> b', b -> a' (swap 1), each forwards (flip 0) or backwards (flip 1); the
+ * cell counts of the interface plane must agree.  off[3] (HOST pointer, may be NULL = 0) is added to the
+ * neighbour's coordinates seen from home: the period vector across a wrap-around link.  Velocities and coordinates are
+ * Cartesian components: only indices are mapped.  Where some link is not the aligned one the direction-by-direction
+ * ghost fills are repeated three times, so that edge and corner ghosts that reach a rotated neighbour's own ghost cells
+ * are the fixed point of the exchange (R29).  MEG6_EINVAL on mismatching sizes / scheme / stream.
+ * A block may be linked to itself (wrap-around).  The link is a pointer: the neighbour must outlive the home grid's
+ * last call.  A link invalidates the home block's metrics (call meg6_metrics_compute[_blocks] again).
+ * meg6_metrics_compute_blocks / meg6_rhs_blocks / meg6_rk3_step_blocks work on n blocks together: geometry -- cell
+ * centres of all blocks, then the ghost coordinates direction by direction over all blocks, then each block's metrics;
+ * flow -- primitives of all blocks, then the ghost exchange direction by direction over all blocks (edge and corner
+ * ghosts come from diagonal neighbours in two steps), then the sweeps of each block; per block the semantics of the
+ * single-grid calls.  g, U, dUdt: HOST arrays of n pointers (grids; DEVICE state arrays).  Every neighbour of a listed
+ * block must be listed.  The single-grid calls return MEG6_ESTATE on a grid that has an interface to another block or
+ * an unlinked one. */
 meg6_status meg6_link_blocks(meg6_grid* home, int face, meg6_grid* neighbour);
+meg6_status meg6_link_blocks_oriented(meg6_grid* home, int face, meg6_grid* neighbour, int nb_face, int swap, int flip_a,
+                                      int flip_b, const double* off);
+meg6_status meg6_metrics_compute_blocks(int n, meg6_grid* const* g, double t);
 meg6_status meg6_rhs_blocks(int n, meg6_grid* const* g, const double* const* U, double* const* dUdt);
 meg6_status meg6_rk3_step_blocks(int n, meg6_grid* const* g, double* const* U, double t, double dt);
 
@@ -129,6 +144,19 @@ meg6_status meg6_rk3_step_blocks(int n, meg6_grid* const* g, double* const* U, d
  *   meg6_stage_sweeps(g, U, NULL, s, dt)                 gradients + sweeps + fused RK stage update of U
  * meg6_stage_sweeps(g, U, dUdt, 0, 0) writes dQ/dt instead (after stage_prim and the ghost fills with s = 0).
  * Identical, kernel for kernel, to what meg6_rk3_step_blocks launches. */
+/* The geometry in pieces, for the same callers: meg6_stage_geom_centres(g, t); for d = 0, 1, 2: [meg6_stage_geom_pack
+ * (g, face, layers) for the interface faces of direction d -- the ten layers of cell-centre coordinates (moving meshes:
+ * and grid velocities) next to `face` over the padded transverse extent, meg6_geom_interface_doubles doubles -- delivered
+ * to the neighbour, which registered its receive buffer with meg6_set_geom_interface_buffer(g, face, layers, off)],
+ * meg6_stage_geom_extend(g, d); then meg6_stage_geom_finish(g).  Remote neighbours are aligned blocks at least ten
+ * cells thick along the link.  Static meshes: once; moving meshes: at every stage time. */
+size_t      meg6_geom_interface_doubles(const meg6_grid* g, int face);
+meg6_status meg6_set_geom_interface_buffer(meg6_grid* g, int face, const double* layers, const double* off);
+meg6_status meg6_stage_geom_centres(meg6_grid* g, double t);
+meg6_status meg6_stage_geom_pack(meg6_grid* g, int face, double* layers);
+meg6_status meg6_stage_geom_extend(meg6_grid* g, int d);
+meg6_status meg6_stage_geom_finish(meg6_grid* g);
+
 size_t      meg6_interface_doubles(const meg6_grid* g, int face);
 meg6_status meg6_set_interface_buffer(meg6_grid* g, int face, const double* layers);
 meg6_status meg6_stage_prim(meg6_grid* g, const double* U);

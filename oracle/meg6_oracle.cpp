@@ -221,6 +221,7 @@ struct meg6o_grid {
   std::vector<double> xn, yn, zn, dxm, dym, dzm;   /* nodes */
   /* geometry at the time of the last metrics_compute */
   Arr xc[3];         /* cell-centre coordinates, ghost 10 */
+  Arr xt[3];         /* cell-centre grid velocities (moving meshes), ghost 10 */
   Arr met[9];        /* hatted metrics at cell centres, valid on [-5,n+5) */
   Arr rj;            /* 1/J */
   Arr mt[3];         /* hatted time metrics */
@@ -241,7 +242,18 @@ struct meg6o_grid {
   bool want_masks = false;
   std::vector<unsigned short> mask[3];
   meg6o_grid* link[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};   /* bc 5: neighbour block per face */
+  /* orientation of the neighbour seen from this block (Sec. 6: "each block possesses its own coordinate
+   * system"; R28/R29): a cell with index vector h of THIS block (ghost ranges included) is the neighbour's cell m with
+   * m[lax[e]] = lsg[e] > 0 ? h[e] + lsh[e] : lsh[e] - h[e]; loff = what is added to the neighbour's coordinates when
+   * they are seen from here (zero, or the period vector across a wrap-around link) */
+  int lax[6][3], lsg[6][3], lsh[6][3];
+  double loff[6][3];
+  bool rotated = false;            /* some link is not the aligned one: the ghost fills are repeated (R29) */
+  bool thin_nb = false;            /* a neighbour has fewer cells along the link than the coordinate ghost depth: its own
+                                      ghost coordinates (from ITS neighbour) are read, so the extension runs twice */
   const double* ibuf[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr}; /* bc 5: or packed neighbour layers */
+  const double* gbuf[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr}; /* ... and packed cell-centre layers */
+  double goff[6][3];
 };
 
 namespace {
@@ -249,8 +261,13 @@ namespace {
 const int GX = 10; /* ghost depth of coordinates (two nested delta of reach 5, R13/R19) */
 const int GP = 6;  /* ghost depth of primitives (R19) */
 
-/* O1.3: extend a cell-centre array along dir: periodic image + offset, or linear extrapolation (R13, R14) */
-void extend_dir(Arr& a, int dir, bool periodic, double offset) {
+/* O1.3: extend a cell-centre array along dir: periodic image + offset, or linear extrapolation (R13, R14), or -- at a
+ * block-interface face (bc 5) -- the neighbour block's own cell centres (R28: the two blocks then difference the same
+ * coordinates across their common face, so the interface metrics of the cut are those of the uncut mesh).
+ * comp = coordinate component (0..2) of `a`, vel: `a` is a grid-velocity array (no offsets).  which: 0 -> G->xc, 1 -> xt
+ * of the neighbour (passed in nbarr per face, null where the face is no linked interface). */
+void extend_dir(Arr& a, int dir, bool periodic, double offset, const meg6o_grid* G = nullptr, int comp = 0,
+                const Arr* const nbarr[2] = nullptr, bool vel = false) {
   const int n = a.n[dir], g = a.g;
   int lo[3], hi[3];
   for (int c = 0; c < 3; ++c) { lo[c] = a.lo[c]; hi[c] = a.hi[c]; }
@@ -263,9 +280,32 @@ void extend_dir(Arr& a, int dir, bool periodic, double offset) {
           if (periodic) {
             base[-q * s] = base[(n - q) * s] - offset;
             base[(n - 1 + q) * s] = base[(q - 1) * s] + offset;
-          } else {
-            base[-q * s] = base[0] - q * (base[s] - base[0]);
-            base[(n - 1 + q) * s] = base[(n - 1) * s] + q * (base[(n - 1) * s] - base[(n - 2) * s]);
+            continue;
+          }
+          for (int side = 0; side < 2; ++side) {
+            const int face = 2 * dir + side;
+            const int hd = side ? n - 1 + q : -q;
+            double v;
+            if (G && G->p.bc[face] == 5 && nbarr && nbarr[side]) {
+              int h[3] = {i, j, k}, m[3];
+              h[dir] = hd;
+              for (int e = 0; e < 3; ++e)
+                m[G->lax[face][e]] = G->lsg[face][e] > 0 ? h[e] + G->lsh[face][e] : G->lsh[face][e] - h[e];
+              v = (*nbarr[side])(m[0], m[1], m[2]) + (vel ? 0.0 : G->loff[face][comp]);
+            } else if (G && G->p.bc[face] == 5 && G->gbuf[face]) {
+              /* packed layers of a remote neighbour (meg6o_stage_geom_pack on its side): [vel*3 + comp][tb][ta][l] */
+              int ta = (dir == 0) ? j : i, tb = (dir == 2) ? j : k;
+              int e1 = (dir == 0) ? 1 : 0, e2 = (dir == 2) ? 1 : 2;
+              const size_t ea = a.n[e1] + 2 * GX, eb = a.n[e2] + 2 * GX;
+              const int l = side ? q - 1 : GX - q;
+              v = G->gbuf[face][((((size_t)(vel ? 3 : 0) + comp) * eb + (size_t)(tb + GX)) * ea + (size_t)(ta + GX)) * GX + l] +
+                  (vel ? 0.0 : G->goff[face][comp]);
+            } else if (!side) {
+              v = base[0] - q * (base[s] - base[0]);
+            } else {
+              v = base[(n - 1) * s] + q * (base[(n - 1) * s] - base[(n - 2) * s]);
+            }
+            base[hd * s] = v;
           }
         }
       }
@@ -316,14 +356,13 @@ meg6o_grid* meg6o_create(const meg6o_params* p, const double* x, const double* y
 void meg6o_destroy(meg6o_grid* G) { delete G; }
 
 /* ---------------------------------- O1 geometry ------------------------------------------- */
-void meg6o_metrics_compute(meg6o_grid* G, double t) {
+namespace {
+/* O1.1-O1.2: node positions and analytic node velocities (form of Eq. 49-50), cell centres */
+void geom_centres(meg6o_grid* G, double t) {
   const meg6o_params& p = G->p;
-  const int sch = p.scheme;
   const double two_pi = 2.0 * M_PI;
-  /* O1.1 node positions and analytic node velocities (form of Eq. 49-50) */
   const std::vector<double>* base[3] = {&G->xn, &G->yn, &G->zn};
   const std::vector<double>* mode[3] = {&G->dxm, &G->dym, &G->dzm};
-  Arr xt[3];
   for (int c = 0; c < 3; ++c) {
     if (G->user_centres) continue;
     if (p.moving) {
@@ -331,16 +370,82 @@ void meg6o_metrics_compute(meg6o_grid* G, double t) {
       std::vector<double> pos(base[c]->size()), vel(base[c]->size());
       for (size_t q = 0; q < pos.size(); ++q) { pos[q] = (*base[c])[q] + s * (*mode[c])[q]; vel[q] = sd * (*mode[c])[q]; }
       cell_mean(*G, pos, G->xc[c]);
-      cell_mean(*G, vel, xt[c]);
+      cell_mean(*G, vel, G->xt[c]);
     } else {
       cell_mean(*G, *base[c], G->xc[c]);
     }
-    /* O1.3 ghost layers, direction by direction */
-    for (int d = 0; d < 3; ++d) {
-      extend_dir(G->xc[c], d, p.periodic[d] != 0, p.period[d][c]);
-      if (p.moving) extend_dir(xt[c], d, p.periodic[d] != 0, 0.0);
-    }
   }
+}
+/* O1.3 ghost layers of direction d (after the lower directions; with several blocks: direction d in every block
+ * before direction d+1 in any, like the ghost fill of the primitives) */
+void geom_extend(meg6o_grid* G, int d) {
+  const meg6o_params& p = G->p;
+  if (G->user_centres) return;
+  for (int c = 0; c < 3; ++c) {
+    const Arr* nbx[2] = {nullptr, nullptr};
+    const Arr* nbv[2] = {nullptr, nullptr};
+    for (int side = 0; side < 2; ++side) {
+      const meg6o_grid* nb = (!p.periodic[d] && p.bc[2 * d + side] == 5) ? G->link[2 * d + side] : nullptr;
+      if (nb) {
+        if (nb->xc[c].d.empty()) { fprintf(stderr, "meg6o geometry: the neighbour block has no cell centres yet (use meg6o_metrics_compute_blocks)\n"); abort(); }
+        nbx[side] = &nb->xc[c]; nbv[side] = &nb->xt[c];
+      }
+    }
+    extend_dir(G->xc[c], d, p.periodic[d] != 0, p.period[d][c], G, c, nbx, false);
+    if (p.moving) extend_dir(G->xt[c], d, p.periodic[d] != 0, 0.0, G, c, nbv, true);
+  }
+}
+void geom_finish(meg6o_grid* G);
+}  // namespace
+
+/* geometry of several linked blocks: centres everywhere, then the ghost coordinates direction by direction over all
+ * blocks (repeated where a link is rotated, R29), then each block's metrics */
+void meg6o_metrics_compute_blocks(int nb, meg6o_grid* const* G, double t) {
+  bool rot = false, thin = false;
+  for (int b = 0; b < nb; ++b) { geom_centres(G[b], t); rot = rot || G[b]->rotated; thin = thin || G[b]->thin_nb; }
+  for (int pass = 0; pass < (rot ? 3 : thin ? 2 : 1); ++pass)
+    for (int d = 0; d < 3; ++d)
+      for (int b = 0; b < nb; ++b) geom_extend(G[b], d);
+  for (int b = 0; b < nb; ++b) geom_finish(G[b]);
+}
+
+void meg6o_metrics_compute(meg6o_grid* G, double t) { meg6o_metrics_compute_blocks(1, &G, t); }
+
+/* staged geometry for blocks in different processes (the caller carries the packed cell-centre layers) */
+void meg6o_stage_geom_centres(meg6o_grid* G, double t) { geom_centres(G, t); }
+void meg6o_stage_geom_extend(meg6o_grid* G, int d) { geom_extend(G, d); }
+void meg6o_stage_geom_finish(meg6o_grid* G) { geom_finish(G); }
+size_t meg6o_geom_interface_doubles(const meg6o_grid* G, int face) {
+  const int d = face / 2;
+  const int e1 = (d == 0) ? 1 : 0, e2 = (d == 2) ? 1 : 2;
+  return (size_t)(G->p.moving ? 6 : 3) * GX * (G->n[e1] + 2 * GX) * (G->n[e2] + 2 * GX);
+}
+void meg6o_set_geom_interface_buffer(meg6o_grid* G, int face, const double* layers, const double* off) {
+  G->gbuf[face] = layers;
+  for (int c = 0; c < 3; ++c) G->goff[face][c] = off ? off[c] : 0.0;
+}
+void meg6o_stage_geom_pack(meg6o_grid* G, int face, double* layers) {
+  const int d = face / 2, side = face & 1;
+  if (G->n[d] < GX) { fprintf(stderr, "meg6o_stage_geom_pack: a block must be at least %d cells thick along a remote link\n", GX); abort(); }
+  const int e1 = (d == 0) ? 1 : 0, e2 = (d == 2) ? 1 : 2;
+  const size_t ea = G->n[e1] + 2 * GX, eb = G->n[e2] + 2 * GX;
+  const int first = side ? G->n[d] - GX : 0;
+  for (int f = 0; f < (G->p.moving ? 6 : 3); ++f) {
+    const Arr& a = (f < 3) ? G->xc[f] : G->xt[f - 3];
+    for (int tb = -GX; tb < G->n[e2] + GX; ++tb)
+      for (int ta = -GX; ta < G->n[e1] + GX; ++ta)
+        for (int l = 0; l < GX; ++l) {
+          int is[3]; is[e1] = ta; is[e2] = tb; is[d] = first + l;
+          layers[((f * eb + (size_t)(tb + GX)) * ea + (size_t)(ta + GX)) * GX + l] = a.d[a.idx(is[0], is[1], is[2])];
+        }
+  }
+}
+
+namespace {
+void geom_finish(meg6o_grid* G) {
+  const meg6o_params& p = G->p;
+  const int sch = p.scheme;
+  Arr* xt = G->xt;
   auto mul = [](double a, double b) { return a * b; };
   auto sub = [](double a, double b) { return a - b; };
 
@@ -439,6 +544,7 @@ void meg6o_metrics_compute(meg6o_grid* G, double t) {
   }
   G->have_metrics = true;
 }
+}  // namespace
 
 /* tests only: supply padded cell-centre coordinates [(nk+20)(nj+20)(ni+20)] (ghost depth 10) directly,
  * bypassing O1.1-O1.3, so that single coefficients of the metric stencils can be probed (Eq. 43). */
@@ -715,10 +821,12 @@ void ghost_dir(meg6o_grid* G, int d) {
              * neighbour block counted from its opposite face, same transverse index (aligned blocks) */
             const meg6o_grid* nb = G->link[face];
             if (nb) {
-              const int nn = nb->n[d];
               for (int q = 1; q <= GP; ++q) {
-                int is[3]; is[a] = ta; is[b] = tb; is[d] = side ? q - 1 : nn - q;
-                for (int f = 0; f < 5; ++f) at(f, last + sg * q) = nb->P[f](is[0], is[1], is[2]);
+                int h[3], m[3];
+                h[a] = ta; h[b] = tb; h[d] = last + sg * q;
+                for (int e = 0; e < 3; ++e)
+                  m[G->lax[face][e]] = G->lsg[face][e] > 0 ? h[e] + G->lsh[face][e] : G->lsh[face][e] - h[e];
+                for (int f = 0; f < 5; ++f) at(f, last + sg * q) = nb->P[f](m[0], m[1], m[2]);
               }
             } else {
               /* packed layers of a neighbour that lives elsewhere (meg6o_stage_pack on its side): layer l = 0..5 in
@@ -806,8 +914,13 @@ void meg6o_rhs_blocks(int nb, meg6o_grid* const* G, const double* const* U, doub
       if (!G[b]->p.periodic[f / 2] && G[b]->p.bc[f] == 5 && !G[b]->link[f] && !G[b]->ibuf[f]) { fprintf(stderr, "meg6o_rhs: unlinked block interface\n"); abort(); }
     prim_interior(G[b], U[b]);
   }
-  for (int d = 0; d < 3; ++d)
-    for (int b = 0; b < nb; ++b) ghost_dir(G[b], d);
+  /* rotated links (R29): the neighbour cell behind an edge or corner ghost may itself be a ghost of a direction the
+   * neighbour fills later; repeating the fill makes every ghost cell the fixed point of the exchange */
+  bool rot = false;
+  for (int b = 0; b < nb; ++b) rot = rot || G[b]->rotated;
+  for (int pass = 0; pass < (rot ? 3 : 1); ++pass)
+    for (int d = 0; d < 3; ++d)
+      for (int b = 0; b < nb; ++b) ghost_dir(G[b], d);
   for (int b = 0; b < nb; ++b) finish_primitives(G[b]);
   for (int b = 0; b < nb; ++b) rhs_from_primitives(G[b], U[b], dUdt[b]);
 }
@@ -948,8 +1061,7 @@ void meg6o_rk3_step_blocks(int nb, meg6o_grid* const* G, double* const* U, doubl
   }
   const double ts[3] = {t, t + dt, t + 0.5 * dt};
   for (int s = 0; s < 3; ++s) {
-    for (int b = 0; b < nb; ++b)
-      if (G[b]->p.moving) meg6o_metrics_compute(G[b], ts[s]);
+    if (G[0]->p.moving) meg6o_metrics_compute_blocks(nb, G, ts[s]);
     meg6o_rhs_blocks(nb, G, Uc.data(), Lp.data());
     for (int b = 0; b < nb; ++b) {
       double* u = U[b];
@@ -996,18 +1108,50 @@ void meg6o_stage_rhs(meg6o_grid* G, const double* U, double* dUdt) {
   rhs_from_primitives(G, U, dUdt);
 }
 
-/* Block interface (Sec. 6; Table 1 last column): face `face` of `home` (bc 5) takes its ghost primitives
- * from the interior cells of `nb` next to nb's opposite face.  Aligned blocks only (same orientation of the three
- * computational axes, equal transverse cell counts): R28.  Returns 0 on success. */
+/* Block interface (Sec. 6; Table 1 last column): face `face` of `home` (bc 5) takes its ghost cells -- the
+ * primitives, and the cell-centre coordinates the metrics are built from -- out of the block `nb`, whose face `nb_face`
+ * is the same surface.  "Each block possesses its own coordinate system": the two transverse axes of the home
+ * face, in storage order (a < b), run along the neighbour's transverse axes (a' < b') as a -> a', b -> b' (swap = 0) or
+ * a -> b', b -> a' (swap = 1), each forwards (flip = 0) or backwards (flip = 1); the cell counts must agree ("the
+ * dimensions of the block interface plane should be identical").  off[3] is added to the neighbour's coordinates
+ * seen from home (zero; the period vector across a wrap-around link).  Returns 0 on success.  R28, R29. */
+int meg6o_link_blocks_oriented(meg6o_grid* home, int face, meg6o_grid* nb, int nb_face, int swap, int flip_a, int flip_b,
+                               const double* off) {
+  if (!home || !nb || face < 0 || face > 5 || nb_face < 0 || nb_face > 5) return 1;
+  const int d = face / 2, dn = nb_face / 2;
+  if (home->p.periodic[d] || home->p.bc[face] != 5) return 1;
+  if (nb->p.periodic[dn] || nb->n[dn] < GP) return 1;
+  int a = (d + 1) % 3, b = (d + 2) % 3, an = (dn + 1) % 3, bn = (dn + 2) % 3;
+  if (a > b) std::swap(a, b);
+  if (an > bn) std::swap(an, bn);
+  const int ta = swap ? bn : an, tb = swap ? an : bn;     /* images of the home axes a, b */
+  if (nb->n[ta] != home->n[a] || nb->n[tb] != home->n[b]) return 1;
+  int* ax = home->lax[face]; int* sg = home->lsg[face]; int* sh = home->lsh[face];
+  ax[a] = ta; sg[a] = flip_a ? -1 : 1; sh[a] = flip_a ? home->n[a] - 1 : 0;
+  ax[b] = tb; sg[b] = flip_b ? -1 : 1; sh[b] = flip_b ? home->n[b] - 1 : 0;
+  /* along the normal: ghost layer q of home = the q-th interior cell of the neighbour counted from nb_face */
+  const int n = home->n[d], nn = nb->n[dn], hs = face & 1, ns = nb_face & 1;
+  ax[d] = dn;
+  if (hs && !ns) { sg[d] = 1; sh[d] = -n; }
+  else if (hs && ns) { sg[d] = -1; sh[d] = nn - 1 + n; }
+  else if (!hs && ns) { sg[d] = 1; sh[d] = nn; }
+  else { sg[d] = -1; sh[d] = -1; }
+  for (int c = 0; c < 3; ++c) home->loff[face][c] = off ? off[c] : 0.0;
+  home->link[face] = nb;
+  home->ibuf[face] = nullptr; home->gbuf[face] = nullptr;
+  const bool aligned = ax[0] == 0 && ax[1] == 1 && ax[2] == 2 && sg[0] > 0 && sg[1] > 0 && sg[2] > 0;
+  if (!aligned) { home->rotated = true; nb->rotated = true; }
+  if (nn < GX) home->thin_nb = true;
+  return 0;
+}
+
+/* aligned blocks: same orientation of the three computational axes, nb's opposite face */
 int meg6o_link_blocks(meg6o_grid* home, int face, meg6o_grid* nb) {
   if (!home || !nb || face < 0 || face > 5) return 1;
   const int d = face / 2;
-  if (home->p.periodic[d] || home->p.bc[face] != 5) return 1;
-  if (nb->p.periodic[d] || nb->n[d] < GP) return 1;
   for (int e = 0; e < 3; ++e)
-    if (e != d && (nb->n[e] != home->n[e] || nb->p.periodic[e] != home->p.periodic[e])) return 1;
-  home->link[face] = nb;
-  return 0;
+    if (e != d && nb->p.periodic[e] != home->p.periodic[e]) return 1;
+  return meg6o_link_blocks_oriented(home, face, nb, face ^ 1, 0, 0, 0, nullptr);
 }
 
 /* Eq. B.2 / B.3: un-hatted metrics = hatted * J; viscous alpha read as alpha^D = 4 (R25) */

@@ -53,6 +53,22 @@ void meg6o_rk3_step(meg6o_grid* g, double* U, double t, double dt);
  * from the interior cells of `nb` next to nb's opposite face; aligned blocks, equal transverse sizes.  Returns 0 if ok.
  * The *_blocks calls advance all blocks together (ghost exchange before every right-hand side). */
 int meg6o_link_blocks(meg6o_grid* home, int face, meg6o_grid* nb);
+/* The same for blocks with their own coordinate systems: home's `face` is the neighbour's `nb_face`; home's
+ * transverse axes (storage order) run along the neighbour's transverse axes in that order (swap 0) or exchanged (swap 1),
+ * forwards or backwards (flip_a, flip_b); off[3] (may be NULL) is added to the neighbour's cell-centre coordinates seen
+ * from home (the period vector across a wrap-around link).  Ghost CELLS come from the neighbour: primitives and the
+ * cell-centre coordinates the metrics are formed from (R28, R29). */
+int meg6o_link_blocks_oriented(meg6o_grid* home, int face, meg6o_grid* nb, int nb_face, int swap, int flip_a, int flip_b,
+                               const double* off);
+/* geometry of linked blocks together: cell centres of all, ghost coordinates direction by direction over all, metrics */
+void meg6o_metrics_compute_blocks(int nb, meg6o_grid* const* g, double t);
+/* staged geometry for blocks in different processes: centres -> for d: [pack / deliver] extend(d) -> finish */
+size_t meg6o_geom_interface_doubles(const meg6o_grid* g, int face);
+void meg6o_set_geom_interface_buffer(meg6o_grid* g, int face, const double* layers, const double* off);
+void meg6o_stage_geom_centres(meg6o_grid* g, double t);
+void meg6o_stage_geom_pack(meg6o_grid* g, int face, double* layers);
+void meg6o_stage_geom_extend(meg6o_grid* g, int d);
+void meg6o_stage_geom_finish(meg6o_grid* g);
 /* Staged evaluation for blocks in different processes: prim -> for d: [pack / deliver / set_interface_buffer] ghosts(d)
  * -> stage_rhs.  The packed layers of a face: meg6o_interface_doubles doubles. */
 size_t meg6o_interface_doubles(const meg6o_grid* g, int face);

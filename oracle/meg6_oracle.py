@@ -63,6 +63,16 @@ def lib():
         L.meg6o_rk3_step.argtypes = [C.c_void_p, _dp, C.c_double, C.c_double]
         L.meg6o_link_blocks.restype = C.c_int
         L.meg6o_link_blocks.argtypes = [C.c_void_p, C.c_int, C.c_void_p]
+        L.meg6o_link_blocks_oriented.restype = C.c_int
+        L.meg6o_link_blocks_oriented.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, _dp]
+        L.meg6o_metrics_compute_blocks.argtypes = [C.c_int, C.POINTER(C.c_void_p), C.c_double]
+        L.meg6o_geom_interface_doubles.restype = C.c_size_t
+        L.meg6o_geom_interface_doubles.argtypes = [C.c_void_p, C.c_int]
+        L.meg6o_set_geom_interface_buffer.argtypes = [C.c_void_p, C.c_int, C.c_void_p, _dp]
+        L.meg6o_stage_geom_centres.argtypes = [C.c_void_p, C.c_double]
+        L.meg6o_stage_geom_pack.argtypes = [C.c_void_p, C.c_int, C.c_void_p]
+        L.meg6o_stage_geom_extend.argtypes = [C.c_void_p, C.c_int]
+        L.meg6o_stage_geom_finish.argtypes = [C.c_void_p]
         L.meg6o_rhs_blocks.argtypes = [C.c_int, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p), C.POINTER(C.c_void_p)]
         L.meg6o_rk3_step_blocks.argtypes = [C.c_int, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p), C.c_double, C.c_double]
         L.meg6o_interface_doubles.restype = C.c_size_t
@@ -186,10 +196,43 @@ class Grid:
         assert U.flags.c_contiguous and U.dtype == np.float64
         lib().meg6o_rk3_step(self.h, _p(U), float(t), float(dt))
 
-    def link(self, face, neighbour):
-        if lib().meg6o_link_blocks(self.h, int(face), neighbour.h) != 0:
+    def link(self, face, neighbour, nb_face=None, swap=0, flip_a=0, flip_b=0, offset=None):
+        """block interface: ghost cells of `face` come from `neighbour` (its face nb_face, default the opposite one;
+        orientation of the transverse axes: swap / flip_a / flip_b; offset added to its coordinates seen from here)"""
+        off = _c(offset if offset is not None else [0.0, 0.0, 0.0])
+        if nb_face is None and not (swap or flip_a or flip_b):
+            rc = lib().meg6o_link_blocks(self.h, int(face), neighbour.h)
+            if rc == 0 and offset is not None:
+                rc = lib().meg6o_link_blocks_oriented(self.h, int(face), neighbour.h, int(face) ^ 1, 0, 0, 0, _p(off))
+        else:
+            rc = lib().meg6o_link_blocks_oriented(self.h, int(face), neighbour.h,
+                                                  int(face) ^ 1 if nb_face is None else int(nb_face), int(swap),
+                                                  int(flip_a), int(flip_b), _p(off))
+        if rc != 0:
             raise ValueError("meg6o_link_blocks rejected the pair")
         self._links = getattr(self, "_links", []) + [neighbour]
+
+    # staged geometry (blocks in different processes)
+    def geom_interface_doubles(self, face):
+        return int(lib().meg6o_geom_interface_doubles(self.h, int(face)))
+
+    def set_geom_interface_buffer(self, face, layers, offset=None):
+        assert layers.dtype == np.float64 and layers.flags["C_CONTIGUOUS"]
+        off = _c(offset if offset is not None else [0.0, 0.0, 0.0])
+        lib().meg6o_set_geom_interface_buffer(self.h, int(face), layers.ctypes.data, _p(off))
+
+    def stage_geom_centres(self, t):
+        lib().meg6o_stage_geom_centres(self.h, float(t))
+
+    def stage_geom_pack(self, face, layers):
+        assert layers.dtype == np.float64 and layers.flags["C_CONTIGUOUS"]
+        lib().meg6o_stage_geom_pack(self.h, int(face), layers.ctypes.data)
+
+    def stage_geom_extend(self, d):
+        lib().meg6o_stage_geom_extend(self.h, int(d))
+
+    def stage_geom_finish(self):
+        lib().meg6o_stage_geom_finish(self.h)
 
     # staged evaluation (blocks in different processes); `layers` are numpy float64 arrays kept alive by the caller
     def interface_doubles(self, face):
@@ -268,6 +311,11 @@ class Grid:
 
 def _vps(ptrs):
     return (C.c_void_p * len(ptrs))(*ptrs)
+
+
+def metrics_compute_blocks(grids, t=0.0):
+    """geometry of several linked blocks together (meg6o_metrics_compute_blocks)"""
+    lib().meg6o_metrics_compute_blocks(len(grids), _vps([g.h for g in grids]), float(t))
 
 
 def rhs_blocks(grids, Us):

@@ -3,4 +3,4 @@
 The Python layer only marshals arguments: every step of the path runs in the CUDA kernels of
 csrc/libmeg6.so.  There is no CPU fallback: a missing library or device raises.
 """
-from .binding import (Grid, Meg6Error, Params, lib, lib_path, make_params, EXPORTS, rhs_blocks, rk3_step_blocks, fp64_peak)  # noqa: F401
+from .binding import (Grid, Meg6Error, Params, lib, lib_path, make_params, EXPORTS, rhs_blocks, rk3_step_blocks, metrics_compute_blocks, fp64_peak)  # noqa: F401

@@ -11,7 +11,9 @@ EXPORTS = ["meg6_workspace_bytes", "meg6_grid_create", "meg6_grid_destroy", "meg
            "meg6_set_inflow", "meg6_set_sponge", "meg6_rhs", "meg6_rk3_step", "meg6_cfl_dt", "meg6_diagnostics",
            "meg6_limiter_stats_enable", "meg6_limiter_stats", "meg6_set_branch_masks", "meg6_get_array", "meg6_profile_enable",
            "meg6_profile_read", "meg6_fp64_peak", "meg6_last_error",
-           "meg6_version", "meg6_link_blocks", "meg6_rhs_blocks", "meg6_rk3_step_blocks",
+           "meg6_version", "meg6_link_blocks", "meg6_link_blocks_oriented", "meg6_metrics_compute_blocks", "meg6_rhs_blocks",
+           "meg6_rk3_step_blocks", "meg6_geom_interface_doubles", "meg6_set_geom_interface_buffer",
+           "meg6_stage_geom_centres", "meg6_stage_geom_pack", "meg6_stage_geom_extend", "meg6_stage_geom_finish",
            "meg6_interface_doubles", "meg6_set_interface_buffer", "meg6_stage_prim", "meg6_stage_pack",
            "meg6_stage_ghosts", "meg6_stage_sweeps"]
 
@@ -101,6 +103,23 @@ def lib():
         L.meg6_profile_read.argtypes = [_vp, C.POINTER(C.c_double), C.POINTER(C.c_ulonglong)]
         L.meg6_link_blocks.restype = C.c_int
         L.meg6_link_blocks.argtypes = [_vp, C.c_int, _vp]
+        L.meg6_link_blocks_oriented.restype = C.c_int
+        L.meg6_link_blocks_oriented.argtypes = [_vp, C.c_int, _vp, C.c_int, C.c_int, C.c_int, C.c_int,
+                                                C.POINTER(C.c_double)]
+        L.meg6_metrics_compute_blocks.restype = C.c_int
+        L.meg6_metrics_compute_blocks.argtypes = [C.c_int, C.POINTER(_vp), C.c_double]
+        L.meg6_geom_interface_doubles.restype = C.c_size_t
+        L.meg6_geom_interface_doubles.argtypes = [_vp, C.c_int]
+        L.meg6_set_geom_interface_buffer.restype = C.c_int
+        L.meg6_set_geom_interface_buffer.argtypes = [_vp, C.c_int, _vp, C.POINTER(C.c_double)]
+        L.meg6_stage_geom_centres.restype = C.c_int
+        L.meg6_stage_geom_centres.argtypes = [_vp, C.c_double]
+        L.meg6_stage_geom_pack.restype = C.c_int
+        L.meg6_stage_geom_pack.argtypes = [_vp, C.c_int, _vp]
+        L.meg6_stage_geom_extend.restype = C.c_int
+        L.meg6_stage_geom_extend.argtypes = [_vp, C.c_int]
+        L.meg6_stage_geom_finish.restype = C.c_int
+        L.meg6_stage_geom_finish.argtypes = [_vp]
         L.meg6_rhs_blocks.restype = C.c_int
         L.meg6_rhs_blocks.argtypes = [C.c_int, C.POINTER(_vp), C.POINTER(_vp), C.POINTER(_vp)]
         L.meg6_rk3_step_blocks.restype = C.c_int
@@ -199,10 +218,43 @@ class Grid:
         self._chk_state(U)
         _check(lib().meg6_rk3_step(self.h, U.data_ptr(), float(t), float(dt)), "meg6_rk3_step")
 
-    def link(self, face, neighbour):
-        """block interface (bc 5): ghost cells of `face` come from `neighbour`'s interior at its opposite face"""
-        _check(lib().meg6_link_blocks(self.h, int(face), neighbour.h), "meg6_link_blocks")
+    def link(self, face, neighbour, nb_face=None, swap=0, flip_a=0, flip_b=0, offset=None):
+        """block interface (bc 5): ghost cells of `face` come from `neighbour` (its face nb_face, default the opposite
+        one; orientation of the transverse axes: swap / flip_a / flip_b; offset added to its coordinates seen from here)"""
+        if nb_face is None and not (swap or flip_a or flip_b) and offset is None:
+            _check(lib().meg6_link_blocks(self.h, int(face), neighbour.h), "meg6_link_blocks")
+        else:
+            off = (C.c_double * 3)(*(offset if offset is not None else (0.0, 0.0, 0.0)))
+            _check(lib().meg6_link_blocks_oriented(self.h, int(face), neighbour.h,
+                                                   int(face) ^ 1 if nb_face is None else int(nb_face), int(swap),
+                                                   int(flip_a), int(flip_b), off), "meg6_link_blocks_oriented")
         self._links = getattr(self, "_links", []) + [neighbour]   # keep the neighbour alive
+
+    # ---- staged geometry (include/meg6.h): the pieces paper_2303_10785_b200.slabs drives ----
+    def new_geom_interface_buffer(self, face):
+        n = lib().meg6_geom_interface_doubles(self.h, int(face))
+        return self.torch.zeros(n, dtype=self.torch.float64, device=self.device)
+
+    def set_geom_interface_buffer(self, face, layers, offset=None):
+        assert layers.is_cuda and layers.dtype == self.torch.float64 and layers.is_contiguous()
+        off = (C.c_double * 3)(*(offset if offset is not None else (0.0, 0.0, 0.0)))
+        _check(lib().meg6_set_geom_interface_buffer(self.h, int(face), layers.data_ptr(), off),
+               "meg6_set_geom_interface_buffer")
+        if not hasattr(self, "_gbufs"):
+            self._gbufs = {}
+        self._gbufs[int(face)] = layers   # keep it alive
+
+    def stage_geom_centres(self, t):
+        _check(lib().meg6_stage_geom_centres(self.h, float(t)), "meg6_stage_geom_centres")
+
+    def stage_geom_pack(self, face, layers):
+        _check(lib().meg6_stage_geom_pack(self.h, int(face), layers.data_ptr()), "meg6_stage_geom_pack")
+
+    def stage_geom_extend(self, d):
+        _check(lib().meg6_stage_geom_extend(self.h, int(d)), "meg6_stage_geom_extend")
+
+    def stage_geom_finish(self):
+        _check(lib().meg6_stage_geom_finish(self.h), "meg6_stage_geom_finish")
 
     # ---- staged stepping (include/meg6.h "Staged stepping"): the pieces paper_2303_10785_b200.slabs drives ----
     def new_interface_buffer(self, face):
@@ -306,6 +358,12 @@ def fp64_peak(device="cuda:0"):
 
 def _ptr_array(ptrs):
     return (_vp * len(ptrs))(*ptrs)
+
+
+def metrics_compute_blocks(grids, t=0.0):
+    """geometry of several linked blocks together (meg6_metrics_compute_blocks)"""
+    _check(lib().meg6_metrics_compute_blocks(len(grids), _ptr_array([g.h.value for g in grids]), float(t)),
+           "meg6_metrics_compute_blocks")
 
 
 def rhs_blocks(grids, Us, outs=None):

@@ -133,7 +133,10 @@ static size_t carve(const meg6_params* p, const Consts& c, meg6_grid* g, char* b
 
 static inline unsigned nblk(long long n, int t) { return (unsigned)((n + t - 1) / t); }
 namespace meg6 {
-cudaError_t launch_geometry(meg6_grid* g, double t);
+cudaError_t geom_centres(meg6_grid* g, double t);
+cudaError_t geom_extend(meg6_grid* g, int d);
+cudaError_t geom_rest(meg6_grid* g);
+cudaError_t geom_pack(meg6_grid* g, int face, double* layers);
 Box launch_ig4(meg6_grid* g, const Lay& L, const double* f, const Box& fb, int dir, double* out);
 Box launch_ig4_batch(meg6_grid* g, const Lay& L, const double* f, const Box& fb, int dir, double* out, int nfields,
                      long long fs_in, long long fs_out);
@@ -366,17 +369,99 @@ void meg6_grid_destroy(meg6_grid* g) {
   delete g;
 }
 
-meg6_status meg6_metrics_compute(meg6_grid* g, double t) {
-  if (!g) return fail(MEG6_EINVAL, "null grid%s");
-  if (g->have_metrics && !g->p.moving) return MEG6_OK;   // static: idempotent
-  cudaError_t e;
+static bool links_ok(const meg6_grid* g, bool single);
+
+// Geometry of n linked blocks together: cell centres of all, then the ghost coordinates direction by direction over all
+// blocks (repeated where a link is rotated, R29), then each block's metrics.
+meg6_status meg6_metrics_compute_blocks(int n, meg6_grid* const* g, double t) {
+  if (n < 1 || !g) return fail(MEG6_EINVAL, "metrics_compute_blocks: no blocks%s");
+  bool todo = false, rot = false;
+  for (int b = 0; b < n; ++b) {
+    if (!g[b]) return fail(MEG6_EINVAL, "metrics_compute_blocks: null grid%s");
+    if (!links_ok(g[b], false)) return fail(MEG6_ESTATE, "metrics_compute: block-interface face without a link%s");
+    for (int f = 0; f < 6; ++f) {   // every neighbour must be in the list: its cell centres are read
+      const meg6_grid* nb = g[b]->link[f];
+      bool found = nb == nullptr;
+      for (int q = 0; q < n && !found; ++q) found = g[q] == nb;
+      if (!found) return fail(MEG6_ESTATE, "metrics_compute: a linked neighbour block is not in the call (use meg6_metrics_compute_blocks)%s");
+    }
+    todo = todo || !g[b]->have_metrics || g[b]->p.moving;
+    rot = rot || g[b]->rotated;
+  }
+  if (!todo) return MEG6_OK;   // static: idempotent
+  cudaError_t e = cudaSuccess;
+  std::vector<ProfScope*> scopes;
+  for (int b = 0; b < n; ++b) g[b]->geom_launches = 0;
   {
-    ProfScope ps(g, 0, 0);
-    g->geom_launches = 0;
-    e = meg6::launch_geometry(g, t);                      // meg6_geom.cu (compiled with -fmad=false)
-    ps.set_launches(g->geom_launches);
+    // one timing scope over the whole call, charged to the first block
+    ProfScope ps(g[0], 0, 0);
+    for (int b = 0; b < n && e == cudaSuccess; ++b) e = meg6::geom_centres(g[b], t);
+    for (int pass = 0; pass < (rot ? 3 : 1); ++pass)
+      for (int d = 0; d < 3; ++d)
+        for (int b = 0; b < n && e == cudaSuccess; ++b) e = meg6::geom_extend(g[b], d);
+    for (int b = 0; b < n && e == cudaSuccess; ++b) e = meg6::geom_rest(g[b]);   // meg6_geom.cu (-fmad=false)
+    int nl = 0;
+    for (int b = 0; b < n; ++b) nl += g[b]->geom_launches;
+    ps.set_launches(nl);
   }
   if (e != cudaSuccess) return fail(MEG6_ECUDA, "metrics_compute: %s", cudaGetErrorString(e));
+  for (int b = 0; b < n; ++b) g[b]->have_metrics = true;
+  return MEG6_OK;
+}
+
+meg6_status meg6_metrics_compute(meg6_grid* g, double t) {
+  if (!g) return fail(MEG6_EINVAL, "null grid%s");
+  return meg6_metrics_compute_blocks(1, &g, t);
+}
+
+// ---- staged geometry (blocks on different devices): centres -> for d: [pack / deliver] extend(d) -> finish ----
+size_t meg6_geom_interface_doubles(const meg6_grid* g, int face) {
+  if (!g || face < 0 || face > 5) return 0;
+  const int d = face / 2;
+  const int e1 = (d == 0) ? 1 : 0, e2 = (d == 2) ? 1 : 2;
+  return (size_t)(g->p.moving ? 6 : 3) * GX * (size_t)(g->c.n[e1] + 2 * GX) * (size_t)(g->c.n[e2] + 2 * GX);
+}
+
+meg6_status meg6_set_geom_interface_buffer(meg6_grid* g, int face, const double* layers, const double* off) {
+  if (!g || face < 0 || face > 5) return fail(MEG6_EINVAL, "set_geom_interface_buffer: bad argument%s");
+  if (g->p.periodic[face / 2] || g->p.bc[face] != 5) return fail(MEG6_EINVAL, "set_geom_interface_buffer: face is not a block-interface face (bc 5)%s");
+  g->gbuf[face] = layers;
+  for (int q = 0; q < 3; ++q) g->goff[face][q] = off ? off[q] : 0.0;
+  return MEG6_OK;
+}
+
+meg6_status meg6_stage_geom_centres(meg6_grid* g, double t) {
+  if (!g) return fail(MEG6_EINVAL, "null grid%s");
+  g->geom_launches = 0;
+  CUDA_OK(meg6::geom_centres(g, t));
+  return MEG6_OK;
+}
+
+meg6_status meg6_stage_geom_pack(meg6_grid* g, int face, double* layers) {
+  if (!g || !layers || face < 0 || face > 5) return fail(MEG6_EINVAL, "stage_geom_pack: bad argument%s");
+  CUDA_OK(meg6::geom_pack(g, face, layers));
+  return MEG6_OK;
+}
+
+meg6_status meg6_stage_geom_extend(meg6_grid* g, int d) {
+  if (!g || d < 0 || d > 2) return fail(MEG6_EINVAL, "stage_geom_extend: bad argument%s");
+  for (int side = 0; side < 2; ++side) {
+    const int f = 2 * d + side;
+    if (!g->p.periodic[d] && g->p.bc[f] == 5 && !g->link[f] && !g->gbuf[f])
+      return fail(MEG6_ESTATE, "stage_geom_extend: block-interface face without a link or a coordinate buffer%s");
+  }
+  CUDA_OK(meg6::geom_extend(g, d));
+  return MEG6_OK;
+}
+
+meg6_status meg6_stage_geom_finish(meg6_grid* g) {
+  if (!g) return fail(MEG6_EINVAL, "null grid%s");
+  {
+    ProfScope ps(g, 0, 0);
+    const cudaError_t e = meg6::geom_rest(g);
+    ps.set_launches(g->geom_launches);
+    if (e != cudaSuccess) return fail(MEG6_ECUDA, "stage_geom_finish: %s", cudaGetErrorString(e));
+  }
   g->have_metrics = true;
   return MEG6_OK;
 }
@@ -416,10 +501,13 @@ static cudaError_t fill_ghosts_dir(meg6_grid* g, int buf, int d) {
     const meg6_grid* nb = g->link[2 * d + side];
     if (nb) {
       gin.nbP[side] = buf ? nb->Pb[0] : nb->P[0];
-      gin.nbL[side] = nb->c.LP; gin.nbfs[side] = nb->c.fsP; gin.nbn[side] = nb->c.n[d];
-    } else if (g->ibuf[2 * d + side]) {   // packed layers of a remote neighbour: a block six cells thick
+      gin.nbL[side] = nb->c.LP; gin.nbfs[side] = nb->c.fsP;
+      for (int e = 0; e < 3; ++e) { gin.nax[side][e] = g->lax[2 * d + side][e]; gin.nsg[side][e] = g->lsg[2 * d + side][e]; gin.nsh[side][e] = g->lsh[2 * d + side][e]; }
+    } else if (g->ibuf[2 * d + side]) {   // packed layers of a remote neighbour: a block six cells thick, aligned
       gin.nbP[side] = g->ibuf[2 * d + side];
-      gin.nbL[side] = pack_lay(c.LP, d); gin.nbfs[side] = gin.nbL[side].n; gin.nbn[side] = 6;
+      gin.nbL[side] = pack_lay(c.LP, d); gin.nbfs[side] = gin.nbL[side].n;
+      for (int e = 0; e < 3; ++e) { gin.nax[side][e] = e; gin.nsg[side][e] = 1; gin.nsh[side][e] = 0; }
+      gin.nsh[side][d] = side ? -c.n[d] : 6;
     }
   }
   ProfScope ps(g, 2, 1);
@@ -428,10 +516,11 @@ static cudaError_t fill_ghosts_dir(meg6_grid* g, int buf, int d) {
 }
 
 static cudaError_t fill_ghosts(meg6_grid* g, int buf) {
-  for (int d = 0; d < 3; ++d) {
-    const cudaError_t e = fill_ghosts_dir(g, buf, d);
-    if (e != cudaSuccess) return e;
-  }
+  for (int pass = 0; pass < (g->rotated ? 3 : 1); ++pass)
+    for (int d = 0; d < 3; ++d) {
+      const cudaError_t e = fill_ghosts_dir(g, buf, d);
+      if (e != cudaSuccess) return e;
+    }
   return cudaSuccess;
 }
 
@@ -572,17 +661,55 @@ meg6_status meg6_rk3_step(meg6_grid* g, double* U, double t, double dt) {
 }
 
 // ---- multi-block (Sec. 6; Table 1 last column; R28) ----
+meg6_status meg6_link_blocks_oriented(meg6_grid* home, int face, meg6_grid* nb, int nb_face, int swap, int flip_a, int flip_b,
+                                      const double* off) {
+  if (!home || !nb || face < 0 || face > 5 || nb_face < 0 || nb_face > 5) return fail(MEG6_EINVAL, "link_blocks: bad argument%s");
+  const int d = face / 2, dn = nb_face / 2;
+  if (home->p.periodic[d] || home->p.bc[face] != 5) return fail(MEG6_EINVAL, "link_blocks: face is not a block-interface face (bc 5)%s");
+  if (nb->p.periodic[dn]) return fail(MEG6_EINVAL, "link_blocks: the neighbour is periodic in that direction%s");
+  int a = (d + 1) % 3, b = (d + 2) % 3, an = (dn + 1) % 3, bn = (dn + 2) % 3;
+  if (a > b) { int t = a; a = b; b = t; }
+  if (an > bn) { int t = an; an = bn; bn = t; }
+  const int ta = swap ? bn : an, tb = swap ? an : bn;   // images of the home axes a, b
+  if (nb->c.n[ta] != home->c.n[a] || nb->c.n[tb] != home->c.n[b])
+    return fail(MEG6_EINVAL, "link_blocks: the interface planes of the two blocks have different cell counts%s");
+  if (nb->stream != home->stream) return fail(MEG6_EINVAL, "link_blocks: the blocks must share one stream%s");
+  if (nb->p.moving != home->p.moving || nb->p.scheme != home->p.scheme || nb->p.viscous != home->p.viscous)
+    return fail(MEG6_EINVAL, "link_blocks: the blocks differ in scheme, viscous or moving%s");
+  int* ax = home->lax[face]; int* sg = home->lsg[face]; int* sh = home->lsh[face];
+  ax[a] = ta; sg[a] = flip_a ? -1 : 1; sh[a] = flip_a ? home->c.n[a] - 1 : 0;
+  ax[b] = tb; sg[b] = flip_b ? -1 : 1; sh[b] = flip_b ? home->c.n[b] - 1 : 0;
+  // along the normal: ghost layer q of home = the q-th interior cell of the neighbour counted from nb_face
+  const int n = home->c.n[d], nn = nb->c.n[dn], hs = face & 1, ns = nb_face & 1;
+  ax[d] = dn;
+  if (hs && !ns) { sg[d] = 1; sh[d] = -n; }
+  else if (hs && ns) { sg[d] = -1; sh[d] = nn - 1 + n; }
+  else if (!hs && ns) { sg[d] = 1; sh[d] = nn; }
+  else { sg[d] = -1; sh[d] = -1; }
+  for (int q = 0; q < 3; ++q) home->loff[face][q] = off ? off[q] : 0.0;
+  home->link[face] = nb;
+  home->ibuf[face] = nullptr; home->gbuf[face] = nullptr;
+  const bool aligned = ax[0] == 0 && ax[1] == 1 && ax[2] == 2 && sg[0] > 0 && sg[1] > 0 && sg[2] > 0;
+  if (!aligned) { home->rotated = true; nb->rotated = true; }
+  home->have_metrics = false;   // the ghost coordinates of this face change with the link
+  return MEG6_OK;
+}
+
 meg6_status meg6_link_blocks(meg6_grid* home, int face, meg6_grid* nb) {
   if (!home || !nb || face < 0 || face > 5) return fail(MEG6_EINVAL, "link_blocks: bad argument%s");
   const int d = face / 2;
-  if (home->p.periodic[d] || home->p.bc[face] != 5) return fail(MEG6_EINVAL, "link_blocks: face is not a block-interface face (bc 5)%s");
-  if (nb->p.periodic[d]) return fail(MEG6_EINVAL, "link_blocks: the neighbour is periodic in that direction%s");
   for (int e = 0; e < 3; ++e)
-    if (e != d && (nb->c.n[e] != home->c.n[e] || nb->c.periodic[e] != home->c.periodic[e]))
+    if (e != d && nb->c.periodic[e] != home->c.periodic[e])
       return fail(MEG6_EINVAL, "link_blocks: transverse sizes or periodicity differ%s");
-  if (nb->stream != home->stream) return fail(MEG6_EINVAL, "link_blocks: the blocks must share one stream%s");
-  home->link[face] = nb;
-  return MEG6_OK;
+  return meg6_link_blocks_oriented(home, face, nb, face ^ 1, 0, 0, 0, nullptr);
+}
+
+// rotated links (R29): the neighbour cell behind an edge or corner ghost may itself be a ghost of a direction the
+// neighbour fills later; repeating the fill makes every ghost cell the fixed point of the exchange
+static int ghost_passes(int n, meg6_grid* const* g) {
+  for (int b = 0; b < n; ++b)
+    if (g[b]->rotated) return 3;
+  return 1;
 }
 
 static meg6_status blocks_ok(int n, meg6_grid* const* g, const char* who) {
@@ -610,8 +737,9 @@ meg6_status meg6_rhs_blocks(int n, meg6_grid* const* g, const double* const* U, 
     if (!g[b]->have_metrics) return fail(MEG6_ESTATE, "rhs_blocks called before metrics_compute%s");
     CUDA_OK(launch_prim(g[b], U[b]));
   }
-  for (int d = 0; d < 3; ++d)
-    for (int b = 0; b < n; ++b) CUDA_OK(fill_ghosts_dir(g[b], 0, d));
+  for (int pass = 0; pass < ghost_passes(n, g); ++pass)
+    for (int d = 0; d < 3; ++d)
+      for (int b = 0; b < n; ++b) CUDA_OK(fill_ghosts_dir(g[b], 0, d));
   for (int b = 0; b < n; ++b) {
     Fuse3 fu = make_fuse(g[b], U[b], dUdt[b]);
     fu.mode = 0;
@@ -633,10 +761,10 @@ meg6_status meg6_rk3_step_blocks(int n, meg6_grid* const* g, double* const* U, d
   for (int s = 0; s < 3; ++s) {
     // every block writes the primitives of its new state into the buffer NOT read by this stage, so the ghost
     // exchange of the next stage finds all neighbours' interiors complete
-    for (int b = 0; b < n; ++b)
-      if (g[b]->p.moving && (st = meg6_metrics_compute(g[b], ts[s])) != MEG6_OK) return st;
-    for (int d = 0; d < 3; ++d)
-      for (int b = 0; b < n; ++b) CUDA_OK(fill_ghosts_dir(g[b], s & 1, d));
+    if (g[0]->p.moving && (st = meg6_metrics_compute_blocks(n, g, ts[s])) != MEG6_OK) return st;
+    for (int pass = 0; pass < ghost_passes(n, g); ++pass)
+      for (int d = 0; d < 3; ++d)
+        for (int b = 0; b < n; ++b) CUDA_OK(fill_ghosts_dir(g[b], s & 1, d));
     for (int b = 0; b < n; ++b)
       if ((st = stage_sweeps(g[b], s & 1, make_fuse_rk(g[b], U[b], s, dt))) != MEG6_OK) return st;
   }

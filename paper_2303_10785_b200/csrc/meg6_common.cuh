@@ -104,8 +104,16 @@ struct meg6_grid {
   double* res;        // [5][N]
   double* U0;         // [5][N]
   double* inflow[6];
-  meg6_grid* link[6];          // bc 5: the neighbour block of each face (meg6_link_blocks)
+  meg6_grid* link[6];          // bc 5: the neighbour block of each face (meg6_link_blocks[_oriented])
+  // orientation of the neighbour seen from this block ("each block possesses its own coordinate system"; R28, R29):
+  // the cell with index vector h of THIS block (ghost ranges included) is the neighbour's cell m with
+  //   m[lax[e]] = lsg[e] > 0 ? h[e] + lsh[e] : lsh[e] - h[e];   loff: added to the neighbour's coordinates seen from here
+  int lax[6][3], lsg[6][3], lsh[6][3];
+  double loff[6][3];
+  bool rotated;                // some link of this block (or to it) is not the aligned one: ghost fills are repeated (R29)
   const double* ibuf[6];       // bc 5: or a packed copy of the neighbour's layers (meg6_set_interface_buffer)
+  const double* gbuf[6];       // ... and of its cell-centre coordinates (meg6_set_geom_interface_buffer)
+  double goff[6][3];
   const double* sigma; const double* uref;
   unsigned long long* stats;   // [2] device counters: limited, tested
   unsigned short* bmask[3];    // caller's branch-record arrays per interface family (meg6_set_branch_masks) or null

@@ -27,7 +27,8 @@ struct GhostIn {
   const double* inflow[2]; const double* mx; const double* my; const double* mz;
   // block interfaces (bc 5): field 0 of the neighbour's primitive buffer, its layout, field stride and cell count
   // along this direction, per side
-  const double* nbP[2]; Lay nbL[2]; long long nbfs[2]; int nbn[2];
+  const double* nbP[2]; Lay nbL[2]; long long nbfs[2];
+  int nax[2][3], nsg[2][3], nsh[2][3];   // index map home -> neighbour: m[nax[e]] = nsg[e] > 0 ? h[e] + nsh[e] : nsh[e] - h[e]
 };
 
 // B: ghost layers of direction d (6 deep), after the lower directions have been filled: periodic wrap, fixed
@@ -67,10 +68,16 @@ __global__ void __launch_bounds__(256) k_ghost(Consts c, int d, P6 P, GhostIn in
   const int bc = c.bc[2 * d + side];
   const int ca = min(max(ta, 0), c.n[a] - 1), cb = min(max(tb, 0), c.n[b] - 1);
   if (bc == 5) {
-    // block interface (Table 1 last column; R28): ghost layer q = the q-th interior cell of the neighbour
-    // block counted from its opposite face, same transverse index
-    int is[3];
-    is[a] = ta; is[b] = tb; is[d] = side ? q - 1 : in.nbn[side] - q;
+    // block interface (Table 1 last column; R28, R29): ghost layer q = the q-th interior cell of the neighbour
+    // block counted from the face it shares with this one, at the transverse position the link's orientation gives
+    int h[3], is[3];
+    h[a] = ta; h[b] = tb; h[d] = last + sg * q;
+#pragma unroll
+    for (int e = 0; e < 3; ++e) {
+      const int m = in.nsg[side][e] > 0 ? h[e] + in.nsh[side][e] : in.nsh[side][e] - h[e];
+      const int ax = in.nax[side][e];
+      if (ax == 0) is[0] = m; else if (ax == 1) is[1] = m; else is[2] = m;
+    }
     const double* src = in.nbP[side] + in.nbL[side].at(is[0], is[1], is[2]);
     double v[6];
 #pragma unroll

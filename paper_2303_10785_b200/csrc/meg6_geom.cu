@@ -1,5 +1,6 @@
 // meg6_geom.cu -- metric / Jacobian kernels and their launcher.  Compiled with -fmad=false (see meg6_geom.cuh).
 #include <cstdlib>
+#include <cstring>
 #include <math.h>
 #include "meg6_geom.cuh"
 #ifndef MEG6_IG4_SEGMENTED
@@ -11,17 +12,70 @@ namespace meg6 {
 
 static inline unsigned nblk(long long n, int t) { return (unsigned)((n + t - 1) / t); }
 
-// cell centres of the interior, then ghost layers direction by direction (xi, eta over the xi-extended array, zeta)
-static void launch_centres(meg6_grid* g, const GeomIn& gi, P3 xc, P3 xt) {
+static GeomIn geom_in(meg6_grid* g, double t) {
+  GeomIn gi;
+  for (int q = 0; q < 3; ++q) { gi.node[q] = g->nodes[q]; gi.mode[q] = g->modes[q]; }
+  const double ph = 2.0 * M_PI * g->p.omega * t;
+  gi.s = g->p.moving ? sin(ph) : 0.0;
+  gi.sd = g->p.moving ? 2.0 * M_PI * g->p.omega * cos(ph) : 0.0;
+  return gi;
+}
+
+// stage 1 of the geometry: cell centres (and grid velocities) of the interior cells
+cudaError_t geom_centres(meg6_grid* g, double t) {
   const Consts& c = g->c;
-  k_centres<<<nblk(c.LC.n, 256), 256, 0, g->stream>>>(c, gi, xc, xt);
-  g->geom_launches += 4;
-  for (int d = 0; d < 3; ++d) {
-    int a = (d + 1) % 3, b = (d + 2) % 3;
-    if (a > b) { int t = a; a = b; b = t; }
-    const long long ea = c.n[a] + ((a < d) ? 2 * GX : 0), eb = c.n[b] + ((b < d) ? 2 * GX : 0);
-    k_extend<<<nblk(ea * eb * 2 * GX, 256), 256, 0, g->stream>>>(c, d, xc, xt);
+  P3 xc, xt;
+  for (int q = 0; q < 3; ++q) { xc.p[q] = g->xc[q]; xt.p[q] = g->xt[q]; }
+  k_centres<<<nblk(c.LC.n, 256), 256, 0, g->stream>>>(c, geom_in(g, t), xc, xt);
+  ++g->geom_launches;
+  return cudaGetLastError();
+}
+
+// stage 2, once per direction (xi, then eta over the xi-extended array, then zeta): ghost layers of direction d.  With
+// several blocks, direction d is extended in every block before direction d+1 in any (block-interface faces read the
+// neighbour's array, ghosts of the lower directions included)
+cudaError_t geom_extend(meg6_grid* g, int d) {
+  const Consts& c = g->c;
+  P3 xc, xt;
+  for (int q = 0; q < 3; ++q) { xc.p[q] = g->xc[q]; xt.p[q] = g->xt[q]; }
+  ExtIn in;
+  memset(&in, 0, sizeof(in));
+  for (int side = 0; side < 2; ++side) {
+    const int face = 2 * d + side;
+    if (c.periodic[d] || c.bc[face] != 5) continue;
+    const meg6_grid* nb = g->link[face];
+    if (nb) {
+      for (int q = 0; q < 3; ++q) { in.nbx[side][q] = nb->xc[q]; in.nbv[side][q] = nb->xt[q]; in.off[side][q] = g->loff[face][q]; }
+      in.nbL[side] = nb->c.LX;
+      for (int e = 0; e < 3; ++e) { in.nax[side][e] = g->lax[face][e]; in.nsg[side][e] = g->lsg[face][e]; in.nsh[side][e] = g->lsh[face][e]; }
+    } else if (g->gbuf[face]) {   // packed layers of a remote neighbour: a block ten cells thick, aligned
+      const Lay LQ = geom_pack_lay(c.LX, d);
+      for (int q = 0; q < 3; ++q) {
+        in.nbx[side][q] = g->gbuf[face] + q * LQ.n;
+        in.nbv[side][q] = g->p.moving ? g->gbuf[face] + (3 + q) * LQ.n : nullptr;
+        in.off[side][q] = g->goff[face][q];
+      }
+      in.nbL[side] = LQ;
+      for (int e = 0; e < 3; ++e) { in.nax[side][e] = e; in.nsg[side][e] = 1; in.nsh[side][e] = 0; }
+      in.nsh[side][d] = side ? -c.n[d] : GX;
+    }
   }
+  int a = (d + 1) % 3, b = (d + 2) % 3;
+  if (a > b) { int t = a; a = b; b = t; }
+  const long long ea = c.n[a] + ((a < d) ? 2 * GX : 0), eb = c.n[b] + ((b < d) ? 2 * GX : 0);
+  k_extend<<<nblk(ea * eb * 2 * GX, 256), 256, 0, g->stream>>>(c, d, xc, xt, in);
+  ++g->geom_launches;
+  return cudaGetLastError();
+}
+
+cudaError_t geom_pack(meg6_grid* g, int face, double* layers) {
+  const int d = face / 2;
+  const Lay LQ = geom_pack_lay(g->c.LX, d);
+  const int first = (face & 1) ? g->c.n[d] - GX : 0;
+  P6c src;
+  for (int q = 0; q < 3; ++q) { src.p[q] = g->xc[q]; src.p[3 + q] = g->xt[q]; }
+  k_pack_geom<<<nblk(LQ.n, 256), 256, 0, g->stream>>>(g->c.LX, LQ, d, first, g->p.moving ? 6 : 3, src, layers);
+  return cudaGetLastError();
 }
 
 // ---- MIG4 (scheme 1): the geometry as whole-array passes, each the operation the discretisation names ----
@@ -94,12 +148,9 @@ static Box delta_pass(meg6_grid* g, const double* f, const Box& fb, int dir, dou
   return db;
 }
 
-static cudaError_t launch_geometry_ig4(meg6_grid* g, const GeomIn& gi) {
+static cudaError_t launch_geometry_ig4(meg6_grid* g) {
   const Consts& c = g->c;
   const Lay& L = c.LX;
-  P3 xc, xt;
-  for (int q = 0; q < 3; ++q) { xc.p[q] = g->xc[q]; xt.p[q] = g->xt[q]; }
-  launch_centres(g, gi, xc, xt);
   double* f1 = g->scr[0]; double* H = g->scr[1]; double* t1 = g->scr[2]; double* t2 = g->scr[3];
   double* d1 = g->scr[4]; double* d2 = g->scr[5];
   const Box all = box_all(c);
@@ -166,19 +217,14 @@ static cudaError_t launch_geometry_ig4(meg6_grid* g, const GeomIn& gi) {
   return cudaGetLastError();
 }
 
-cudaError_t launch_geometry(meg6_grid* g, double t) {
+// stage 3: everything after the ghost coordinates (derivatives, metrics, 1/J, time metrics, interface values, GCL)
+cudaError_t geom_rest(meg6_grid* g) {
   const Consts& c = g->c;
-  GeomIn gi;
-  for (int q = 0; q < 3; ++q) { gi.node[q] = g->nodes[q]; gi.mode[q] = g->modes[q]; }
-  const double ph = 2.0 * M_PI * g->p.omega * t;
-  gi.s = g->p.moving ? sin(ph) : 0.0;
-  gi.sd = g->p.moving ? 2.0 * M_PI * g->p.omega * cos(ph) : 0.0;
   P3 xc, xt, mt; P9 cd, met;
   for (int q = 0; q < 3; ++q) { xc.p[q] = g->xc[q]; xt.p[q] = g->xt[q]; mt.p[q] = g->mt[q]; }
   for (int q = 0; q < 9; ++q) { cd.p[q] = g->cd[q]; met.p[q] = g->met[q]; }
-  if (g->p.scheme == 1) return launch_geometry_ig4(g, gi);
+  if (g->p.scheme == 1) return launch_geometry_ig4(g);
   const int T = 256;
-  launch_centres(g, gi, xc, xt);
   // blocking along the grid line trades threads for shared intermediates: it pays once the grid fills the GPU several
   // times over (256^3: -7 % per call), not on config 2's 64^3 (+3 %)
   // MEG6_GEOM_BLOCKED=0/1 in the environment at grid_create forces the choice (the parity tests run both forms on the

@@ -48,7 +48,17 @@ __global__ void __launch_bounds__(256) k_centres(Consts c, GeomIn g, P3 xc, P3 x
 // M1b: ghost layers of direction d (R13, R14), after the lower directions: periodic -> image -/+ period (velocities:
 // plain copy); otherwise linear extrapolation of the last spacing.  The same values, operation by operation, as the
 // recursive definition ext_val (xi innermost, zeta outermost).  One thread per ghost cell.
-__global__ void __launch_bounds__(256) k_extend(Consts c, int d, P3 xc, P3 xt) {
+// Block-interface faces (bc 5; R28, R29): the ghost cell centres are the neighbour block's own cell centres (plus the
+// period across a wrap-around link) -- both blocks then difference the same coordinates across their common face, and
+// the interface metrics of a cut mesh are those of the uncut one, bit for bit.  Per side: field 0 of the neighbour's
+// coordinate (velocity) array, or of a packed copy of its ten layers next to the face; index map as in k_ghost.
+struct ExtIn {
+  const double* nbx[2][3]; const double* nbv[2][3]; Lay nbL[2];
+  int nax[2][3], nsg[2][3], nsh[2][3];
+  double off[2][3];
+};
+
+__global__ void __launch_bounds__(256) k_extend(Consts c, int d, P3 xc, P3 xt, ExtIn in) {
   int a = (d + 1) % 3, b = (d + 2) % 3;
   if (a > b) { int t = a; a = b; b = t; }
   const int loa = (a < d) ? -GX : 0, ea = c.n[a] + ((a < d) ? 2 * GX : 0);
@@ -72,7 +82,19 @@ __global__ void __launch_bounds__(256) k_extend(Consts c, int d, P3 xc, P3 xt) {
     for (int vel = 0; vel < 2; ++vel) {
       if (vel && !c.moving) continue;
       double* f = vel ? xt.p[comp] : xc.p[comp];
-      if (c.periodic[d]) {
+      const double* nbf = vel ? in.nbv[side][comp] : in.nbx[side][comp];
+      if (!c.periodic[d] && c.bc[2 * d + side] == 5 && nbf) {
+        int h[3], is[3];
+        h[a] = ta; h[b] = tb; h[d] = ai;
+#pragma unroll
+        for (int e = 0; e < 3; ++e) {
+          const int m = in.nsg[side][e] > 0 ? h[e] + in.nsh[side][e] : in.nsh[side][e] - h[e];
+          const int ax = in.nax[side][e];
+          if (ax == 0) is[0] = m; else if (ax == 1) is[1] = m; else is[2] = m;
+        }
+        const double v = nbf[in.nbL[side].at(is[0], is[1], is[2])];
+        f[dst] = vel ? v : v + in.off[side][comp];
+      } else if (c.periodic[d]) {
         const double off = vel ? 0.0 : c.period[d][comp];
         f[dst] = side ? f[base + (long long)(ai - n) * s] + off : f[base + (long long)(ai + n) * s] - off;
       } else if (!side) {
@@ -84,6 +106,26 @@ __global__ void __launch_bounds__(256) k_extend(Consts c, int d, P3 xc, P3 xt) {
       }
     }
   }
+}
+
+// Packed cell-centre layers of one face (meg6_stage_geom_pack): the ten layers of direction d next to the face over the
+// whole padded transverse extent, coordinates (and grid velocities).  The packed array is a padded layout itself: LX
+// with ten cells and no ghosts along d; k_extend of the receiving block reads it like a neighbour ten cells thick.
+inline Lay geom_pack_lay(const Lay& LX, int d) {
+  Lay L = LX;
+  if (d == 0) { L.gi = 0; L.pi = GX; } else if (d == 1) { L.gj = 0; L.pj = GX; } else { L.gk = 0; L.pk = GX; }
+  L.sj = L.pi; L.sk = (long long)L.pi * L.pj; L.n = L.sk * L.pk;
+  return L;
+}
+struct P6c { const double* p[6]; };
+__global__ void __launch_bounds__(256) k_pack_geom(Lay LX, Lay LQ, int d, int first, int nf, P6c src, double* __restrict__ out) {
+  const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (tid >= LQ.n) return;
+  const int pi = (int)(tid % LQ.pi), pj = (int)((tid / LQ.pi) % LQ.pj), pk = (int)(tid / LQ.sk);
+  int ix[3] = {pi - LQ.gi, pj - LQ.gj, pk - LQ.gk};
+  ix[d] += first;
+  const long long at = LX.at(ix[0], ix[1], ix[2]);
+  for (int f = 0; f < nf; ++f) out[f * LQ.n + tid] = src.p[f][at];
 }
 
 // ---- linear operators in the paper's own step-by-step form (Eq. 17, 19, 16, 36-38), evaluated in exactly

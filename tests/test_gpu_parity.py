@@ -606,12 +606,13 @@ def test_blocks_rhs_and_steps_parity(mods, name):
     blocks, links = W.split_blocks(wl, cuts)
     og = [O.Grid(b) for b in blocks]
     gg = [M.Grid(b) for b in blocks]
-    for home, face, nb in links:
-        og[home].link(face, og[nb])
-        gg[home].link(face, gg[nb])
-    for a, b in zip(og, gg):
-        a.metrics_compute(0.0)
-        b.metrics_compute(0.0)
+    W.link_all(og, blocks, links)
+    W.link_all(gg, blocks, links)
+    O.metrics_compute_blocks(og, 0.0)
+    M.metrics_compute_blocks(gg, 0.0)
+    for a, b in zip(og, gg):        # geometry of every block, ghost coordinates from the neighbours: bit for bit
+        for q in range(10):
+            assert np.array_equal(b.get_array(0, q), a.cell(q)), (name, q)
     ref = O.rhs_blocks(og, [b["U0"] for b in blocks])
     Us = [torch.as_tensor(b["U0"], device="cuda").contiguous() for b in blocks]
     out = M.rhs_blocks(gg, Us)
@@ -626,8 +627,9 @@ def test_blocks_rhs_and_steps_parity(mods, name):
     for b, uo, u in zip(blocks, Uo, Us):
         e = rel(u.cpu().numpy(), uo)
         assert np.all(e <= STEP_TOL), (name, b["name"], e)
-    if name.startswith("cart"):
-        # and the cut run equals the uncut one on the GPU as well
+    if True:
+        # and the cut run equals the uncut one on the GPU as well, curved meshes included (ghost coordinates of an
+        # interface face are the neighbour's cell centres, R28); walls of both kinds on the outer faces
         g1 = M.Grid(wl)
         g1.metrics_compute(0.0)
         U1 = torch.as_tensor(wl["U0"], device="cuda").contiguous()
@@ -648,12 +650,14 @@ def test_blocks_call_order_errors(mods):
     blocks, links = W.split_blocks(wl, ((10, 10), (12,), (12,)))
     gg = [M.Grid(b) for b in blocks]
     Us = [torch.as_tensor(b["U0"], device="cuda").contiguous() for b in blocks]
-    for g in gg:
-        g.metrics_compute(0.0)
     with pytest.raises(M.Meg6Error):
-        M.rhs_blocks(gg, Us)                       # interfaces not linked yet
-    for home, face, nb in links:
-        gg[home].link(face, gg[nb])
+        M.metrics_compute_blocks(gg, 0.0)          # interfaces not linked yet
+    W.link_all(gg, blocks, links)
+    with pytest.raises(M.Meg6Error):
+        gg[0].metrics_compute(0.0)                 # single-grid call on a block with a foreign neighbour
+    with pytest.raises(M.Meg6Error):
+        M.rhs_blocks(gg, Us)                       # before the metrics
+    M.metrics_compute_blocks(gg, 0.0)
     with pytest.raises(M.Meg6Error):
         gg[0].rhs(Us[0])                           # single-grid call on a block with a foreign neighbour
     with pytest.raises(M.Meg6Error):
@@ -674,16 +678,34 @@ def test_staged_api_with_packed_layers_equals_linked_blocks(mods):
     cuts = ((26,), (11, 13), (10, 12))      # eta and zeta interfaces: edge ghosts travel inside the packed layers
     blocks, links = W.split_blocks(wl, cuts)
     ref = [M.Grid(b) for b in blocks]
-    for home, face, nb in links:
-        ref[home].link(face, ref[nb])
+    W.link_all(ref, blocks, links)
+    M.metrics_compute_blocks(ref, 0.0)
     gg = [M.Grid(b) for b in blocks]
-    send, recv = {}, {}
+    send, recv, gsend, grecv = {}, {}, {}, {}
     for home, face, nb in links:
         send[(home, face)] = gg[home].new_interface_buffer(face)
         recv[(home, face)] = gg[home].new_interface_buffer(face)
         gg[home].set_interface_buffer(face, recv[(home, face)])
-    for g in ref + gg:
-        g.metrics_compute(0.0)
+        gsend[(home, face)] = gg[home].new_geom_interface_buffer(face)
+        grecv[(home, face)] = gg[home].new_geom_interface_buffer(face)
+        gg[home].set_geom_interface_buffer(face, grecv[(home, face)], blocks[home]["link_offset"].get(face))
+    # staged geometry: centres, then per direction pack / hand over / extend, then the metrics
+    for g in gg:
+        g.stage_geom_centres(0.0)
+    for d in range(3):
+        for home, face, nb in links:
+            if face // 2 == d:
+                gg[home].stage_geom_pack(face, gsend[(home, face)])
+        for home, face, nb in links:
+            if face // 2 == d:
+                grecv[(nb, face ^ 1)].copy_(gsend[(home, face)])
+        for g in gg:
+            g.stage_geom_extend(d)
+    for g in gg:
+        g.stage_geom_finish()
+    for a, b in zip(gg, ref):
+        for q in range(10):
+            assert np.array_equal(a.get_array(0, q), b.get_array(0, q))
     Ur = [torch.as_tensor(b["U0"], device="cuda").contiguous() for b in blocks]
     Us = [u.clone() for u in Ur]
     dt = 1.5e-3
@@ -815,3 +837,195 @@ def test_full_step_counts_of_configs_3_4_5_stay_finite_and_bounded(mods):
     assert ke1 > ke0                     # the jet has entered the quiescent domain
     assert frac > 1e-4                   # and the limiter is at work
     print("C4 after 500 steps: limited fraction %.4f" % frac)
+
+
+# ------------------------------------------------------------------ ghost coordinates from the neighbour, rotated blocks
+def test_cut_stretched_jet_mesh_equals_the_uncut_one_on_gpu(mods):
+    """Config-4-type mesh (tanh-stretched, inflow / outflow / sponge, viscous) cut into 2 x 2 x 2 blocks: the metrics of
+    every block are those of the uncut mesh BIT FOR BIT (ghost coordinates of an interface face = the neighbour's cell
+    centres), dQ/dt and three RK3 steps agree with the uncut run to round-off, and with the oracle's blocks."""
+    torch, O, M = mods
+    wl = small_cases()["c4"]
+    cuts = ((26, 26), (20, 17), (17, 16))
+    blocks, links = W.split_blocks(wl, cuts)
+    gg = [M.Grid(b) for b in blocks]
+    W.link_all(gg, blocks, links)
+    M.metrics_compute_blocks(gg, 0.0)
+    g1 = M.Grid(wl)
+    g1.metrics_compute(0.0)
+    for b, g in zip(blocks, gg):
+        for q in range(10):
+            assert np.array_equal(g.get_array(0, q), g1.get_array(0, q)[b["slices"]]), (b["name"], q)
+        for d in range(3):
+            fsl = list(b["slices"])
+            fsl[2 - d] = slice(fsl[2 - d].start, fsl[2 - d].stop + 1)
+            for q in range(10):
+                assert np.array_equal(g.get_array(1, 16 * d + q), g1.get_array(1, 16 * d + q)[tuple(fsl)])
+    U1 = torch.as_tensor(wl["U0"], device="cuda").contiguous()
+    Us = [torch.as_tensor(b["U0"], device="cuda").contiguous() for b in blocks]
+    r1 = g1.rhs(U1).cpu().numpy()
+    out = M.rhs_blocks(gg, Us)
+    for b, o in zip(blocks, out):
+        e = rhs_err(o.cpu().numpy(), r1[(slice(None),) + b["slices"]], b["U0"])
+        assert np.all(e <= 1e-12), (b["name"], e)
+    for s in range(3):
+        g1.rk3_step(U1, s * wl["dt"], wl["dt"])
+        M.rk3_step_blocks(gg, Us, s * wl["dt"], wl["dt"])
+    U1 = U1.cpu().numpy()
+    for b, u in zip(blocks, Us):
+        assert np.all(rel(u.cpu().numpy(), U1[(slice(None),) + b["slices"]]) <= 1e-12)
+    for g in gg + [g1]:
+        g.close()
+
+
+def _link_oriented(grids, blocks, periods=()):
+    for home, face, nb, nb_face, swap, fa, fb, off in W.auto_links(blocks, periods):
+        grids[home].link(face, grids[nb], nb_face=nb_face, swap=swap, flip_a=fa, flip_b=fb, offset=off)
+
+
+@pytest.mark.parametrize("case", ["wavy_periodic_3d", "jet_mesh_quadrants", "mig4_quadrants"])
+def test_blocks_with_rotated_coordinate_systems_on_gpu(mods, case):
+    """Sec. 6 (SURVEY NEXT-3 "4-block butterfly"): blocks stored in frames rotated against their neighbours'
+    (quarter turns about zeta: the four wings of a butterfly-type section; cyclic and x-axis rotations in the 3-D case),
+    linked by node matching.  Against the oracle's blocks (same links): geometry bit for bit, dQ/dt <= 1e-11, three
+    steps <= 1e-9; and turned back, against the UNCUT single block on the GPU, which never sees a link."""
+    torch, O, M = mods
+    if case == "wavy_periodic_3d":
+        wl = W.c3_tgv(n=24)
+        cuts, rots = ((12, 12), (10, 14), (14, 10)), ["id", "z90", "cyc", "x90", "z270", "id", "z180", "cyc"]
+        periods = wl["params"]["period"]
+    else:
+        # outflow faces around, four quadrant blocks about the jet axis direction (here zeta), each turned by a quarter
+        wl = W.c4_jet(ni=26, nj=24, nk=22)
+        wl["params"] = dict(wl["params"], bc=[2, 2, 2, 2, 2, 2], scheme=1 if case == "mig4_quadrants" else 0)
+        wl["inflow"] = {}
+        rng = np.random.default_rng(12)
+        sh = wl["U0"].shape[1:]
+        wl["U0"] = W.conservative(1.0 + 0.1 * rng.uniform(-1, 1, sh), *(0.2 * rng.uniform(-1, 1, sh) for _ in range(3)),
+                                  (1.0 + 0.1 * rng.uniform(-1, 1, sh)) / 1.4)
+        cuts, rots = ((14, 12), (12, 12), (22,)), ["id", "z90", "z270", "z180"]
+        periods = ()
+    plain, _ = W.split_blocks(wl, cuts)
+    blocks = [W.rotate_block(b, r) for b, r in zip(plain, rots)]
+    og = [O.Grid(b) for b in blocks]
+    gg = [M.Grid(b) for b in blocks]
+    _link_oriented(og, blocks, periods)
+    _link_oriented(gg, blocks, periods)
+    O.metrics_compute_blocks(og, 0.0)
+    M.metrics_compute_blocks(gg, 0.0)
+    for a, b in zip(og, gg):
+        for q in range(10):
+            assert np.array_equal(b.get_array(0, q), a.cell(q)), (case, q)
+    ref = O.rhs_blocks(og, [b["U0"] for b in blocks])
+    Us = [torch.as_tensor(b["U0"], device="cuda").contiguous() for b in blocks]
+    out = [o.cpu().numpy() for o in M.rhs_blocks(gg, Us)]
+    for b, r, o in zip(blocks, ref, out):
+        e = rhs_err(o, r, b["U0"])
+        assert np.all(e <= RHS_TOL), (case, b["name"], e)
+    # turned back: the uncut block
+    g1 = M.Grid(wl)
+    g1.metrics_compute(0.0)
+    U1 = torch.as_tensor(wl["U0"], device="cuda").contiguous()
+    r1 = g1.rhs(U1).cpu().numpy()
+    tol = 1e-10 if case == "wavy_periodic_3d" else 1e-11     # Ma 0.1: see tests/test_oracle_blocks.py
+    if case != "jet_mesh_quadrants" and case != "mig4_quadrants":
+        for b, p, o in zip(blocks, plain, out):
+            e = rhs_err(W.unrotate_state(o, b["rotation"]), r1[(slice(None),) + p["slices"]], p["U0"])
+            assert np.all(e <= tol), (case, b["name"], e)
+    dt = min(g.cfl_dt(b["U0"], 0.4) for g, b in zip(og, blocks))
+    Uo = [b["U0"].copy() for b in blocks]
+    for s in range(3):
+        O.rk3_step_blocks(og, Uo, s * dt, dt)
+        M.rk3_step_blocks(gg, Us, s * dt, dt)
+    for b, uo, u in zip(blocks, Uo, Us):
+        assert np.all(rel(u.cpu().numpy(), uo) <= STEP_TOL), (case, b["name"])
+    for g in gg + [g1]:
+        g.close()
+
+
+def test_slab_stepper_on_two_cuda_grids_through_an_in_process_transport(mods, monkeypatch):
+    """paper_2303_10785_b200.slabs.SlabStepper itself (geometry exchange, per-direction pack / exchange / ghost fill,
+    sweeps) driven for two zeta slabs of the stretched jet mesh on the ONE device: torch.distributed's point-to-point
+    calls are replaced by a shim that hands the tensors over with device-to-device copies (NCCL cannot put two ranks
+    on one GPU; the NCCL leg itself stays unexecuted on this pool).  Result: bit for bit meg6_rk3_step_blocks."""
+    torch, O, M = mods
+    from paper_2303_10785_b200 import slabs
+    wl = small_cases()["c4"]
+    blocks, links = W.split_blocks(wl, ((52,), (37,), (17, 16)))
+    ref = [M.Grid(b) for b in blocks]
+    W.link_all(ref, blocks, links)
+    M.metrics_compute_blocks(ref, 0.0)
+    gg = [M.Grid(b) for b in blocks]
+
+    import threading
+
+    class Shim:
+        """mailbox transport for ranks that are threads of this process: a send parks a copy of the tensor, a receive
+        waits for it and copies it in (device-to-device, on the one stream both grids use)"""
+        isend, irecv = "send", "recv"
+
+        def __init__(self):
+            self.tls, self.box, self.cv = threading.local(), {}, threading.Condition()
+
+        def P2POp(self, op, tensor, peer, group=None, tag=0):
+            return (op, tensor, peer, tag)
+
+        def batch_isend_irecv(self, ops):
+            me, works = self.tls.rank, []
+            for op, t, peer, tag in ops:
+                if op == "send":
+                    with self.cv:
+                        self.box[(me, peer, tag)] = t.clone()
+                        self.cv.notify_all()
+                else:
+                    works.append(self._Recv(self, (peer, me, tag), t))
+            return works
+
+        class _Recv:
+            def __init__(self, shim, key, t):
+                self.shim, self.key, self.t = shim, key, t
+
+            def wait(self):
+                with self.shim.cv:
+                    assert self.shim.cv.wait_for(lambda: self.key in self.shim.box, timeout=60)
+                    src = self.shim.box.pop(self.key)
+                self.t.copy_(src)
+    shim = Shim()
+    monkeypatch.setattr(slabs, "dist", shim)
+    steppers = []
+    for r in range(2):
+        remote = {face: nb for home, face, nb in links if home == r}
+        steppers.append(slabs.SlabStepper(gg[r], remote, offsets=blocks[r]["link_offset"]))
+
+    def on_ranks(fn):
+        """fn(rank) on one thread per rank, as torchrun would on one process per rank"""
+        errs = []
+
+        def body(r):
+            shim.tls.rank = r
+            try:
+                with torch.cuda.device(0):
+                    fn(r)
+            except BaseException as e:   # noqa: BLE001
+                errs.append(e)
+        th = [threading.Thread(target=body, args=(r,)) for r in range(2)]
+        for t in th:
+            t.start()
+        for t in th:
+            t.join()
+        if errs:
+            raise errs[0]
+    on_ranks(lambda r: steppers[r].metrics_compute(0.0))
+    for a, b in zip(gg, ref):
+        for q in range(10):
+            assert np.array_equal(a.get_array(0, q), b.get_array(0, q))
+    Ur = [torch.as_tensor(b["U0"], device="cuda").contiguous() for b in blocks]
+    Us = [u.clone() for u in Ur]
+    for n in range(2):
+        M.rk3_step_blocks(ref, Ur, n * wl["dt"], wl["dt"])
+        on_ranks(lambda r: steppers[r].rk3_step(Us[r], n * wl["dt"], wl["dt"]))
+    for a, b, blk in zip(Us, Ur, blocks):
+        assert torch.equal(a, b)
+        assert (a.cpu().numpy() - blk["U0"]).__abs__().max() > 1e-6
+    for g in ref + gg:
+        g.close()

@@ -24,8 +24,23 @@ class OracleBlock:
         self.g = O.Grid(wl)
         self.U0 = None
 
-    def metrics_compute(self, t):
-        self.g.metrics_compute(t)
+    def new_geom_interface_buffer(self, face):
+        return torch.zeros(self.g.geom_interface_doubles(face), dtype=torch.float64)
+
+    def set_geom_interface_buffer(self, face, layers, offset=None):
+        self.g.set_geom_interface_buffer(face, layers.numpy(), offset)
+
+    def stage_geom_centres(self, t):
+        self.g.stage_geom_centres(t)
+
+    def stage_geom_pack(self, face, layers):
+        self.g.stage_geom_pack(face, layers.numpy())
+
+    def stage_geom_extend(self, d):
+        self.g.stage_geom_extend(d)
+
+    def stage_geom_finish(self):
+        self.g.stage_geom_finish()
 
     def new_interface_buffer(self, face):
         return torch.zeros(self.g.interface_doubles(face), dtype=torch.float64)
@@ -59,7 +74,7 @@ class OracleBlock:
 
 def _case(kind):
     if kind == "periodic_zeta":      # two slabs, wrap-around: both faces of a rank talk to the same peer
-        return W.cartesian_periodic(ni=12, nj=10, nk=20, viscous=1), ((12,), (10,), (12, 8))
+        return W.cartesian_periodic(ni=12, nj=10, nk=22, viscous=1), ((12,), (10,), (12, 10))
     return W.wall_box(ni=14, nj=12, nk=22, viscous=1), ((14,), (12,), (10, 12))   # curved, walls outside, one interface
 
 
@@ -71,9 +86,9 @@ def _worker(rank, world, port, kind, out):
     wl, cuts = _case(kind)
     blocks, links = W.split_blocks(wl, cuts)
     blk = OracleBlock(blocks[rank])
-    blk.metrics_compute(0.0)
     remote = {face: nb for home, face, nb in links if home == rank}
-    st = SlabStepper(blk, remote)
+    st = SlabStepper(blk, remote, offsets=blocks[rank]["link_offset"])
+    st.metrics_compute(0.0)
     U = blocks[rank]["U0"].copy()
     rhs = np.empty_like(U)
     st.rhs(U, rhs)
@@ -90,10 +105,8 @@ def _reference(kind):
     wl, cuts = _case(kind)
     blocks, links = W.split_blocks(wl, cuts)
     grids = [O.Grid(b) for b in blocks]
-    for home, face, nb in links:
-        grids[home].link(face, grids[nb])
-    for g in grids:
-        g.metrics_compute(0.0)
+    W.link_all(grids, blocks, links)
+    O.metrics_compute_blocks(grids, 0.0)
     rhs = O.rhs_blocks(grids, [b["U0"] for b in blocks])
     Us = [b["U0"].copy() for b in blocks]
     dt = 2.0e-3

@@ -314,7 +314,8 @@ def cartesian_periodic(ni=24, nj=20, nk=16, viscous=1, seed=77, scheme=0):
 
 
 def split_blocks(wl, cuts):
-    """Cuts a static single-block workload into aligned blocks.  cuts = (cells of the xi pieces, eta pieces, zeta
+    """Cuts a static single-block workload into aligned blocks (each block dict carries `link_offset`: per linked face
+    the vector added to the neighbour's coordinates seen from the block -- the period across a wrap-around link).  cuts = (cells of the xi pieces, eta pieces, zeta
     pieces), e.g. ((12, 12), (20,), (16,)).  Returns (blocks, links): blocks in storage order (xi piece fastest),
     links = [(home, face, neighbour)].  Cut directions become non-periodic with bc 5 on the cut faces; a periodic
     direction that is cut wraps around through links; outer faces of non-periodic directions keep their bc."""
@@ -337,6 +338,7 @@ def split_blocks(wl, cuts):
                 p["ni"], p["nj"], p["nk"] = (hi[d] - lo[d] for d in range(3))
                 p["periodic"] = list(prm["periodic"])
                 p["bc"] = list(prm["bc"])
+                link_offset = {}
                 for d in range(3):
                     if nb[d] == 1:
                         continue
@@ -348,6 +350,10 @@ def split_blocks(wl, cuts):
                             npos = list(pos)
                             npos[d] = q % nb[d]
                             links.append((idx(*pos), 2 * d + side, idx(*npos)))
+                            # what is added to the neighbour's coordinates seen from here: the period vector where
+                            # the link wraps around a periodic direction, else nothing
+                            wrap = (1.0 if q >= nb[d] else -1.0 if q < 0 else 0.0)
+                            link_offset[2 * d + side] = [wrap * float(v) for v in prm["period"][d]]
                 sl_n = tuple(slice(lo[d], hi[d] + 1) for d in (2, 1, 0))
                 sl_c = tuple(slice(lo[d], hi[d]) for d in (2, 1, 0))
                 extra = {}
@@ -363,9 +369,132 @@ def split_blocks(wl, cuts):
                     inflow[int(face)] = np.ascontiguousarray(pin[:, lo[t2]:hi[t2], lo[t1]:hi[t1]])
                 if inflow:
                     extra["inflow"] = inflow
-                blocks.append(dict(extra, name="%s_block%d" % (wl["name"], idx(*pos)), params=p,
+                blocks.append(dict(extra, name="%s_block%d" % (wl["name"], idx(*pos)), params=p, link_offset=link_offset,
                                    x=np.ascontiguousarray(wl["x"][sl_n]), y=np.ascontiguousarray(wl["y"][sl_n]),
                                    z=np.ascontiguousarray(wl["z"][sl_n]),
                                    U0=np.ascontiguousarray(wl["U0"][(slice(None),) + sl_c]),
                                    dt=wl.get("dt"), cfl=wl.get("cfl"), steps=wl.get("steps"), t0=0.0, slices=sl_c))
     return blocks, links
+
+
+def link_all(grids, blocks, links):
+    """plumbing: grids[home].link(face, grids[nb]) for every link of split_blocks, with its coordinate offset"""
+    for home, face, nb in links:
+        grids[home].link(face, grids[nb], offset=blocks[home]["link_offset"].get(face))
+
+
+# --------------------------------------------------------------------------------------------------
+# Blocks with their own coordinate systems (Sec. 6, P:344): index plumbing only.
+ROTATIONS = {
+    # name: (source axis of the new xi, eta, zeta; +1 forwards / -1 backwards) -- proper rotations (right-handed)
+    "id": ((0, 1), (1, 1), (2, 1)),
+    "z90": ((1, 1), (0, -1), (2, 1)),      # new xi = old eta, new eta = -old xi
+    "z180": ((0, -1), (1, -1), (2, 1)),
+    "z270": ((1, -1), (0, 1), (2, 1)),
+    "cyc": ((1, 1), (2, 1), (0, 1)),       # new (xi, eta, zeta) = old (eta, zeta, xi)
+    "x90": ((0, 1), (2, 1), (1, -1)),      # new eta = old zeta, new zeta = -old eta
+}
+
+
+def _reindex(a, rot, lead=0):
+    """array with trailing axes (k, j, i) re-expressed in the rotated computational frame"""
+    # numpy axis of computational direction e is lead + 2 - e
+    src = [lead + 2 - rot[e][0] for e in range(3)]          # numpy source axis of new direction e
+    out = np.transpose(a, list(range(lead)) + [src[2], src[1], src[0]])
+    for e in range(3):
+        if rot[e][1] < 0:
+            out = np.flip(out, axis=lead + 2 - e)
+    return np.ascontiguousarray(out)
+
+
+def rotate_block(blk, name):
+    """The same block of cells stored in another computational frame: node arrays, state and boundary data re-indexed,
+    face numbers and periodicity permuted.  Cartesian vector components (u, v, w; x, y, z) are untouched."""
+    rot = ROTATIONS[name]
+    p = dict(blk["params"])
+    n_old = (p["ni"], p["nj"], p["nk"])
+    p["ni"], p["nj"], p["nk"] = (n_old[rot[e][0]] for e in range(3))
+    p["periodic"] = [blk["params"]["periodic"][rot[e][0]] for e in range(3)]
+    p["period"] = [[rot[e][1] * v for v in blk["params"]["period"][rot[e][0]]] for e in range(3)]
+    bc, link_offset, face_map = [0] * 6, {}, {}
+    for e in range(3):
+        for side in range(2):
+            old_face = 2 * rot[e][0] + (side if rot[e][1] > 0 else 1 - side)
+            bc[2 * e + side] = blk["params"]["bc"][old_face]
+            face_map[old_face] = 2 * e + side
+            if old_face in blk.get("link_offset", {}):
+                link_offset[2 * e + side] = blk["link_offset"][old_face]
+    p["bc"] = bc
+    out = dict(blk, params=p, link_offset=link_offset, face_map=face_map, rotation=name,
+               name=blk["name"] + "_" + name)
+    for key in ("x", "y", "z", "dx_mode", "dy_mode", "dz_mode"):
+        if blk.get(key) is not None:
+            out[key] = _reindex(blk[key], rot)
+    out["U0"] = _reindex(blk["U0"], rot, lead=1)
+    if blk.get("sigma") is not None:
+        out["sigma"] = _reindex(blk["sigma"], rot)
+        out["U_ref"] = _reindex(blk["U_ref"], rot, lead=1)
+    assert not blk.get("inflow"), "rotate_block: inflow faces are not re-indexed"
+    return out
+
+
+def unrotate_state(a, name):
+    """inverse of the re-indexing of rotate_block for a state array (5, nk, nj, ni)"""
+    rot = ROTATIONS[name]
+    out = a
+    for e in range(3):
+        if rot[e][1] < 0:
+            out = np.flip(out, axis=1 + 2 - e)
+    src = [1 + 2 - rot[e][0] for e in range(3)]
+    perm = [0, src[2], src[1], src[0]]
+    inv = np.argsort(perm)
+    return np.ascontiguousarray(np.transpose(out, inv))
+
+
+def _face_nodes(blk, face):
+    """node coordinates of a block face, shape (nb+1, na+1, 3), transverse axes in storage order (a fast)"""
+    d, side = face // 2, face % 2
+    sl = [slice(None)] * 3
+    sl[2 - d] = -1 if side else 0
+    return np.stack([blk[k][tuple(sl)] for k in ("x", "y", "z")], axis=-1)
+
+
+def auto_links(blocks, periods=()):
+    """Finds, for every block-interface face (bc 5), the neighbour block, its face and the orientation of its axes by
+    matching the node coordinates of the faces (up to one of the given period vectors).  Returns
+    [(home, face, nb, nb_face, swap, flip_a, flip_b, offset)]: the arguments of the oriented link call."""
+    offs = [np.zeros(3)] + [s * np.asarray(v, dtype=float) for v in periods for s in (1.0, -1.0)]
+    faces = [(b, f, _face_nodes(blk, f)) for b, blk in enumerate(blocks) for f in range(6)
+             if not blk["params"]["periodic"][f // 2] and blk["params"]["bc"][f] == 5]
+    links = []
+    for b, f, N in faces:
+        h = np.linalg.norm(N[1, 1] - N[0, 0]) if min(N.shape[:2]) > 1 else 1.0
+        found = None
+        for c, g, M in faces:
+            if (c, g) == (b, f) and not periods:
+                continue
+            for swap in (0, 1):
+                Ms = np.swapaxes(M, 0, 1) if swap else M     # home a runs along the neighbour's b' when swapped
+                if Ms.shape != N.shape:
+                    continue
+                for fa in (0, 1):
+                    for fb in (0, 1):
+                        T = Ms[:, ::-1] if fa else Ms
+                        T = T[::-1] if fb else T
+                        for off in offs:
+                            if (c, g) == (b, f) and not off.any():
+                                continue
+                            if np.abs(T + off - N).max() <= 1e-9 * max(h, 1e-30) + 1e-12:
+                                found = (b, f, c, g, swap, fa, fb, [float(v) for v in off])
+                        if found:
+                            break
+                    if found:
+                        break
+                if found:
+                    break
+            if found:
+                break
+        if found is None:
+            raise ValueError("auto_links: no partner for block %d face %d" % (b, f))
+        links.append(found)
+    return links
