@@ -814,8 +814,11 @@ void ghost_dir(meg6o_grid* G, int d) {
         for (int side = 0; side < 2; ++side) {
           const int face = 2 * d + side, bc = p.bc[face];
           const int last = side ? n - 1 : 0, sg = side ? 1 : -1;
-          /* transverse position clamped to the interior for the lookups of face data / metrics */
+          /* transverse position clamped to the interior for the lookup of face data, and to the range on which the
+           * cell-centre metrics exist (five ghost layers) for the metric lookups of the wall and outflow rules: in the
+           * ghost columns beyond a block interface those are the neighbour's true metrics (R27, R28) */
           const int ca = std::min(std::max(ta, 0), G->n[a] - 1), cb = std::min(std::max(tb, 0), G->n[b] - 1);
+          const int ma = std::min(std::max(ta, -5), G->n[a] + 4), mb = std::min(std::max(tb, -5), G->n[b] + 4);
           if (bc == 5) {
             /* block interface, Table 1 last column, R28: ghost layer q = the q-th interior cell of the
              * neighbour block counted from its opposite face, same transverse index (aligned blocks) */
@@ -856,7 +859,7 @@ void ghost_dir(meg6o_grid* G, int d) {
               double pv[5];
               for (int f = 0; f < 5; ++f) pv[f] = at(f, m);
               if (bc == 3) {
-                int im[3]; im[a] = ca; im[b] = cb; im[d] = m;
+                int im[3]; im[a] = ma; im[b] = mb; im[d] = m;
                 const double mx = G->met[3 * d](im[0], im[1], im[2]), my = G->met[3 * d + 1](im[0], im[1], im[2]),
                              mz = G->met[3 * d + 2](im[0], im[1], im[2]);
                 const double gm = std::sqrt(mx * mx + my * my + mz * mz);
@@ -873,7 +876,7 @@ void ghost_dir(meg6o_grid* G, int d) {
              * normal Mach number of that cell is below one */
             double pv[5];
             for (int f = 0; f < 5; ++f) pv[f] = at(f, last);
-            int im[3]; im[a] = ca; im[b] = cb; im[d] = last;
+            int im[3]; im[a] = ma; im[b] = mb; im[d] = last;
             const double mx = G->met[3 * d](im[0], im[1], im[2]), my = G->met[3 * d + 1](im[0], im[1], im[2]),
                          mz = G->met[3 * d + 2](im[0], im[1], im[2]);
             const double gm = std::sqrt(mx * mx + my * my + mz * mz);

@@ -66,7 +66,10 @@ __global__ void __launch_bounds__(256) k_ghost(Consts c, int d, P6 P, GhostIn in
     return;
   }
   const int bc = c.bc[2 * d + side];
-  const int ca = min(max(ta, 0), c.n[a] - 1), cb = min(max(tb, 0), c.n[b] - 1);
+  const int ca = min(max(ta, 0), c.n[a] - 1), cb = min(max(tb, 0), c.n[b] - 1);   // face data: interior positions
+  // metric lookups of the wall / outflow rules: wherever the cell-centre metrics exist (five ghost layers; beyond a block
+  // interface those are the neighbour's true metrics, R27 / R28)
+  const int ma = min(max(ta, -5), c.n[a] + 4), mb = min(max(tb, -5), c.n[b] + 4);
   if (bc == 5) {
     // block interface (Table 1 last column; R28, R29): ghost layer q = the q-th interior cell of the neighbour
     // block counted from the face it shares with this one, at the transverse position the link's orientation gives
@@ -104,7 +107,7 @@ __global__ void __launch_bounds__(256) k_ghost(Consts c, int d, P6 P, GhostIn in
     for (int f = 0; f < 5; ++f) pv[f] = P.p[f][mir];
     if (bc == 3) {
       int im[3];
-      im[a] = ca; im[b] = cb; im[d] = m;
+      im[a] = ma; im[b] = mb; im[d] = m;
       const long long am = c.LX.at(im[0], im[1], im[2]);
       const double mx = in.mx[am], my = in.my[am], mz = in.mz[am];
       const double gm = sqrt(mx * mx + my * my + mz * mz);
@@ -122,7 +125,7 @@ __global__ void __launch_bounds__(256) k_ghost(Consts c, int d, P6 P, GhostIn in
 #pragma unroll
     for (int f = 0; f < 5; ++f) pv[f] = P.p[f][base + (long long)last * s];
     int im[3];
-    im[a] = ca; im[b] = cb; im[d] = last;
+    im[a] = ma; im[b] = mb; im[d] = last;
     const long long am = c.LX.at(im[0], im[1], im[2]);
     const double mx = in.mx[am], my = in.my[am], mz = in.mz[am];
     const double gm = sqrt(mx * mx + my * my + mz * mz);

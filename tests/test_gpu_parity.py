@@ -627,9 +627,10 @@ def test_blocks_rhs_and_steps_parity(mods, name):
     for b, uo, u in zip(blocks, Uo, Us):
         e = rel(u.cpu().numpy(), uo)
         assert np.all(e <= STEP_TOL), (name, b["name"], e)
-    if True:
+    if wl["params"].get("scheme", 0) == 0:
         # and the cut run equals the uncut one on the GPU as well, curved meshes included (ghost coordinates of an
-        # interface face are the neighbour's cell centres, R28); walls of both kinds on the outer faces
+        # interface face are the neighbour's cell centres, R28); walls of both kinds on the outer faces.  Not for MIG4:
+        # its implicit gradients are line solves, and a cut line is two systems with their own closures (R26)
         g1 = M.Grid(wl)
         g1.metrics_compute(0.0)
         U1 = torch.as_tensor(wl["U0"], device="cuda").contiguous()
