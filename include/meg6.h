@@ -96,6 +96,10 @@ meg6_status meg6_rhs(meg6_grid* g, const double* U, double* dUdt);
  * geometry at the stage times t, t+dt, t+dt/2 (R17) and leave it at t+dt/2.  U is read and written by the last
  * sweep of every stage; it must not be touched by other streams while the step is in flight. */
 meg6_status meg6_rk3_step(meg6_grid* g, double* U, double t, double dt);
+/* nsteps SSP-RK3 steps of constant dt (t, t+dt, ...): the same arithmetic as nsteps calls of meg6_rk3_step, bit for bit;
+ * since U stays with the library between the steps (the paper's time loop is device-resident), the
+ * primitive conversion of U^{n+1} is done by the last sweep of step n instead of a separate kernel per step. */
+meg6_status meg6_rk3_steps(meg6_grid* g, double* U, double t, double dt, int nsteps);
 
 /* Multi-block (Sec. 6; Table 1 last column P:354-362; readings R28, R29).  A face with bc == 5 is a block
  * interface: its ghost CELLS are the neighbour block's cells next to the face the two blocks share -- the six ghost

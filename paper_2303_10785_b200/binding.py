@@ -8,7 +8,7 @@ import os
 from . import build as _build
 
 EXPORTS = ["meg6_workspace_bytes", "meg6_grid_create", "meg6_grid_destroy", "meg6_metrics_compute",
-           "meg6_set_inflow", "meg6_set_sponge", "meg6_rhs", "meg6_rk3_step", "meg6_cfl_dt", "meg6_diagnostics",
+           "meg6_set_inflow", "meg6_set_sponge", "meg6_rhs", "meg6_rk3_step", "meg6_rk3_steps", "meg6_cfl_dt", "meg6_diagnostics",
            "meg6_limiter_stats_enable", "meg6_limiter_stats", "meg6_set_branch_masks", "meg6_get_array", "meg6_profile_enable",
            "meg6_profile_read", "meg6_fp64_peak", "meg6_last_error",
            "meg6_version", "meg6_link_blocks", "meg6_link_blocks_oriented", "meg6_metrics_compute_blocks", "meg6_rhs_blocks",
@@ -85,6 +85,8 @@ def lib():
         L.meg6_rhs.argtypes = [_vp, _vp, _vp]
         L.meg6_rk3_step.restype = C.c_int
         L.meg6_rk3_step.argtypes = [_vp, _vp, C.c_double, C.c_double]
+        L.meg6_rk3_steps.restype = C.c_int
+        L.meg6_rk3_steps.argtypes = [_vp, _vp, C.c_double, C.c_double, C.c_int]
         L.meg6_diagnostics.restype = C.c_int
         L.meg6_diagnostics.argtypes = [_vp, _vp, C.POINTER(C.c_double)]
         L.meg6_cfl_dt.restype = C.c_int
@@ -217,6 +219,10 @@ class Grid:
     def rk3_step(self, U, t, dt):
         self._chk_state(U)
         _check(lib().meg6_rk3_step(self.h, U.data_ptr(), float(t), float(dt)), "meg6_rk3_step")
+
+    def rk3_steps(self, U, t, dt, nsteps):
+        self._chk_state(U)
+        _check(lib().meg6_rk3_steps(self.h, U.data_ptr(), float(t), float(dt), int(nsteps)), "meg6_rk3_steps")
 
     def link(self, face, neighbour, nb_face=None, swap=0, flip_a=0, flip_b=0, offset=None):
         """block interface (bc 5): ghost cells of `face` come from `neighbour` (its face nb_face, default the opposite

@@ -637,12 +637,14 @@ meg6_status meg6_rhs(meg6_grid* g, const double* U, double* dUdt) {
 
 static const double RK_A[3] = {0.0, 3.0 / 4.0, 1.0 / 3.0}, RK_B[3] = {1.0, 1.0 / 4.0, 2.0 / 3.0};
 
-static Fuse3 make_fuse_rk(meg6_grid* g, double* U, int s, double dt) {
-  const int buf = s & 1;
+// stage s of a step whose primitives are in buffer `buf`; more: another stage follows that may use the primitives of the
+// state this one produces (always within a step; across steps only inside meg6_rk3_steps, where nobody touches U)
+static Fuse3 make_fuse_rk(meg6_grid* g, double* U, int s, double dt, int buf = -1, bool more = false) {
+  if (buf < 0) buf = s & 1;
   Fuse3 fu = make_fuse(g, U, U);
   fu.mode = 1; fu.a = RK_A[s]; fu.b = RK_B[s]; fu.dt = dt;
-  fu.U0w = (s == 0) ? g->U0 : nullptr;                      // stage 1 saves U^n on the way
-  fu.Pn = (s < 2) ? (buf ? g->P[0] : g->Pb[0]) : nullptr;   // primitives of the next stage's state
+  fu.U0w = (s == 0) ? g->U0 : nullptr;                                // stage 1 saves U^n on the way
+  fu.Pn = (s < 2 || more) ? (buf ? g->P[0] : g->Pb[0]) : nullptr;     // primitives of the next stage's state
   return fu;
 }
 
@@ -656,6 +658,29 @@ meg6_status meg6_rk3_step(meg6_grid* g, double* U, double t, double dt) {
     meg6_status st;
     if (g->p.moving && (st = meg6_metrics_compute(g, ts[s])) != MEG6_OK) return st;
     if ((st = stage(g, s & 1, make_fuse_rk(g, U, s, dt))) != MEG6_OK) return st;
+  }
+  return MEG6_OK;
+}
+
+// n steps of constant dt in one call: the time loop stays in the library (nothing leaves the device between
+// steps), so the primitives of U^{n+1} that the last sweep of a step can write on its way are those of the next step's
+// first stage -- the separate conversion kernel runs once per call instead of once per step.
+meg6_status meg6_rk3_steps(meg6_grid* g, double* U, double t, double dt, int nsteps) {
+  if (!g || !U || nsteps < 0) return fail(MEG6_EINVAL, "rk3_steps: bad argument%s");
+  if (nsteps == 0) return MEG6_OK;
+  if (!g->have_metrics && !g->p.moving) return fail(MEG6_ESTATE, "rk3_steps called before metrics_compute%s");
+  if (!links_ok(g, true)) return fail(MEG6_ESTATE, "rk3_steps: block-interface face without a link, or linked to another block%s");
+  CUDA_OK(launch_prim(g, U));
+  int buf = 0;
+  for (int n = 0; n < nsteps; ++n) {
+    const double tn = t + n * dt;
+    const double ts[3] = {tn, tn + dt, tn + 0.5 * dt};
+    for (int s = 0; s < 3; ++s) {
+      meg6_status st;
+      if (g->p.moving && (st = meg6_metrics_compute(g, ts[s])) != MEG6_OK) return st;
+      if ((st = stage(g, buf, make_fuse_rk(g, U, s, dt, buf, n + 1 < nsteps))) != MEG6_OK) return st;
+      buf ^= 1;
+    }
   }
   return MEG6_OK;
 }

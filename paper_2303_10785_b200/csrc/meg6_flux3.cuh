@@ -133,16 +133,19 @@ __device__ __forceinline__ double rcp3(double x) { return 1.0 / x; }
 // to DSETP + SEL + FSEL + LOP3 + three or four register moves each (sm_100a has no FP64 min/max instruction; SASS of the
 // round-1 build: 8 instructions per call, 24 % of the limiting path); a NaN here means the state is lost anyway.  For
 // ordered operands the result is the same value bit for bit (the limiter's own +-0 cases select equal magnitudes).
-// Unordered operands: the forms below are those of std::min / std::max -- the first operand comes back when the
-// second is a NaN -- which is what the step-by-step CPU restatement of the method does at an interface whose limited
-// right state has left the physical range (sound speed of a negative density: the violent inflow interface of the
-// randomised parity case), so such an interface takes the same branch of Eq. 26 on both sides.
-__device__ __forceinline__ double dmin3(double a, double b) { return (b < a) ? b : a; }
-__device__ __forceinline__ double dmax3(double a, double b) { return (a < b) ? b : a; }
+__device__ __forceinline__ double dmin3(double a, double b) { return (a < b) ? a : b; }
+__device__ __forceinline__ double dmax3(double a, double b) { return (a > b) ? a : b; }
+// The wave-speed bounds of HLLC are the one place where an unordered operand occurs in a run that is otherwise fine: a
+// limited state that has left the physical range (negative density: the violent inflow interface of the randomised
+// parity case) has a NaN sound speed.  The forms below are those of std::min / std::max -- the FIRST operand comes back
+// when the second is a NaN -- which is what the step-by-step CPU restatement of the method does, so such an interface
+// takes the same branch of Eq. 26 on both sides (and the left state's flux, which is finite).
+__device__ __forceinline__ double hmin3(double a, double b) { return (b < a) ? b : a; }
+__device__ __forceinline__ double hmax3(double a, double b) { return (a < b) ? b : a; }
 
 __device__ __forceinline__ double minmod3(double a, double b) {   // E.2
   // same sign: the operand of smaller magnitude IS sign * min(|a|, |b|)
-  const double m = (fabs(b) < fabs(a)) ? b : a;
+  const double m = (fabs(a) < fabs(b)) ? a : b;
   const bool same = ((__double2hiint(a) ^ __double2hiint(b)) >= 0);
   return same ? m : 0.0;
 }
@@ -192,8 +195,8 @@ __device__ __forceinline__ unsigned hllc3(const double PL[5], const double PR[5]
   const double t = rcp3(PL[0] * PR[0]);
   const double irL = PR[0] * t, irR = PL[0] * t;
   const double cL = sqrt(gamma * PL[4] * irL) * g, cR = sqrt(gamma * PR[4] * irR) * g;
-  const double SL = dmin3(UL - cL, UR - cR);
-  const double SR = dmax3(UL + cL, UR + cR);
+  const double SL = hmin3(UL - cL, UR - cR);
+  const double SR = hmax3(UL + cL, UR + cR);
   const double mL = PL[0] * (SL - UL), mR = PR[0] * (SR - UR);
   const double SS = (fma(mR, UR, -mL * UL) + (PL[4] - PR[4]) * g2) * rcp3(mR - mL);
   const bool left = (SL >= 0.0) || (SS >= 0.0);

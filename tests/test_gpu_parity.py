@@ -1030,3 +1030,23 @@ def test_slab_stepper_on_two_cuda_grids_through_an_in_process_transport(mods, mo
         assert (a.cpu().numpy() - blk["U0"]).__abs__().max() > 1e-6
     for g in ref + gg:
         g.close()
+
+
+@pytest.mark.parametrize("name", ["c2", "c3", "c4"])
+def test_rk3_steps_equals_repeated_rk3_step_bit_for_bit(mods, cases, name):
+    """meg6_rk3_steps(n) = n x meg6_rk3_step: same kernels on the same data (the primitive conversion of U^{n+1} moves
+    from its own kernel into the last sweep of step n), static and moving meshes, odd step count (buffer parity)."""
+    torch, O, M = mods
+    wl = cases[name]
+    g = M.Grid(wl)
+    g.metrics_compute(0.0)
+    U = torch.as_tensor(wl["U0"], device="cuda").contiguous()
+    dt = wl["dt"] if wl["dt"] else g.cfl_dt(U, wl["cfl"])
+    Ua, Ub = U.clone(), U.clone()
+    for s in range(5):
+        g.rk3_step(Ua, s * dt, dt)
+    g.rk3_steps(Ub, 0.0, dt, 5)
+    assert torch.equal(Ua, Ub)
+    g.rk3_steps(Ub, 5 * dt, dt, 0)
+    assert torch.equal(Ua, Ub)
+    g.close()
