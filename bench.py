@@ -79,8 +79,8 @@ def bytes_per_cell_stage(prm, sponge_frac):
     k["prim"] = 0.0                                # once per meg6_rk3_steps call (11 doubles / (3 K) per cell-stage)
     met = (10 if v else 3) + (1 if m else 0)
     if ig:
-        # MIG4: 3 nf line solves (read f, write d, read d, write x) ; sweeps read P, P' and two 5-field gradient groups
-        k["grad"] = 3 * nf * 4
+        # MIG4: 3 nf segmented line solves (read f, write the gradient); sweeps read P, P' and two 5-field gradient groups
+        k["grad"] = 3 * nf * 2
         base = nf + nf + met + (10 if v else 0)
     else:
         k["grad"] = GRAD_DOUBLES if v else 0

@@ -115,10 +115,20 @@ Box launch_ig4(meg6_grid* g, const Lay& L, const double* f, const Box& fb, int d
 Box launch_ig4_flow(meg6_grid* g, const Lay& L, const double* f, const Box& fb, int dir, double* out, int nfields,
                     long long fs_in, long long fs_out) {
   const int m = fb.hi[dir] - fb.lo[dir] - 4;
-  if (!MEG6_IG4_SEGMENTED || dir == 0 || m - 2 > IG4S_NSEG * IG4S_SEGMAX || m < 3)
+  if (!MEG6_IG4_SEGMENTED || m - 2 > IG4S_NSEG * IG4S_SEGMAX || m < 3)
     return launch_ig4_batch(g, L, f, fb, dir, out, nfields, fs_in, fs_out);
   Box ob = fb;
   ob.lo[dir] += 2; ob.hi[dir] -= 2;
+  if (dir == 0) {
+    // lanes of a warp = segments of one xi line, or of several short lines
+    const int spl = (m - 2 + IG4S_SEGMAX - 1) / IG4S_SEGMAX;        // segments per line (<= 32)
+    const int lpw = 32 / spl;                                        // lines per warp
+    if ((long long)lpw * (m + 4) > IG4SX_TILE) return launch_ig4_batch(g, L, f, fb, dir, out, nfields, fs_in, fs_out);
+    const long long lines = (long long)(ob.hi[1] - ob.lo[1]) * (ob.hi[2] - ob.lo[2]);
+    const dim3 grid((unsigned)nblk(lines, (long long)IG4SX_WARPS * lpw), (unsigned)nfields);
+    k_ig4sx<<<grid, 32 * IG4SX_WARPS, 0, g->stream>>>(L, f, out, ob, g->ig4_cc, fs_in, fs_out, spl, lpw);
+    return ob;
+  }
   const int od = (dir == 1) ? 2 : 1;
   const dim3 grid((unsigned)nblk(ob.hi[0] - ob.lo[0], IG4S_LANES), (unsigned)(ob.hi[od] - ob.lo[od]), (unsigned)nfields);
   const int nseg = (m - 2 + IG4S_SEGMAX - 1) / IG4S_SEGMAX;   // segments of (nearly) full length, fewer threads for short lines

@@ -233,6 +233,90 @@ __global__ void __launch_bounds__(IG4S_LANES * IG4S_NSEG, 2) k_ig4s(Lay L, const
   if (last) px[(long long)(m - 1) * s] = sX[1][lane];
 }
 
+// The segmented solve for lines along xi (flow gradients only, like k_ig4s).  A xi line is contiguous in memory, so the
+// lanes of a warp are the segments of one line (or of several short lines: LPW lines of SPL segments each): the warp
+// copies its lines into shared memory with full-width coalesced loads, every lane takes its SEG-cell window from
+// there (lane stride 13 doubles: conflict-free), the affine maps of the two Thomas sweeps are chained with warp shuffles,
+// and the gradients leave through the same tile.  f is read once and the gradient written once (k_ig4x: four passes).
+constexpr int IG4SX_WARPS = 4, IG4SX_TILE = 32 * IG4S_SEGMAX + 8;
+__global__ void __launch_bounds__(32 * IG4SX_WARPS) k_ig4sx(Lay L, const double* __restrict__ f, double* __restrict__ out, Box ob,
+                                                            const double* __restrict__ cc, long long fs_in, long long fs_out,
+                                                            int spl, int lpw) {
+  constexpr int SMAX = IG4S_SEGMAX;
+  __shared__ double tile[IG4SX_WARPS][IG4SX_TILE];
+  f += blockIdx.y * fs_in; out += blockIdx.y * fs_out;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  double* T = tile[warp];
+  const int n1 = ob.hi[1] - ob.lo[1], n2 = ob.hi[2] - ob.lo[2];
+  const long long nl = (long long)n1 * n2;
+  const int m = ob.hi[0] - ob.lo[0];                // unknowns 0 .. m-1 of a line; 0 and m-1 explicit (R26)
+  const int W = m + 4;                              // f window of a line: cells -2 .. m+1 relative to the first unknown
+  const long long line0 = ((long long)blockIdx.x * IG4SX_WARPS + warp) * lpw;   // first line of this warp
+  const double al = 5.0 / 14.0, ial = 14.0 / 5.0, ca = (2.0 + al) / 3.0, cb = (4.0 * al - 1.0) / 12.0;
+  // ---- stage the windows of the warp's lines ----
+  for (int l = 0; l < lpw; ++l) {
+    const long long lid = line0 + l;
+    if (lid >= nl) break;
+    const double* pf = f + L.at(ob.lo[0], ob.lo[1] + (int)(lid % n1), ob.lo[2] + (int)(lid / n1)) - 2;
+    for (int q = lane; q < W; q += 32) T[l * W + q] = pf[q];
+  }
+  __syncwarp();
+  const int ln = lane / spl, seg = lane % spl;      // this lane: segment `seg` of the warp's line `ln`
+  const long long lid = line0 + ln;
+  const bool act = ln < lpw && lid < nl;
+  const int len = (m - 2 + spl - 1) / spl;          // interior unknowns per segment (<= SMAX)
+  const int reach = (48 + len - 1) / len;           // see k_ig4s
+  const int q0 = 1 + seg * len;
+  const int nq = act ? max(0, min(len, m - 1 - q0)) : 0;
+  const double* Tl = T + (act ? ln : 0) * W + 2;    // Tl[q] = f at unknown q of this lane's line
+  double r[SMAX];
+#pragma unroll
+  for (int u = 0; u < SMAX; ++u) {
+    const double* w = Tl + q0 + u;
+    r[u] = (u < nq) ? fma(cb, w[2] - w[-2], ca * (w[1] - w[-1])) : 0.0;
+  }
+  const double x0 = 2.0 / 3.0 * (Tl[1] - Tl[-1]) - 1.0 / 12.0 * (Tl[2] - Tl[-2]);                    // Eq. D.2 at unknown 0
+  const double xm = 2.0 / 3.0 * (Tl[m] - Tl[m - 2]) - 1.0 / 12.0 * (Tl[m + 1] - Tl[m - 3]);          // ... and at m-1
+  const double* __restrict__ cs = cc + q0;
+  const unsigned full = 0xffffffffu;
+  // ---- forward sweep ----
+  double a = 0.0, b = 1.0;
+#pragma unroll
+  for (int u = 0; u < SMAX; ++u)
+    if (u < nq) { const double c = __ldg(cs + u); a = fma(-al, a, r[u]) * (c * ial); b = -c * b; }
+  double din = (seg <= reach) ? x0 : 0.0;
+  for (int k = reach; k >= 1; --k) {                // maps of the segments seg-k .. seg-1 of the same line, in order
+    const double at = __shfl_up_sync(full, a, k), bt = __shfl_up_sync(full, b, k);
+    if (seg - k >= 0) din = fma(bt, din, at);
+  }
+#pragma unroll
+  for (int u = 0; u < SMAX; ++u)
+    if (u < nq) { din = fma(-al, din, r[u]) * (__ldg(cs + u) * ial); r[u] = din; }
+  // ---- backward sweep ----
+  a = 0.0; b = 1.0;
+#pragma unroll
+  for (int u = SMAX - 1; u >= 0; --u)
+    if (u < nq) { const double c = __ldg(cs + u); a = fma(-c, a, r[u]); b = -c * b; }
+  const int nsg = (m - 2 + len - 1) / len;          // segments that hold unknowns
+  double xin = (seg + reach >= nsg - 1) ? xm : 0.0;
+  for (int k = reach; k >= 1; --k) {                // maps of the segments seg+k .. seg+1
+    const double at = __shfl_down_sync(full, a, k), bt = __shfl_down_sync(full, b, k);
+    if (seg + k <= nsg - 1 && seg + k < spl) xin = fma(bt, xin, at);
+  }
+  __syncwarp();                                     // every lane has read its window: the tile now takes the results
+#pragma unroll
+  for (int u = SMAX - 1; u >= 0; --u)
+    if (u < nq) { xin = fma(-__ldg(cs + u), xin, r[u]); T[ln * W + 2 + q0 + u] = xin; }
+  if (act && seg == 0) { T[ln * W + 2] = x0; T[ln * W + 2 + m - 1] = xm; }
+  __syncwarp();
+  for (int l = 0; l < lpw; ++l) {
+    const long long lo = line0 + l;
+    if (lo >= nl) break;
+    double* po = out + L.at(ob.lo[0], ob.lo[1] + (int)(lo % n1), ob.lo[2] + (int)(lo / n1));
+    for (int q = lane; q < m; q += 32) po[q] = T[l * W + 2 + q];
+  }
+}
+
 // Central interface value Eq. 36/38 from f and its gradient f1: index i of `out` = interface between
 // cells i and i+1 along dir.  The second derivative is Eq. 19.  `out` may have another layout (interface
 // arrays): LO, and an index shift `sh` along dir (interface arrays number the face between cells i-1 and i as i).
