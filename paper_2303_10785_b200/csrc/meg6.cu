@@ -366,6 +366,7 @@ meg6_status meg6_grid_create(const meg6_params* p, const double* x, const double
 void meg6_grid_destroy(meg6_grid* g) {
   if (!g) return;
   for (cudaEvent_t e : g->prof_pool) cudaEventDestroy(e);
+  if (g->steps_graph) cudaGraphExecDestroy(g->steps_graph);
   delete g;
 }
 
@@ -671,8 +672,33 @@ meg6_status meg6_rk3_steps(meg6_grid* g, double* U, double t, double dt, int nst
   if (!g->have_metrics && !g->p.moving) return fail(MEG6_ESTATE, "rk3_steps called before metrics_compute%s");
   if (!links_ok(g, true)) return fail(MEG6_ESTATE, "rk3_steps: block-interface face without a link, or linked to another block%s");
   CUDA_OK(launch_prim(g, U));
-  int buf = 0;
-  for (int n = 0; n < nsteps; ++n) {
+  int buf = 0, n0 = 0;
+  if (!g->p.moving && !g->prof_on && nsteps >= 4) {
+    // static mesh: two steps (six stages: the primitive buffers swap roles every stage) as one CUDA graph.  Small grids
+    // are bound by the launch rate of the host (config 1: 18 launches of ~5 us of work each per step)
+    meg6_grid::GraphKey key;
+    memset(&key, 0, sizeof(key));
+    key.U = U; key.dt = dt; key.sigma = g->sigma; key.uref = g->uref; key.stats_on = g->stats_on;
+    for (int d = 0; d < 3; ++d) key.bm[d] = g->bmask[d];
+    if (!g->steps_graph || memcmp(&key, &g->steps_key, sizeof(key)) != 0) {
+      if (g->steps_graph) { cudaGraphExecDestroy(g->steps_graph); g->steps_graph = nullptr; }
+      (void)make_fuse(g, U, U);   // tensor maps of the caller's arrays encoded before the capture
+      cudaGraph_t graph = nullptr;
+      CUDA_OK(cudaStreamBeginCapture(g->stream, cudaStreamCaptureModeThreadLocal));
+      meg6_status st = MEG6_OK;
+      int b = 0;
+      for (int q = 0; q < 6 && st == MEG6_OK; ++q, b ^= 1) st = stage(g, b, make_fuse_rk(g, U, q % 3, dt, b, true));
+      const cudaError_t ec = cudaStreamEndCapture(g->stream, &graph);
+      if (st != MEG6_OK) { if (graph) cudaGraphDestroy(graph); return st; }
+      CUDA_OK(ec);
+      const cudaError_t ei = cudaGraphInstantiate(&g->steps_graph, graph, 0);
+      cudaGraphDestroy(graph);
+      CUDA_OK(ei);
+      g->steps_key = key;
+    }
+    for (; n0 + 2 <= nsteps; n0 += 2) CUDA_OK(cudaGraphLaunch(g->steps_graph, g->stream));
+  }
+  for (int n = n0; n < nsteps; ++n) {
     const double tn = t + n * dt;
     const double ts[3] = {tn, tn + dt, tn + 0.5 * dt};
     for (int s = 0; s < 3; ++s) {

@@ -122,6 +122,10 @@ struct meg6_grid {
   bool have_metrics;
   int geom_blocked;            // -1 by size, 0 / 1 forced (MEG6_GEOM_BLOCKED in the environment at grid_create; tests)
   int geom_launches;           // kernels launched by the last metrics_compute
+  // meg6_rk3_steps on static meshes: the launches of two consecutive steps (the period of the primitive-buffer parity)
+  // captured once as a CUDA graph and replayed; the key is what the captured kernel arguments depend on
+  cudaGraphExec_t steps_graph;
+  struct GraphKey { const double* U; double dt; const double* sigma; const double* uref; int stats_on; unsigned short* bm[3]; } steps_key;
   // per-kernel timing (meg6_profile_*): event pairs of the launches since the last read
   int prof_on;
   std::vector<cudaEvent_t> prof_pool;

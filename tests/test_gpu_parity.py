@@ -1049,4 +1049,10 @@ def test_rk3_steps_equals_repeated_rk3_step_bit_for_bit(mods, cases, name):
     assert torch.equal(Ua, Ub)
     g.rk3_steps(Ub, 5 * dt, dt, 0)
     assert torch.equal(Ua, Ub)
+    # again from the new state (static meshes replay the captured two-step graph), then with another dt (re-captured)
+    for dt2, n in ((dt, 6), (0.5 * dt, 4)):
+        for s in range(n):
+            g.rk3_step(Ua, s * dt2, dt2)
+        g.rk3_steps(Ub, 0.0, dt2, n)
+        assert torch.equal(Ua, Ub)
     g.close()
