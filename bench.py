@@ -261,6 +261,8 @@ def run_ours(args):
         raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
+    # everything on one stream of our own (the library captures CUDA graphs, which the legacy default stream cannot)
+    torch.cuda.set_stream(torch.cuda.Stream(dev))
     dist = None
     if world > 1:
         import torch.distributed as dist

@@ -673,7 +673,9 @@ meg6_status meg6_rk3_steps(meg6_grid* g, double* U, double t, double dt, int nst
   if (!links_ok(g, true)) return fail(MEG6_ESTATE, "rk3_steps: block-interface face without a link, or linked to another block%s");
   CUDA_OK(launch_prim(g, U));
   int buf = 0, n0 = 0;
-  if (!g->p.moving && !g->prof_on && nsteps >= 4) {
+  // (stream capture is not available on the legacy default stream: callers that want the graph pass their own stream)
+  if (!g->p.moving && !g->prof_on && nsteps >= 4 && g->stream != nullptr && g->stream != cudaStreamLegacy &&
+      g->stream != cudaStreamPerThread) {
     // static mesh: two steps (six stages: the primitive buffers swap roles every stage) as one CUDA graph.  Small grids
     // are bound by the launch rate of the host (config 1: 18 launches of ~5 us of work each per step)
     meg6_grid::GraphKey key;

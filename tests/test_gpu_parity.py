@@ -1038,6 +1038,14 @@ def test_rk3_steps_equals_repeated_rk3_step_bit_for_bit(mods, cases, name):
     from its own kernel into the last sweep of step n), static and moving meshes, odd step count (buffer parity)."""
     torch, O, M = mods
     wl = cases[name]
+    side = torch.cuda.Stream()                    # graphs need a stream of the caller's own
+    torch.cuda.current_stream().synchronize()
+    with torch.cuda.stream(side):
+        _rk3_steps_body(torch, M, wl)
+    side.synchronize()
+
+
+def _rk3_steps_body(torch, M, wl):
     g = M.Grid(wl)
     g.metrics_compute(0.0)
     U = torch.as_tensor(wl["U0"], device="cuda").contiguous()
