@@ -498,3 +498,49 @@ def auto_links(blocks, periods=()):
             raise ValueError("auto_links: no partner for block %d face %d" % (b, f))
         links.append(found)
     return links
+
+
+def butterfly(n=12, nr=12, nk=10, a=0.5, R=2.0, Lz=1.0, viscous=1, scheme=0, seed=627, uniform=False):
+    """Butterfly-type O-grid section (Fig. 13b "to avoid singularity at the axis"), synthetic: a square core block
+    of n x n cells and four outer blocks of nr x n cells between the square and a circle of radius R, each in its own
+    frame (xi radial, eta along the core's side; quarter turns about the axis from one to the next), extruded along a
+    periodic zeta.  Three blocks meet along each of the core's four corner edges.  Returns the five block workloads
+    (interfaces bc 5, outer rim outflow); link them with auto_links.  (The paper's jet grid has four blocks and is not
+    in the container; this one only has its topology class: rotated frames around a core, singular corner edges.)"""
+    s = np.linspace(-1.0, 1.0, n + 1)
+    r = np.linspace(0.0, 1.0, nr + 1)
+    zk = np.linspace(-Lz / 2, Lz / 2, nk + 1)
+
+    def extrude(X2, Y2):
+        shp = (nk + 1,) + X2.shape
+        return (np.ascontiguousarray(np.broadcast_to(X2, shp)), np.ascontiguousarray(np.broadcast_to(Y2, shp)),
+                np.ascontiguousarray(np.broadcast_to(zk[:, None, None], shp)))
+    X, Y = np.meshgrid(a * s, a * s, indexing="xy")
+    grids = [extrude(X, Y)]
+    P0 = np.stack([a * np.ones_like(s), a * s], -1)                                  # the core's east side
+    P1 = np.stack([R * np.cos(s * np.pi / 4), R * np.sin(s * np.pi / 4)], -1)        # the rim arc facing it
+    N = (1 - r)[None, :, None] * P0[:, None, :] + r[None, :, None] * P1[:, None, :]  # (eta = s, xi = r, 2)
+    for q in range(4):
+        c, sn = np.cos(q * np.pi / 2), np.sin(q * np.pi / 2)
+        c, sn = round(c), round(sn)                                                  # exact quarter turns
+        grids.append(extrude(c * N[..., 0] - sn * N[..., 1], sn * N[..., 0] + c * N[..., 1]))
+    rng = np.random.default_rng(seed)
+    ph = rng.uniform(0.0, 2.0 * np.pi, size=(5, 3))
+    blocks = []
+    for b, (x, y, z) in enumerate(grids):
+        nj_, ni_ = x.shape[1] - 1, x.shape[2] - 1
+        bc = [5, 5, 5, 5, 0, 0] if b == 0 else [5, 2, 5, 5, 0, 0]
+        prm = _base_params(ni_, nj_, nk, periodic=[0, 0, 1], period=[[0, 0, 0], [0, 0, 0], [0, 0, Lz]], bc=bc,
+                           viscous=viscous, scheme=scheme, p_out=1.0 / GAMMA)
+        if viscous:
+            prm.update(mu_ref=0.3 * 1.0 / 200.0, t_ref=1.0 / GAMMA, s_suth=0.4 / GAMMA)
+        xc, yc, zc = cell_centres(x), cell_centres(y), cell_centres(z)
+        if uniform:
+            one = np.ones_like(xc)
+            prim = (one, 0.3 * one, 0.2 * one, -0.1 * one, one / GAMMA)
+        else:
+            f = lambda qq: np.sin(1.3 * xc + ph[qq, 0]) * np.cos(1.1 * yc + ph[qq, 1]) * np.sin(2 * np.pi * zc / Lz + ph[qq, 2])
+            prim = (1.0 + 0.05 * f(0), 0.3 * (1.0 + 0.1 * f(1)), 0.03 * f(2), 0.03 * f(3), (1.0 + 0.05 * f(4)) / GAMMA)
+        blocks.append(dict(name="butterfly_block%d" % b, params=prm, x=x, y=y, z=z, U0=conservative(*prim), dt=None,
+                           cfl=0.4, steps=3, t0=0.0))
+    return blocks
