@@ -128,6 +128,7 @@ static size_t carve(const meg6_params* p, const Consts& c, meg6_grid* g, char* b
   }
   G->stats = (unsigned long long*)take(2);
   G->red = take(4 * CFL_BLOCKS);
+  G->tp = take(16);
   return off;
 }
 
@@ -674,10 +675,10 @@ meg6_status meg6_rk3_steps(meg6_grid* g, double* U, double t, double dt, int nst
   CUDA_OK(launch_prim(g, U));
   int buf = 0, n0 = 0;
   // (stream capture is not available on the legacy default stream: callers that want the graph pass their own stream)
-  if (!g->p.moving && !g->prof_on && nsteps >= 4 && g->stream != nullptr && g->stream != cudaStreamLegacy &&
+  if (!g->prof_on && nsteps >= 4 && g->stream != nullptr && g->stream != cudaStreamLegacy &&
       g->stream != cudaStreamPerThread) {
-    // static mesh: two steps (six stages: the primitive buffers swap roles every stage) as one CUDA graph.  Small grids
-    // are bound by the launch rate of the host (config 1: 18 launches of ~5 us of work each per step)
+    // two steps (six stages: the primitive buffers swap roles every stage) as one CUDA graph.  Small grids are bound by the
+    // launch rate of the host (config 1: 18 launches of ~5 us of work each per step; config 2: 54 with the geometry)
     meg6_grid::GraphKey key;
     memset(&key, 0, sizeof(key));
     key.U = U; key.dt = dt; key.sigma = g->sigma; key.uref = g->uref; key.stats_on = g->stats_on;
@@ -689,7 +690,14 @@ meg6_status meg6_rk3_steps(meg6_grid* g, double* U, double t, double dt, int nst
       CUDA_OK(cudaStreamBeginCapture(g->stream, cudaStreamCaptureModeThreadLocal));
       meg6_status st = MEG6_OK;
       int b = 0;
-      for (int q = 0; q < 6 && st == MEG6_OK; ++q, b ^= 1) st = stage(g, b, make_fuse_rk(g, U, q % 3, dt, b, true));
+      for (int q = 0; q < 6 && st == MEG6_OK; ++q, b ^= 1) {
+        if (g->p.moving) {   // the geometry of stage q at ITS time: the two time factors are read from g->tp at replay
+          g->tp_cur = g->tp + 2 * q;
+          st = meg6_metrics_compute(g, 0.0);
+          g->tp_cur = nullptr;
+        }
+        if (st == MEG6_OK) st = stage(g, b, make_fuse_rk(g, U, q % 3, dt, b, true));
+      }
       const cudaError_t ec = cudaStreamEndCapture(g->stream, &graph);
       if (st != MEG6_OK) { if (graph) cudaGraphDestroy(graph); return st; }
       CUDA_OK(ec);
@@ -698,7 +706,21 @@ meg6_status meg6_rk3_steps(meg6_grid* g, double* U, double t, double dt, int nst
       CUDA_OK(ei);
       g->steps_key = key;
     }
-    for (; n0 + 2 <= nsteps; n0 += 2) CUDA_OK(cudaGraphLaunch(g->steps_graph, g->stream));
+    for (; n0 + 2 <= nsteps; n0 += 2) {
+      if (g->p.moving) {
+        // moving mesh: the stage times of these two steps, as the factors meg6_metrics_compute(t) forms on the host
+        // (same expressions, same bits); the copy is ordered after the previous replay on the stream
+        double tp[12];
+        for (int q = 0; q < 6; ++q) {
+          const double tn = t + (n0 + q / 3) * dt;
+          const double ts = (q % 3 == 0) ? tn : (q % 3 == 1) ? tn + dt : tn + 0.5 * dt;
+          const double ph = 2.0 * M_PI * g->p.omega * ts;
+          tp[2 * q] = sin(ph); tp[2 * q + 1] = 2.0 * M_PI * g->p.omega * cos(ph);
+        }
+        CUDA_OK(cudaMemcpyAsync(g->tp, tp, sizeof(tp), cudaMemcpyHostToDevice, g->stream));
+      }
+      CUDA_OK(cudaGraphLaunch(g->steps_graph, g->stream));
+    }
   }
   for (int n = n0; n < nsteps; ++n) {
     const double tn = t + n * dt;

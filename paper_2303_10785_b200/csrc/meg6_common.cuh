@@ -124,6 +124,8 @@ struct meg6_grid {
   int geom_launches;           // kernels launched by the last metrics_compute
   // meg6_rk3_steps on static meshes: the launches of two consecutive steps (the period of the primitive-buffer parity)
   // captured once as a CUDA graph and replayed; the key is what the captured kernel arguments depend on
+  double* tp;                  // 12 doubles: (sin, 2 pi omega cos) of the six stage times of a replayed two-step graph
+  const double* tp_cur;        // non-null while such a graph is captured: where k_centres reads its two numbers
   cudaGraphExec_t steps_graph;
   struct GraphKey { const double* U; double dt; const double* sigma; const double* uref; int stats_on; unsigned short* bm[3]; } steps_key;
   // per-kernel timing (meg6_profile_*): event pairs of the launches since the last read

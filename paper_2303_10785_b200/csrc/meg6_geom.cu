@@ -18,6 +18,7 @@ static GeomIn geom_in(meg6_grid* g, double t) {
   const double ph = 2.0 * M_PI * g->p.omega * t;
   gi.s = g->p.moving ? sin(ph) : 0.0;
   gi.sd = g->p.moving ? 2.0 * M_PI * g->p.omega * cos(ph) : 0.0;
+  gi.tp = g->tp_cur;   // set while a graph of meg6_rk3_steps is being captured: the two numbers come from device memory
   return gi;
 }
 

@@ -8,6 +8,7 @@ struct GeomIn {
   const double* node[3];
   const double* mode[3];
   double s, sd;   // sin(2 pi omega t), 2 pi omega cos(2 pi omega t)
+  const double* tp;   // or, if not null: the same two numbers in device memory (tp[0], tp[1]; replayed CUDA graphs)
 };
 
 // 8-vertex mean of node positions x0 + s*mode (vel == false) or node velocities sd*mode.
@@ -16,13 +17,14 @@ __device__ __forceinline__ double cell_mean(const Consts& c, const GeomIn& g, in
   const long long b = (long long)k * sk + (long long)j * sj + i;
   const long long o[8] = {0, 1, sj, sj + 1, sk, sk + 1, sk + sj, sk + sj + 1};
   double acc = 0.0;
+  const double gs = g.tp ? g.tp[0] : g.s, gsd = g.tp ? g.tp[1] : g.sd;
 #pragma unroll
   for (int q = 0; q < 8; ++q) {
     double v;
-    if (vel) v = g.sd * g.mode[comp][b + o[q]];
+    if (vel) v = gsd * g.mode[comp][b + o[q]];
     else {
       v = g.node[comp][b + o[q]];
-      if (c.moving) v = v + g.s * g.mode[comp][b + o[q]];
+      if (c.moving) v = v + gs * g.mode[comp][b + o[q]];
     }
     acc = (q == 0) ? v : acc + v;
   }
