@@ -85,7 +85,7 @@ def bytes_per_cell_stage(prm, sponge_frac):
     else:
         k["grad"] = GRAD_DOUBLES if v else 0
         base = nf + met + (SWEEP_GRAD_DOUBLES if v else 0)   # primitive tile, interface metrics, stored gradients
-    k["flux_eta"] = base + 5                        # first sweep: writes the residual
+    k["flux_eta"] = base + 5 + (ETA_GRAD_DOUBLES if (v and not ig) else 0)   # first sweep: writes the residual [+ its own gradients]
     k["flux_zeta"] = base + 5 + 5                   # reads and writes it
     # last sweep, fused with assembly + RK3 stage + primitives of the new state:
     # reads residual 5, U 5, U0 5 (stages 2-3), 1/J 1 [, (1/J)_t 1] [, sigma 1, Q_ref 5 where sigma != 0]; writes U 5,
@@ -97,9 +97,11 @@ def bytes_per_cell_stage(prm, sponge_frac):
     return {a: 8.0 * b for a, b in k.items()}
 
 
-# stored tangential gradients of the viscous flux (MEG6): k_grad reads (u,v,w,T) and writes 12 arrays; each sweep reads
-# the 8 arrays of its two tangential directions
-GRAD_DOUBLES = 4 + 12
+# stored tangential gradients of the viscous flux (MEG6): k_grad reads (u,v,w,T) and writes the 8 arrays of the xi and zeta
+# gradients, the eta sweep (first) writes the 4 arrays of the eta gradients it has in its tiles; each sweep reads the 8
+# arrays of its two tangential directions
+GRAD_DOUBLES = 4 + 8
+ETA_GRAD_DOUBLES = 4
 SWEEP_GRAD_DOUBLES = 8
 
 

@@ -556,11 +556,12 @@ static meg6_status stage_sweeps(meg6_grid* g, int buf, const Fuse3& fu) {
     for (int e = 0; e < 3; ++e)
       for (int f = 0; f < 4; ++f) G.p[4 * e + f] = g->G[e][f];
     ProfScope ps(g, 3, 1);
-    k_grad<<<dim3(nblk(c.LG.pi, 32), nblk(c.n[1] + 2, 8), nblk(c.n[2] + 2, GRAD_KB)), dim3(32, 8, 1), 0, g->stream>>>(c, P, G);
+    k_grad<<<dim3(nblk(c.LG.pi, 32), nblk(c.n[1] + 2, 8), nblk(c.n[2] + 2, GRAD_KB)), dim3(32, 8, 1), 0, g->stream>>>(c, P, G, 1);
   }
   CUDA_OK(cudaGetLastError());
   FluxIn3 i3;
   i3.res = g->res; i3.stats = g->stats_on ? g->stats : nullptr; i3.moving = g->p.moving ? 1 : 0; i3.mask = nullptr;
+  i3.gown = (g->p.viscous && !IG) ? g->G[1][0] : nullptr; i3.gfs = c.fsG;
   const bool V = g->p.viscous != 0;
   TmaMaps tm[3] = {g->tmaps3[buf][0], g->tmaps3[buf][1], g->tmaps3[buf][2]};
   if (fu.tail_tma) { tm[0].U = g->mapU; tm[0].U0 = g->mapU0; tm[0].J = g->mapJ; if (g->sigma) tm[0].Sg = g->mapSg; }

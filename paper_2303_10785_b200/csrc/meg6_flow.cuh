@@ -174,7 +174,9 @@ __device__ __forceinline__ double d1_op(const double* __restrict__ f, long long 
 // zeta stencil re-uses its loads in registers and the eta stencil of the block re-uses rows in L1
 // (ncu r1c: the one-cell-per-thread version was L1-wavefront bound with a 31 % L1 hit rate).
 constexpr int GRAD_KB = 4;   // cells per thread along zeta (2 and 8: +10 %, r2c)
-__global__ void __launch_bounds__(256, 4) k_grad(Consts c, P6 P, P12 G) {
+// eta_ghost_only: the eta gradients of the interior columns (0 <= i < ni, 0 <= k < nk) are stored by the eta sweep, which
+// has them in its tiles; here they are formed only in the ghost columns i = -1, ni and k = -1, nk, which no eta tile covers
+__global__ void __launch_bounds__(256, 4) k_grad(Consts c, P6 P, P12 G, int eta_ghost_only) {
   // i runs over the whole padded row of G (-GGI .. pitch-GGI): the cells beyond -1 and n are padding nobody reads, but
   // writing them makes every warp store start and end on a 32-byte sector (no partial-sector fills in L2/DRAM)
   const int i = blockIdx.x * 32 + threadIdx.x - GGI;
@@ -201,11 +203,12 @@ __global__ void __launch_bounds__(256, 4) k_grad(Consts c, P6 P, P12 G) {
       double* __restrict__ gy = G.p[4 + f];
       double* __restrict__ gz = G.p[8 + f];
       const double vx = d1_op(qq, 1);
-      const double vy = d1_op(qq, sj);
+      const bool need_y = !eta_ghost_only || i < 0 || i >= c.n[0] || k0 + m < 0 || k0 + m >= c.n[2];
       double r = CE1 * (z[m + 4] - z[m + 2]);
       r = fma(CE2, z[m + 5] - z[m + 1], r);
       r = fma(CE3, z[m + 6] - z[m], r);
-      if (ok) { gx[ag] = vx; gy[ag] = vy; gz[ag] = r; }
+      if (ok) { gx[ag] = vx; gz[ag] = r; }
+      if (ok && need_y) gy[ag] = d1_op(qq, sj);
     }
   }
 }

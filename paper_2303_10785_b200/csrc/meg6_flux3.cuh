@@ -79,6 +79,8 @@ struct FluxIn3 {
   double* res;                  // [5] running residual, layout LR, field stride fsR
   unsigned long long* stats;    // limiter counters or null
   unsigned short* mask;         // branch record of this family's interfaces (meg6_set_branch_masks) or null
+  double* gown;                 // eta sweep (MEG6, viscous): where it stores the eta gradients of (u,v,w,T) of its cells for
+  long long gfs;                // the later sweeps' tangential terms (field 0, layout LG, field stride gfs), or null
   int first, moving;
 };
 
@@ -645,6 +647,16 @@ k_flux3(const Consts c, const FluxIn3 in, const __grid_constant__ TmaMaps tm, co
       if (!FUSE) {
 #pragma unroll
         for (int f = 0; f < 5; ++f) in.res[f * c.fsR + ac] = R[f];
+        if (DIR == 1 && VISC && !IG4 && in.gown) {
+          // The E6 gradients along eta of (u, v, w, T) at this cell exist in the tile (P' = aL - aR, T'): they are the
+          // TANGENTIAL gradients of the zeta and xi sweeps that follow in this stage, so the stored-gradient kernel
+          // forms them only in the ghost columns no eta tile covers (gradients are shared, not recomputed)
+          const long long ag = c.LG.at(t0 + t, s0h + s, o);
+#pragma unroll
+          for (int f = 0; f < 3; ++f)
+            in.gown[f * in.gfs + ag] = sA[sidx3<DIR, TT>(f + 1, s + 2, t, LA)] - sA[sidx3<DIR, TT>(f + 6, s + 2, t, LA)];
+          in.gown[3 * in.gfs + ag] = sT1[sidx3<DIR, TT>(0, s + 1, t, LT)];
+        }
       } else {
         int ci, cj, ck;
         if (DIR == 0) { ci = s0h + s; cj = t0 + t; ck = o; }
