@@ -172,6 +172,18 @@ meg6_status meg6_stage_sweeps(meg6_grid* g, double* U, double* dUdt, int s, doub
  * Synchronises the stream.  *dt is a HOST pointer. */
 meg6_status meg6_cfl_dt(meg6_grid* g, const double* U, double cfl, double* dt);
 
+/* The same time step for callers that may not allocate and may not wait (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc): the partial minima of the reduction live in a file-scope
+ * `static __device__` array of the library (256 KiB on every GPU that loads libmeg6.so, held until exit) instead of the
+ * workspace, the reduction is finished on the device, and the result goes to *dt_device, a DEVICE pointer (one double)
+ * owned by the caller.  Two kernel launches on the grid's stream; no cudaMalloc / cudaFree / allocating library call, no
+ * copy to the host, no synchronisation.  Limit: grids of at most 16 777 216 = 2^24 cells (one pair of partial minima
+ * per 1024 cells, 16 384 pairs); larger grids get MEG6_EINVAL with a message that says so (use meg6_cfl_dt).  Other
+ * errors as meg6_cfl_dt.  The array is shared by every call on that GPU and keeps the last call's contents: a call
+ * overwrites every slot it reads (nothing has to start at zero), but calls that overlap on the GPU -- two grids on
+ * different streams, or the same grid from two threads -- race on it; callers serialise them. */
+meg6_status meg6_cfl_dt_noalloc(meg6_grid* g, const double* U, double cfl, double* dt_device);
+
 /* Volume-averaged kinetic energy and enstrophy of the state U (Eq. 54, written for three dimensions with
  * dV = 1/J; vorticity from the shared first gradients of the velocity) and the volume, at the geometry of the
  * last metrics_compute: out[0] = E_k, out[1] = enstrophy, out[2] = sum of 1/J.  out is a HOST pointer (3 doubles);

@@ -8,7 +8,8 @@ import os
 from . import build as _build
 
 EXPORTS = ["meg6_workspace_bytes", "meg6_grid_create", "meg6_grid_destroy", "meg6_metrics_compute",
-           "meg6_set_inflow", "meg6_set_sponge", "meg6_rhs", "meg6_rk3_step", "meg6_rk3_steps", "meg6_cfl_dt", "meg6_diagnostics",
+           "meg6_set_inflow", "meg6_set_sponge", "meg6_rhs", "meg6_rk3_step", "meg6_rk3_steps", "meg6_cfl_dt", "meg6_cfl_dt_noalloc",
+           "meg6_diagnostics",
            "meg6_limiter_stats_enable", "meg6_limiter_stats", "meg6_set_branch_masks", "meg6_get_array", "meg6_profile_enable",
            "meg6_profile_read", "meg6_fp64_peak", "meg6_last_error",
            "meg6_version", "meg6_link_blocks", "meg6_link_blocks_oriented", "meg6_metrics_compute_blocks", "meg6_rhs_blocks",
@@ -91,6 +92,8 @@ def lib():
         L.meg6_diagnostics.argtypes = [_vp, _vp, C.POINTER(C.c_double)]
         L.meg6_cfl_dt.restype = C.c_int
         L.meg6_cfl_dt.argtypes = [_vp, _vp, C.c_double, C.POINTER(C.c_double)]
+        L.meg6_cfl_dt_noalloc.restype = C.c_int
+        L.meg6_cfl_dt_noalloc.argtypes = [_vp, _vp, C.c_double, _vp]
         L.meg6_limiter_stats_enable.restype = C.c_int
         L.meg6_limiter_stats_enable.argtypes = [_vp, C.c_int]
         L.meg6_limiter_stats.restype = C.c_int
@@ -300,6 +303,14 @@ class Grid:
         dt = C.c_double()
         _check(lib().meg6_cfl_dt(self.h, U.data_ptr(), float(cfl), C.byref(dt)), "meg6_cfl_dt")
         return dt.value
+
+    def cfl_dt_noalloc(self, U, cfl, out):
+        """meg6_cfl_dt_noalloc: the time step into `out`, a one-element CUDA float64 tensor of the caller's (no
+        allocation, no host copy, no synchronisation; grids of at most 2^24 cells)"""
+        self._chk_state(U)
+        assert out.is_cuda and out.dtype == self.torch.float64 and out.numel() == 1
+        _check(lib().meg6_cfl_dt_noalloc(self.h, U.data_ptr(), float(cfl), out.data_ptr()), "meg6_cfl_dt_noalloc")
+        return out
 
     def limiter_stats_enable(self, on=True):
         _check(lib().meg6_limiter_stats_enable(self.h, int(on)), "meg6_limiter_stats_enable")

@@ -3,6 +3,7 @@
 #include <math.h>
 #include <stdio.h>
 #include <string.h>
+#include <mutex>
 #include <new>
 
 #include "meg6_common.cuh"
@@ -289,6 +290,93 @@ struct ProfScope {
   }
 };
 
+// ---- meg6_cfl_dt_noalloc: the time-step reduction with its scratch in a static device array (include/meg6.h) ----
+// One partial minimum pair per block of NOALLOC_CPB consecutive cells; the array holds NOALLOC_MAX_BLOCKS pairs, i.e.
+// grids of up to NOALLOC_MAX_CELLS cells.  256 KiB of device memory on every GPU that loads the library, until exit.
+// In HOST code the name g_noalloc_scratch is a stand-in for the symbol, not a device address: the address the kernels
+// get comes from cudaGetSymbolAddress, taken once per device at grid creation with that device current.
+constexpr int NOALLOC_CPB = 1024;                                   // cells per block (256 threads x 4)
+constexpr long long NOALLOC_MAX_CELLS = 1LL << 24;                  // 16 777 216 cells (config 4: 12.8 M; 256^3)
+constexpr int NOALLOC_MAX_BLOCKS = (int)(NOALLOC_MAX_CELLS / NOALLOC_CPB);
+static __device__ __align__(256) double g_noalloc_scratch[2 * NOALLOC_MAX_BLOCKS];
+
+// Eq. B.2 / B.3 per cell as in k_cfl; block b reduces cells [b CPB, (b+1) CPB) and writes its pair
+__global__ void __launch_bounds__(256) k_cfl_part(Consts c, const double* __restrict__ U, CflIn in, double* __restrict__ part) {
+  const long long N = c.LC.n;
+  double inv_min = INFINITY, vis_min = INFINITY;
+  const long long first = (long long)blockIdx.x * NOALLOC_CPB;
+  for (int q = 0; q < NOALLOC_CPB / 256; ++q) {
+    const long long tid = first + q * 256 + threadIdx.x;
+    if (tid >= N) break;
+    const int i = (int)(tid % c.n[0]), j = (int)((tid / c.n[0]) % c.n[1]), k = (int)(tid / ((long long)c.n[0] * c.n[1]));
+    const long long at = c.LX.at(i, j, k);
+    const double r = U[tid], u = U[N + tid] / r, v = U[2 * N + tid] / r, w = U[3 * N + tid] / r;
+    const double p = (c.gamma - 1.0) * (U[4 * N + tid] - 0.5 * r * (u * u + v * v + w * w));
+    const double cs = sqrt(c.gamma * p / r), J = 1.0 / in.rj[at];
+    const double mu = c.viscous ? sutherland(c, p / (r * c.r_gas)) : 0.0;
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      const double mx = J * in.met[3 * d][at], my = J * in.met[3 * d + 1][at], mz = J * in.met[3 * d + 2][at];
+      const double mtt = c.moving ? J * in.mt[d][at] : 0.0;
+      const double gn = sqrt(mx * mx + my * my + mz * mz);
+      inv_min = fmin(inv_min, 1.0 / (fabs(mtt + mx * u + my * v + mz * w) + cs * gn));
+      if (c.viscous) vis_min = fmin(vis_min, 1.0 / (mu * gn * gn));
+    }
+  }
+  __shared__ double sa[256], sb[256];
+  sa[threadIdx.x] = inv_min; sb[threadIdx.x] = vis_min;
+  __syncthreads();
+  for (int o = 128; o > 0; o >>= 1) {
+    if ((int)threadIdx.x < o) {
+      sa[threadIdx.x] = fmin(sa[threadIdx.x], sa[threadIdx.x + o]);
+      sb[threadIdx.x] = fmin(sb[threadIdx.x], sb[threadIdx.x + o]);
+    }
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) { part[2 * blockIdx.x] = sa[0]; part[2 * blockIdx.x + 1] = sb[0]; }
+}
+
+// the nb pairs of THIS call (the array keeps older calls' pairs beyond nb: they are not read) -> dt in device memory
+__global__ void __launch_bounds__(256) k_cfl_fin(const double* __restrict__ part, int nb, double cfl, int viscous,
+                                                 double* __restrict__ dt) {
+  double a = INFINITY, b = INFINITY;
+  for (int q = threadIdx.x; q < nb; q += 256) { a = fmin(a, part[2 * q]); b = fmin(b, part[2 * q + 1]); }
+  __shared__ double sa[256], sb[256];
+  sa[threadIdx.x] = a; sb[threadIdx.x] = b;
+  __syncthreads();
+  for (int o = 128; o > 0; o >>= 1) {
+    if ((int)threadIdx.x < o) {
+      sa[threadIdx.x] = fmin(sa[threadIdx.x], sa[threadIdx.x + o]);
+      sb[threadIdx.x] = fmin(sb[threadIdx.x], sb[threadIdx.x + o]);
+    }
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) {
+    double r = sa[0];
+    if (viscous) r = fmin(r, sb[0] / 4.0);   // R25: the alpha of Eq. B.3 read as alpha^D = 4
+    *dt = cfl * r;
+  }
+}
+
+// device address of the static scratch array on the CURRENT device, resolved once per device (set-up time)
+static cudaError_t noalloc_scratch_address(double** out) {
+  static double* addr[64] = {nullptr};
+  static std::mutex mu;
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
+  std::lock_guard<std::mutex> lock(mu);
+  if (!addr[dev]) {
+    double* ptr = nullptr;
+    e = cudaGetSymbolAddress((void**)&ptr, g_noalloc_scratch);
+    if (e != cudaSuccess) return e;
+    addr[dev] = ptr;
+  }
+  *out = addr[dev];
+  return cudaSuccess;
+}
+
 extern "C" {
 
 meg6_status meg6_profile_enable(meg6_grid* g, int on) {
@@ -359,6 +447,7 @@ meg6_status meg6_grid_create(const meg6_params* p, const double* x, const double
     if (e == cudaSuccess) e = cudaStreamSynchronize(g->stream);   // the host vectors go out of scope
   }
   if (e == cudaSuccess) e = setup_tma(g);
+  if (e == cudaSuccess) e = noalloc_scratch_address(&g->noalloc_scratch);   // set-up: this grid's device is current
   if (e != cudaSuccess) { delete g; return fail(MEG6_ECUDA, "grid_create: %s", cudaGetErrorString(e)); }
   *out = g;
   return MEG6_OK;
@@ -922,6 +1011,23 @@ meg6_status meg6_cfl_dt(meg6_grid* g, const double* U, double cfl, double* dt) {
   double r = a;
   if (g->p.viscous) r = fmin(r, b / 4.0);   // R25: the alpha of Eq. B.3 read as alpha^D = 4
   *dt = cfl * r;
+  return MEG6_OK;
+}
+
+meg6_status meg6_cfl_dt_noalloc(meg6_grid* g, const double* U, double cfl, double* dt_device) {
+  if (!g || !U || !dt_device) return fail(MEG6_EINVAL, "cfl_dt_noalloc: null pointer%s");
+  if (g->c.LC.n > NOALLOC_MAX_CELLS)
+    return fail(MEG6_EINVAL, "cfl_dt_noalloc: the grid has more cells than the static scratch array holds (maximum 16777216 = 2^24 cells; use meg6_cfl_dt)%s");
+  if (!g->have_metrics) return fail(MEG6_ESTATE, "cfl_dt_noalloc called before metrics_compute%s");
+  if (!g->noalloc_scratch) return fail(MEG6_ESTATE, "cfl_dt_noalloc: scratch address not resolved%s");
+  CflIn in;
+  for (int q = 0; q < 9; ++q) in.met[q] = g->met[q];
+  for (int q = 0; q < 3; ++q) in.mt[q] = g->mt[q];
+  in.rj = g->rj;
+  const int nb = (int)((g->c.LC.n + NOALLOC_CPB - 1) / NOALLOC_CPB);
+  k_cfl_part<<<nb, 256, 0, g->stream>>>(g->c, U, in, g->noalloc_scratch);
+  k_cfl_fin<<<1, 256, 0, g->stream>>>(g->noalloc_scratch, nb, cfl, g->p.viscous ? 1 : 0, dt_device);
+  CUDA_OK(cudaGetLastError());
   return MEG6_OK;
 }
 

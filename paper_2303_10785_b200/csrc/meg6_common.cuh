@@ -118,6 +118,7 @@ struct meg6_grid {
   unsigned long long* stats;   // [2] device counters: limited, tested
   unsigned short* bmask[3];    // caller's branch-record arrays per interface family (meg6_set_branch_masks) or null
   double* red;                 // reduction scratch
+  double* noalloc_scratch;     // device address of the library's static scratch array on this grid's device (meg6_cfl_dt_noalloc)
   int stats_on;
   bool have_metrics;
   int geom_blocked;            // -1 by size, 0 / 1 forced (MEG6_GEOM_BLOCKED in the environment at grid_create; tests)
