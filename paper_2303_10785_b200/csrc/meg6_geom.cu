@@ -3,9 +3,6 @@
 #include <cstring>
 #include <math.h>
 #include "meg6_geom.cuh"
-#ifndef MEG6_IG4_SEGMENTED
-#define MEG6_IG4_SEGMENTED 1
-#endif
 #include "meg6_ig4.cuh"
 
 namespace meg6 {
@@ -116,7 +113,7 @@ Box launch_ig4(meg6_grid* g, const Lay& L, const double* f, const Box& fb, int d
 Box launch_ig4_flow(meg6_grid* g, const Lay& L, const double* f, const Box& fb, int dir, double* out, int nfields,
                     long long fs_in, long long fs_out) {
   const int m = fb.hi[dir] - fb.lo[dir] - 4;
-  if (!MEG6_IG4_SEGMENTED || m - 2 > IG4S_NSEG * IG4S_SEGMAX || m < 3)
+  if (m - 2 > IG4S_NSEG * IG4S_SEGMAX || m < 3)
     return launch_ig4_batch(g, L, f, fb, dir, out, nfields, fs_in, fs_out);
   Box ob = fb;
   ob.lo[dir] += 2; ob.hi[dir] -= 2;
@@ -242,10 +239,8 @@ cudaError_t geom_rest(meg6_grid* g) {
   // same small grids)
   const bool blocked = g->geom_blocked >= 0 ? (g->geom_blocked == 1) : (c.LC.n >= (1LL << 21));
   g->geom_launches += 1 + 3 + 3 + (g->p.moving ? 1 : 0);   // coordinate derivatives, metric sweeps, interface families, GCL
-#if MEG6_CD_KB > 1
-  if (blocked) k_coord_deriv_blk<MEG6_CD_KB><<<nblk((long long)c.LX.pi * c.LX.pj * nblk(c.n[2] + 2 * GX, MEG6_CD_KB), T), T, 0, g->stream>>>(c, xc, cd, g->rj);
+  if (blocked) k_coord_deriv_blk<CD_KB><<<nblk((long long)c.LX.pi * c.LX.pj * nblk(c.n[2] + 2 * GX, CD_KB), T), T, 0, g->stream>>>(c, xc, cd, g->rj);
   else
-#endif
   k_coord_deriv<<<nblk(c.LX.n, T), T, 0, g->stream>>>(c, xc, cd, g->rj);
   {
     const int e0 = c.n[0] + 10, e1 = c.n[1] + 10, e2 = c.n[2] + 10;
@@ -262,8 +257,8 @@ cudaError_t geom_rest(meg6_grid* g) {
     if (d == 0 || !blocked) k_face_metrics<<<nblk(c.LF[d].n, T), T, 0, g->stream>>>(c, d, job);
     else {
       const Lay& LF = c.LF[d];
-      const long long nthr = (long long)LF.pi * nblk(d == 1 ? LF.pj : LF.pk, MEG6_FACE_KB) * (d == 1 ? LF.pk : LF.pj);
-      k_face_metrics_blk<MEG6_FACE_KB><<<nblk(nthr, T), T, 0, g->stream>>>(c, d, job);
+      const long long nthr = (long long)LF.pi * nblk(d == 1 ? LF.pj : LF.pk, FACE_KB) * (d == 1 ? LF.pk : LF.pj);
+      k_face_metrics_blk<FACE_KB><<<nblk(nthr, T), T, 0, g->stream>>>(c, d, job);
     }
   }
   if (g->p.moving) k_rjt<<<nblk(c.LC.n, T), T, 0, g->stream>>>(c, g->fmt[0], g->fmt[1], g->fmt[2], g->rjt);

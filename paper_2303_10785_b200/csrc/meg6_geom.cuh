@@ -221,9 +221,7 @@ __global__ void k_coord_deriv(Consts c, P3 xc, P9 cd, double* __restrict__ rj) {
 // block share their E6 gradients, second derivatives, one-sided states and interface values in registers (33 FP64
 // operations per derivative instead of 76 at KB = 6; the kernel is FP64-pipe-bound, ncu r1m); the xi and eta derivatives
 // are formed per cell as before.  Every value goes through the operations of delta_vals in its order (bit-identical).
-#ifndef MEG6_CD_KB
-#define MEG6_CD_KB 6
-#endif
+constexpr int CD_KB = 6;      // cells of a zeta column per thread (measured: 4 and 8 no better, r1m)
 template <int KB>
 __global__ void __launch_bounds__(256) k_coord_deriv_blk(Consts c, P3 xc, P9 cd, double* __restrict__ rj) {
   const int ext[3] = {c.n[0] + 2 * GX, c.n[1] + 2 * GX, c.n[2] + 2 * GX};
@@ -386,9 +384,7 @@ __global__ void k_face_metrics(Consts c, int d, FaceJob job) {
 // interfaces share the E6 gradients, second derivatives and one-sided states of their cells, which the thread keeps in
 // registers: 30 FP64 operations per interface instead of 56 at KB = 4 (k_face_metrics is FP64-pipe-bound, ncu r1m);
 // the operations on every value are those of H_vals, in its order (bit-identical results).  Lanes run along xi.
-#ifndef MEG6_FACE_KB
-#define MEG6_FACE_KB 6
-#endif
+constexpr int FACE_KB = 6;    // interfaces of a grid line per thread
 template <int KB>
 __global__ void __launch_bounds__(256) k_face_metrics_blk(Consts c, int d, FaceJob job) {
   const Lay& LF = c.LF[d];

@@ -18,6 +18,8 @@ pytestmark = [pytest.mark.gpu, pytest.mark.slow]
 
 
 def run_both(torch, O, M, wl, U0, steps, t0=0.0, dt=None, label=""):
+    import os
+    O.set_threads(os.cpu_count() or 1)          # these runs are minutes of oracle time: every host core
     og = O.Grid(wl)
     og.metrics_compute(t0)
     g = M.Grid(wl)
