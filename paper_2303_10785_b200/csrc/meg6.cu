@@ -607,6 +607,16 @@ static cudaError_t fill_ghosts_dir(meg6_grid* g, int buf, int d) {
 }
 
 static cudaError_t fill_ghosts(meg6_grid* g, int buf) {
+  const Consts& c = g->c;
+  if (c.periodic[0] && c.periodic[1] && c.periodic[2]) {   // all wraps: one launch (k_ghost_periodic)
+    P6 P;
+    for (int f = 0; f < 6; ++f) P.p[f] = buf ? g->Pb[f] : g->P[f];
+    const long long e0 = c.n[0] + 12, e1 = c.n[1] + 12;
+    const long long nthr = e0 * e1 * 12 + e0 * 12 * c.n[2] + 12LL * c.n[1] * c.n[2];
+    ProfScope ps(g, 2, 1);
+    k_ghost_periodic<<<nblk(nthr, 256), 256, 0, g->stream>>>(c, P);
+    return cudaGetLastError();
+  }
   for (int pass = 0; pass < (g->rotated ? 3 : 1); ++pass)
     for (int d = 0; d < 3; ++d) {
       const cudaError_t e = fill_ghosts_dir(g, buf, d);

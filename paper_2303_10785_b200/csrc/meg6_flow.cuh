@@ -138,6 +138,41 @@ __global__ void __launch_bounds__(256) k_ghost(Consts c, int d, P6 P, GhostIn in
   }
 }
 
+// B for a block that is periodic in all three directions (configs 1, 2, 3, 5): every ghost cell is the copy of the interior
+// cell at the wrapped index -- what the three direction-ordered passes of k_ghost produce, value for value -- in ONE
+// launch (the small configs are bound by launches: three ghost kernels were 45 % of a 32^3 stage).  One thread per
+// ghost cell: the zeta slabs over the whole padded (i, j) extent, the eta slabs over the padded i extent, the xi slabs.
+__global__ void __launch_bounds__(256) k_ghost_periodic(Consts c, P6 P) {
+  constexpr int NG = 6;
+  const int n0 = c.n[0], n1 = c.n[1], n2 = c.n[2];
+  const long long e0 = n0 + 2 * NG, e1 = n1 + 2 * NG;
+  const long long nz = e0 * e1 * (2 * NG), ny = e0 * (2 * NG) * n2, nx = (long long)(2 * NG) * n1 * n2;
+  long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  int i, j, k;
+  if (tid < nz) {
+    i = (int)(tid % e0) - NG; j = (int)((tid / e0) % e1) - NG;
+    const int q = (int)(tid / (e0 * e1));
+    k = q < NG ? q - NG : n2 + q - NG;
+  } else if ((tid -= nz) < ny) {
+    i = (int)(tid % e0) - NG;
+    const int q = (int)((tid / e0) % (2 * NG));
+    j = q < NG ? q - NG : n1 + q - NG;
+    k = (int)(tid / (e0 * 2 * NG));
+  } else if ((tid -= ny) < nx) {
+    const int q = (int)(tid % (2 * NG));
+    i = q < NG ? q - NG : n0 + q - NG;
+    j = (int)((tid / (2 * NG)) % n1); k = (int)(tid / ((long long)(2 * NG) * n1));
+  } else return;
+  const int si = i < 0 ? i + n0 : i >= n0 ? i - n0 : i, sj = j < 0 ? j + n1 : j >= n1 ? j - n1 : j,
+            sk = k < 0 ? k + n2 : k >= n2 ? k - n2 : k;
+  const long long src = c.LP.at(si, sj, sk), dst = c.LP.at(i, j, k);
+  double v[6];
+#pragma unroll
+  for (int f = 0; f < 6; ++f) v[f] = P.p[f][src];
+#pragma unroll
+  for (int f = 0; f < 6; ++f) P.p[f][dst] = v[f];
+}
+
 // Packed interface layers (meg6_stage_pack): the six cell layers of direction d next to one face, all six fields,
 // every transverse position of the padded primitive array.  The packed array is a padded layout itself: as LP, but
 // with 6 cells and no ghosts along d -- k_ghost reads it like a neighbour block that is six cells thick.
