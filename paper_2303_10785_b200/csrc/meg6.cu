@@ -655,7 +655,7 @@ static meg6_status stage_sweeps(meg6_grid* g, int buf, const Fuse3& fu) {
     for (int e = 0; e < 3; ++e)
       for (int f = 0; f < 4; ++f) G.p[4 * e + f] = g->G[e][f];
     ProfScope ps(g, 3, 1);
-    k_grad<<<dim3(nblk(c.LG.pi, 32), nblk(c.n[1] + 2, 8), nblk(c.n[2] + 2, GRAD_KB)), dim3(32, 8, 1), 0, g->stream>>>(c, P, G, 1);
+    k_grad<<<dim3(nblk(c.LG.pi / 2, 32), nblk(c.n[1] + 2, 8), nblk(c.n[2] + 2, GRAD_KB)), dim3(32, 8, 1), 0, g->stream>>>(c, P, G, 1);
   }
   CUDA_OK(cudaGetLastError());
   FluxIn3 i3;

@@ -203,47 +203,60 @@ __device__ __forceinline__ double d1_op(const double* __restrict__ f, long long 
   return r;
 }
 
-// G(b): stored gradients of (u,v,w,T) along xi, eta, zeta on cells [-1, n+1)^3 (viscous flux, Fig. 5 P:295;
+// G(b): stored gradients of (u,v,w,T) along xi and zeta on cells [-1, n+1)^3 (viscous flux, Fig. 5 P:295;
 // R18: T is differentiated with the same E6 scheme).  G.p[4*e + f].
-// A block of 32 x 8 threads covers 32 x 8 x GRAD_KB cells: each thread walks GRAD_KB cells along zeta, so the
-// zeta stencil re-uses its loads in registers and the eta stencil of the block re-uses rows in L1
-// (ncu r1c: the one-cell-per-thread version was L1-wavefront bound with a 31 % L1 hit rate).
+// A thread takes TWO xi-neighbouring cells (an aligned pair: every load and store is 16 bytes wide) and walks GRAD_KB cells
+// along zeta: the zeta stencil re-uses its loads in registers, the xi stencils of the pair share one ten-value window
+// (4 + 1 wide loads instead of 12 narrow ones; ncu r2: the one-cell form was bound by L1 wavefronts, 66-72 %, half of its
+// instructions address arithmetic around 8.5 loads per value).  A block of 32 x 8 threads covers 64 x 8 x GRAD_KB cells.
+// The eta gradients of the interior columns (0 <= i < ni, 0 <= k < nk) are stored by the eta sweep, which has them in its
+// tiles; with eta_ghost_only they are formed here only in the ghost columns i = -1, ni and k = -1, nk, which no eta tile covers.
 constexpr int GRAD_KB = 4;   // cells per thread along zeta (2 and 8: +10 %, r2c)
-// eta_ghost_only: the eta gradients of the interior columns (0 <= i < ni, 0 <= k < nk) are stored by the eta sweep, which
-// has them in its tiles; here they are formed only in the ghost columns i = -1, ni and k = -1, nk, which no eta tile covers
-__global__ void __launch_bounds__(256, 4) k_grad(Consts c, P6 P, P12 G, int eta_ghost_only) {
+__device__ __forceinline__ double e6_vals(double m3, double m2, double m1, double p1, double p2, double p3) {   // as d1_op
+  double r = CE1 * (p1 - m1);
+  r = fma(CE2, p2 - m2, r);
+  r = fma(CE3, p3 - m3, r);
+  return r;
+}
+__global__ void __launch_bounds__(256, 3) k_grad(Consts c, P6 P, P12 G, int eta_ghost_only) {
   // i runs over the whole padded row of G (-GGI .. pitch-GGI): the cells beyond -1 and n are padding nobody reads, but
   // writing them makes every warp store start and end on a 32-byte sector (no partial-sector fills in L2/DRAM)
-  const int i = blockIdx.x * 32 + threadIdx.x - GGI;
+  const int i0 = 2 * (blockIdx.x * 32 + threadIdx.x) - GGI;     // even: the pair (i0, i0 + 1) is 16-byte aligned in P and G
   const int j = blockIdx.y * 8 + threadIdx.y - 1;
   const int k0 = blockIdx.z * GRAD_KB - 1;
-  if (i >= c.LG.pi - GGI || j > c.n[1]) return;
+  if (i0 >= c.LG.pi - GGI || j > c.n[1]) return;
   const long long sj = c.LP.sj, sk = c.LP.sk;
-  const long long ap0 = c.LP.at(i, j, k0), ag0 = c.LG.at(i, j, k0);
+  const long long ap0 = c.LP.at(i0, j, k0), ag0 = c.LG.at(i0, j, k0);
 #pragma unroll
   for (int f = 0; f < 4; ++f) {
     const double* __restrict__ q = P.p[(f < 3) ? f + 1 : 5] + ap0;
-    double z[GRAD_KB + 6];
+    double2 z[GRAD_KB + 6];
 #pragma unroll
-    for (int m = 0; m < GRAD_KB + 6; ++m) z[m] = (k0 + m - 3 <= c.n[2] + 3) ? q[(m - 3) * sk] : 0.0;
+    for (int m = 0; m < GRAD_KB + 6; ++m)
+      z[m] = (k0 + m - 3 <= c.n[2] + 3) ? *reinterpret_cast<const double2*>(q + (m - 3) * sk) : make_double2(0.0, 0.0);
 #pragma unroll
     for (int m = 0; m < GRAD_KB; ++m) {
       // no early exit: the planes beyond n+1 are inside the 6-deep ghost padding of P, only the stores are guarded, so
-      // the loads of the next cells can be issued before the stores of this one (the kernel was a chain of 16
-      // load-wait-store rounds per thread)
+      // the loads of the next cells can be issued before the stores of this one
       const bool ok = k0 + m <= c.n[2];
       const double* __restrict__ qq = q + m * sk;
       const long long ag = ag0 + m * c.LG.sk;
-      double* __restrict__ gx = G.p[f];
-      double* __restrict__ gy = G.p[4 + f];
-      double* __restrict__ gz = G.p[8 + f];
-      const double vx = d1_op(qq, 1);
-      const bool need_y = !eta_ghost_only || i < 0 || i >= c.n[0] || k0 + m < 0 || k0 + m >= c.n[2];
-      double r = CE1 * (z[m + 4] - z[m + 2]);
-      r = fma(CE2, z[m + 5] - z[m + 1], r);
-      r = fma(CE3, z[m + 6] - z[m], r);
-      if (ok) { gx[ag] = vx; gz[ag] = r; }
-      if (ok && need_y) gy[ag] = d1_op(qq, sj);
+      const double2 a = *reinterpret_cast<const double2*>(qq - 4), b = *reinterpret_cast<const double2*>(qq - 2),
+                    d = *reinterpret_cast<const double2*>(qq + 2), e = *reinterpret_cast<const double2*>(qq + 4);
+      const double2 cc = z[m + 3];
+      double2 vx, vz;
+      vx.x = e6_vals(a.y, b.x, b.y, cc.y, d.x, d.y);
+      vx.y = e6_vals(b.x, b.y, cc.x, d.x, d.y, e.x);
+      vz.x = e6_vals(z[m].x, z[m + 1].x, z[m + 2].x, z[m + 4].x, z[m + 5].x, z[m + 6].x);
+      vz.y = e6_vals(z[m].y, z[m + 1].y, z[m + 2].y, z[m + 4].y, z[m + 5].y, z[m + 6].y);
+      if (ok) {
+        *reinterpret_cast<double2*>(G.p[f] + ag) = vx;
+        *reinterpret_cast<double2*>(G.p[8 + f] + ag) = vz;
+        const bool kg = k0 + m < 0 || k0 + m >= c.n[2];
+#pragma unroll
+        for (int h = 0; h < 2; ++h)
+          if (!eta_ghost_only || kg || i0 + h < 0 || i0 + h >= c.n[0]) G.p[4 + f][ag + h] = d1_op(qq + h, sj);
+      }
     }
   }
 }
