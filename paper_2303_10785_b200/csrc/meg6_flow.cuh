@@ -218,7 +218,7 @@ __device__ __forceinline__ double e6_vals(double m3, double m2, double m1, doubl
   r = fma(CE3, p3 - m3, r);
   return r;
 }
-__global__ void __launch_bounds__(256, 3) k_grad(Consts c, P6 P, P12 G, int eta_ghost_only) {
+__global__ void __launch_bounds__(256, 4) k_grad(Consts c, P6 P, P12 G, int eta_ghost_only) {
   // i runs over the whole padded row of G (-GGI .. pitch-GGI): the cells beyond -1 and n are padding nobody reads, but
   // writing them makes every warp store start and end on a 32-byte sector (no partial-sector fills in L2/DRAM)
   const int i0 = 2 * (blockIdx.x * 32 + threadIdx.x) - GGI;     // even: the pair (i0, i0 + 1) is 16-byte aligned in P and G
