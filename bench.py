@@ -105,6 +105,23 @@ ETA_GRAD_DOUBLES = 4
 SWEEP_GRAD_DOUBLES = 8
 
 
+def default_develop(wl, wl_name, develop):
+    """untimed steps that advance the flow before the timed ones: half of the config's step count for the jet"""
+    return develop if develop is not None else (wl["steps"] // 2 if wl_name.startswith("c4_jet") else 0)
+
+
+def make_config(wl, wl_name, prm, cells, dt, world, slabs, develop, warmup):
+    """The `config` object of the JSON line: the workload BASELINE.json's metric is quoted on.  Both arms print the same
+    object (the reference arm times a bounded sample of it and says so in `cpu_baseline.sample`)."""
+    stage_bytes = sum(bytes_per_cell_stage(prm, sponge_fraction(wl)).values())
+    return {"workload": wl_name, "cells": cells, "viscous": prm["viscous"], "moving": prm["moving"],
+            "scheme": "MIG4" if prm.get("scheme", 0) == 1 else "MEG6", "dt": dt,
+            "parallelism": ("zeta slabs x%d, 6-layer halo exchange per stage" if slabs else "replicas x%d") % world,
+            "l2": "working set %.1f GB per stage >> 126 MB L2 (no flush needed)" % (stage_bytes * cells / max(world if slabs else 1, 1) / 1e9),
+            "state": "timed after %d untimed steps of the config's %s-step run (warm-up included)" % (
+                max(develop, warmup), wl.get("steps"))}
+
+
 def sponge_fraction(wl):
     sg = wl.get("sigma")
     return None if sg is None else float(np.count_nonzero(sg)) / sg.size
@@ -215,6 +232,17 @@ def cpu_baseline():
     return rec
 
 
+def ref_config(args):
+    """our arm's `config` for the default workload (no GPU needed: the jet has a fixed dt)"""
+    wl = W.c4_jet(ni=20, nj=20, nk=20)               # parameters and step count only; the sizes are set below
+    full = dict(ni=320, nj=200, nk=200)
+    prm = dict(wl["params"], **full)
+    name = "c4_jet_%dx%dx%d" % (full["ni"], full["nj"], full["nk"])
+    sg = W.c4_jet(**SAMPLE)                           # sponge fraction of the sample mesh (same relative layer widths)
+    return make_config(dict(wl, sigma=sg["sigma"]), name, prm, full["ni"] * full["nj"] * full["nk"], wl["dt"], 1, False,
+                       default_develop(wl, name, args.develop), max(args.warmup, 3))
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -232,7 +260,7 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": "c4_jet_320x200x200", "sample": base["sample"]},
+            "config": ref_config(args),
             "cpu_baseline": base,
             "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line))
@@ -334,7 +362,7 @@ def run_ours(args):
     # form: the MP limiter's slow path, almost idle at t = 0, costs more and more.  The timed
     # steps are therefore taken in the MIDDLE of the config's run (after `develop` untimed steps); the throughput of
     # the first steps is reported beside it as `startup`.
-    develop = args.develop if args.develop is not None else (wl["steps"] // 2 if wl_name.startswith("c4_jet") else 0)
+    develop = default_develop(wl, wl_name, args.develop)
     startup = None
     if develop > 0:
         barrier()
@@ -433,10 +461,7 @@ def run_ours(args):
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
             "scaling": "strong" if slabs else "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": wl_name, "cells": ncell_job if slabs else ncell, "viscous": prm["viscous"], "moving": prm["moving"],
-                       "scheme": "MIG4" if prm.get("scheme", 0) == 1 else "MEG6",
-                       "dt": dt, "parallelism": ("zeta slabs x%d, 6-layer halo exchange per stage" if slabs else "replicas x%d") % world,
-                       "l2": "working set %.1f GB per stage >> 126 MB L2 (no flush needed)" % (stage_bytes * ncell / 1e9)},
+            "config": make_config(wl, wl_name, prm, ncell_job if slabs else ncell, dt, world, slabs, develop, args.warmup),
             "clocks": clocks, "gpu_launches": int(launches), "finite": finite,
             "profiled_ms_per_step": ms_prof / args.steps, "inputs_sha256": input_hashes(wl),
             "sponge_cell_fraction": sponge_fraction(wl),
@@ -448,8 +473,6 @@ def run_ours(args):
                                   "frac": stage_bytes * ncell_job * 3 * args.steps / (ms * 1e-3) / 1e9 / world / hbm,
                                   "peak": hbm, "peak_source": peak_src},
             "kernels": kernels}
-    line["config"]["state"] = "timed after %d untimed steps of the config's %s-step run (warm-up included)" % (
-        max(develop, args.warmup), wl.get("steps"))
     if startup is not None:
         line["startup"] = {"value": whole_job_throughput(ncell_job / world, args.steps, world, startup), "unit": UNIT,
                            "ms_per_step": startup / args.steps,
