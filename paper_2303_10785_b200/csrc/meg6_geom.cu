@@ -36,6 +36,14 @@ cudaError_t geom_extend(meg6_grid* g, int d) {
   const Consts& c = g->c;
   P3 xc, xt;
   for (int q = 0; q < 3; ++q) { xc.p[q] = g->xc[q]; xt.p[q] = g->xt[q]; }
+  if (c.periodic[0] && c.periodic[1] && c.periodic[2]) {   // all wraps: the three passes as one launch, at d == 0
+    if (d != 0) return cudaSuccess;
+    const long long e0 = c.n[0] + 2 * GX, e1 = c.n[1] + 2 * GX;
+    const long long nthr = e0 * e1 * 2 * GX + e0 * 2 * GX * c.n[2] + 2LL * GX * c.n[1] * c.n[2];
+    k_extend_periodic<<<nblk(nthr, 256), 256, 0, g->stream>>>(c, xc, xt);
+    ++g->geom_launches;
+    return cudaGetLastError();
+  }
   ExtIn in;
   memset(&in, 0, sizeof(in));
   for (int side = 0; side < 2; ++side) {
@@ -238,7 +246,7 @@ cudaError_t geom_rest(meg6_grid* g) {
   // MEG6_GEOM_BLOCKED=0/1 in the environment at grid_create forces the choice (the parity tests run both forms on the
   // same small grids)
   const bool blocked = g->geom_blocked >= 0 ? (g->geom_blocked == 1) : (c.LC.n >= (1LL << 21));
-  g->geom_launches += 1 + 3 + 3 + (g->p.moving ? 1 : 0);   // coordinate derivatives, metric sweeps, interface families, GCL
+  g->geom_launches += 1 + 3 + (blocked ? 3 : 1) + (g->p.moving ? 1 : 0);   // coordinate derivatives, metric sweeps, interface families, GCL
   if (blocked) k_coord_deriv_blk<CD_KB><<<nblk((long long)c.LX.pi * c.LX.pj * nblk(c.n[2] + 2 * GX, CD_KB), T), T, 0, g->stream>>>(c, xc, cd, g->rj);
   else
   k_coord_deriv<<<nblk(c.LX.n, T), T, 0, g->stream>>>(c, xc, cd, g->rj);
@@ -248,13 +256,22 @@ cudaError_t geom_rest(meg6_grid* g) {
     k_met_dir<1><<<dim3(nblk(e0, MetCfg<1>::TW), nblk(e1, MetCfg<1>::TS), e2), 256, 0, g->stream>>>(c, xc, xt, cd, met, mt);
     k_met_dir<2><<<dim3(nblk(e0, MetCfg<2>::TW), nblk(e2, MetCfg<2>::TS), e1), 256, 0, g->stream>>>(c, xc, xt, cd, met, mt);
   }
+  FaceJob3 jobs;
   for (int d = 0; d < 3; ++d) {
-    FaceJob job;
+    FaceJob& job = jobs.job[d];
     job.n = 0;
     for (int q = 0; q < 10; ++q)
       if (g->fmet[d][q]) { job.src[job.n] = (q < 9) ? g->met[q] : g->rj; job.dst[job.n] = g->fmet[d][q]; ++job.n; }
     if (g->p.moving) { job.src[job.n] = g->mt[d]; job.dst[job.n] = g->fmt[d]; ++job.n; }
-    if (d == 0 || !blocked) k_face_metrics<<<nblk(c.LF[d].n, T), T, 0, g->stream>>>(c, d, job);
+  }
+  if (!blocked) {
+    long long nmax = c.LF[0].n;
+    for (int d = 1; d < 3; ++d) nmax = c.LF[d].n > nmax ? c.LF[d].n : nmax;
+    k_face_metrics3<<<dim3(nblk(nmax, T), 3), T, 0, g->stream>>>(c, jobs);
+  }
+  for (int d = 0; d < 3 && blocked; ++d) {
+    const FaceJob& job = jobs.job[d];
+    if (d == 0) k_face_metrics<<<nblk(c.LF[d].n, T), T, 0, g->stream>>>(c, d, job);
     else {
       const Lay& LF = c.LF[d];
       const long long nthr = (long long)LF.pi * nblk(d == 1 ? LF.pj : LF.pk, FACE_KB) * (d == 1 ? LF.pk : LF.pj);

@@ -110,6 +110,43 @@ __global__ void __launch_bounds__(256) k_extend(Consts c, int d, P3 xc, P3 xt, E
   }
 }
 
+// M1b for a block that is periodic in all three directions: every ghost cell centre in ONE launch.  The three
+// direction-ordered passes give  ((interior -+ period_xi) -+ period_eta) -+ period_zeta  with the offsets of the directions
+// in which the index wrapped, added in that order; the same additions in the same order here (bit-identical), velocities
+// plain copies.  One thread per ghost cell: zeta slabs over the padded (i, j) extent, eta slabs over padded i, xi slabs.
+__global__ void __launch_bounds__(256) k_extend_periodic(Consts c, P3 xc, P3 xt) {
+  const int n0 = c.n[0], n1 = c.n[1], n2 = c.n[2];
+  const long long e0 = n0 + 2 * GX, e1 = n1 + 2 * GX;
+  const long long nz = e0 * e1 * (2 * GX), ny = e0 * (2 * GX) * n2, nx = (long long)(2 * GX) * n1 * n2;
+  long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  int i, j, k;
+  if (tid < nz) {
+    i = (int)(tid % e0) - GX; j = (int)((tid / e0) % e1) - GX;
+    const int q = (int)(tid / (e0 * e1));
+    k = q < GX ? q - GX : n2 + q - GX;
+  } else if ((tid -= nz) < ny) {
+    i = (int)(tid % e0) - GX;
+    const int q = (int)((tid / e0) % (2 * GX));
+    j = q < GX ? q - GX : n1 + q - GX;
+    k = (int)(tid / (e0 * 2 * GX));
+  } else if ((tid -= ny) < nx) {
+    const int q = (int)(tid % (2 * GX));
+    i = q < GX ? q - GX : n0 + q - GX;
+    j = (int)((tid / (2 * GX)) % n1); k = (int)(tid / ((long long)(2 * GX) * n1));
+  } else return;
+  const int wi = i < 0 ? -1 : i >= n0 ? 1 : 0, wj = j < 0 ? -1 : j >= n1 ? 1 : 0, wk = k < 0 ? -1 : k >= n2 ? 1 : 0;
+  const long long src = c.LX.at(i - wi * n0, j - wj * n1, k - wk * n2), dst = c.LX.at(i, j, k);
+#pragma unroll
+  for (int comp = 0; comp < 3; ++comp) {
+    double v = xc.p[comp][src];
+    if (wi) v = wi > 0 ? v + c.period[0][comp] : v - c.period[0][comp];
+    if (wj) v = wj > 0 ? v + c.period[1][comp] : v - c.period[1][comp];
+    if (wk) v = wk > 0 ? v + c.period[2][comp] : v - c.period[2][comp];
+    xc.p[comp][dst] = v;
+    if (c.moving) xt.p[comp][dst] = xt.p[comp][src];
+  }
+}
+
 // Packed cell-centre layers of one face (meg6_stage_geom_pack): the ten layers of direction d next to the face over the
 // whole padded transverse extent, coordinates (and grid velocities).  The packed array is a padded layout itself: LX
 // with ten cells and no ghosts along d; k_extend of the receiving block reads it like a neighbour ten cells thick.
@@ -377,6 +414,20 @@ __global__ void k_face_metrics(Consts c, int d, FaceJob job) {
   if (tid >= LF.n) return;
   const int i = (int)(tid % LF.pi), j = (int)((tid / LF.pi) % LF.pj), k = (int)(tid / LF.sk);
   const long long at = c.LX.at(i, j, k), s = c.LX.stride(d);
+  for (int q = 0; q < job.n; ++q) job.dst[q][tid] = H_op(job.src[q] + at, s);
+}
+
+// M4, the three families in one launch (blockIdx.y = family): on small grids each family alone is less than one wave of
+// CTAs (64^3: 1040 of 1184 slots, three launches of 10 us each)
+struct FaceJob3 { FaceJob job[3]; };
+__global__ void k_face_metrics3(Consts c, FaceJob3 jobs) {
+  const int d = blockIdx.y;
+  const Lay& LF = c.LF[d];
+  const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (tid >= LF.n) return;
+  const int i = (int)(tid % LF.pi), j = (int)((tid / LF.pi) % LF.pj), k = (int)(tid / LF.sk);
+  const long long at = c.LX.at(i, j, k), s = c.LX.stride(d);
+  const FaceJob& job = jobs.job[d];
   for (int q = 0; q < job.n; ++q) job.dst[q][tid] = H_op(job.src[q] + at, s);
 }
 
