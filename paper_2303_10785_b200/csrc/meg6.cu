@@ -775,7 +775,7 @@ meg6_status meg6_rk3_steps(meg6_grid* g, double* U, double t, double dt, int nst
   CUDA_OK(launch_prim(g, U));
   int buf = 0, n0 = 0;
   // (stream capture is not available on the legacy default stream: callers that want the graph pass their own stream)
-  if (!g->prof_on && nsteps >= 4 && g->stream != nullptr && g->stream != cudaStreamLegacy &&
+  if (!g->prof_on && nsteps >= 2 && g->stream != nullptr && g->stream != cudaStreamLegacy &&
       g->stream != cudaStreamPerThread) {
     // two steps (six stages: the primitive buffers swap roles every stage) as one CUDA graph.  Small grids are bound by the
     // launch rate of the host (config 1: 18 launches of ~5 us of work each per step; config 2: 54 with the geometry)
