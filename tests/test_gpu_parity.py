@@ -807,7 +807,7 @@ def test_c3_full_size_conservation_and_symmetry_of_the_step(mods):
 def test_full_step_counts_of_configs_3_4_5_stay_finite_and_bounded(mods):
     """BASELINE.json's step counts at full size on the GPU: config 3 (128^3, 200 RK3 steps), config 4 (320x200x200,
     500 steps: the jet starts up, shocks form at the nozzle lip, the limiter becomes active) and the MIG4 variant
-    (config 5's flow at 192^3, 50 steps).  The oracle would need hours for these; the checks are properties: finite
+    (config 5 in full: 384^3, 50 steps).  The oracle would need hours for these; the checks are properties: finite
     state, positive density and pressure, kinetic energy of the Taylor-Green vortex decaying."""
     torch, O, M = mods
 
@@ -832,7 +832,7 @@ def test_full_step_counts_of_configs_3_4_5_stay_finite_and_bounded(mods):
 
     ke0, ke1, _ = run(W.c3_tgv(n=128), 200)
     assert 0.9 * ke0 < ke1 < ke0
-    ke0, ke1, _ = run(W.c5_tgv_mig4(n=192), 50)
+    ke0, ke1, _ = run(W.c5_tgv_mig4(n=384), 50)      # config 5 at its own size: 56.6 M cells, 50 GB of workspace
     assert 0.95 * ke0 < ke1 < ke0
     ke0, ke1, frac = run(W.c4_jet(), 500)
     assert ke1 > ke0                     # the jet has entered the quiescent domain
