@@ -104,3 +104,15 @@ def test_mig4_128_20_steps(mods):
     Ug, Uo, rep, touched, hist = run_both(torch, O, M, wl, wl["U0"], 20, label="c5 mig4 128^3")
     e = rel(Ug, Uo)
     assert np.all(e <= STEP_TOL), e
+
+
+def test_mig4_256_3_steps(mods):
+    """Config 5's scheme and flow at 256^3 (the middle of its 128^3..384^3 sweep; at 384^3 the oracle's arrays alone
+    would take tens of GB of host memory): geometry of the implicit scheme on 16.8 M cells, dQ/dt and three RK3 steps,
+    every cell."""
+    torch, O, M = mods
+    wl = W.c5_tgv_mig4(n=256, steps=3)
+    Ug, Uo, rep, touched, hist = run_both(torch, O, M, wl, wl["U0"], 3, label="c5 mig4 256^3")
+    e = rel(Ug, Uo)
+    assert np.all(e <= STEP_TOL), e
+    assert rep["e1_flips"] + rep["hllc_flips"] <= 20, rep
