@@ -122,36 +122,41 @@ def test_mig4_256_3_steps(mods):
 def test_c4_full_config_all_500_steps(mods):
     """Config 4 exactly as BASELINE.json states it: 320 x 200 x 200, all 500 RK3 steps from the initial state, GPU against
     the oracle, every cell (north_star: "1e-9 after the config's step count").  Not part of the default `-m gpu` run (the
-    oracle needs about 18 s per step on 16 cores); the result of the run made in round 2 is in profiles/r2_c4_500_steps.md.
+    oracle needs about 13 s per step on 16 cores, and one call on the GPU pool is limited to an hour: round 2 ran it in two
+    legs, steps 1-250 from the initial state and steps 251-500 from the GPU's state at step 250 -- MEG6_LONG_START=250
+    MEG6_LONG_STEPS=250); the results are in profiles/r2_c4_500_steps.md.
     Progress goes to MEG6_LONG_LOG (a line every 25 steps), so an interrupted run still leaves its numbers."""
     import os
     torch, O, M = mods
     O.set_threads(os.cpu_count() or 1)
     wl = W.c4_jet()
     steps = int(os.environ.get("MEG6_LONG_STEPS", "500"))
-    log = os.environ.get("MEG6_LONG_LOG")
+    start = int(os.environ.get("MEG6_LONG_START", "0"))       # > 0: the GPU advances that many steps first, then both sides
+    log = os.environ.get("MEG6_LONG_LOG")                     # continue from ITS state (a run in two legs)
     og = O.Grid(wl)
     og.metrics_compute(0.0)
     g = M.Grid(wl)
     g.metrics_compute(0.0)
+    U = torch.as_tensor(wl["U0"], device="cuda").contiguous()
+    dt = wl["dt"]
+    for s in range(start):
+        g.rk3_step(U, s * dt, dt)
+    Uo = U.cpu().numpy().copy()
     g.limiter_stats_enable(True)
     g.branch_masks_enable(True)
     og.branch_masks_enable(True)
-    Uo = wl["U0"].copy()
-    U = torch.as_tensor(wl["U0"], device="cuda").contiguous()
-    dt = wl["dt"]
     lo0 = lg0 = 0
     worst = np.zeros(5)
     ndiff = 0
     t0 = time.time()
-    for s in range(steps):
+    for s in range(start, start + steps):
         og.rk3_step(Uo, s * dt, dt)
         g.rk3_step(U, s * dt, dt)
         lo, to = og.limiter_stats()
         lg, tg = g.limiter_stats()
         assert tg == to
         ndiff += int((lo - lo0) != (lg - lg0))
-        if (s + 1) % 25 == 0 or s + 1 == steps:
+        if (s + 1) % 25 == 0 or s + 1 == start + steps:
             e = rel(U.cpu().numpy(), Uo)
             worst = np.maximum(worst, e)
             rep, _ = flip_report(g, og, wl["U0"].shape[1:])
