@@ -171,3 +171,15 @@ def test_c4_full_config_all_500_steps(mods):
             assert np.all(e <= STEP_TOL), (s + 1, e)
         lo0, lg0 = lo, lg
     g.close()
+
+
+@pytest.mark.skipif(not __import__("os").environ.get("MEG6_LONG"), reason="15 minutes of CPU oracle: set MEG6_LONG=1")
+def test_mig4_256_all_50_steps(mods):
+    """Config 5's scheme, flow and STEP COUNT (50) at 256^3 -- the largest grid of its sweep whose oracle arrays fit the
+    host comfortably (384^3 would need tens of GB).  Result of the round-2 run in profiles/r2_c4_500_steps.md."""
+    torch, O, M = mods
+    wl = W.c5_tgv_mig4(n=256, steps=50)
+    Ug, Uo, rep, touched, hist = run_both(torch, O, M, wl, wl["U0"], 50, label="c5 mig4 256^3 x 50")
+    e = rel(Ug, Uo)
+    assert np.all(e <= STEP_TOL), e
+    assert rep["e1_flips"] + rep["hllc_flips"] <= 20, rep
