@@ -14,7 +14,9 @@
  * fixes the choice; oracle and CUDA path simply share the reading):
  *   - eigenvector averaging state (R5), MP alpha value (R7), tangential viscous gradients (R11),
  *     un-hatted interface metrics (R12), Sutherland constants (R15), sponge form (R16),
- *     inflow/outflow ghost rules (R20), the VALUE of the alpha in Eq. B.3 (R25; the formula around it is pinned),
+ *     WHICH inflow/outflow ghost rules the garbled Table 1 meant (R20; the rules as read are pinned: the box is the
+ *     inner part of a longer periodic box holding the ghost states, tests/test_oracle_inout.py),
+ *     the VALUE of the alpha in Eq. B.3 (R25; the formula around it is pinned),
  *     the cell whose metrics give the wall normal of the inviscid-wall rule (R27),
  *     where the IG4 line systems of the MIG4 variant end and how they are closed (R26):
  *     parity unpinned.

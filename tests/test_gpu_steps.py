@@ -48,7 +48,7 @@ def run_both(torch, O, M, wl, U0, steps, t0=0.0, dt=None, label=""):
         lo0, lg0, to0, tg0 = lo, lg, to, tg
         if s in (0, 1, 4, 9, 19, 49, 99, 199) or s == steps - 1:
             print("%s step %d: rel %s, limited this step oracle %d gpu %d of %d" % (
-                label, s + 1, rel(U.cpu().numpy(), Uo), hist[-1][0], hist[-1][1], tested))
+                label, s + 1, rel(U.cpu().numpy(), Uo), hist[-1][0], hist[-1][1], tested), flush=True)
     wall = time.time() - wall
     Ug = U.cpu().numpy()
     rep, touched = flip_report(g, og, U0.shape[1:])
@@ -175,11 +175,13 @@ def test_c4_full_config_all_500_steps(mods):
 
 @pytest.mark.skipif(not __import__("os").environ.get("MEG6_LONG"), reason="15 minutes of CPU oracle: set MEG6_LONG=1")
 def test_mig4_256_all_50_steps(mods):
-    """Config 5's scheme, flow and STEP COUNT (50) at 256^3 -- the largest grid of its sweep whose oracle arrays fit the
-    host comfortably (384^3 would need tens of GB).  Result of the round-2 run in profiles/r2_c4_500_steps.md."""
+    """Config 5's scheme, flow and STEP COUNT (50) at 256^3 -- or, with MEG6_LONG_N=384, at the config's own 384^3 (the
+    oracle then holds 64 GB of arrays and needs most of an hour on 16 cores).  Results of the round-2 runs in
+    profiles/r2_c4_500_steps.md."""
     torch, O, M = mods
-    wl = W.c5_tgv_mig4(n=256, steps=50)
-    Ug, Uo, rep, touched, hist = run_both(torch, O, M, wl, wl["U0"], 50, label="c5 mig4 256^3 x 50")
+    n = int(__import__("os").environ.get("MEG6_LONG_N", "256"))
+    wl = W.c5_tgv_mig4(n=n, steps=50)
+    Ug, Uo, rep, touched, hist = run_both(torch, O, M, wl, wl["U0"], 50, label="c5 mig4 %d^3 x 50" % n)
     e = rel(Ug, Uo)
     assert np.all(e <= STEP_TOL), e
     assert rep["e1_flips"] + rep["hllc_flips"] <= 20, rep
