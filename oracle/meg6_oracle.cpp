@@ -819,7 +819,10 @@ void ghost_dir(meg6o_grid* G, int d) {
           /* transverse position clamped to the interior for the lookup of face data, and to the range on which the
            * cell-centre metrics exist (five ghost layers) for the metric lookups of the wall and outflow rules: in the
            * ghost columns beyond a block interface those are the neighbour's true metrics (R27, R28) */
-          const int ca = std::min(std::max(ta, 0), G->n[a] - 1), cb = std::min(std::max(tb, 0), G->n[b] - 1);
+          /* (face data in the ghost columns of a PERIODIC transverse direction: the periodic image's, Table 1 periodic
+           * column -- a ghost cell is its image cell, boundary data included) */
+          const int ca = p.periodic[a] ? (ta % G->n[a] + G->n[a]) % G->n[a] : std::min(std::max(ta, 0), G->n[a] - 1);
+          const int cb = p.periodic[b] ? (tb % G->n[b] + G->n[b]) % G->n[b] : std::min(std::max(tb, 0), G->n[b] - 1);
           const int ma = std::min(std::max(ta, -5), G->n[a] + 4), mb = std::min(std::max(tb, -5), G->n[b] + 4);
           if (bc == 5) {
             /* block interface, Table 1 last column, R28: ghost layer q = the q-th interior cell of the

@@ -66,7 +66,9 @@ __global__ void __launch_bounds__(256) k_ghost(Consts c, int d, P6 P, GhostIn in
     return;
   }
   const int bc = c.bc[2 * d + side];
-  const int ca = min(max(ta, 0), c.n[a] - 1), cb = min(max(tb, 0), c.n[b] - 1);   // face data: interior positions
+  // face data: interior positions; in the ghost columns of a periodic transverse direction the periodic image's
+  const int ca = c.periodic[a] ? (ta % c.n[a] + c.n[a]) % c.n[a] : min(max(ta, 0), c.n[a] - 1);
+  const int cb = c.periodic[b] ? (tb % c.n[b] + c.n[b]) % c.n[b] : min(max(tb, 0), c.n[b] - 1);
   // metric lookups of the wall / outflow rules: wherever the cell-centre metrics exist (five ghost layers; beyond a block
   // interface those are the neighbour's true metrics, R27 / R28)
   const int ma = min(max(ta, -5), c.n[a] + 4), mb = min(max(tb, -5), c.n[b] + 4);

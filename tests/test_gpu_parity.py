@@ -578,6 +578,42 @@ def test_wall_ghosts_rhs_and_steps_parity(mods, name):
     g.close()
 
 
+INOUT_CASES = [(0, False, 1.0, 1, 0), (0, True, 0.5, 0, 0), (1, False, 1.0, 1, 0), (1, True, 1.6, 1, 1),
+               (2, False, 0.5, 1, 1), (2, True, 1.0, 1, 0)]
+
+
+@pytest.mark.parametrize("axis,flip,u_mean,viscous,scheme", INOUT_CASES)
+def test_inflow_outflow_faces_in_every_direction_parity(mods, axis, flip, u_mean, viscous, scheme):
+    """Inflow / outflow ghost rules (Table 1, R20) on each of the six faces, the other two directions
+    periodic, non-uniform inflow data, sub- and supersonic outflow cells in one face (u_mean = 1): one dQ/dt and three
+    RK3 steps against the oracle.  The inflow data of a ghost column of a periodic transverse direction are those of
+    its periodic image (the corner ghost cells the viscous tangential gradients read)."""
+    torch, O, M = mods
+    n = [13, 11, 12]
+    n[axis] = 21
+    wl = W.inout_box(n=tuple(n), axis=axis, flip=flip, viscous=viscous, u_mean=u_mean, scheme=scheme)
+    og = O.Grid(wl)
+    og.metrics_compute(0.0)
+    ref = og.rhs(wl["U0"])
+    g = M.Grid(wl)
+    g.metrics_compute(0.0)
+    U = torch.as_tensor(wl["U0"], device="cuda").contiguous()
+    out = g.rhs(U).cpu().numpy()
+    e = rhs_err(out, ref, wl["U0"])
+    assert np.all(e <= RHS_TOL), (wl["name"], e, rel(out, ref))
+    dt = og.cfl_dt(wl["U0"], wl["cfl"])
+    assert g.cfl_dt(U, wl["cfl"]) == pytest.approx(dt, rel=1e-12)
+    Uo = wl["U0"].copy()
+    t = 0.0
+    for s in range(3):
+        og.rk3_step(Uo, t, dt)
+        g.rk3_step(U, t, dt)
+        t += dt
+    e = rel(U.cpu().numpy(), Uo)
+    assert np.all(e <= STEP_TOL), (wl["name"], e)
+    g.close()
+
+
 def test_walls_on_a_moving_mesh_are_einval(mods):
     torch, O, M = mods
     wl = W.c2_dynamic_freestream(n=12, steps=1)

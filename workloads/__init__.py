@@ -297,6 +297,51 @@ def wall_box(ni=22, nj=19, nk=17, bc=(3, 4, 3, 3, 4, 3), viscous=1, scheme=0, se
 
 
 # --------------------------------------------------------------------------------------------------
+def inout_box(n=(18, 9, 8), axis=0, flip=False, viscous=0, u_mean=1.0, scheme=0, seed=77, h=0.1):
+    """Uniform Cartesian box with an inflow and an outflow face (bc 1 / 2, Table 1) across direction `axis`
+    (flip: inflow on the max side, flow towards the min side), periodic in the two other directions; smooth + seeded
+    state with the stream along `axis` at mean Mach number u_mean (sound speed ~ 1: u_mean = 1 puts sub- and supersonic
+    outflow cells into one face), non-uniform inflow data.  wl["P0"] = the primitive state (rho, u, v, w, p)."""
+    ni, nj, nk = n
+    X, E, Z = _comp_coords(n, (ni * h, nj * h, nk * h))
+    rng = np.random.default_rng(seed)
+    xc, yc, zc = cell_centres(X), cell_centres(E), cell_centres(Z)
+    cc = (xc, yc, zc)
+    kk = [2 * np.pi / (m * h) for m in n]
+    kk[axis] = 3.0                                                # not periodic along the stream
+    wob = lambda ph: np.sin(kk[0] * xc + ph) * np.cos(kk[1] * yc + ph) * np.cos(kk[2] * zc - ph)
+    sgn = -1.0 if flip else 1.0
+    rho = 1.0 + 0.08 * wob(0.3) + 0.01 * rng.uniform(-1, 1, xc.shape)
+    vel = [0.10 * wob(2.0), -0.07 * wob(0.7), 0.05 * wob(1.4)]
+    vel[axis] = sgn * (u_mean + 0.12 * wob(1.1) + 0.01 * rng.uniform(-1, 1, xc.shape))
+    p = (1.0 + 0.08 * wob(1.9) + 0.01 * rng.uniform(-1, 1, xc.shape)) / GAMMA
+    ta, tb = [d for d in range(3) if d != axis]                   # transverse directions, storage order: tb slow
+    take = [slice(None)] * 3
+    take[2 - axis] = 0
+    ca, cb = cc[ta][tuple(take)], cc[tb][tuple(take)]             # (n_tb, n_ta)
+    pin = np.empty((5,) + ca.shape)
+    pin[0] = 1.0 + 0.05 * np.cos(kk[ta] * ca)
+    pin[1:4] = 0.0
+    pin[1 + ta] = 0.03 * np.sin(kk[ta] * ca)
+    pin[1 + tb] = -0.02 * np.sin(kk[tb] * cb)
+    pin[1 + axis] = sgn * (u_mean + 0.05 * np.cos(kk[tb] * cb))
+    pin[4] = (1.0 + 0.04 * np.cos(kk[ta] * ca + kk[tb] * cb)) / GAMMA
+    periodic, bc = [1, 1, 1], [0] * 6
+    periodic[axis] = 0
+    bc[2 * axis + (1 if flip else 0)] = 1
+    bc[2 * axis + (0 if flip else 1)] = 2
+    period = [[0.0] * 3 for _ in range(3)]
+    for d in (ta, tb):
+        period[d][d] = n[d] * h
+    prm = _base_params(ni, nj, nk, periodic=periodic, period=period, viscous=viscous, scheme=scheme,
+                       mu_ref=2e-3 if viscous else 0.0, bc=bc, p_out=0.93 / GAMMA)
+    P0 = np.stack([rho, vel[0], vel[1], vel[2], p])
+    return dict(name="inout_box_%dx%dx%d_axis%d%s" % (ni, nj, nk, axis, "_flip" if flip else ""), params=prm,
+                x=np.ascontiguousarray(X), y=np.ascontiguousarray(E), z=np.ascontiguousarray(Z), U0=conservative(*P0),
+                P0=P0, inflow={2 * axis + (1 if flip else 0): pin}, sigma=None, dt=None, cfl=0.4, steps=3, t0=0.0)
+
+
+# --------------------------------------------------------------------------------------------------
 # Multi-block inputs (Sec. 6, P:342-352): a single-block workload cut into aligned blocks.
 def cartesian_periodic(ni=24, nj=20, nk=16, viscous=1, seed=77, scheme=0):
     """Uniform Cartesian periodic box (spacing 1/8: exactly representable coordinates) with a seeded smooth state:
