@@ -147,7 +147,12 @@ meg6_status meg6_rk3_step_blocks(int n, meg6_grid* const* g, double* const* U, d
  *       meg6_stage_ghosts(g, s, d)                       ghost fill of direction d (all boundary kinds)
  *   meg6_stage_sweeps(g, U, NULL, s, dt)                 gradients + sweeps + fused RK stage update of U
  * meg6_stage_sweeps(g, U, dUdt, 0, 0) writes dQ/dt instead (after stage_prim and the ghost fills with s = 0).
- * Identical, kernel for kernel, to what meg6_rk3_step_blocks launches. */
+ * Identical, kernel for kernel, to what meg6_rk3_step_blocks launches -- except for its edge round: after the three
+ * directions the block calls copy, once more and over the ghost ranges of BOTH transverse directions, the ghost layers
+ * of every face linked by pointer, so that an edge ghost cell beyond an interface is the neighbour's own ghost cell
+ * there (R28).  That matters only where a fixed-inflow face with non-uniform data lies in a direction filled AFTER a
+ * cut direction (the block's own P_in at a clamped index otherwise); a slab decomposition cuts the last direction and
+ * needs no such round, and the staged calls have none. */
 /* The geometry in pieces, for the same callers: meg6_stage_geom_centres(g, t); for d = 0, 1, 2: [meg6_stage_geom_pack
  * (g, face, layers) for the interface faces of direction d -- the ten layers of cell-centre coordinates (moving meshes:
  * and grid velocities) next to `face` over the padded transverse extent, meg6_geom_interface_doubles doubles -- delivered

@@ -795,10 +795,17 @@ void prim_interior(meg6o_grid* G, const double* U) {
 
 /* ghost fill of direction d, after the lower directions: xi over interior (j,k); eta over all filled i; zeta over
  * all (i,j).  With several blocks, direction d is filled in every block before direction d+1 in any. */
-void ghost_dir(meg6o_grid* G, int d) {
+void ghost_dir(meg6o_grid* G, int d, bool edges = false) {
   const meg6o_params& p = G->p;
   int lo[3] = {0, 0, 0}, hi[3] = {G->n[0], G->n[1], G->n[2]};
   for (int e = 0; e < d; ++e) { lo[e] = -GP; hi[e] = G->n[e] + GP; }
+  /* edges (R28): the second round of a multi-block fill -- the faces linked to a neighbour block only, over the ghost
+   * ranges of BOTH transverse directions: an edge ghost cell beyond an interface is the neighbour's own ghost cell
+   * there (its boundary rule with ITS face data), also where the other direction is filled after this one */
+  if (edges) {
+    if (p.periodic[d]) return;
+    for (int e = d + 1; e < 3; ++e) { lo[e] = -GP; hi[e] = G->n[e] + GP; }
+  }
   {
     const int n = G->n[d];
     int a = (d + 1) % 3, b = (d + 2) % 3;
@@ -816,6 +823,7 @@ void ghost_dir(meg6o_grid* G, int d) {
         for (int side = 0; side < 2; ++side) {
           const int face = 2 * d + side, bc = p.bc[face];
           const int last = side ? n - 1 : 0, sg = side ? 1 : -1;
+          if (edges && !(bc == 5 && G->link[face])) continue;
           /* transverse position clamped to the interior for the lookup of face data, and to the range on which the
            * cell-centre metrics exist (five ghost layers) for the metric lookups of the wall and outflow rules: in the
            * ghost columns beyond a block interface those are the neighbour's true metrics (R27, R28) */
@@ -929,6 +937,12 @@ void meg6o_rhs_blocks(int nb, meg6o_grid* const* G, const double* const* U, doub
   for (int pass = 0; pass < (rot ? 3 : 1); ++pass)
     for (int d = 0; d < 3; ++d)
       for (int b = 0; b < nb; ++b) ghost_dir(G[b], d);
+  bool linked = false;
+  for (int b = 0; b < nb; ++b)
+    for (int f = 0; f < 6; ++f) linked = linked || (!G[b]->p.periodic[f / 2] && G[b]->p.bc[f] == 5 && G[b]->link[f]);
+  if (linked)
+    for (int d = 0; d < 3; ++d)
+      for (int b = 0; b < nb; ++b) ghost_dir(G[b], d, true);
   for (int b = 0; b < nb; ++b) finish_primitives(G[b]);
   for (int b = 0; b < nb; ++b) rhs_from_primitives(G[b], U[b], dUdt[b]);
 }

@@ -576,16 +576,19 @@ meg6_status meg6_set_sponge(meg6_grid* g, const double* sigma, const double* U_r
 // ghost layers of direction d in primitive buffer `buf` (the lower directions are filled already).  Block interfaces
 // read the SAME buffer of the neighbour block: with several blocks, direction d is filled in every block before
 // direction d+1 in any (edge and corner ghosts then arrive from the diagonal neighbours in two steps).
-static cudaError_t fill_ghosts_dir(meg6_grid* g, int buf, int d) {
+static cudaError_t fill_ghosts_dir(meg6_grid* g, int buf, int d, bool edges = false) {
   const Consts& c = g->c;
+  if (edges && (c.periodic[d] || (!g->link[2 * d] && !g->link[2 * d + 1]))) return cudaSuccess;
   double* const* Pc = buf ? g->Pb : g->P;
   P6 P;
   for (int f = 0; f < 6; ++f) P.p[f] = Pc[f];
   int a = (d + 1) % 3, b = (d + 2) % 3;
   if (a > b) { int t = a; a = b; b = t; }
-  const long long ea = c.n[a] + ((a < d) ? 12 : 0), eb = c.n[b] + ((b < d) ? 12 : 0);
+  const long long ea = c.n[a] + ((a < d || edges) ? 12 : 0), eb = c.n[b] + ((b < d || edges) ? 12 : 0);
   GhostIn gin;
   memset(&gin, 0, sizeof(gin));
+  gin.edges = edges ? 1 : 0;
+  for (int side = 0; side < 2; ++side) gin.edge[side] = (c.bc[2 * d + side] == 5 && g->link[2 * d + side]) ? 1 : 0;
   gin.inflow[0] = g->inflow[2 * d]; gin.inflow[1] = g->inflow[2 * d + 1];
   gin.mx = g->met[3 * d]; gin.my = g->met[3 * d + 1]; gin.mz = g->met[3 * d + 2];
   for (int side = 0; side < 2; ++side) {
@@ -622,6 +625,10 @@ static cudaError_t fill_ghosts(meg6_grid* g, int buf) {
       const cudaError_t e = fill_ghosts_dir(g, buf, d);
       if (e != cudaSuccess) return e;
     }
+  for (int d = 0; d < 3; ++d) {   // edge round (R28): a block linked to itself
+    const cudaError_t e = fill_ghosts_dir(g, buf, d, true);
+    if (e != cudaSuccess) return e;
+  }
   return cudaSuccess;
 }
 
@@ -915,6 +922,8 @@ meg6_status meg6_rhs_blocks(int n, meg6_grid* const* g, const double* const* U, 
   for (int pass = 0; pass < ghost_passes(n, g); ++pass)
     for (int d = 0; d < 3; ++d)
       for (int b = 0; b < n; ++b) CUDA_OK(fill_ghosts_dir(g[b], 0, d));
+  for (int d = 0; d < 3; ++d)   // edge round (R28; nothing is launched for a block without linked faces along d)
+    for (int b = 0; b < n; ++b) CUDA_OK(fill_ghosts_dir(g[b], 0, d, true));
   for (int b = 0; b < n; ++b) {
     Fuse3 fu = make_fuse(g[b], U[b], dUdt[b]);
     fu.mode = 0;
@@ -940,6 +949,8 @@ meg6_status meg6_rk3_step_blocks(int n, meg6_grid* const* g, double* const* U, d
     for (int pass = 0; pass < ghost_passes(n, g); ++pass)
       for (int d = 0; d < 3; ++d)
         for (int b = 0; b < n; ++b) CUDA_OK(fill_ghosts_dir(g[b], s & 1, d));
+    for (int d = 0; d < 3; ++d)
+      for (int b = 0; b < n; ++b) CUDA_OK(fill_ghosts_dir(g[b], s & 1, d, true));
     for (int b = 0; b < n; ++b)
       if ((st = stage_sweeps(g[b], s & 1, make_fuse_rk(g[b], U[b], s, dt))) != MEG6_OK) return st;
   }

@@ -29,6 +29,10 @@ struct GhostIn {
   // along this direction, per side
   const double* nbP[2]; Lay nbL[2]; long long nbfs[2];
   int nax[2][3], nsg[2][3], nsh[2][3];   // index map home -> neighbour: m[nax[e]] = nsg[e] > 0 ? h[e] + nsh[e] : nsh[e] - h[e]
+  // edge round of a multi-block fill (R28): only the sides with edge[side] set (faces linked to a block of this call),
+  // over the ghost ranges of BOTH transverse directions -- an edge ghost cell beyond an interface is the neighbour's
+  // own ghost cell there (its boundary rule with its face data), also where the other direction is filled later
+  int edges, edge[2];
 };
 
 // B: ghost layers of direction d (6 deep), after the lower directions have been filled: periodic wrap, fixed
@@ -40,8 +44,8 @@ __global__ void __launch_bounds__(256) k_ghost(Consts c, int d, P6 P, GhostIn in
   if (a > b) { int t = a; a = b; b = t; }
   constexpr int NG = 6;
   // transverse ranges: directions below d are already extended
-  const int loa = (a < d) ? -NG : 0, ea = c.n[a] + ((a < d) ? 2 * NG : 0);
-  const int lob = (b < d) ? -NG : 0, eb = c.n[b] + ((b < d) ? 2 * NG : 0);
+  const int loa = (a < d || in.edges) ? -NG : 0, ea = c.n[a] + ((a < d || in.edges) ? 2 * NG : 0);
+  const int lob = (b < d || in.edges) ? -NG : 0, eb = c.n[b] + ((b < d || in.edges) ? 2 * NG : 0);
   const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (tid >= (long long)ea * eb * 2 * NG) return;
   int qs, ta, tb;   // qs = layer + 6 * side
@@ -56,6 +60,7 @@ __global__ void __launch_bounds__(256) k_ghost(Consts c, int d, P6 P, GhostIn in
   const long long base = c.LP.at(ix[0], ix[1], ix[2]);   // cell 0 of this line
   const int last = side ? n - 1 : 0, sg = side ? 1 : -1;
   const long long dst = base + (long long)(last + sg * q) * s;
+  if (in.edges && !in.edge[side]) return;
   if (c.periodic[d]) {
     const long long src = side ? base + (long long)(q - 1) * s : base + (long long)(n - q) * s;
     double v[6];

@@ -629,6 +629,10 @@ def _block_sets():
         "cart_zeta_cut_inviscid": (W.cartesian_periodic(nk=22, viscous=0), ((24,), (20,), (12, 10))),
         "curved_box_walls_2x2x2": (W.wall_box(ni=26, nj=24, nk=22), ((14, 12), (11, 13), (10, 12))),
         "curved_box_walls_mig4": (W.wall_box(ni=26, nj=24, nk=22, scheme=1), ((14, 12), (24,), (10, 12))),
+        # inflow / outflow faces across zeta with non-uniform P_in, cut in xi and eta: the corner ghost cells beyond the
+        # block edges are the NEIGHBOUR's inflow ghosts (edge round of the fill, R28)
+        "inout_zeta_cut_xi_eta": (W.inout_box(n=(23, 21, 21), axis=2, viscous=1, u_mean=1.0), ((12, 11), (10, 11), (21,))),
+        "inout_eta_cut_xi": (W.inout_box(n=(23, 21, 12), axis=1, flip=True, viscous=1, u_mean=0.5), ((12, 11), (21,), (12,))),
     }
 
 

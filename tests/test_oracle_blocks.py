@@ -56,15 +56,14 @@ def test_cut_periodic_cartesian_box_equals_the_uncut_one(cuts, viscous):
     assert relerr(gather(blocks, Us, U.shape), U) <= 1e-12
 
 
-@pytest.mark.parametrize("axis,cuts", [(0, ((21,), (11, 10), (12,))), (0, ((21,), (11,), (11, 10))),
-                                       (1, ((13,), (21,), (10, 11))), (0, ((11, 10), (11,), (12,)))])
+@pytest.mark.parametrize("axis,cuts", [(0, ((21,), (11, 10), (12,))), (1, ((13,), (21,), (10, 11))),
+                                       (0, ((11, 10), (11,), (12,))), (1, ((11, 10), (21,), (12,))),
+                                       (2, ((12, 11), (10, 11), (21,)))])
 def test_cut_inflow_outflow_box_equals_the_uncut_one(axis, cuts):
-    """Non-uniform inflow data, sub- and supersonic outflow, viscous, cut ACROSS the stream or along a direction that
-    comes after the stream's in the ghost-fill order (xi, eta, zeta): exactly the uncut box.  (A cut in a direction
-    BEFORE the inflow face's -- e.g. a zeta inflow face on a domain cut in xi -- is the one combination that is not: the
-    corner ghost cells beyond the block edge take the block's own inflow data at the clamped index, not the
-    neighbour's; 1e-4 of the viscous dQ/dt in the edge cells, R28 "limits".  Config 4 and the slab mode,
-    inflow at imin and cuts in zeta, are of the exact kind.)"""
+    """Non-uniform inflow data, sub- and supersonic outflow, viscous; cut across the stream, in a direction after the
+    stream's in the ghost-fill order (xi, eta, zeta), and in directions BEFORE it: exactly the uncut box.  The last kind
+    needs the edge round of the multi-block fill (R28): the corner ghost cells beyond a block edge are the neighbour's
+    own inflow ghosts, formed with the neighbour's P_in, not the block's P_in at a clamped index."""
     n = tuple(sum(c) for c in cuts)
     wl = W.inout_box(n=n, axis=axis, viscous=1, u_mean=1.0)
     g1 = O.Grid(wl)
