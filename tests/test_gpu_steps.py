@@ -185,3 +185,22 @@ def test_mig4_256_all_50_steps(mods):
     e = rel(Ug, Uo)
     assert np.all(e <= STEP_TOL), e
     assert rep["e1_flips"] + rep["hllc_flips"] <= 20, rep
+
+
+def test_c2_mesh_and_step_count_with_a_nontrivial_flow(mods):
+    """Config 2's mesh, motion, size and STEP COUNT (64^3 jittered mesh, nodes moving at omega = 1, 100 RK3 steps) with a
+    smooth non-uniform flow instead of the freestream (whose parity is trivial: both sides stay uniform to 1e-12): 300
+    geometry evaluations at the stage times, grid velocities, time metrics and GCL terms against the oracle's over the
+    whole run (a minute of oracle time on 16 cores)."""
+    torch, O, M = mods
+    wl = W.c2_dynamic_freestream(n=64)
+    xc, yc, zc = (W.cell_centres(wl[k]) for k in ("x", "y", "z"))
+    s2 = lambda a: np.sin(2 * np.pi * a)
+    U0 = W.conservative(1 + 0.1 * s2(xc) * s2(yc), 1 + 0.2 * s2(yc + 0.1), 0.1 * s2(zc) * s2(xc),
+                        -0.15 * s2(xc + 0.3), (1 + 0.05 * s2(zc + 0.2)) / (1.4 * 0.25))
+    Ug, Uo, rep, touched, hist = run_both(torch, O, M, wl, U0, 100, label="c2 mesh 64^3 x 100, smooth flow")
+    e = rel(Ug, Uo)
+    assert np.all(e <= STEP_TOL), e
+    assert np.abs(Ug - U0).max() > 1e-2
+    assert rep["e1_flips"] + rep["hllc_flips"] <= 20, rep
+
