@@ -3,6 +3,12 @@ import sys
 
 import pytest
 
+# The oracle's OpenMP threads sleep at the end of a parallel loop instead of spinning (read by libgomp when it is first
+# loaded, hence here, before anything imports it): most oracle pins are tiny grids with thousands of short loops, and
+# on a shared host whose cores are taken away now and then spinning threads made the CPU suite five to ten times slower.
+# Timing is not what tests measure; bench.py's cpu_baseline does not go through here.
+os.environ.setdefault("OMP_WAIT_POLICY", "passive")
+
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
