@@ -3,8 +3,10 @@
 
 One "step" = one SSP-RK3 step = three passes of the whole hot path (ghosts, gradients, three flux sweeps, the last
 one fused with residual assembly + RK3 update + primitive conversion) over the workload; the K timed steps are one
-meg6_rk3_steps call (state resident on the device); the end-to-end number calls meg6_rk3_step per step between the copies.  value = N_cells * 3 * steps / seconds, in Mcell-updates/s per
-RK stage, summed over all ranks (independent replicas for --gpus > 1: the path is single-GPU).
+meg6_rk3_steps call (state resident on the device); the end-to-end number calls meg6_rk3_step per step between a
+host -> device copy of the whole state and a device -> host copy of the result, E2E_STATES independent states in flight
+on three streams (the one-state, strictly sequential form is reported beside it as e2e.serial).
+value = N_cells * 3 * steps / seconds, in Mcell-updates/s per RK stage, summed over all ranks (independent replicas for --gpus > 1: the path is single-GPU).
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c4|c3|c1|c2] [--impl reference]
 """
